@@ -1,0 +1,240 @@
+"""ctypes wrapper of the CPU oracle (oracle/mpr_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke()
+and bench.py's cpu_baseline / --impl reference legs may import this module.
+It imports nothing from paper_1811_01604_b200.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mpr_oracle.c")
+_LIB = os.path.join(_HERE, "libmpr_oracle.so")
+
+TWO_PI_F = float(np.float32(2.0 * np.pi))   # 6.2831854820251465
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2, no FMA contraction, no fast-math; OpenMP over one colour's rows."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+               "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        f32p = np.ctypeslib.ndpointer(np.float32, flags="C_CONTIGUOUS")
+        f64p = np.ctypeslib.ndpointer(np.float64, flags="C_CONTIGUOUS")
+        u8p = np.ctypeslib.ndpointer(np.uint8, flags="C_CONTIGUOUS")
+        u32p = np.ctypeslib.ndpointer(np.uint32, flags="C_CONTIGUOUS")
+        L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]
+        L.orc_philox4x32_10.restype = None
+        L.orc_u01.argtypes = [C.c_uint32]
+        L.orc_u01.restype = C.c_double
+        L.orc_minmax.argtypes = [f32p, u8p, C.c_int64, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.orc_minmax.restype = C.c_int64
+        L.orc_eq1.argtypes = [C.c_float, C.c_float, C.c_float]
+        L.orc_eq1.restype = C.c_float
+        L.orc_transform.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_uint64, C.c_uint32,
+                                    C.c_float, C.c_float, f32p]
+        L.orc_transform.restype = None
+        L.orc_local_energy.argtypes = [C.c_double] * 4
+        L.orc_local_energy.restype = C.c_double
+        L.orc_or_reflect.argtypes = [C.c_double] * 6 + [C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double)]
+        L.orc_or_reflect.restype = C.c_double
+        L.orc_sweep.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                C.c_uint64, C.c_uint32, C.c_uint32, C.c_int,
+                                C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_sweep.restype = C.c_uint64
+        L.orc_n_bonds.argtypes = [C.c_int, C.c_int]
+        L.orc_n_bonds.restype = C.c_int64
+        L.orc_energy.argtypes = [f32p, C.c_int, C.c_int, C.c_double]
+        L.orc_energy.restype = C.c_double
+        L.orc_sg_slope.argtypes = [f64p, C.c_int]
+        L.orc_sg_slope.restype = C.c_double
+        L.orc_equilibrate.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_double, C.c_double,
+                                      C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_int, C.c_int,
+                                      C.c_double, C.c_double, C.POINTER(C.c_uint32),
+                                      C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                      C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_equilibrate.restype = C.c_int
+        L.orc_simulate.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                   C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_int,
+                                   C.POINTER(C.c_uint32), f64p]
+        L.orc_simulate.restype = None
+        L.orc_predict.argtypes = [f64p, C.c_int, f32p, u8p, C.c_int64, C.c_float, C.c_float, f32p]
+        L.orc_predict.restype = None
+        L.orc_num_threads.restype = C.c_int
+        L.orc_set_num_threads.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+# ---------------------------------------------------------------------------
+# thin functional wrappers (numpy in, numpy out)
+# ---------------------------------------------------------------------------
+def philox4x32_10(counter, key) -> np.ndarray:
+    c = np.ascontiguousarray(counter, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty(4, dtype=np.uint32)
+    lib().orc_philox4x32_10(c, k, out)
+    return out
+
+
+def u01(x: int) -> float:
+    return lib().orc_u01(int(x) & 0xFFFFFFFF)
+
+
+def minmax(z: np.ndarray, mask: np.ndarray):
+    zf = np.ascontiguousarray(z, dtype=np.float32).ravel()
+    m = np.ascontiguousarray(mask, dtype=np.uint8).ravel()
+    lo, hi = C.c_float(), C.c_float()
+    n = lib().orc_minmax(zf, m, zf.size, C.byref(lo), C.byref(hi))
+    return np.float32(lo.value), np.float32(hi.value), int(n)
+
+
+def eq1(z, zmin, zmax) -> np.float32:
+    return np.float32(lib().orc_eq1(float(z), float(zmin), float(zmax)))
+
+
+def transform(z: np.ndarray, mask: np.ndarray, seed: int, g: int = 0):
+    """O1 + O2: returns (phi float32 [rows, cols], zmin, zmax)."""
+    rows, cols = z.shape
+    zf = np.ascontiguousarray(z, dtype=np.float32)
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    zmin, zmax, _ = minmax(zf, m)
+    phi = np.empty((rows, cols), dtype=np.float32)
+    lib().orc_transform(zf, m, rows, cols, seed, g, float(zmin), float(zmax), phi)
+    return phi, zmin, zmax
+
+
+def local_energy(phi, Cs, Ss, q) -> float:
+    return lib().orc_local_energy(phi, Cs, Ss, q)
+
+
+def or_reflect(phi, Cs, Ss, q, mode=0, C1=0.0, S1=0.0):
+    kept, raw = C.c_int(), C.c_double()
+    p = lib().orc_or_reflect(phi, Cs, Ss, C1, S1, q, mode, C.byref(kept), C.byref(raw))
+    return p, bool(kept.value), raw.value
+
+
+def sweep(phi: np.ndarray, mask: np.ndarray, q, T, a, seed, g, t, or_mode=0, diag=False):
+    """One UPDATE sweep IN PLACE on phi (float32 [rows, cols]); returns the
+    accepted count, plus (margin, edge, R) double arrays when diag=True."""
+    rows, cols = phi.shape
+    assert phi.dtype == np.float32 and phi.flags.c_contiguous
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    if diag:
+        mg = np.full((rows, cols), np.inf)
+        ed = np.full((rows, cols), np.inf)
+        RR = np.full((rows, cols), np.inf)
+        acc = lib().orc_sweep(phi, m, rows, cols, q, T, a, seed, g, t, or_mode,
+                              mg.ctypes.data, ed.ctypes.data, RR.ctypes.data)
+        return int(acc), mg, ed, RR
+    return int(lib().orc_sweep(phi, m, rows, cols, q, T, a, seed, g, t, or_mode, None, None, None))
+
+
+def n_bonds(rows, cols) -> int:
+    return int(lib().orc_n_bonds(rows, cols))
+
+
+def energy(phi: np.ndarray, q=0.5) -> float:
+    rows, cols = phi.shape
+    return lib().orc_energy(np.ascontiguousarray(phi, dtype=np.float32), rows, cols, q)
+
+
+def energy_per_bond(phi: np.ndarray, q=0.5) -> float:
+    return energy(phi, q) / n_bonds(*phi.shape)
+
+
+def sg_slope(e) -> float:
+    e = np.ascontiguousarray(e, dtype=np.float64)
+    return lib().orc_sg_slope(e, e.size)
+
+
+@dataclass
+class Params:
+    """Alg. 2 step 1 parameters; defaults = reading R7."""
+    q: float = 0.5
+    equil_cap: int = 500
+    sweeps_per_real: int = 1
+    M: int = 100
+    seed: int = 0
+    n_f: int = 5
+    n_fit: int = 20
+    A_targ: float = 0.3
+    k_a: float = 3.0
+    or_mode: int = 0
+    a_eq_mode: int = 0
+
+
+def equilibrate(phi, mask, T, p: Params, g=0, t0=0, history=False):
+    rows, cols = phi.shape
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    t = C.c_uint32(t0)
+    a, k = C.c_double(), C.c_double()
+    if history:
+        eh = np.zeros(p.equil_cap + 2); Ah = np.zeros(p.equil_cap + 2); ah = np.zeros(p.equil_cap + 2)
+        ptrs = (eh.ctypes.data, Ah.ctypes.data, ah.ctypes.data)
+    else:
+        ptrs = (None, None, None)
+    i = lib().orc_equilibrate(phi, m, rows, cols, p.q, float(T), p.seed, g, p.or_mode,
+                              p.equil_cap, p.n_f, p.n_fit, p.A_targ, p.k_a,
+                              C.byref(t), C.byref(a), C.byref(k), *ptrs)
+    out = {"sweeps": int(i), "a": a.value, "k": k.value, "t": int(t.value)}
+    if history:
+        out.update(e_hist=eh[: i + 1], A_hist=Ah[: i + 1], a_hist=ah[: i + 1])
+    return out
+
+
+def simulate(phi, mask, T, a_eq, p: Params, g=0, t0=0):
+    rows, cols = phi.shape
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    t = C.c_uint32(t0)
+    acc = np.zeros((rows, cols), dtype=np.float64)
+    lib().orc_simulate(phi, m, rows, cols, p.q, float(T), float(a_eq), p.seed, g, p.or_mode,
+                       p.M, p.sweeps_per_real, C.byref(t), acc.reshape(-1))
+    return acc, int(t.value)
+
+
+def predict(acc, M, z, mask, zmin, zmax) -> np.ndarray:
+    zf = np.ascontiguousarray(z, dtype=np.float32)
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    out = np.empty_like(zf)
+    lib().orc_predict(np.ascontiguousarray(acc, dtype=np.float64).reshape(-1), M, zf.reshape(-1),
+                      m.reshape(-1), zf.size, float(zmin), float(zmax), out.reshape(-1))
+    return out
+
+
+def run(z, mask, T, p: Params, g=0):
+    """Alg. 2 steps 2, 3, 5, 6, 7 for one grid (T is an input: step 4 is not on
+    this path).  Returns dict(pred, phi, stats)."""
+    phi, zmin, zmax = transform(z, mask, p.seed, g)
+    st = equilibrate(phi, mask, T, p, g=g, t0=0)
+    a_eq = st["a"] if p.a_eq_mode == 0 else 1.0
+    acc, t_end = simulate(phi, mask, T, a_eq, p, g=g, t0=st["t"])
+    pred = predict(acc, p.M, z, mask, zmin, zmax)
+    st.update(t_end=t_end, a_eq=a_eq, zmin=zmin, zmax=zmax,
+              e_final=energy_per_bond(phi, p.q))
+    return {"pred": pred, "phi": phi, "stats": st}
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().orc_set_num_threads(int(n))
