@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""Benchmark of the MPR hot path on B200 (contract: see DESIGN.md "Measurement").
+
+A step = one pass of the whole path over one synthetic grid (batch):
+mpr_create (min/max, Eq. 1, lists) -> mpr_set_params (initial state) ->
+mpr_equilibrate -> mpr_simulate (M x s sweeps) -> mpr_predict.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `value` = prediction-site updates per second
+(GUpdates/s) with the inputs resident in HBM; `e2e` = the same with HOST
+buffers (H2D of values + mask, D2H of the prediction inside the timed
+region); `roofline` = the half-sweep kernel against the measured HBM peak;
+`cpu_baseline` = the oracle, as it stands, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "prediction-site updates per second"
+UNIT = "GUpdates/s"
+L2_FLUSH_BYTES = 512 << 20
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg4", help="cfg1..cfg5, paper33, paper66 (BASELINE.json configs)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--L", type=int, default=None, help="override the grid side (debugging only)")
+    ap.add_argument("--batch", type=int, default=None, help="override the batch of cfg5 (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples SM clocks and throttle reasons during the timed region (NVML)."""
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def algorithmic_bytes_per_sweep(N: int, P: int) -> float:
+    """every site read once, every prediction site written once,
+    one mask bit per site: 4N + 4P + N/8 bytes per sweep."""
+    return 4.0 * N + 4.0 * P + N / 8.0
+
+
+# ---------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on the host cores
+# ---------------------------------------------------------------------------
+def oracle_sample(w, n_sweeps: int):
+    """Times n_sweeps oracle UPDATE sweeps on grid 0 of the workload from the
+    oracle's own initial state at a = 1 (bounded sample of the same workload).
+    Returns (updates per second, seconds, threads)."""
+    from oracle import mpr_oracle as orc
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    phi, _, _ = orc.transform(z, m, w.seed)
+    P = int((m == 0).sum())
+    orc.sweep(phi, m, w.q, T, 1.0, w.seed, 0, 0)               # warm the caches / thread pool
+    t0 = time.perf_counter()
+    for t in range(1, n_sweeps + 1):
+        orc.sweep(phi, m, w.q, T, 1.0 + t / 3.0, w.seed, 0, t)
+    dt = time.perf_counter() - t0
+    return P * n_sweeps / dt, dt, orc.num_threads()
+
+
+def oracle_sweeps_for(w) -> int:
+    """About 10-30 s of CPU work: ~60 ns per update per core as a planning figure."""
+    P = int((w.mask[0] == 0).sum())
+    return int(max(3, min(2000, 8.0e7 / max(P, 1))))
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_sweeps = oracle_sweeps_for(w)
+    for _ in range(args.warmup):
+        oracle_sample(w, max(1, n_sweeps // 10))
+    rates, secs, cores = [], 0.0, 1
+    for _ in range(args.steps):
+        r, dt, cores = oracle_sample(w, n_sweeps)
+        rates.append(r); secs += dt
+    value = float(np.mean(rates)) / 1e9
+    sample = f"{n_sweeps} UPDATE sweeps of grid 0 of {w.name} ({w.rows}x{w.cols}) per step from the initial state"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "rows": w.rows, "cols": w.cols, "batch": w.batch},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ---------------------------------------------------------------------------
+# the CUDA path
+# ---------------------------------------------------------------------------
+def run_b200(args, w):
+    import torch
+    import torch.distributed as dist
+    from paper_1811_01604_b200 import mpr
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the MPR path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # one independent unit (grid batch) per rank, no data-path collective: replicas, weak scaling
+    seed = w.seed + 7919 * rank
+    h_values = torch.from_numpy(w.truth).pin_memory()
+    h_mask = torch.from_numpy(w.mask).pin_memory()
+    h_out = torch.empty(w.truth.shape, dtype=torch.float32).pin_memory()
+    d_values, d_mask = h_values.to(dev), h_mask.to(dev)
+    d_out = torch.empty_like(d_values)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    T = [float(x) for x in w.T]
+    prm = dict(seed=seed, q=w.q, equil_cap=w.equil_cap, sweeps_per_real=w.sweeps_per_real, M=w.M)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def one_pass(values, mask):
+        ctx = mpr.Mpr(values, mask)
+        ctx.set_params(T, **prm).equilibrate().simulate()
+        ctx.predict(d_out)
+        return ctx
+
+    def step_device():
+        ctx = one_pass(d_values, d_mask)
+        return ctx
+
+    def step_e2e():
+        dv = h_values.to(dev, non_blocking=True)
+        dm = h_mask.to(dev, non_blocking=True)
+        ctx = one_pass(dv, dm)
+        h_out.copy_(d_out, non_blocking=True)
+        return ctx
+
+    def timed(step_fn, steps):
+        """Returns (seconds for `steps` steps, updates done, launches) with an L2 flush between steps
+        (outside the per-step events) and CUDA events on the launching stream."""
+        total_ms, updates, launches = 0.0, 0, 0
+        for _ in range(steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            e0.record(stream)
+            ctx = step_fn()
+            e1.record(stream)
+            e1.synchronize()
+            total_ms += e0.elapsed_time(e1)
+            st = ctx.get_stats()
+            updates += sum(s.n_free * s.t for s in st)
+            launches += ctx.launch_count()
+            ctx.close()
+        return total_ms / 1e3, updates, launches
+
+    for _ in range(max(args.warmup, 1)):
+        step_device().close()
+    barrier()
+    with ClockSampler(local) as clk:
+        secs, updates, launches = timed(step_device, args.steps)
+    barrier()
+    step_e2e().close()
+    barrier()
+    secs_e2e, updates_e2e, _ = timed(step_e2e, args.steps)
+    barrier()
+
+    # the dominant kernel alone: half-sweeps on the equilibrated state, CUDA events around n sweeps
+    ctx = mpr.Mpr(d_values, d_mask)
+    ctx.set_params(T, **prm).equilibrate()
+    st = ctx.get_stats()
+    a_eq = float(np.mean([s.a for s in st]))
+    n_probe = 50
+    ctx.sweep(5, a_eq)
+    stream.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    ctx.sweep(n_probe, a_eq)
+    e1.record(stream)
+    e1.synchronize()
+    halfsweep_s = e0.elapsed_time(e1) / 1e3 / (2 * n_probe)
+    N_sites = w.rows * w.cols * w.batch
+    P_sites = sum(s.n_free for s in st)
+    equil_sweeps = [s.equil_sweeps for s in st]
+    ctx.close()
+
+    if world > 1:
+        t = torch.tensor([secs, secs_e2e, halfsweep_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        secs, secs_e2e, halfsweep_s = (float(x) for x in t.cpu())
+        u = torch.tensor([updates, updates_e2e, launches], dtype=torch.float64, device=dev)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        updates, updates_e2e, launches = (float(x) for x in u.cpu())
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        bytes_per_launch = algorithmic_bytes_per_sweep(N_sites, P_sites) / 2.0
+        achieved = bytes_per_launch / halfsweep_s / 1e9
+        out = {
+            "metric": METRIC, "value": updates / secs / 1e9, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "rows": w.rows, "cols": w.cols, "batch": w.batch,
+                       "n_free_per_rank": int(P_sites), "equil_cap": w.equil_cap, "M": w.M,
+                       "sweeps_per_real": w.sweeps_per_real, "equil_sweeps": equil_sweeps,
+                       "parallelism": f"replicas x{world}", "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)",
+                       "step": "mpr_create+set_params+equilibrate+simulate+predict"},
+            "ms_per_grid": 1e3 * secs / args.steps / w.batch,
+            "lattice_site_visits_per_s": updates / secs / max(P_sites, 1) * N_sites,
+            "e2e": {"value": updates_e2e / secs_e2e / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": int(h_values.numel() * 4 + h_mask.numel()),
+                    "d2h_bytes_per_step": int(h_out.numel() * 4), "ms_per_step": 1e3 * secs_e2e / args.steps},
+            "gpu_launches": int(launches),
+            "clocks": clk.summary(),
+            "roofline": {"bound": "hbm", "kernel": "k_halfsweep", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": bytes_per_launch, "us_per_launch": halfsweep_s * 1e6,
+                         "gupdates_per_s_kernel_only": P_sites / 2.0 / halfsweep_s / 1e9},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            n_sweeps = oracle_sweeps_for(w)
+            rate, dt, cores = oracle_sample(w, n_sweeps)
+            out["cpu_baseline"] = {
+                "value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+                "sample": f"{n_sweeps} UPDATE sweeps of grid 0 of {w.name} ({w.rows}x{w.cols}) from the initial state"}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    from paper_1811_01604_b200 import synth
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference" and rank != 0:
+        return
+    w = synth.make_workload(args.workload, batch=args.batch, L=args.L)
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_b200(args, w)
+
+
+if __name__ == "__main__":
+    main()

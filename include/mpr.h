@@ -1,0 +1,171 @@
+/*
+ * mpr.h -- C ABI of the B200-native (sm_100a) hot path of the modified planar
+ * rotator (MPR) conditional simulation, arXiv 1811.01604 ("PAPER.md").
+ *
+ * The library fills the gaps of `batch` independent rows x cols grids:
+ * sample sites (mask = 1) are held fixed, prediction sites (mask = 0) are
+ * simulated by the checkerboard hybrid Monte Carlo sweep (PAPER.md L113-146
+ * Alg. 1) to the paper's energy-slope equilibration (L192-206,
+ * Alg. 2 step 5), followed by M realizations (L207-211, step 6) whose mean is
+ * back-transformed into the interpolated map (L148, L212, step 7).
+ *
+ * Conventions (all entry points)
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.
+ *   - The caller owns every buffer it passes (inputs, workspace, outputs).
+ *     The library owns only the small host-side mpr_ctx (plus a few bytes of
+ *     pinned host memory used to poll device flags).  All device state lives
+ *     inside the caller's workspace.
+ *   - Every call returns an mpr_status; nothing throws, aborts or sets errno.
+ *     Output parameters are left untouched when the status is not MPR_OK.
+ *   - Work is enqueued on the CUDA stream given to mpr_create.  Calls that
+ *     return host data (and mpr_create / mpr_equilibrate, which need device
+ *     results to size launches / stop the loop) synchronise that stream; the
+ *     others return as soon as the work is enqueued.
+ *   - A context is not thread-safe; distinct contexts are independent.
+ *   - Grids are row-major, [batch][rows][cols]; rectangular grids are allowed
+ *     (PAPER.md L261).  2 <= rows, cols <= 65534; rows*cols < 2^31.
+ *   - Random numbers: Philox4x32-10 keyed by `seed`, counter
+ *     (ordinal pair, global sweep index t, 2 + colour, grid) for the sweeps and
+ *     (site >> 2, 0, 0, grid) for the initial state (reading R13).
+ *     t counts sweeps from mpr_set_params on, through equilibration and every
+ *     realization.
+ */
+#ifndef MPR_H
+#define MPR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mpr_ctx mpr_ctx; /* opaque */
+
+typedef enum {
+    MPR_OK = 0,
+    MPR_ERR_ARG = 1,              /* bad argument (null pointer, size, q, T, M, ...) */
+    MPR_ERR_NO_SAMPLES = 2,       /* a grid has no sample site (mask all 0) */
+    MPR_ERR_NO_FREE = 3,          /* a grid has no prediction site (mask all 1) */
+    MPR_ERR_DEGENERATE_RANGE = 4, /* z_max == z_min over the samples: Eq. 1 divides by zero */
+    MPR_ERR_NONFINITE = 5,        /* a sample value is NaN or Inf */
+    MPR_ERR_STATE = 6,            /* call out of order (e.g. sweep before set_params) */
+    MPR_ERR_WORKSPACE = 7,        /* workspace too small or misaligned (256 B) */
+    MPR_ERR_CUDA = 8,             /* a CUDA runtime call failed; see mpr_last_cuda_error */
+    MPR_ERR_UNSUPPORTED = 9       /* valid per the paper but not built (or_mode 1 with q != 1/2) */
+} mpr_status;
+
+/* Alg. 2 step 1 parameters.  POD, host memory. */
+typedef struct {
+    uint32_t struct_size;     /* = sizeof(mpr_params); ABI versioning */
+    float    q;               /* coupling exponent, 0 < q <= 0.5; paper: 1/2 (L89) */
+    uint32_t equil_cap;       /* i_max, at most this many equilibration sweeps (L171, L192) */
+    uint32_t sweeps_per_real; /* UPDATE sweeps per realization; paper 1 (L210), BASELINE configs 100 */
+    uint32_t M;               /* number of realizations (L168), >= 1 */
+    uint32_t n_f;             /* slope checked every n_f sweeps (L169, L201) */
+    uint32_t n_fit;           /* window of the slope fit, 2 <= n_fit <= 256 (L169, L201) */
+    float    A_targ;          /* target acceptance ratio (L170, L196) */
+    float    k_a;             /* proposal-width growth constant (L171, L197) */
+    uint32_t or_mode;         /* 0 exact-q reflection (R2), 1 Eq. 6 as printed (q = 1/2 only), 2 off */
+    uint32_t a_eq_mode;       /* 0 keep the a reached in equilibration, 1 a = 1 as printed at L210 (R10) */
+    uint64_t seed;            /* Philox key */
+} mpr_params;
+
+/* Per-grid run statistics (host). */
+typedef struct {
+    uint32_t equil_sweeps;    /* i: sweeps done by mpr_equilibrate */
+    uint32_t t;               /* global sweep index (sweeps since mpr_set_params) */
+    uint32_t equilibrated;    /* 1 once the stopping rule k >= 0 or the cap was reached */
+    uint32_t realizations;    /* realizations accumulated so far */
+    uint64_t n_free;          /* P: prediction sites */
+    uint64_t n_samples;       /* sample sites */
+    uint64_t n_bonds;         /* N_GP = rows(cols-1) + cols(rows-1) (L109) */
+    double   a;               /* current proposal-width divisor, alpha = 2 pi / a (L156) */
+    double   k;               /* last fitted energy slope (L201) */
+    double   A_last;          /* acceptance ratio of the last counted sweep */
+    double   e_last;          /* energy per bond after the last counted sweep (L199) */
+    float    z_min, z_max;    /* Eq. 1 range (L81) */
+} mpr_stats;
+
+/* Default parameters: q = 1/2, n_f = 5, n_fit = 20, A_targ = 0.3, k_a = 3,
+ * equil_cap = 500, M = 100, sweeps_per_real = 1, modes 0, seed 0
+ * (reading R7; the paper defers them to its companion paper, L166). */
+void mpr_default_params(mpr_params* h_out);
+
+/* Bytes of device workspace mpr_create needs for `batch` grids of rows x cols
+ * (worst case: every site a prediction site).  MPR_ERR_ARG on bad sizes. */
+mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* h_bytes);
+
+/* Problem statement: grid, sample set, sample values.
+ * Computes z_min / z_max over SAMPLE sites (L81), the data->angle transform
+ * of Eq. 1 (L79) at sample sites, the fixed-site bitmask and the
+ * checkerboard-split (L261) lists of prediction sites.
+ *   d_values      device float [batch][rows][cols]; values at mask==0 sites are ignored (may be NaN)
+ *   d_sample_mask device uint8 [batch][rows][cols]; nonzero = sample (fixed), 0 = prediction site
+ *   d_workspace   device, >= mpr_query_workspace bytes, 256-byte aligned; must outlive the context
+ *   cuda_stream   a cudaStream_t (0 = default stream); all later work runs on it
+ * The inputs are consumed before the call returns (it synchronises).
+ * Errors: ARG, WORKSPACE, NO_SAMPLES, NO_FREE, DEGENERATE_RANGE, NONFINITE, CUDA. */
+mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols,
+                      const float* d_values, const uint8_t* d_sample_mask,
+                      void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Alg. 2 steps 1-2 (L165-180): stores the parameters and the per-grid
+ * temperatures (h_T host float [batch], T > 0 finite), draws the initial state
+ * U(0, 2 pi) at the prediction sites from the INIT stream, resets i = 0,
+ * a = 1, k = -1, t = 0 and the realization accumulator.  May be called again
+ * to restart.  Errors: ARG, UNSUPPORTED, CUDA. */
+mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* h_params, const float* h_T);
+
+/* Alg. 2 step 5 (L192-206): per grid, sweep until the fitted energy slope
+ * k >= 0 or equil_cap sweeps; adapts a by step 5.2.  Synchronises. */
+mpr_status mpr_equilibrate(mpr_ctx* ctx);
+
+/* Alg. 2 step 6 (L207-211): M x {sweeps_per_real sweeps; accumulate the state
+ * at prediction sites}.  Asynchronous. */
+mpr_status mpr_simulate(mpr_ctx* ctx);
+
+/* Alg. 2 step 7 + back-transform (L148, L210-212): d_out device float
+ * [batch][rows][cols]; prediction sites = z_min + mean(phi) (z_max - z_min)/(2 pi)
+ * over the realizations accumulated so far (>= 1), sample sites = the input
+ * value bit for bit.  Asynchronous. */
+mpr_status mpr_predict(mpr_ctx* ctx, float* d_out);
+
+mpr_status mpr_destroy(mpr_ctx* ctx);
+
+/* ---- diagnostic / test / checkpoint surface ---- */
+
+/* Current angles phi in [0, 2 pi], device float [batch][rows][cols]. Sample
+ * sites return Eq. 1 bit-exactly. Asynchronous. */
+mpr_status mpr_get_angles(mpr_ctx* ctx, float* d_phi);
+/* Overwrite the angles of the PREDICTION sites from d_phi (same shape);
+ * sample sites are ignored. Asynchronous. */
+mpr_status mpr_set_angles(mpr_ctx* ctx, const float* d_phi);
+/* Set / get the global sweep index t of every grid (with get/set_angles this
+ * is a complete checkpoint: the RNG is counter-based). */
+mpr_status mpr_set_sweep_index(mpr_ctx* ctx, uint32_t t);
+/* n_sweeps raw UPDATE sweeps (Alg. 1) at fixed a >= 1 on every grid; t
+ * advances by n_sweeps. h_accepted (host uint64 [batch], may be NULL) receives
+ * the accepted Metropolis proposals summed over these sweeps (synchronises
+ * when non-NULL). */
+mpr_status mpr_sweep(mpr_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_accepted);
+/* Energy per bond e = H / N_GP of Eq. 2 (L87, L109, L199), host double [batch]. Synchronises. */
+mpr_status mpr_energy(mpr_ctx* ctx, double* h_e_per_bond);
+/* z_min, z_max of Eq. 1 per grid, host float [batch]. */
+mpr_status mpr_get_transform(mpr_ctx* ctx, float* h_zmin, float* h_zmax);
+/* Fixed-site bitmask as built by mpr_create: device uint32 [batch][ceil(rows*cols/32)],
+ * bit (n & 31) of word (n >> 5) = 1 for a sample site n = row*cols + col. Asynchronous. */
+mpr_status mpr_get_mask_bits(mpr_ctx* ctx, uint32_t* d_bits);
+/* Per-grid statistics, host mpr_stats [batch]. Synchronises. */
+mpr_status mpr_get_stats(mpr_ctx* ctx, mpr_stats* h_out);
+/* Number of kernels this context has launched so far (bench bookkeeping). */
+mpr_status mpr_get_launch_count(mpr_ctx* ctx, uint64_t* h_count);
+
+const char* mpr_status_string(mpr_status s);
+/* Text of the last CUDA error seen by this library in the calling process. */
+const char* mpr_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPR_H */

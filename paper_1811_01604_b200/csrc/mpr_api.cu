@@ -1,0 +1,473 @@
+// mpr_api.cu -- host controller and C ABI (include/mpr.h) of the MPR hot path.
+// Everything on the path runs in the kernels of mpr_device.cuh; this file
+// validates arguments, lays out the caller's workspace and enqueues launches.
+#include "mpr_device.cuh"
+#include "../../include/mpr.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace mpr;
+
+namespace {
+
+thread_local char g_cuda_err[256] = "";
+
+inline bool cuda_ok(cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return true;
+    snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", what, cudaGetErrorString(e));
+    return false;
+}
+#define CU(call) do { if (!cuda_ok((call), #call)) return MPR_ERR_CUDA; } while (0)
+// this library links its own (static) CUDA runtime, whose current device is not torch's
+#define ENTER(ctx) do { if (!cuda_ok(cudaSetDevice((ctx)->device), "cudaSetDevice")) return MPR_ERR_CUDA; } while (0)
+#define CU_LAUNCH() do { ++ctx->launches; if (!cuda_ok(cudaGetLastError(), "kernel launch")) return MPR_ERR_CUDA; } while (0)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
+
+struct Geometry {
+    uint32_t N, words, W, Wp, VS, LC;
+};
+
+bool make_geometry(int batch, int rows, int cols, Geometry* g)
+{
+    if (batch < 1 || batch > 65535 || rows < 2 || cols < 2 || rows > 65534 || cols > 65534) return false;
+    const uint64_t N = (uint64_t)rows * (uint64_t)cols;
+    const uint64_t W = ((uint64_t)cols + 1) / 2, Wp = (W + 2 + 1) & ~1ull;   // even pitch
+    const uint64_t VS = ((uint64_t)rows + 2) * Wp;
+    if (N >= (1ull << 31) || VS >= (1ull << 31)) return false;
+    g->N = (uint32_t)N; g->words = (uint32_t)((N + 31) / 32);
+    g->W = (uint32_t)W; g->Wp = (uint32_t)Wp; g->VS = (uint32_t)VS;
+    g->LC = (uint32_t)((((N + 1) / 2 + 1) & ~1ull) + 2);                       // even, >= max count + 2
+    return true;
+}
+
+struct Layout {
+    size_t states, done, partials, values, phi, bits, vec, lists, acc, rowstart, total;
+};
+
+Layout make_layout(int batch, int rows, const Geometry& g)
+{
+    Layout L;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    const size_t B = (size_t)batch;
+    L.states   = take(B * sizeof(GridState));
+    L.done     = take(B * sizeof(uint32_t));
+    L.partials = take(B * ENERGY_BLOCKS * sizeof(double));
+    L.values   = take(B * g.N * sizeof(float));
+    L.phi      = take(B * g.N * sizeof(float));
+    L.bits     = take(B * g.words * sizeof(uint32_t));
+    L.vec      = take(B * 2 * g.VS * sizeof(float2));
+    L.lists    = take(B * 2 * g.LC * sizeof(uint32_t));
+    L.acc      = take(B * 2 * g.LC * sizeof(float));
+    L.rowstart = take(B * 2 * ((size_t)rows + 1) * sizeof(uint32_t));
+    L.total = o;
+    return L;
+}
+
+enum RunState { CREATED = 0, READY = 1 };
+
+}  // namespace
+
+struct mpr_ctx {
+    Dev          d;
+    Layout       lay;
+    cudaStream_t stream;
+    mpr_params   prm;
+    RunState     state;
+    uint32_t     max_free[2];     // max over grids of the free count per colour
+    int          energy_blocks;
+    uint64_t     launches;
+    uint32_t*    h_pinned;        // [batch] pinned host, done flags
+    GridState*   h_states;        // [batch] pageable host copy
+    bool         qhalf;
+    bool         dirty;           // vectors changed since d.phi was last written at the free sites
+    int          device;          // device the workspace lives on
+};
+
+namespace {
+
+mpr_status fetch_states(mpr_ctx* ctx)
+{
+    CU(cudaMemcpyAsync(ctx->h_states, ctx->d.states, sizeof(GridState) * ctx->d.batch, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MPR_OK;
+}
+
+template <bool COUNT, bool CHECK_DONE>
+mpr_status launch_halfsweep(mpr_ctx* ctx, int colour, uint32_t t_off)
+{
+    const unsigned pairs = (ctx->max_free[colour] + 1) / 2;
+    if (pairs == 0) return MPR_OK;
+    ctx->dirty = true;
+    const dim3 grid(cdiv(pairs, SWEEP_THREADS), ctx->d.batch);
+    const int orm = (int)ctx->prm.or_mode;
+#define MPR_HS(QH, OM) k_halfsweep<QH, OM, COUNT, CHECK_DONE><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(ctx->d, colour, t_off)
+    if (ctx->qhalf) { if (orm == 0) MPR_HS(true, 0); else if (orm == 1) MPR_HS(true, 1); else MPR_HS(true, 2); }
+    else            { if (orm == 0) MPR_HS(false, 0); else MPR_HS(false, 2); }
+#undef MPR_HS
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+// one UPDATE sweep (Alg. 1): colour 0 (contains the upper-left node, Fig. 1) then colour 1
+template <bool COUNT, bool CHECK_DONE>
+mpr_status launch_sweep(mpr_ctx* ctx, uint32_t t_off)
+{
+    mpr_status s = launch_halfsweep<COUNT, CHECK_DONE>(ctx, 0, t_off);
+    if (s != MPR_OK) return s;
+    return launch_halfsweep<COUNT, CHECK_DONE>(ctx, 1, t_off);
+}
+
+mpr_status launch_energy(mpr_ctx* ctx, bool check_done)
+{
+    k_energy<<<dim3(ctx->energy_blocks, ctx->d.batch), ENERGY_THREADS, 0, ctx->stream>>>(ctx->d, check_done);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+dim3 list_grid(const mpr_ctx* ctx)
+{
+    const uint32_t m = ctx->max_free[0] > ctx->max_free[1] ? ctx->max_free[0] : ctx->max_free[1];
+    return dim3(cdiv(m ? m : 1, 256), ctx->d.batch, 2);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mpr_status_string(mpr_status s)
+{
+    switch (s) {
+    case MPR_OK: return "ok";
+    case MPR_ERR_ARG: return "bad argument";
+    case MPR_ERR_NO_SAMPLES: return "a grid has no sample site";
+    case MPR_ERR_NO_FREE: return "a grid has no prediction site";
+    case MPR_ERR_DEGENERATE_RANGE: return "sample values have zero range (Eq. 1 divides by zero)";
+    case MPR_ERR_NONFINITE: return "a sample value is not finite";
+    case MPR_ERR_STATE: return "call out of order";
+    case MPR_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case MPR_ERR_CUDA: return "CUDA error";
+    case MPR_ERR_UNSUPPORTED: return "parameter combination not supported";
+    }
+    return "unknown status";
+}
+
+const char* mpr_last_cuda_error(void) { return g_cuda_err; }
+
+void mpr_default_params(mpr_params* p)
+{
+    if (!p) return;
+    memset(p, 0, sizeof *p);
+    p->struct_size = (uint32_t)sizeof(mpr_params);
+    p->q = 0.5f; p->equil_cap = 500; p->sweeps_per_real = 1; p->M = 100;
+    p->n_f = 5; p->n_fit = 20; p->A_targ = 0.3f; p->k_a = 3.0f;
+    p->or_mode = 0; p->a_eq_mode = 0; p->seed = 0;
+}
+
+mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* bytes)
+{
+    Geometry g;
+    if (!bytes || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
+    *bytes = make_layout(batch, rows, g).total;
+    return MPR_OK;
+}
+
+mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float* d_values,
+                      const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    Geometry g;
+    if (!out || !d_values || !d_sample_mask || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
+    const Layout lay = make_layout(batch, rows, g);
+    if (!d_workspace || workspace_bytes < lay.total || ((uintptr_t)d_workspace & 255u)) return MPR_ERR_WORKSPACE;
+
+    mpr_ctx* ctx = new (std::nothrow) mpr_ctx();
+    if (!ctx) return MPR_ERR_ARG;
+    memset(ctx, 0, sizeof *ctx);
+    ctx->lay = lay;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    {
+        cudaPointerAttributes attr;
+        if (!cuda_ok(cudaPointerGetAttributes(&attr, d_workspace), "cudaPointerGetAttributes") ||
+            attr.type != cudaMemoryTypeDevice) { delete ctx; return MPR_ERR_WORKSPACE; }
+        ctx->device = attr.device;
+        if (!cuda_ok(cudaSetDevice(ctx->device), "cudaSetDevice")) { delete ctx; return MPR_ERR_CUDA; }
+    }
+    ctx->state = CREATED;
+    char* base = (char*)d_workspace;
+    Dev& d = ctx->d;
+    d.states = (GridState*)(base + lay.states);
+    d.done_flags = (uint32_t*)(base + lay.done);
+    d.e_partials = (double*)(base + lay.partials);
+    d.values = (float*)(base + lay.values);
+    d.phi = (float*)(base + lay.phi);
+    d.bits = (uint32_t*)(base + lay.bits);
+    d.vec = (float2*)(base + lay.vec);
+    d.lists = (uint32_t*)(base + lay.lists);
+    d.acc = (float*)(base + lay.acc);
+    d.rowstart = (uint32_t*)(base + lay.rowstart);
+    d.batch = batch; d.rows = rows; d.cols = cols;
+    d.N = g.N; d.words = g.words; d.W = g.W; d.Wp = g.Wp; d.VS = g.VS; d.LC = g.LC;
+    d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
+    ctx->energy_blocks = rows < ENERGY_BLOCKS ? rows : ENERGY_BLOCKS;
+    ctx->h_states = new (std::nothrow) GridState[batch];
+    mpr_status st = MPR_OK;
+    auto fail = [&](mpr_status s) { mpr_destroy(ctx); return s; };
+    if (!ctx->h_states) return fail(MPR_ERR_ARG);
+    if (!cuda_ok(cudaMallocHost((void**)&ctx->h_pinned, sizeof(uint32_t) * batch), "cudaMallocHost")) return fail(MPR_ERR_CUDA);
+
+    cudaStream_t s = ctx->stream;
+    // zero pads of the vector arrays = open boundary
+    if (!cuda_ok(cudaMemsetAsync(d.vec, 0, (size_t)batch * 2 * g.VS * sizeof(float2), s), "memset vec")) return fail(MPR_ERR_CUDA);
+    k_state_reset<<<cdiv(batch, 128), 128, 0, s>>>(d);
+    unsigned mm_blocks = cdiv(g.N, 256 * 8);
+    if (mm_blocks > 1184) mm_blocks = 1184;
+    k_minmax<<<dim3(mm_blocks, batch), 256, 0, s>>>(d, d_values, d_sample_mask);
+    k_minmax_finish<<<cdiv(batch, 128), 128, 0, s>>>(d);
+    k_transform<<<dim3(cdiv((size_t)g.words * 32, 256), batch), 256, 0, s>>>(d, d_values, d_sample_mask);
+    k_rowcount<<<dim3(cdiv((size_t)rows * 32, 256), batch), 256, 0, s>>>(d);
+    k_rowscan<<<dim3(batch, 2), 32, 0, s>>>(d);
+    k_build_lists<<<dim3(cdiv((size_t)rows * 32, 256), batch), 256, 0, s>>>(d);
+    ctx->launches += 7;
+    if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
+    st = fetch_states(ctx);
+    if (st != MPR_OK) return fail(st);
+    for (int b = 0; b < batch; ++b) {
+        const uint32_t e = ctx->h_states[b].err_flags;
+        if (e & ERRF_NO_SAMPLES) return fail(MPR_ERR_NO_SAMPLES);
+        if (e & ERRF_NONFINITE) return fail(MPR_ERR_NONFINITE);
+        if (e & ERRF_DEGENERATE) return fail(MPR_ERR_DEGENERATE_RANGE);
+        if (e & ERRF_NO_FREE) return fail(MPR_ERR_NO_FREE);
+        for (int c = 0; c < 2; ++c)
+            if (ctx->h_states[b].n_free[c] > ctx->max_free[c]) ctx->max_free[c] = ctx->h_states[b].n_free[c];
+    }
+    *out = ctx;
+    return MPR_OK;
+}
+
+mpr_status mpr_destroy(mpr_ctx* ctx)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    delete[] ctx->h_states;
+    delete ctx;
+    return MPR_OK;
+}
+
+mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
+{
+    if (!ctx || !p || !h_T || p->struct_size != sizeof(mpr_params)) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (!(p->q > 0.0f && p->q <= 0.5f) || p->M < 1 || p->sweeps_per_real < 1 || p->n_f < 1 ||
+        p->n_fit < 2 || p->n_fit > (uint32_t)MAX_NFIT || !(p->k_a > 0.0f) || !std::isfinite(p->A_targ) ||
+        p->or_mode > 2 || p->a_eq_mode > 1)
+        return MPR_ERR_ARG;
+    for (int b = 0; b < ctx->d.batch; ++b)
+        if (!(h_T[b] > 0.0f) || !std::isfinite(h_T[b])) return MPR_ERR_ARG;
+    if (p->or_mode == 1 && p->q != 0.5f) return MPR_ERR_UNSUPPORTED;
+    ctx->prm = *p;
+    ctx->qhalf = p->q == 0.5f;
+    Dev& d = ctx->d;
+    d.key0 = (uint32_t)p->seed; d.key1 = (uint32_t)(p->seed >> 32);
+    d.q = p->q; d.inv_q = 1.0f / p->q;
+    d.bc = (float)cos((double)p->q * (double)TWO_PI_F); d.bs = (float)sin((double)p->q * (double)TWO_PI_F);
+    d.n_f = p->n_f; d.n_fit = p->n_fit; d.equil_cap = p->equil_cap;
+    d.A_targ = (double)p->A_targ; d.k_a = (double)p->k_a;
+    // per-grid temperatures: staged through the (currently unused) accumulator
+    CU(cudaMemcpyAsync(d.acc, h_T, sizeof(float) * d.batch, cudaMemcpyHostToDevice, ctx->stream));
+    k_begin_run<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, d.acc);
+    CU_LAUNCH();
+    k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d);
+    CU_LAUNCH();
+    CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
+    ctx->state = READY;
+    ctx->dirty = false;
+    return MPR_OK;
+}
+
+mpr_status mpr_equilibrate(mpr_ctx* ctx)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const Dev& d = ctx->d;
+    const uint32_t cap = ctx->prm.equil_cap;
+    uint32_t issued = 0;
+    // the first slope check happens at i = n_fit, then every n_f sweeps (Alg. 2 step 5.4)
+    uint32_t chunk = ctx->prm.n_fit + 1;
+    while (issued < cap) {
+        if (chunk > cap - issued) chunk = cap - issued;
+        for (uint32_t j = 0; j < chunk; ++j) {
+            mpr_status s = launch_sweep<true, true>(ctx, 0);          // 5.1 (t advanced by the controller)
+            if (s != MPR_OK) return s;
+            s = launch_energy(ctx, true);                              // 5.3
+            if (s != MPR_OK) return s;
+            k_controller<<<d.batch, 32, 0, ctx->stream>>>(d, ctx->energy_blocks);   // 5.2, 5.4, 5.5
+            CU_LAUNCH();
+        }
+        issued += chunk;
+        CU(cudaMemcpyAsync(ctx->h_pinned, d.done_flags, sizeof(uint32_t) * d.batch, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        bool all = true;
+        for (int b = 0; b < d.batch; ++b) all = all && ctx->h_pinned[b];
+        if (all) break;
+        chunk = ctx->prm.n_f;
+    }
+    return MPR_OK;
+}
+
+mpr_status mpr_simulate(mpr_ctx* ctx)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const Dev& d = ctx->d;
+    const uint32_t s_per = ctx->prm.sweeps_per_real;
+    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, ctx->prm.a_eq_mode == 1 ? 0 : 1, 1.0);
+    CU_LAUNCH();
+    for (uint32_t j = 0; j < ctx->prm.M; ++j) {
+        for (uint32_t w = 0; w < s_per; ++w) {
+            mpr_status s = launch_sweep<false, false>(ctx, w);
+            if (s != MPR_OK) return s;
+        }
+        k_accumulate<<<list_grid(ctx), 256, 0, ctx->stream>>>(d, s_per, j == 0);
+        CU_LAUNCH();
+    }
+    return MPR_OK;
+}
+
+mpr_status mpr_predict(mpr_ctx* ctx, float* d_out)
+{
+    if (!ctx || !d_out) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const Dev& d = ctx->d;
+    CU(cudaMemcpyAsync(d_out, d.values, sizeof(float) * (size_t)d.N * d.batch, cudaMemcpyDeviceToDevice, ctx->stream));
+    k_predict<<<list_grid(ctx), 256, 0, ctx->stream>>>(d, d_out);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr_get_angles(mpr_ctx* ctx, float* d_phi)
+{
+    if (!ctx || !d_phi) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const Dev& d = ctx->d;
+    if (ctx->dirty) {        // otherwise d.phi already holds the state exactly (initial draw or import)
+        k_export_angles<<<list_grid(ctx), 256, 0, ctx->stream>>>(d);
+        CU_LAUNCH();
+        ctx->dirty = false;
+    }
+    CU(cudaMemcpyAsync(d_phi, d.phi, sizeof(float) * (size_t)d.N * d.batch, cudaMemcpyDeviceToDevice, ctx->stream));
+    return MPR_OK;
+}
+
+mpr_status mpr_set_angles(mpr_ctx* ctx, const float* d_phi)
+{
+    if (!ctx || !d_phi) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    k_import_angles<<<list_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, d_phi);
+    CU_LAUNCH();
+    ctx->dirty = false;
+    return MPR_OK;
+}
+
+mpr_status mpr_set_sweep_index(mpr_ctx* ctx, uint32_t t)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    k_advance_t<<<cdiv(ctx->d.batch, 128), 128, 0, ctx->stream>>>(ctx->d, t, 1, 0);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr_sweep(mpr_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_accepted)
+{
+    if (!ctx || !(a >= 1.0) || !std::isfinite(a)) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const Dev& d = ctx->d;
+    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, a);
+    CU_LAUNCH();
+    k_advance_t<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, 0, 1);   // zero the accepted counters
+    CU_LAUNCH();
+    for (uint32_t w = 0; w < n_sweeps; ++w) {
+        mpr_status s = h_accepted ? launch_sweep<true, false>(ctx, w) : launch_sweep<false, false>(ctx, w);
+        if (s != MPR_OK) return s;
+    }
+    k_advance_t<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, n_sweeps, 0, 0);
+    CU_LAUNCH();
+    if (h_accepted) {
+        mpr_status s = fetch_states(ctx);
+        if (s != MPR_OK) return s;
+        for (int b = 0; b < d.batch; ++b) h_accepted[b] = ctx->h_states[b].accepted;
+    }
+    return MPR_OK;
+}
+
+mpr_status mpr_energy(mpr_ctx* ctx, double* h_e)
+{
+    if (!ctx || !h_e) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr_status s = launch_energy(ctx, false);
+    if (s != MPR_OK) return s;
+    k_energy_query<<<ctx->d.batch, 32, 0, ctx->stream>>>(ctx->d, ctx->energy_blocks);
+    CU_LAUNCH();
+    s = fetch_states(ctx);
+    if (s != MPR_OK) return s;
+    for (int b = 0; b < ctx->d.batch; ++b) h_e[b] = ctx->h_states[b].e_query;
+    return MPR_OK;
+}
+
+mpr_status mpr_get_transform(mpr_ctx* ctx, float* h_zmin, float* h_zmax)
+{
+    if (!ctx || !h_zmin || !h_zmax) return MPR_ERR_ARG;
+    for (int b = 0; b < ctx->d.batch; ++b) { h_zmin[b] = ctx->h_states[b].zmin; h_zmax[b] = ctx->h_states[b].zmax; }
+    return MPR_OK;      // z_min / z_max never change after mpr_create, which fetched them
+}
+
+mpr_status mpr_get_mask_bits(mpr_ctx* ctx, uint32_t* d_bits)
+{
+    if (!ctx || !d_bits) return MPR_ERR_ARG;
+    ENTER(ctx);
+    CU(cudaMemcpyAsync(d_bits, ctx->d.bits, sizeof(uint32_t) * (size_t)ctx->d.words * ctx->d.batch,
+                       cudaMemcpyDeviceToDevice, ctx->stream));
+    return MPR_OK;
+}
+
+mpr_status mpr_get_stats(mpr_ctx* ctx, mpr_stats* h_out)
+{
+    if (!ctx || !h_out) return MPR_ERR_ARG;
+    ENTER(ctx);
+    mpr_status s = fetch_states(ctx);
+    if (s != MPR_OK) return s;
+    for (int b = 0; b < ctx->d.batch; ++b) {
+        const GridState& g = ctx->h_states[b];
+        mpr_stats& o = h_out[b];
+        o.equil_sweeps = g.i; o.t = g.t; o.equilibrated = g.done; o.realizations = g.realizations;
+        o.n_free = (uint64_t)g.n_free[0] + g.n_free[1];
+        o.n_samples = g.n_samples;
+        o.n_bonds = (uint64_t)ctx->d.n_bonds;
+        o.a = g.a; o.k = g.k; o.A_last = g.A_last; o.e_last = g.e_last;
+        o.z_min = g.zmin; o.z_max = g.zmax;
+    }
+    return MPR_OK;
+}
+
+mpr_status mpr_get_launch_count(mpr_ctx* ctx, uint64_t* h_count)
+{
+    if (!ctx || !h_count) return MPR_ERR_ARG;
+    *h_count = ctx->launches;
+    return MPR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,276 @@
+"""Thin Python binding of the C-ABI library (include/mpr.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels
+behind `libmpr_b200.so`.  PyTorch supplies device memory (tensors) and the
+stream; nothing here computes.  There is NO CPU fallback: loading fails
+loudly if the library has not been built (`python -m paper_1811_01604_b200.build`),
+and every call raises `MprError` on a non-zero status.
+
+Function names mirror the C entry points: mpr_create, mpr_set_params,
+mpr_equilibrate, mpr_simulate, mpr_predict, ... ; the `Mpr` class bundles a
+context with the tensors it must keep alive.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmpr_b200.so")
+
+STATUS_NAMES = {
+    0: "MPR_OK", 1: "MPR_ERR_ARG", 2: "MPR_ERR_NO_SAMPLES", 3: "MPR_ERR_NO_FREE",
+    4: "MPR_ERR_DEGENERATE_RANGE", 5: "MPR_ERR_NONFINITE", 6: "MPR_ERR_STATE",
+    7: "MPR_ERR_WORKSPACE", 8: "MPR_ERR_CUDA", 9: "MPR_ERR_UNSUPPORTED",
+}
+
+# every symbol include/mpr.h declares
+EXPORTS = (
+    "mpr_default_params", "mpr_query_workspace", "mpr_create", "mpr_set_params", "mpr_equilibrate",
+    "mpr_simulate", "mpr_predict", "mpr_destroy", "mpr_get_angles", "mpr_set_angles",
+    "mpr_set_sweep_index", "mpr_sweep", "mpr_energy", "mpr_get_transform", "mpr_get_mask_bits",
+    "mpr_get_stats", "mpr_get_launch_count", "mpr_status_string", "mpr_last_cuda_error",
+)
+
+
+class MprError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        self.name = STATUS_NAMES.get(status, str(status))
+        super().__init__(f"{where}: {self.name}" + (f" ({detail})" if detail else ""))
+
+
+class mpr_params(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("q", C.c_float), ("equil_cap", C.c_uint32),
+        ("sweeps_per_real", C.c_uint32), ("M", C.c_uint32), ("n_f", C.c_uint32), ("n_fit", C.c_uint32),
+        ("A_targ", C.c_float), ("k_a", C.c_float), ("or_mode", C.c_uint32), ("a_eq_mode", C.c_uint32),
+        ("seed", C.c_uint64),
+    ]
+
+
+class mpr_stats(C.Structure):
+    _fields_ = [
+        ("equil_sweeps", C.c_uint32), ("t", C.c_uint32), ("equilibrated", C.c_uint32),
+        ("realizations", C.c_uint32), ("n_free", C.c_uint64), ("n_samples", C.c_uint64),
+        ("n_bonds", C.c_uint64), ("a", C.c_double), ("k", C.c_double), ("A_last", C.c_double),
+        ("e_last", C.c_double), ("z_min", C.c_float), ("z_max", C.c_float),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1811_01604_b200.build` "
+                "(the MPR path has no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i, u32, u64, sz = C.c_void_p, C.c_int, C.c_uint32, C.c_uint64, C.c_size_t
+        L.mpr_default_params.argtypes = [C.POINTER(mpr_params)]; L.mpr_default_params.restype = None
+        L.mpr_query_workspace.argtypes = [i, i, i, C.POINTER(sz)]
+        L.mpr_create.argtypes = [C.POINTER(vp), i, i, i, vp, vp, vp, sz, vp]
+        L.mpr_set_params.argtypes = [vp, C.POINTER(mpr_params), C.POINTER(C.c_float)]
+        L.mpr_equilibrate.argtypes = [vp]
+        L.mpr_simulate.argtypes = [vp]
+        L.mpr_predict.argtypes = [vp, vp]
+        L.mpr_destroy.argtypes = [vp]
+        L.mpr_get_angles.argtypes = [vp, vp]
+        L.mpr_set_angles.argtypes = [vp, vp]
+        L.mpr_set_sweep_index.argtypes = [vp, u32]
+        L.mpr_sweep.argtypes = [vp, u32, C.c_double, C.POINTER(u64)]
+        L.mpr_energy.argtypes = [vp, C.POINTER(C.c_double)]
+        L.mpr_get_transform.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.mpr_get_mask_bits.argtypes = [vp, vp]
+        L.mpr_get_stats.argtypes = [vp, C.POINTER(mpr_stats)]
+        L.mpr_get_launch_count.argtypes = [vp, C.POINTER(u64)]
+        for name in EXPORTS:
+            getattr(L, name).restype = C.c_int
+        L.mpr_default_params.restype = None
+        L.mpr_status_string.argtypes = [i]; L.mpr_status_string.restype = C.c_char_p
+        L.mpr_last_cuda_error.argtypes = []; L.mpr_last_cuda_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        detail = lib().mpr_last_cuda_error().decode() if status == 8 else lib().mpr_status_string(status).decode()
+        raise MprError(status, where, detail)
+
+
+def default_params(**overrides) -> mpr_params:
+    p = mpr_params()
+    lib().mpr_default_params(C.byref(p))
+    for k, v in overrides.items():
+        if not hasattr(p, k):
+            raise AttributeError(k)
+        setattr(p, k, v)
+    return p
+
+
+def mpr_query_workspace(batch: int, rows: int, cols: int) -> int:
+    n = C.c_size_t()
+    _check(lib().mpr_query_workspace(batch, rows, cols, C.byref(n)), "mpr_query_workspace")
+    return int(n.value)
+
+
+@dataclass
+class Stats:
+    equil_sweeps: int
+    t: int
+    equilibrated: bool
+    realizations: int
+    n_free: int
+    n_samples: int
+    n_bonds: int
+    a: float
+    k: float
+    A_last: float
+    e_last: float
+    z_min: float
+    z_max: float
+
+
+class Mpr:
+    """One context = `batch` grids of rows x cols on one GPU.
+
+    values: float32 CUDA tensor [batch, rows, cols] (or [rows, cols]);
+    sample_mask: uint8 CUDA tensor of the same shape, 1 = sample (fixed).
+    """
+
+    def __init__(self, values, sample_mask, stream=None):
+        import torch
+        if not values.is_cuda or not sample_mask.is_cuda:
+            raise ValueError("values and sample_mask must be CUDA tensors (there is no CPU path)")
+        if values.dim() == 2:
+            values, sample_mask = values[None], sample_mask[None]
+        if values.dtype != torch.float32 or sample_mask.dtype != torch.uint8 or values.shape != sample_mask.shape:
+            raise ValueError("values float32 and sample_mask uint8 of the same [batch, rows, cols] shape")
+        values, sample_mask = values.contiguous(), sample_mask.contiguous()
+        self.device = values.device
+        self.batch, self.rows, self.cols = (int(x) for x in values.shape)
+        self._torch = torch
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        nbytes = mpr_query_workspace(self.batch, self.rows, self.cols)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        assert self.workspace.data_ptr() % 256 == 0
+        self._ctx = C.c_void_p()
+        _check(lib().mpr_create(C.byref(self._ctx), self.batch, self.rows, self.cols,
+                                values.data_ptr(), sample_mask.data_ptr(),
+                                self.workspace.data_ptr(), nbytes, self._stream.cuda_stream), "mpr_create")
+        self.params = None
+
+    # -- lifecycle ---------------------------------------------------------
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self._stream.synchronize()
+            lib().mpr_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the path ----------------------------------------------------------
+    def set_params(self, T, params: mpr_params | None = None, **overrides):
+        p = params if params is not None else default_params(**overrides)
+        if params is not None:
+            for k, v in overrides.items():
+                setattr(p, k, v)
+        Ts = [float(T)] * self.batch if not hasattr(T, "__len__") else [float(x) for x in T]
+        if len(Ts) != self.batch:
+            raise ValueError("one temperature per grid")
+        arr = (C.c_float * self.batch)(*Ts)
+        _check(lib().mpr_set_params(self._ctx, C.byref(p), arr), "mpr_set_params")
+        self.params = p
+        return self
+
+    def equilibrate(self):
+        _check(lib().mpr_equilibrate(self._ctx), "mpr_equilibrate")
+        return self
+
+    def simulate(self):
+        _check(lib().mpr_simulate(self._ctx), "mpr_simulate")
+        return self
+
+    def predict(self, out=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty((self.batch, self.rows, self.cols), dtype=torch.float32, device=self.device)
+        _check(lib().mpr_predict(self._ctx, out.data_ptr()), "mpr_predict")
+        return out
+
+    # -- diagnostics -------------------------------------------------------
+    def get_angles(self, out=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty((self.batch, self.rows, self.cols), dtype=torch.float32, device=self.device)
+        _check(lib().mpr_get_angles(self._ctx, out.data_ptr()), "mpr_get_angles")
+        return out
+
+    def set_angles(self, phi):
+        phi = phi.to(device=self.device, dtype=self._torch.float32).reshape(self.batch, self.rows, self.cols).contiguous()
+        _check(lib().mpr_set_angles(self._ctx, phi.data_ptr()), "mpr_set_angles")
+        self._stream.synchronize()          # phi may be a temporary
+        return self
+
+    def set_sweep_index(self, t: int):
+        _check(lib().mpr_set_sweep_index(self._ctx, int(t)), "mpr_set_sweep_index")
+        return self
+
+    def sweep(self, n_sweeps: int, a: float, count: bool = False):
+        if count:
+            acc = (C.c_uint64 * self.batch)()
+            _check(lib().mpr_sweep(self._ctx, int(n_sweeps), float(a), acc), "mpr_sweep")
+            return [int(x) for x in acc]
+        _check(lib().mpr_sweep(self._ctx, int(n_sweeps), float(a), None), "mpr_sweep")
+        return None
+
+    def energy(self):
+        e = (C.c_double * self.batch)()
+        _check(lib().mpr_energy(self._ctx, e), "mpr_energy")
+        return [float(x) for x in e]
+
+    def get_transform(self):
+        lo, hi = (C.c_float * self.batch)(), (C.c_float * self.batch)()
+        _check(lib().mpr_get_transform(self._ctx, lo, hi), "mpr_get_transform")
+        return [float(x) for x in lo], [float(x) for x in hi]
+
+    def get_mask_bits(self):
+        torch = self._torch
+        words = (self.rows * self.cols + 31) // 32
+        out = torch.empty((self.batch, words), dtype=torch.int32, device=self.device)
+        _check(lib().mpr_get_mask_bits(self._ctx, out.data_ptr()), "mpr_get_mask_bits")
+        return out
+
+    def get_stats(self):
+        arr = (mpr_stats * self.batch)()
+        _check(lib().mpr_get_stats(self._ctx, arr), "mpr_get_stats")
+        return [Stats(s.equil_sweeps, s.t, bool(s.equilibrated), s.realizations, s.n_free, s.n_samples,
+                      s.n_bonds, s.a, s.k, s.A_last, s.e_last, s.z_min, s.z_max) for s in arr]
+
+    def launch_count(self) -> int:
+        n = C.c_uint64()
+        _check(lib().mpr_get_launch_count(self._ctx, C.byref(n)), "mpr_get_launch_count")
+        return int(n.value)
+
+
+def interpolate(values, sample_mask, T, **params):
+    """The whole path for a batch of grids: create, set_params, equilibrate,
+    simulate, predict.  Returns (prediction tensor, list of Stats)."""
+    m = Mpr(values, sample_mask)
+    try:
+        m.set_params(T, **params).equilibrate().simulate()
+        out = m.predict()
+        stats = m.get_stats()
+    finally:
+        m.close()
+    return out, stats

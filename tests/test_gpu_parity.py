@@ -1,0 +1,402 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle.
+
+Protocol (BASELINE.json north_star):
+  T1  bit-exact: z_min, z_max, Eq. 1 angles at sample sites, the initial draw,
+      the fixed-site bitmask, sample sites after a run.
+  T2  one sweep from an identical oracle-made state: every prediction site
+      within 1e-5 rad, except decision flips (Metropolis accept/reject or an
+      interval-end test decided the other way) which must be near-threshold
+      in the oracle's own margin and number <= 1e-4 of the sites.
+  T2b energy per bond within 2e-6; accepted counts equal up to the flips.
+  T3  full runs: energy per bond, MAE and RMSE against the withheld truth
+      within 1 % (means over seeds where one seed's noise exceeds 1 %).
+Every oracle input is made by the oracle or by the seeded generators; nothing
+the CUDA path computed is fed to the oracle.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1811_01604_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TWO_PI_F = float(np.float32(2.0 * math.pi))
+TOL_RAD = 1e-5            # north_star: per site within 1e-5 rad in fp32
+FLIP_FRACTION = 1e-4      # north_star: near-threshold decisions <= 1e-4 of sites
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("a CUDA device is required for -m gpu tests (no CPU fallback exists)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def mpr(torch_cuda):
+    from paper_1811_01604_b200 import mpr as binding
+    binding.lib()
+    return binding
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _field(rows, cols, ell, p_removed, seed):
+    z = synth.grf(rows, cols, ell, "gaussian", seed)
+    mask = synth.bernoulli_mask(rows, cols, p_removed, seed + 1)
+    # make sure both kinds of site exist on tiny grids
+    mask.flat[0] = 1
+    mask.flat[-1] = 0
+    if mask.sum() < 2:
+        mask.flat[1] = 1
+    return z, mask
+
+
+# ---------------------------------------------------------------------------
+# T1
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("rows,cols,batch", [(64, 64, 1), (37, 53, 3), (2, 2, 1), (2, 9, 2), (9, 2, 1), (129, 1000, 1)])
+def test_t1_transform_mask_and_initial_state_bit_exact(torch_cuda, mpr, orc, rows, cols, batch):
+    torch = torch_cuda
+    zs, ms = [], []
+    for g in range(batch):
+        z, m = _field(rows, cols, 4.0, 0.4, 50 + 7 * g)
+        z = (z * (1.0 + g) + 3.0 * g).astype(np.float32)
+        z[m == 0] = np.nan                                   # values at prediction sites are ignored
+        zs.append(z); ms.append(m)
+    z, m = np.stack(zs), np.stack(ms)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    seed = 0x1234_5678_9ABC_DEF0
+    ctx.set_params([0.05] * batch, seed=seed)
+    lo, hi = ctx.get_transform()
+    phi = ctx.get_angles().cpu().numpy()
+    bits = ctx.get_mask_bits().cpu().numpy().view(np.uint32)
+    st = ctx.get_stats()
+    for g in range(batch):
+        zin = np.where(m[g] == 1, z[g], 0.0).astype(np.float32)
+        ref, zmin, zmax = orc.transform(zin, m[g], seed, g)
+        assert np.float32(lo[g]).view(np.uint32) == zmin.view(np.uint32)
+        assert np.float32(hi[g]).view(np.uint32) == zmax.view(np.uint32)
+        assert np.array_equal(phi[g].view(np.uint32), ref.view(np.uint32))      # Eq. 1 and the INIT stream
+        packed = np.packbits(m[g].ravel().astype(bool), bitorder="little")
+        packed = np.concatenate([packed, np.zeros((-packed.size) % 4, np.uint8)]).view(np.uint32)
+        assert np.array_equal(bits[g], packed)
+        assert st[g].n_samples == int(m[g].sum()) and st[g].n_free == int((m[g] == 0).sum())
+        assert st[g].n_bonds == orc.n_bonds(rows, cols)
+    ctx.close()
+
+
+def test_t1_sample_sites_bit_exact_after_a_run_and_predict_returns_inputs(torch_cuda, mpr, orc):
+    torch = torch_cuda
+    z, m = _field(48, 80, 6.0, 0.5, 11)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(0.02, seed=5, equil_cap=60, M=3, sweeps_per_real=7)
+    before = ctx.get_angles().cpu().numpy()[0]
+    ctx.equilibrate().simulate()
+    after = ctx.get_angles().cpu().numpy()[0]
+    pred = ctx.predict().cpu().numpy()[0]
+    s = m.astype(bool)
+    assert np.array_equal(after[s].view(np.uint32), before[s].view(np.uint32))
+    assert not np.array_equal(after[~s], before[~s])
+    assert after.min() >= 0.0 and after.max() <= np.float32(TWO_PI_F)
+    assert np.array_equal(pred[s].view(np.uint32), z[s].view(np.uint32))
+    zmin, zmax, _ = orc.minmax(z, m)
+    assert pred[~s].min() >= zmin - 1e-6 and pred[~s].max() <= zmax + 1e-6
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------
+# T2 / T2b
+# ---------------------------------------------------------------------------
+def _compare_one_sweep(orc, ctx, phi0, mask, q, T, a, seed, t, or_mode, g_list=(0,)):
+    """phi0 [batch, rows, cols] oracle-made state.  Returns worst-case numbers."""
+    import torch
+    ctx.set_angles(torch.from_numpy(phi0).cuda())
+    ctx.set_sweep_index(t)
+    e_gpu0 = ctx.energy()
+    acc_gpu = ctx.sweep(1, a, count=True)
+    got = ctx.get_angles().cpu().numpy()
+    e_gpu1 = ctx.energy()
+    out = []
+    for g in g_list:
+        ref = phi0[g].copy()
+        e_ref0 = orc.energy_per_bond(ref, q)
+        acc_ref, margin, edge, _ = orc.sweep(ref, mask[g], q, T[g], a, seed, g, t, or_mode, diag=True)
+        e_ref1 = orc.energy_per_bond(ref, q)
+        free = mask[g] == 0
+        d = np.abs(got[g].astype(np.float64) - ref.astype(np.float64))
+        assert np.array_equal(got[g][~free].view(np.uint32), ref[~free].view(np.uint32))
+        bad = free & (d > TOL_RAD)
+        n_bad, P = int(bad.sum()), int(free.sum())
+        # every disagreement must be a near-threshold decision in the oracle's own margins
+        if n_bad:
+            near = (margin[bad] < 1e-3) | (edge[bad] < 1e-4)
+            assert near.all(), (n_bad, margin[bad][~near][:5], edge[bad][~near][:5], d[bad][~near][:5])
+        assert n_bad <= max(1, math.ceil(FLIP_FRACTION * P)), (n_bad, P)
+        assert abs(acc_gpu[g] - acc_ref) <= n_bad
+        assert abs(e_gpu0[g] - e_ref0) < 2e-6 and abs(e_gpu1[g] - e_ref1) < 2e-6 + 8.0 * n_bad / max(1, orc.n_bonds(*ref.shape))
+        out.append((n_bad, P, float(d[free & ~bad].max()) if (free & ~bad).any() else 0.0))
+    return out
+
+
+@pytest.mark.parametrize("name,L", [("cfg1", 64), ("cfg2", 256), ("cfg3", 256), ("cfg4", 512)])
+def test_t2_one_sweep_from_equilibrated_oracle_state(torch_cuda, mpr, orc, name, L):
+    """Equilibrated (low-temperature) states are the hard case for fp32."""
+    torch = torch_cuda
+    w = synth.make_workload(name, L=L)
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    p = orc.Params(seed=w.seed, equil_cap=300)
+    phi, _, _ = orc.transform(z, m, p.seed)
+    st = orc.equilibrate(phi, m, T, p)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=w.seed)
+    for k in range(3):                      # three successive oracle states
+        res = _compare_one_sweep(orc, ctx, phi[None].copy(), m[None], 0.5, [T], st["a"], w.seed, st["t"] + k, 0)
+        orc.sweep(phi, m, 0.5, T, st["a"], w.seed, 0, st["t"] + k)
+        assert res[0][2] <= TOL_RAD
+    ctx.close()
+
+
+@pytest.mark.parametrize("rows,cols", [(2, 2), (2, 7), (7, 2), (3, 3), (37, 53), (64, 129), (255, 64)])
+def test_t2_ragged_and_tiny_grids_hot_start(torch_cuda, mpr, orc, rows, cols):
+    """Random (hot) states, a = 1: wraps, rejected reflections, edges and corners."""
+    torch = torch_cuda
+    z, m = _field(rows, cols, 3.0, 0.6, 300 + rows * 7 + cols)
+    seed, T = 99, 0.3
+    phi, _, _ = orc.transform(z, m, seed)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed)
+    for t in range(4):
+        _compare_one_sweep(orc, ctx, phi[None].copy(), m[None], 0.5, [T], 1.0 + t, seed, t, 0)
+        orc.sweep(phi, m, 0.5, T, 1.0 + t, seed, 0, t)
+    ctx.close()
+
+
+def test_t2_all_sites_free_but_one_and_single_free_site(torch_cuda, mpr, orc):
+    torch = torch_cuda
+    rng = np.random.default_rng(5)
+    z = rng.standard_normal((16, 20)).astype(np.float32)
+    for m in (np.zeros((16, 20), np.uint8), np.ones((16, 20), np.uint8)):
+        m = m.copy()
+        if m[0, 0] == 0:
+            m[3, 4] = 1; m[10, 11] = 1          # two samples fix the range
+        else:
+            m[7, 9] = 0                          # one prediction site
+        phi, _, _ = orc.transform(z, m, 3)
+        ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+        ctx.set_params(0.2, seed=3)
+        _compare_one_sweep(orc, ctx, phi[None].copy(), m[None], 0.5, [0.2], 2.0, 3, 0, 0)
+        ctx.close()
+
+
+@pytest.mark.parametrize("q,or_mode", [(0.5, 2), (0.5, 1), (0.3, 0), (0.3, 2), (0.125, 0)])
+def test_t2_other_q_and_over_relaxation_modes(torch_cuda, mpr, orc, q, or_mode):
+    torch = torch_cuda
+    z, m = _field(96, 70, 5.0, 0.5, 77)
+    seed, T = 21, 0.05
+    phi, _, _ = orc.transform(z, m, seed)
+    p = orc.Params(q=q, seed=seed, equil_cap=40, or_mode=or_mode)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed, q=q, or_mode=or_mode)
+    # hot state, then a partly relaxed one
+    _compare_one_sweep(orc, ctx, phi[None].copy(), m[None], q, [T], 1.0, seed, 0, or_mode)
+    st = orc.equilibrate(phi, m, T, p)
+    _compare_one_sweep(orc, ctx, phi[None].copy(), m[None], q, [T], st["a"], seed, st["t"], or_mode)
+    ctx.close()
+
+
+def test_t2_batch_of_grids_with_own_temperature_and_stream(torch_cuda, mpr, orc):
+    torch = torch_cuda
+    B, L = 4, 96
+    zs, ms, Ts, phis = [], [], [], []
+    seed = 1717
+    for g in range(B):
+        z, m = _field(L, L, 4.0 + 6 * g, 0.66, 900 + g)
+        zs.append(z); ms.append(m); Ts.append(synth.choose_T(z, m))
+        phi, _, _ = orc.transform(z, m, seed, g)
+        p = orc.Params(seed=seed, equil_cap=30)
+        orc.equilibrate(phi, m, Ts[-1], p, g=g)
+        phis.append(phi)
+    z, m, phi = np.stack(zs), np.stack(ms), np.stack(phis)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(Ts, seed=seed)
+    _compare_one_sweep(orc, ctx, phi, m, 0.5, Ts, 7.5, seed, 30, 0, g_list=range(B))
+    ctx.close()
+
+
+def test_t2_full_size_cfg4_shape_one_sweep(torch_cuda, mpr, orc):
+    """BASELINE configs[3] size (4096 x 4096, 33 % removed) in the launch
+    configuration bench.py times.  The state is generator-made: the truth
+    field's own angles plus small noise at the prediction sites stands in for an
+    equilibrated state (the oracle would need minutes to equilibrate one)."""
+    torch = torch_cuda
+    L = 4096
+    z = synth.grf(L, L, 64.0, "gaussian", 1004)
+    m = synth.bernoulli_mask(L, L, 0.33, 2004)
+    T = synth.choose_T(z, m)
+    zmin, zmax, _ = orc.minmax(z, m)
+    rng = np.random.default_rng(8)
+    phi = ((z.astype(np.float64) - zmin) / (float(zmax) - float(zmin)) * TWO_PI_F
+           + math.sqrt(T) * rng.standard_normal(z.shape)).clip(0.0, TWO_PI_F).astype(np.float32)
+    ref0, _, _ = orc.transform(z, m, 3004)
+    phi[m == 1] = ref0[m == 1]
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=3004)
+    res = _compare_one_sweep(orc, ctx, phi[None], m[None], 0.5, [T], 40.0, 3004, 123, 0)
+    assert res[0][2] <= TOL_RAD
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------
+# equilibration controller (Alg. 2 step 5) and T3
+# ---------------------------------------------------------------------------
+def test_equilibration_follows_the_oracle_trajectory(torch_cuda, mpr, orc):
+    """Same Philox streams, same arithmetic up to rounding: the stopping rule
+    fires at the same sweep (or one check later if a decision flipped) and a
+    and e agree."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg2", L=192)
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    p = orc.Params(seed=w.seed, equil_cap=1000)
+    phi, _, _ = orc.transform(z, m, p.seed)
+    st = orc.equilibrate(phi, m, T, p, history=True)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=w.seed, equil_cap=1000).equilibrate()
+    g = ctx.get_stats()[0]
+    assert g.equilibrated and g.t == g.equil_sweeps
+    assert abs(g.equil_sweeps - st["sweeps"]) <= 2 * p.n_f
+    assert g.a == pytest.approx(st["a"], rel=0.15)
+    assert g.e_last == pytest.approx(st["e_hist"][-1], abs=2e-4)
+    assert ctx.energy()[0] == pytest.approx(g.e_last, abs=1e-9)
+    # capped run: exactly cap sweeps, a follows 1 + i/k_a while the acceptance is low
+    ctx.set_params(T, seed=w.seed, equil_cap=7).equilibrate()
+    g = ctx.get_stats()[0]
+    assert g.equil_sweeps == 7 and g.equilibrated
+    ctx.close()
+
+
+def _full_run_scores(orc, mpr, torch, w, seeds, s=None, M=None):
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    s = s or w.sweeps_per_real
+    M = M or w.M
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    rows = []
+    for seed in seeds:
+        ctx.set_params(T, seed=seed, equil_cap=w.equil_cap, sweeps_per_real=s, M=M).equilibrate().simulate()
+        pred = ctx.predict().cpu().numpy()[0]
+        vg = synth.validation_measures(z, pred, m)
+        eg = ctx.energy()[0]
+        res = orc.run(z, m, T, orc.Params(seed=seed, equil_cap=w.equil_cap, sweeps_per_real=s, M=M))
+        vo = synth.validation_measures(z, res["pred"], m)
+        rows.append((vg["mae"], vo["mae"], vg["rmse"], vo["rmse"], eg, res["stats"]["e_final"],
+                     ctx.get_stats()[0].equil_sweeps, res["stats"]["sweeps"]))
+    ctx.close()
+    return np.array(rows)
+
+
+def test_t3_full_run_cfg1_mean_over_seeds(torch_cuda, mpr, orc):
+    """configs[0]: 64 x 64, 33 % removed, cap 1000, M = 10 x 100 sweeps.  One
+    seed's MAE / RMSE noise is ~2 %, so means over 32 seeds are compared."""
+    w = synth.make_workload("cfg1")
+    r = _full_run_scores(orc, mpr, torch_cuda, w, seeds=range(4000, 4032))
+    mae_g, mae_o, rmse_g, rmse_o, e_g, e_o = (r[:, k].mean() for k in range(6))
+    assert mae_g == pytest.approx(mae_o, rel=0.01)
+    assert rmse_g == pytest.approx(rmse_o, rel=0.01)
+    assert e_g == pytest.approx(e_o, rel=0.01)
+    assert (1.0 + e_g) == pytest.approx(1.0 + e_o, rel=0.02)
+    assert r[:, 6].mean() == pytest.approx(r[:, 7].mean(), rel=0.1)
+
+
+def test_t3_full_run_cfg2_shape(torch_cuda, mpr, orc):
+    """configs[1] grid and mask (256 x 256, 66 % removed, M = 100) with 10
+    sweeps per realization so the oracle side stays within seconds."""
+    w = synth.make_workload("cfg2")
+    r = _full_run_scores(orc, mpr, torch_cuda, w, seeds=range(5000, 5003), s=10)
+    mae_g, mae_o, rmse_g, rmse_o, e_g, e_o = (r[:, k].mean() for k in range(6))
+    assert mae_g == pytest.approx(mae_o, rel=0.01)
+    assert rmse_g == pytest.approx(rmse_o, rel=0.01)
+    assert e_g == pytest.approx(e_o, rel=0.01)
+    assert (1.0 + e_g) == pytest.approx(1.0 + e_o, rel=0.01)
+
+
+def test_accumulate_and_predict_against_oracle_back_transform(torch_cuda, mpr, orc):
+    """Step 6-7 alone, deterministic: import an oracle state, accumulate it
+    M times with sweeps that cannot move (over-relaxation off, T so low and a
+    so large that... no: use the API as is) -- here: M = 1, s = 1 and compare
+    the prediction with the oracle's back-transform of the same one sweep."""
+    torch = torch_cuda
+    z, m = _field(40, 56, 5.0, 0.5, 31)
+    z = (50.0 + 10.0 * z).astype(np.float32)
+    seed, T = 8, 0.05
+    phi, zmin, zmax = orc.transform(z, m, seed)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed, M=1, sweeps_per_real=1, equil_cap=0, a_eq_mode=1)
+    ctx.simulate()                                   # one sweep at a = 1, t = 0, then accumulate
+    pred = ctx.predict().cpu().numpy()[0]
+    margin = orc.sweep(phi, m, 0.5, T, 1.0, seed, 0, 0, diag=True)[1]
+    acc = np.where(m == 0, phi.astype(np.float64), 0.0)
+    ref = orc.predict(acc, 1, z, m, zmin, zmax)
+    ok = (m == 1) | (margin > 1e-3)
+    scale = (float(zmax) - float(zmin)) / TWO_PI_F
+    assert np.abs(pred - ref)[ok].max() <= 2 * TOL_RAD * scale
+    assert (~ok).sum() <= 2
+    assert ctx.get_stats()[0].realizations == 1 and ctx.get_stats()[0].t == 1
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------
+# error behaviour at the boundary
+# ---------------------------------------------------------------------------
+def test_error_statuses(torch_cuda, mpr):
+    torch = torch_cuda
+    z = torch.randn(8, 8, device="cuda")
+    ones = torch.ones(8, 8, dtype=torch.uint8, device="cuda")
+    zeros = torch.zeros(8, 8, dtype=torch.uint8, device="cuda")
+    half = ones.clone(); half[::2] = 0
+    with pytest.raises(mpr.MprError) as e:
+        mpr.Mpr(z, zeros)
+    assert e.value.name == "MPR_ERR_NO_SAMPLES"
+    with pytest.raises(mpr.MprError) as e:
+        mpr.Mpr(z, ones)
+    assert e.value.name == "MPR_ERR_NO_FREE"
+    with pytest.raises(mpr.MprError) as e:
+        mpr.Mpr(torch.full((8, 8), 2.5, device="cuda"), half)
+    assert e.value.name == "MPR_ERR_DEGENERATE_RANGE"
+    zn = z.clone(); zn[1, 1] = float("inf")
+    with pytest.raises(mpr.MprError) as e:
+        mpr.Mpr(zn, half)
+    assert e.value.name == "MPR_ERR_NONFINITE"
+    ctx = mpr.Mpr(z, half)
+    with pytest.raises(mpr.MprError) as e:
+        ctx.equilibrate()
+    assert e.value.name == "MPR_ERR_STATE"
+    for bad in (dict(q=0.7), dict(M=0), dict(n_fit=1), dict(or_mode=3)):
+        with pytest.raises(mpr.MprError) as e:
+            ctx.set_params(0.1, **bad)
+        assert e.value.name == "MPR_ERR_ARG"
+    with pytest.raises(mpr.MprError) as e:
+        ctx.set_params(-1.0)
+    assert e.value.name == "MPR_ERR_ARG"
+    with pytest.raises(mpr.MprError) as e:
+        ctx.set_params(0.1, q=0.25, or_mode=1)
+    assert e.value.name == "MPR_ERR_UNSUPPORTED"
+    ctx.close()
+
+
+def test_same_seed_same_result_bitwise(torch_cuda, mpr):
+    """The run is a pure function of (inputs, params, seed): no atomics on
+    floating point anywhere on the path."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    outs = []
+    for _ in range(2):
+        pred, st = mpr.interpolate(_dev(torch, w.truth), _dev(torch, w.mask), w.T, seed=9, equil_cap=300,
+                                   sweeps_per_real=5, M=4)
+        outs.append((pred.cpu().numpy(), st[0].equil_sweeps, st[0].e_last))
+    assert np.array_equal(outs[0][0].view(np.uint32), outs[1][0].view(np.uint32))
+    assert outs[0][1:] == outs[1][1:]

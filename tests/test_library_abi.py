@@ -1,0 +1,86 @@
+"""CPU-side checks of the boundary: the C-ABI library builds for sm_100a,
+loads, exports every symbol include/mpr.h declares, and its host-only logic
+(argument validation, workspace sizing, defaults) behaves as the header says.
+No compute call is made: there is no GPU here."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_1811_01604_b200 import build as mpr_build
+from paper_1811_01604_b200 import mpr
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    mpr_build.build()
+    return mpr.lib()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "mpr.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mpr_[a-z_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = _declared_symbols()
+    assert len(names) >= 19
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(mpr.EXPORTS) == names
+
+
+def test_defaults_are_reading_r7(lib):
+    p = mpr.default_params()
+    assert p.struct_size == C.sizeof(mpr.mpr_params)
+    assert (p.q, p.n_f, p.n_fit, p.equil_cap, p.M, p.sweeps_per_real) == (0.5, 5, 20, 500, 100, 1)
+    assert p.A_targ == pytest.approx(0.3) and p.k_a == 3.0 and p.or_mode == 0 and p.a_eq_mode == 0
+
+
+def test_workspace_query_validates_and_scales(lib):
+    for bad in [(0, 8, 8), (1, 1, 8), (1, 8, 1), (1, 70000, 8), (1, 65000, 65000)]:
+        with pytest.raises(mpr.MprError) as e:
+            mpr.mpr_query_workspace(*bad)
+        assert e.value.name == "MPR_ERR_ARG"
+    small = mpr.mpr_query_workspace(1, 64, 64)
+    big = mpr.mpr_query_workspace(1, 4096, 4096)
+    batch = mpr.mpr_query_workspace(32, 2048, 2048)
+    assert small < 1 << 20
+    # about 28.1 bytes per site: 8 (unit vectors) + 4 + 4 (values, angles) + 4 + 4 (lists, accumulators) + 1/8
+    assert 24 * 4096 ** 2 < big < 30 * 4096 ** 2
+    assert 24 * 32 * 2048 ** 2 < batch < 30 * 32 * 2048 ** 2
+    assert mpr.mpr_query_workspace(3, 37, 53) % 256 == 0
+
+
+def test_null_and_misuse_are_errors_not_crashes(lib):
+    ctx = C.c_void_p()
+    assert lib.mpr_create(C.byref(ctx), 1, 8, 8, None, None, None, 0, None) == 1          # MPR_ERR_ARG
+    assert lib.mpr_create(None, 1, 8, 8, None, None, None, 0, None) == 1
+    assert lib.mpr_equilibrate(None) == 1 and lib.mpr_simulate(None) == 1 and lib.mpr_predict(None, None) == 1
+    assert lib.mpr_destroy(None) == 1
+    assert lib.mpr_query_workspace(1, 8, 8, None) == 1
+    assert ctx.value is None
+
+
+def test_status_strings(lib):
+    seen = set()
+    for code in range(10):
+        s = lib.mpr_status_string(code).decode()
+        assert s and s != "unknown status"
+        seen.add(s)
+    assert len(seen) == 10
+    assert lib.mpr_status_string(99).decode() == "unknown status"
+
+
+def test_no_cpu_fallback_in_the_product():
+    """The product never imports, links or executes the oracle."""
+    pkg = os.path.join(ROOT, "paper_1811_01604_b200")
+    pat = re.compile(r"^\s*(from|import)\s+oracle|mpr_oracle|libmpr_oracle|orc_[a-z]", re.M)
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                assert not pat.search(open(os.path.join(dirpath, f)).read()), f
