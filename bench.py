@@ -134,9 +134,9 @@ def oracle_sample(w, n_sweeps: int):
 
 
 def oracle_sweeps_for(w) -> int:
-    """About 10-30 s of CPU work: ~60 ns per update per core as a planning figure."""
+    """About 10-30 s of CPU work at the ~5e7-1e8 updates/s the OpenMP oracle reaches on a host."""
     P = int((w.mask[0] == 0).sum())
-    return int(max(3, min(2000, 8.0e7 / max(P, 1))))
+    return int(max(3, min(20000, 1.2e9 / max(P, 1))))
 
 
 def run_reference(args, w):

@@ -70,21 +70,22 @@ double orc_u01(uint32_t x)
     return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0);
 }
 
-/* Random-stream layout (reading R13).  key = (seed_lo, seed_hi).
+/* Random-stream layout (reading R13; the paper only says "two numbers per
+ * spin per MC step" from Philox4_32_10, L267).  key = (seed_lo, seed_hi).
  *   INIT  stream: counter = (n >> 2, 0, 0, g), word n & 3, n = row*cols+col.
- *   SWEEP stream: counter = (o >> 1, t, 2 + colour, g); o = ordinal of the
- *     site among the FREE sites of its colour in row-major order; words
- *     (2*(o&1), 2*(o&1)+1) give (u, r).  t = global sweep index, increasing
- *     from the first equilibration sweep through all realizations.
+ *   SWEEP stream: counter = (n, t >> 1, 2, g), keyed by the SITE n and the
+ *     pair of sweeps (t, t+1): words (x0, x1) give (u, r) at even t, words
+ *     (x2, x3) at odd t.  t = global sweep index, increasing from the first
+ *     equilibration sweep through all realizations.
  */
-static void sweep_uniforms(uint64_t seed, uint32_t g, uint32_t t, int colour,
-                           uint64_t ordinal, double *u, double *r)
+static void sweep_uniforms(uint64_t seed, uint32_t g, uint32_t t, uint32_t n,
+                           double *u, double *r)
 {
-    uint32_t ctr[4] = { (uint32_t)(ordinal >> 1), t, 2u + (uint32_t)colour, g };
+    uint32_t ctr[4] = { n, t >> 1, 2u, g };
     uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
     uint32_t x[4];
     orc_philox4x32_10(ctr, key, x);
-    int slot = (int)(ordinal & 1u);
+    int slot = (int)(t & 1u);
     *u = orc_u01(x[2 * slot]);
     *r = orc_u01(x[2 * slot + 1]);
 }
@@ -209,22 +210,12 @@ uint64_t orc_sweep(float *phi, const uint8_t *mask, int rows, int cols,
                    double *d_margin, double *d_edge, double *d_R)
 {
     uint64_t accepted_total = 0;
-    uint64_t *row_start = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)(rows + 1));
     for (int colour = 0; colour < 2; ++colour) {
-        /* ordinal of the first free site of this colour in each row */
-        row_start[0] = 0;
-        for (int r = 0; r < rows; ++r) {
-            uint64_t cnt = 0;
-            for (int c = (r + colour) & 1; c < cols; c += 2)
-                if (!mask[(int64_t)r * cols + c]) ++cnt;
-            row_start[r + 1] = row_start[r] + cnt;
-        }
         uint64_t accepted = 0;
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static) reduction(+:accepted)
 #endif
         for (int r = 0; r < rows; ++r) {
-            uint64_t ordinal = row_start[r];
             for (int c = (r + colour) & 1; c < cols; c += 2) {
                 int64_t n = (int64_t)r * cols + c;
                 if (mask[n]) continue;               /* sample sites stay fixed (L148) */
@@ -240,7 +231,7 @@ uint64_t orc_sweep(float *phi, const uint8_t *mask, int rows, int cols,
                 double p1 = orc_or_reflect(p_old, C, S, C1, S1, q, or_mode, &kept, &p_raw);
                 /* line 2: u ~ U(0,1);  line 6: r ~ U(0,1) */
                 double u, rr;
-                sweep_uniforms(seed, g, t, colour, ordinal, &u, &rr);
+                sweep_uniforms(seed, g, t, (uint32_t)n, &u, &rr);
                 /* line 3: phi'' = phi' + 2 pi (u - 0.5)/a (mod 2 pi) */
                 double p2_raw = p1 + TWO_PI * (u - 0.5) / a;
                 double p2 = p2_raw;
@@ -262,12 +253,10 @@ uint64_t orc_sweep(float *phi, const uint8_t *mask, int rows, int cols,
                     d_edge[n] = e1 < e2 ? e1 : e2;
                 }
                 if (d_R) d_R[n] = sqrt(C * C + S * S);
-                ++ordinal;
             }
         }
         accepted_total += accepted;
     }
-    free(row_start);
     return accepted_total;
 }
 
