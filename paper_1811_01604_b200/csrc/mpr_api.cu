@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -31,7 +32,28 @@ inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 struct Geometry {
     uint32_t N, words, W, Wp, VS, LC;
+    int TR, TC, H, FR, FC, ntx, nty, ntiles;
+    uint32_t n_partials;
+    size_t entry_stride;
 };
+
+// Tile shape.  A grid that fits one frame is a single tile with a
+// one-site zero border (any number of sweeps per pass); otherwise TR x TC cores with a halo of H
+// (H/2 sweeps per pass).  MPR_TILE="TR,TC,H" overrides the default for experiments.
+void choose_tiles(int rows, int cols, Geometry* g)
+{
+    int TR = 64, TC = 64, H = 8;
+    if (const char* e = getenv("MPR_TILE")) {
+        int a, b, c;
+        if (sscanf(e, "%d,%d,%d", &a, &b, &c) == 3 && a >= 8 && b >= 8 && c >= 2 && c <= MAX_H && (c & 1) == 0 &&
+            (a + 2 * c) * (b + 2 * c) <= 65536 && a + 2 * c <= 255) { TR = a; TC = b; H = c; }
+    }
+    if ((long)rows * cols <= 128L * 128L && rows <= 250 && cols <= 1024) { TR = rows; TC = cols; H = 1; }
+    g->TR = TR; g->TC = TC; g->H = H; g->FR = TR + 2 * H; g->FC = TC + 2 * H;
+    g->ntx = (cols + TC - 1) / TC; g->nty = (rows + TR - 1) / TR; g->ntiles = g->ntx * g->nty;
+    g->n_partials = (uint32_t)(g->ntiles > ENERGY_BLOCKS ? g->ntiles : ENERGY_BLOCKS);
+    g->entry_stride = (size_t)g->ntiles * g->FR * g->FC;
+}
 
 bool make_geometry(int batch, int rows, int cols, Geometry* g)
 {
@@ -43,11 +65,12 @@ bool make_geometry(int batch, int rows, int cols, Geometry* g)
     g->N = (uint32_t)N; g->words = (uint32_t)((N + 31) / 32);
     g->W = (uint32_t)W; g->Wp = (uint32_t)Wp; g->VS = (uint32_t)VS;
     g->LC = (uint32_t)((((N + 1) / 2 + 1) & ~1ull) + 2);                       // even, >= max count + 2
-    return true;
+    choose_tiles(rows, cols, g);
+    return g->entry_stride < (1ull << 32);
 }
 
 struct Layout {
-    size_t states, done, partials, values, phi, bits, vec, lists, acc, rowstart, total;
+    size_t states, done, partials, values, phi, bits, vec, lists, acc, rowstart, tile_meta, entries, total;
 };
 
 Layout make_layout(int batch, int rows, const Geometry& g)
@@ -56,16 +79,18 @@ Layout make_layout(int batch, int rows, const Geometry& g)
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     const size_t B = (size_t)batch;
-    L.states   = take(B * sizeof(GridState));
-    L.done     = take(B * sizeof(uint32_t));
-    L.partials = take(B * ENERGY_BLOCKS * sizeof(double));
-    L.values   = take(B * g.N * sizeof(float));
-    L.phi      = take(B * g.N * sizeof(float));
-    L.bits     = take(B * g.words * sizeof(uint32_t));
-    L.vec      = take(B * 2 * g.VS * sizeof(float2));
-    L.lists    = take(B * 2 * g.LC * sizeof(uint32_t));
-    L.acc      = take(B * 2 * g.LC * sizeof(float));
-    L.rowstart = take(B * 2 * ((size_t)rows + 1) * sizeof(uint32_t));
+    L.states    = take(B * sizeof(GridState));
+    L.done      = take(B * sizeof(uint32_t));
+    L.partials  = take(B * g.n_partials * sizeof(double));
+    L.values    = take(B * g.N * sizeof(float));
+    L.phi       = take(B * g.N * sizeof(float));
+    L.bits      = take(B * g.words * sizeof(uint32_t));
+    L.vec       = take(2 * B * 2 * g.VS * sizeof(float2));
+    L.lists     = take(B * 2 * g.LC * sizeof(uint32_t));
+    L.acc       = take(B * 2 * g.VS * sizeof(float));
+    L.rowstart  = take(B * 2 * ((size_t)rows + 1) * sizeof(uint32_t));
+    L.tile_meta = take(B * g.ntiles * sizeof(TileMeta));
+    L.entries   = take(B * g.entry_stride * sizeof(uint32_t));
     L.total = o;
     return L;
 }
@@ -82,6 +107,8 @@ struct mpr_ctx {
     RunState     state;
     uint32_t     max_free[2];     // max over grids of the free count per colour
     int          energy_blocks;
+    uint32_t     k_max;           // sweeps per tile pass
+    size_t       smem_bytes;      // dynamic shared memory of k_tilepass
     uint64_t     launches;
     uint32_t*    h_pinned;        // [batch] pinned host, done flags
     GridState*   h_states;        // [batch] pageable host copy
@@ -99,34 +126,39 @@ mpr_status fetch_states(mpr_ctx* ctx)
     return MPR_OK;
 }
 
-template <bool COUNT, bool CHECK_DONE>
-mpr_status launch_halfsweep(mpr_ctx* ctx, int colour, uint32_t t_off)
+typedef void (*pass_kernel)(Dev, uint32_t, uint32_t, uint32_t, uint32_t);
+
+pass_kernel pick_pass_kernel(bool qhalf, int or_mode)
 {
-    const unsigned pairs = (ctx->max_free[colour] + 1) / 2;
-    if (pairs == 0) return MPR_OK;
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0> : or_mode == 1 ? k_tilepass<true, 1> : k_tilepass<true, 2>;
+    return or_mode == 0 ? k_tilepass<false, 0> : k_tilepass<false, 2>;
+}
+
+// K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile
+mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
+{
     ctx->dirty = true;
-    const dim3 grid(cdiv(pairs, SWEEP_THREADS), ctx->d.batch);
-    const int orm = (int)ctx->prm.or_mode;
-#define MPR_HS(QH, OM) k_halfsweep<QH, OM, COUNT, CHECK_DONE><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(ctx->d, colour, t_off)
-    if (ctx->qhalf) { if (orm == 0) MPR_HS(true, 0); else if (orm == 1) MPR_HS(true, 1); else MPR_HS(true, 2); }
-    else            { if (orm == 0) MPR_HS(false, 0); else MPR_HS(false, 2); }
-#undef MPR_HS
+    pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode)
+        <<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(ctx->d, K, t_off, flip, flags);
     CU_LAUNCH();
     return MPR_OK;
 }
 
-// one UPDATE sweep (Alg. 1): colour 0 (contains the upper-left node, Fig. 1) then colour 1
-template <bool COUNT, bool CHECK_DONE>
-mpr_status launch_sweep(mpr_ctx* ctx, uint32_t t_off)
+// n sweeps at the current a as passes of at most k_max sweeps; *t_off and *flip carry the uncommitted progress
+mpr_status launch_sweeps(mpr_ctx* ctx, uint32_t n, uint32_t* t_off, uint32_t* flip, uint32_t flags, uint32_t last_flags)
 {
-    mpr_status s = launch_halfsweep<COUNT, CHECK_DONE>(ctx, 0, t_off);
-    if (s != MPR_OK) return s;
-    return launch_halfsweep<COUNT, CHECK_DONE>(ctx, 1, t_off);
+    while (n) {
+        const uint32_t K = n < ctx->k_max ? n : ctx->k_max;
+        mpr_status s = launch_pass(ctx, K, *t_off, *flip, flags | (n == K ? last_flags : 0u));
+        if (s != MPR_OK) return s;
+        *t_off += K; *flip ^= 1u; n -= K;
+    }
+    return MPR_OK;
 }
 
-mpr_status launch_energy(mpr_ctx* ctx, bool check_done)
+mpr_status launch_energy(mpr_ctx* ctx)
 {
-    k_energy<<<dim3(ctx->energy_blocks, ctx->d.batch), ENERGY_THREADS, 0, ctx->stream>>>(ctx->d, check_done);
+    k_energy<<<dim3(ctx->energy_blocks, ctx->d.batch), ENERGY_THREADS, 0, ctx->stream>>>(ctx->d);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -211,6 +243,11 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     d.lists = (uint32_t*)(base + lay.lists);
     d.acc = (float*)(base + lay.acc);
     d.rowstart = (uint32_t*)(base + lay.rowstart);
+    d.tile_meta = (TileMeta*)(base + lay.tile_meta);
+    d.entries = (uint32_t*)(base + lay.entries);
+    d.VB = (size_t)batch * 2 * g.VS;
+    d.entry_stride = g.entry_stride; d.n_partials = g.n_partials;
+    d.TR = g.TR; d.TC = g.TC; d.H = g.H; d.FR = g.FR; d.FC = g.FC; d.ntx = g.ntx; d.nty = g.nty; d.ntiles = g.ntiles;
     d.batch = batch; d.rows = rows; d.cols = cols;
     d.N = g.N; d.words = g.words; d.W = g.W; d.Wp = g.Wp; d.VS = g.VS; d.LC = g.LC;
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
@@ -223,7 +260,7 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
 
     cudaStream_t s = ctx->stream;
     // zero pads of the vector arrays = open boundary
-    if (!cuda_ok(cudaMemsetAsync(d.vec, 0, (size_t)batch * 2 * g.VS * sizeof(float2), s), "memset vec")) return fail(MPR_ERR_CUDA);
+    if (!cuda_ok(cudaMemsetAsync(d.vec, 0, 2 * d.VB * sizeof(float2), s), "memset vec")) return fail(MPR_ERR_CUDA);
     k_state_reset<<<cdiv(batch, 128), 128, 0, s>>>(d);
     unsigned mm_blocks = cdiv(g.N, 256 * 8);
     if (mm_blocks > 1184) mm_blocks = 1184;
@@ -233,7 +270,10 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     k_rowcount<<<dim3(cdiv((size_t)rows * 32, 256), batch), 256, 0, s>>>(d);
     k_rowscan<<<dim3(batch, 2), 32, 0, s>>>(d);
     k_build_lists<<<dim3(cdiv((size_t)rows * 32, 256), batch), 256, 0, s>>>(d);
-    ctx->launches += 7;
+    k_tile_count<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
+    k_tile_scan<<<batch, 32, 0, s>>>(d);
+    k_tile_fill<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
+    ctx->launches += 10;
     if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
     st = fetch_states(ctx);
     if (st != MPR_OK) return fail(st);
@@ -246,6 +286,31 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
         for (int c = 0; c < 2; ++c)
             if (ctx->h_states[b].n_free[c] > ctx->max_free[c]) ctx->max_free[c] = ctx->h_states[b].n_free[c];
     }
+    // shared memory of the tile pass: frame + entries (+ the odd sweeps' random words when they fit)
+    uint32_t max_entries = 0;
+    for (int b = 0; b < batch; ++b)
+        if (ctx->h_states[b].max_tile_entries > max_entries) max_entries = ctx->h_states[b].max_tile_entries;
+    max_entries = (max_entries + 1u) & ~1u;
+    d.max_entries = max_entries;
+    const size_t frame_bytes = (size_t)g.FR * g.FC * sizeof(float2);
+    int smem_max = 0;
+    if (!cuda_ok(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device), "smem attr")) return fail(MPR_ERR_CUDA);
+    const size_t budget = (size_t)smem_max - 2048;               // static shared memory of the kernel
+    d.use_spare = g.ntiles == 1 || g.H >= 4;                       // pointless when every pass is a single sweep
+    if (frame_bytes + 12ull * max_entries > budget) d.use_spare = 0;
+    ctx->smem_bytes = frame_bytes + (d.use_spare ? 12ull : 4ull) * max_entries;
+    if (ctx->smem_bytes > budget) return fail(MPR_ERR_WORKSPACE);
+    ctx->k_max = g.ntiles == 1 ? 1024u : (uint32_t)(g.H / 2);
+    if (const char* e = getenv("MPR_KMAX")) {
+        const int k = atoi(e);
+        if (k >= 1 && (g.ntiles == 1 || k <= g.H / 2)) ctx->k_max = (uint32_t)k;
+    }
+    for (int qh = 0; qh < 2; ++qh)
+        for (int om = 0; om < 3; ++om) {
+            if (!qh && om == 1) continue;
+            if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
+        }
     *out = ctx;
     return MPR_OK;
 }
@@ -278,10 +343,11 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     d.bc = (float)cos((double)p->q * (double)TWO_PI_F); d.bs = (float)sin((double)p->q * (double)TWO_PI_F);
     d.n_f = p->n_f; d.n_fit = p->n_fit; d.equil_cap = p->equil_cap;
     d.A_targ = (double)p->A_targ; d.k_a = (double)p->k_a;
-    // per-grid temperatures: staged through the (currently unused) accumulator
-    CU(cudaMemcpyAsync(d.acc, h_T, sizeof(float) * d.batch, cudaMemcpyHostToDevice, ctx->stream));
-    k_begin_run<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, d.acc);
+    // per-grid temperatures: staged through the energy partials (free between calls)
+    CU(cudaMemcpyAsync(d.e_partials, h_T, sizeof(float) * d.batch, cudaMemcpyHostToDevice, ctx->stream));
+    k_begin_run<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, (const float*)d.e_partials);
     CU_LAUNCH();
+    CU(cudaMemsetAsync(d.acc, 0, (size_t)d.batch * 2 * d.VS * sizeof(float), ctx->stream));
     k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d);
     CU_LAUNCH();
     CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
@@ -303,11 +369,11 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
     while (issued < cap) {
         if (chunk > cap - issued) chunk = cap - issued;
         for (uint32_t j = 0; j < chunk; ++j) {
-            mpr_status s = launch_sweep<true, true>(ctx, 0);          // 5.1 (t advanced by the controller)
+            // 5.1 one sweep with the energy (5.3) and the accepted count fused; the controller does
+            // 5.2, 5.4, 5.5 and commits the sweep (t, buffer swap) for the grids still running
+            mpr_status s = launch_pass(ctx, 1, 0, 0, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
             if (s != MPR_OK) return s;
-            s = launch_energy(ctx, true);                              // 5.3
-            if (s != MPR_OK) return s;
-            k_controller<<<d.batch, 32, 0, ctx->stream>>>(d, ctx->energy_blocks);   // 5.2, 5.4, 5.5
+            k_controller<<<d.batch, 32, 0, ctx->stream>>>(d);
             CU_LAUNCH();
         }
         issued += chunk;
@@ -328,16 +394,16 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
     const uint32_t s_per = ctx->prm.sweeps_per_real;
-    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, ctx->prm.a_eq_mode == 1 ? 0 : 1, 1.0);
+    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, ctx->prm.a_eq_mode == 1 ? 0 : 1, 1.0, 0);
     CU_LAUNCH();
+    uint32_t t_off = 0, flip = 0;
     for (uint32_t j = 0; j < ctx->prm.M; ++j) {
-        for (uint32_t w = 0; w < s_per; ++w) {
-            mpr_status s = launch_sweep<false, false>(ctx, w);
-            if (s != MPR_OK) return s;
-        }
-        k_accumulate<<<list_grid(ctx), 256, 0, ctx->stream>>>(d, s_per, j == 0);
-        CU_LAUNCH();
+        // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
+        mpr_status s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE);
+        if (s != MPR_OK) return s;
     }
+    k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, t_off, flip, ctx->prm.M);
+    CU_LAUNCH();
     return MPR_OK;
 }
 
@@ -384,7 +450,7 @@ mpr_status mpr_set_sweep_index(mpr_ctx* ctx, uint32_t t)
     if (!ctx) return MPR_ERR_ARG;
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
-    k_advance_t<<<cdiv(ctx->d.batch, 128), 128, 0, ctx->stream>>>(ctx->d, t, 1, 0);
+    k_set_t<<<cdiv(ctx->d.batch, 128), 128, 0, ctx->stream>>>(ctx->d, t);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -395,15 +461,12 @@ mpr_status mpr_sweep(mpr_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_acce
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
-    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, a);
+    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, a, 1);       // also zeroes the accepted counters
     CU_LAUNCH();
-    k_advance_t<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, 0, 1);   // zero the accepted counters
-    CU_LAUNCH();
-    for (uint32_t w = 0; w < n_sweeps; ++w) {
-        mpr_status s = h_accepted ? launch_sweep<true, false>(ctx, w) : launch_sweep<false, false>(ctx, w);
-        if (s != MPR_OK) return s;
-    }
-    k_advance_t<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, n_sweeps, 0, 0);
+    uint32_t t_off = 0, flip = 0;
+    mpr_status rs = launch_sweeps(ctx, n_sweeps, &t_off, &flip, h_accepted ? PASS_COUNT : 0u, 0);
+    if (rs != MPR_OK) return rs;
+    k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, t_off, flip, 0);
     CU_LAUNCH();
     if (h_accepted) {
         mpr_status s = fetch_states(ctx);
@@ -418,7 +481,7 @@ mpr_status mpr_energy(mpr_ctx* ctx, double* h_e)
     if (!ctx || !h_e) return MPR_ERR_ARG;
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
-    mpr_status s = launch_energy(ctx, false);
+    mpr_status s = launch_energy(ctx);
     if (s != MPR_OK) return s;
     k_energy_query<<<ctx->d.batch, 32, 0, ctx->stream>>>(ctx->d, ctx->energy_blocks);
     CU_LAUNCH();

@@ -19,20 +19,25 @@ namespace mpr {
 constexpr float    TWO_PI_F      = 6.28318530717958647692f;  // float nearest 2 pi; state space [0, TWO_PI_F]
 constexpr int      MAX_NFIT      = 256;
 constexpr uint32_t LIST_SENTINEL = 0xFFFFFFFFu;
-constexpr int      SWEEP_THREADS = 256;
+constexpr int      TILE_THREADS  = 512;
+constexpr int      MAX_H         = 16;                       // largest halo: up to 8 sweeps per tile pass
 constexpr int      ENERGY_BLOCKS = 592;                      // 4 x 148 SMs; fixed so the sum order is deterministic
 constexpr int      ENERGY_THREADS = 256;
 
 enum : uint32_t { ERRF_NO_SAMPLES = 1u, ERRF_NO_FREE = 2u, ERRF_DEGENERATE = 4u, ERRF_NONFINITE = 8u };
+// k_tilepass flags
+enum : uint32_t { PASS_COUNT = 1u, PASS_ENERGY = 2u, PASS_ACCUMULATE = 4u, PASS_CHECK_DONE = 8u };
 
 // One per grid, in the workspace.
 struct GridState {
-    // --- read by every half-sweep ---
-    uint32_t t;                  // global sweep index (Philox counter word 1)
+    // --- read by every tile pass ---
+    uint32_t t;                  // global sweep index (Philox counter word 1 is t >> 1)
     uint32_t done;               // equilibration stopped (Alg. 2 step 5 loop condition false)
+    uint32_t cur;                // which of the two vector buffers holds the current state
     float    hd_scale;           // q * pi / a: half of the rotation q*delta per unit (u - 1/2)
     float    neg_log2e_over_T;   // AP = 2^(dH * this)
     uint32_t n_free[2];          // prediction sites per colour
+    uint32_t max_tile_entries;   // largest free-site count of one tile frame
     // --- reductions ---
     unsigned long long accepted; // accepted Metropolis proposals since last reset
     uint32_t zmin_enc, zmax_enc; // order-preserving encodings for atomicMin/Max
@@ -47,20 +52,35 @@ struct GridState {
     double   e_ring[MAX_NFIT];   // e(i) at slot i % n_fit
 };
 
+// Free sites of one tile frame (core + halo), see k_tile_fill.
+struct TileMeta {
+    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid)
+    uint32_t cge[2][MAX_H + 1];       // cge[c][k] = entries of colour c with ring >= k (ring = distance outside the core)
+};
+
 // Device view of one context (passed by value to kernels).
 struct Dev {
     GridState* states;
     uint32_t*  done_flags;     // [batch] copy of GridState::done for cheap host polling
-    double*    e_partials;     // [batch][ENERGY_BLOCKS]
+    double*    e_partials;     // [batch][n_partials]
     float*     values;         // [batch][N] verbatim copy of the input values
     float*     phi;            // [batch][N] angle view: Eq. 1 at sample sites (never rewritten), export buffer at free sites
     uint32_t*  bits;           // [batch][words] fixed-site bitmask
-    float2*    vec;            // [batch][2][VS] colour-split padded unit vectors; pad = (0,0)
+    float2*    vec;            // [2 buffers][batch][2 colours][VS] colour-split padded unit vectors; pad = (0,0)
     uint32_t*  lists;          // [batch][2][LC] padded index | parity<<31 of the free sites, row-major order
-    float*     acc;            // [batch][2][LC] sum over realizations of phi at free sites (list order)
+    float*     acc;            // [batch][2][VS] sum over realizations of phi at free sites (same index as vec)
     uint32_t*  rowstart;       // [batch][2][rows+1] ordinal of the first free site of each row
+    TileMeta*  tile_meta;      // [batch][ntiles]
+    uint32_t*  entries;        // [batch][entry_stride] tile frames' free sites: off | local row << 16
     int        batch, rows, cols;
     uint32_t   N, words, W, Wp, VS, LC;
+    size_t     VB;             // float2 elements per vector buffer = batch * 2 * VS
+    size_t     entry_stride;
+    uint32_t   n_partials;
+    // tiling
+    int        TR, TC, H, FR, FC, ntx, nty, ntiles;
+    uint32_t   max_entries;    // smem capacity for entries (even)
+    int        use_spare;      // keep the odd sweep's random words in shared memory
     uint32_t   key0, key1;     // Philox key = (seed lo, seed hi)
     float      q, inv_q;
     float      bc, bs;         // (cos 2 pi q, sin 2 pi q): upper end of the q*phi range
@@ -68,6 +88,11 @@ struct Dev {
     uint32_t   n_f, n_fit, equil_cap;
     double     A_targ, k_a, n_bonds;
 };
+
+__device__ __forceinline__ float2* cur_vec(const Dev& d, int g, uint32_t which)
+{
+    return d.vec + (size_t)which * d.VB + (size_t)g * 2 * d.VS;
+}
 
 // ---------------------------------------------------------------------------
 // Philox4x32-10 (Salmon et al., SC'11), the generator PAPER.md L267 names.
@@ -167,8 +192,8 @@ __global__ void k_state_reset(Dev d)
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= d.batch) return;
     GridState& s = d.states[g];
-    s.t = 0; s.done = 0; s.hd_scale = 0.f; s.neg_log2e_over_T = 0.f;
-    s.n_free[0] = s.n_free[1] = 0;
+    s.t = 0; s.done = 0; s.cur = 0; s.hd_scale = 0.f; s.neg_log2e_over_T = 0.f;
+    s.n_free[0] = s.n_free[1] = 0; s.max_tile_entries = 0;
     s.accepted = 0ull;
     s.zmin_enc = 0xFFFFFFFFu; s.zmax_enc = 0u;
     s.n_samples = 0; s.err_flags = 0; s.i = 0; s.realizations = 0;
@@ -332,8 +357,110 @@ __global__ void __launch_bounds__(256) k_build_lists(Dev d)
 }
 
 // ---------------------------------------------------------------------------
+// a2  tile frames.  The grid is cut into TR x TC core tiles; a tile's frame is
+// its core plus a halo of H sites on every side.  For each tile the free
+// sites of the frame with ring < H (ring = Chebyshev distance outside the
+// core, 0 inside) are listed per colour, outermost ring first, so that the
+// sites a half-sweep of a K-sweep pass still needs are a suffix of the list.
+// ---------------------------------------------------------------------------
+struct TileGeom { int r0, c0, TRc, TCc; };
+
+__device__ __forceinline__ TileGeom tile_geom(const Dev& d, int tile)
+{
+    TileGeom t;
+    const int ty = tile / d.ntx, tx = tile - ty * d.ntx;
+    t.r0 = ty * d.TR; t.c0 = tx * d.TC;
+    t.TRc = min(d.TR, d.rows - t.r0); t.TCc = min(d.TC, d.cols - t.c0);
+    return t;
+}
+
+// class of frame site (lr, lc): returns false if outside the grid, fixed, or on the outermost ring
+__device__ __forceinline__ bool frame_site_class(const Dev& d, const uint32_t* __restrict__ bits, const TileGeom& t,
+                                                 int lr, int lc, int& colour, int& ring)
+{
+    const int r = t.r0 - d.H + lr, col = t.c0 - d.H + lc;
+    if (r < 0 || r >= d.rows || col < 0 || col >= d.cols) return false;
+    const uint32_t n = (uint32_t)r * d.cols + col;
+    if ((bits[n >> 5] >> (n & 31)) & 1u) return false;
+    const int dr = max(max(d.H - lr, lr - (d.H + t.TRc - 1)), 0);
+    const int dc = max(max(d.H - lc, lc - (d.H + t.TCc - 1)), 0);
+    ring = max(dr, dc);
+    colour = (r + col) & 1;
+    return ring < d.H;
+}
+
+__global__ void __launch_bounds__(256) k_tile_count(Dev d)
+{
+    const int tile = blockIdx.x, g = blockIdx.y;
+    __shared__ uint32_t hist[2][MAX_H + 1];
+    for (int i = threadIdx.x; i < 2 * (MAX_H + 1); i += blockDim.x) (&hist[0][0])[i] = 0;
+    __syncthreads();
+    const TileGeom t = tile_geom(d, tile);
+    const uint32_t* bits = d.bits + (size_t)g * d.words;
+    for (int i = threadIdx.x; i < d.FR * d.FC; i += blockDim.x) {
+        const int lr = i / d.FC, lc = i - lr * d.FC;
+        int colour, ring;
+        if (frame_site_class(d, bits, t, lr, lc, colour, ring)) atomicAdd(&hist[colour][ring], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        TileMeta& m = d.tile_meta[(size_t)g * d.ntiles + tile];
+        const int c = threadIdx.x;
+        uint32_t run = 0;
+        for (int k = MAX_H; k >= 0; --k) { run += hist[c][k]; m.cge[c][k] = run; }
+    }
+}
+
+// one warp per grid: exclusive scan of the tiles' entry counts, and their maximum
+__global__ void k_tile_scan(Dev d)
+{
+    const int g = blockIdx.x;
+    const uint32_t lane = threadIdx.x;
+    TileMeta* m = d.tile_meta + (size_t)g * d.ntiles;
+    uint32_t carry = 0, mx = 0;
+    for (int base = 0; base < d.ntiles; base += 32) {
+        const int i = base + lane;
+        const uint32_t c = i < d.ntiles ? m[i].cge[0][0] + m[i].cge[1][0] : 0u;
+        mx = max(mx, c);
+        uint32_t x = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, o);
+            if (lane >= (uint32_t)o) x += y;
+        }
+        if (i < d.ntiles) m[i].base = carry + x - c;
+        carry += __shfl_sync(0xFFFFFFFFu, x, 31);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+    if (lane == 0) d.states[g].max_tile_entries = mx;
+}
+
+__global__ void __launch_bounds__(256) k_tile_fill(Dev d)
+{
+    const int tile = blockIdx.x, g = blockIdx.y;
+    __shared__ uint32_t cursor[2][MAX_H + 1];
+    for (int i = threadIdx.x; i < 2 * (MAX_H + 1); i += blockDim.x) (&cursor[0][0])[i] = 0;
+    __syncthreads();
+    const TileGeom t = tile_geom(d, tile);
+    const TileMeta& m = d.tile_meta[(size_t)g * d.ntiles + tile];
+    const uint32_t* bits = d.bits + (size_t)g * d.words;
+    uint32_t* out = d.entries + (size_t)g * d.entry_stride + m.base;
+    for (int i = threadIdx.x; i < d.FR * d.FC; i += blockDim.x) {
+        const int lr = i / d.FC, lc = i - lr * d.FC;
+        int colour, ring;
+        if (frame_site_class(d, bits, t, lr, lc, colour, ring)) {
+            // colour 0 first; within a colour the rings in descending order
+            const uint32_t pos = (colour ? m.cge[0][0] : 0u) + m.cge[colour][ring + 1] + atomicAdd(&cursor[colour][ring], 1u);
+            out[pos] = (uint32_t)i | ((uint32_t)lr << 16);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------
 // a2  initial state (Alg. 2 step 2.2, L176): phi ~ U(0, 2 pi) at prediction
-// sites from the INIT stream; every site's unit vector (cos q phi, sin q phi).
+// sites from the INIT stream; every site's unit vector (cos q phi, sin q phi)
+// into BOTH vector buffers (sample sites are never written again).
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_init_state(Dev d)
 {
@@ -353,39 +480,21 @@ __global__ void __launch_bounds__(256) k_init_state(Dev d)
     const uint32_t r = n / d.cols, col = n - r * d.cols;
     float sn, cs;
     sincosf(__fmul_rn(d.q, p), &sn, &cs);
-    d.vec[((size_t)g * 2 + ((r + col) & 1u)) * d.VS + padded_index(r, col, d.Wp)] = make_float2(cs, sn);
+    const size_t at = (size_t)((r + col) & 1u) * d.VS + padded_index(r, col, d.Wp);
+    cur_vec(d, g, 0)[at] = make_float2(cs, sn);
+    cur_vec(d, g, 1)[at] = make_float2(cs, sn);
 }
 
 // ---------------------------------------------------------------------------
-// a3  the hot kernel: one half-sweep = UPDATE (Alg. 1) of
-// every prediction site of one checkerboard colour (L261-265).
-// One thread updates the two sites with ordinals (2p, 2p+1): one Philox call,
-// words (x0,x1) -> (u,r) of the first site, (x2,x3) of the second.
+// a3  UPDATE of one prediction site (Alg. 1) in vector form.
+// v = (cos q phi, sin q phi); (hx, hy) = (C, S) = sum over the neighbours.
 // ---------------------------------------------------------------------------
-struct Nbhd { float2 v, up, dn, lf, rt; };
-
-__device__ __forceinline__ Nbhd load_nbhd(const float2* __restrict__ own, const float2* __restrict__ oth,
-                                          uint32_t idx, uint32_t Wp)
-{
-    const uint32_t li = idx & 0x7FFFFFFFu, par = idx >> 31;
-    Nbhd n;
-    n.v  = own[li];
-    n.up = oth[li - Wp];
-    n.dn = oth[li + Wp];
-    n.lf = oth[li - 1u + par];
-    n.rt = oth[li + par];
-    return n;
-}
-
-// Returns the new unit vector; accepted = 1 when the Metropolis proposal was taken.
 template <bool QHALF, int ORMODE>
-__device__ __forceinline__ float2 update_site(const Nbhd& nb, float uc, float r, float hd_scale, float nlT,
-                                              float bc, float bs, uint32_t& accepted)
+__device__ __forceinline__ float2 update_site(float2 v, float hx, float hy, float2 n_up, float2 n_dn, float2 n_lf,
+                                              float2 n_rt, float uc, float r, float hd_scale, float nlT,
+                                              float bc, float bs, bool renorm, uint32_t& accepted)
 {
-    // neighbours' field (C, S) = sum_j (cos q phi_j, sin q phi_j); open boundary = zero pads (L109)
-    const float hx = (nb.up.x + nb.dn.x) + (nb.lf.x + nb.rt.x);
-    const float hy = (nb.up.y + nb.dn.y) + (nb.lf.y + nb.rt.y);
-    float px = nb.v.x, py = nb.v.y;
+    float px = v.x, py = v.y;
     // Alg. 1 line 1: over-relaxation.  Reflect v about h: q phi' = 2 Theta - q phi keeps h.v,
     // i.e. the local energy (L156, L265; R2).  Out of [0, 2 pi]: keep the spin.
     if (ORMODE == 0) {
@@ -400,9 +509,9 @@ __device__ __forceinline__ float2 update_site(const Nbhd& nb, float uc, float r,
     } else if (ORMODE == 1) {
         // Eq. 6 as printed (L158), q = 1/2 only: phi' = [2 atan2(sum sin phi_j, sum cos phi_j) - phi] mod 2 pi,
         // with cos phi_j = c^2 - s^2, sin phi_j = 2 c s; q phi' = Theta_1 - q phi (mod pi)
-        const float C1 = (nb.up.x * nb.up.x - nb.up.y * nb.up.y) + (nb.dn.x * nb.dn.x - nb.dn.y * nb.dn.y)
-                       + (nb.lf.x * nb.lf.x - nb.lf.y * nb.lf.y) + (nb.rt.x * nb.rt.x - nb.rt.y * nb.rt.y);
-        const float S1 = 2.0f * (nb.up.x * nb.up.y + nb.dn.x * nb.dn.y + nb.lf.x * nb.lf.y + nb.rt.x * nb.rt.y);
+        const float C1 = (n_up.x * n_up.x - n_up.y * n_up.y) + (n_dn.x * n_dn.x - n_dn.y * n_dn.y)
+                       + (n_lf.x * n_lf.x - n_lf.y * n_lf.y) + (n_rt.x * n_rt.x - n_rt.y * n_rt.y);
+        const float S1 = 2.0f * (n_up.x * n_up.y + n_dn.x * n_dn.y + n_lf.x * n_lf.y + n_rt.x * n_rt.y);
         const float R2 = fmaf(C1, C1, S1 * S1);
         const float inv = R2 > 0.0f ? rsqrtf(R2) : 0.0f;
         const float ex = R2 > 0.0f ? C1 * inv : 1.0f, ey = S1 * inv;      // atan2(0,0) = 0
@@ -438,55 +547,181 @@ __device__ __forceinline__ float2 update_site(const Nbhd& nb, float uc, float r,
     const bool acc = dH <= 0.0f || ex2_approx(dH * nlT) > r;
     accepted += acc;
     float nx = acc ? rx : px, ny = acc ? ry : py;
-    // keep |v| = 1 against rounding drift (first-order Newton step of 1/|v|)
-    const float sc = fmaf(-0.5f, fmaf(nx, nx, ny * ny), 1.5f);
-    return make_float2(nx * sc, ny * sc);
+    if (renorm) {   // keep |v| = 1 against rounding drift (first-order Newton step of 1/|v|), once per pass
+        const float sc = fmaf(-0.5f, fmaf(nx, nx, ny * ny), 1.5f);
+        nx *= sc; ny *= sc;
+    }
+    return make_float2(nx, ny);
 }
 
-template <bool QHALF, int ORMODE, bool COUNT, bool CHECK_DONE>
-__global__ void __launch_bounds__(SWEEP_THREADS) k_halfsweep(Dev d, int colour, uint32_t t_off)
+// ---------------------------------------------------------------------------
+// a3/a4  the hot kernel: K whole sweeps (colour 0 then colour 1, L261-265) of
+// one tile, on a copy of its frame in shared memory (temporal blocking).
+// Reads the state from one vector buffer and writes the tile's core to the
+// other, so tiles of one launch never see each other's writes.  Sites of the
+// halo are updated redundantly; they reproduce the neighbouring tiles'
+// results bit for bit because the random numbers are keyed by (site, sweep).
+// After half-sweep number hs (0-based) the frame is valid up to ring
+// 2K-1-hs, so each half-sweep only updates the suffix of the entry list
+// with ring <= 2K-1-hs.  Optionally fused at the end of the pass:
+//   PASS_ENERGY      a5: - sum over the core's colour-1 sites of v.h (each bond once)
+//   PASS_COUNT       a5: accepted proposals of the core sites
+//   PASS_ACCUMULATE  a7: acc += phi at the core's prediction sites
+// ---------------------------------------------------------------------------
+template <bool QHALF, int ORMODE>
+__global__ void __launch_bounds__(TILE_THREADS, 2) k_tilepass(Dev d, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
 {
-    const int g = blockIdx.y;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t s_cge[2][MAX_H + 1];
+    __shared__ uint32_t s_accepted;
+    __shared__ double s_red[TILE_THREADS / 32];
+
+    const int tile = blockIdx.x, g = blockIdx.y;
     const GridState& st = d.states[g];
-    if (CHECK_DONE && st.done) return;
-    const uint32_t nfree = st.n_free[colour];
-    const uint32_t pair = blockIdx.x * SWEEP_THREADS + threadIdx.x;
-    uint32_t accepted = 0;
-    if (2u * pair < nfree) {
-        const uint2 idx = reinterpret_cast<const uint2*>(d.lists + ((size_t)g * 2 + colour) * d.LC)[pair];
-        float2* own = d.vec + ((size_t)g * 2 + colour) * d.VS;
-        const float2* oth = d.vec + ((size_t)g * 2 + (1 - colour)) * d.VS;
-        const bool two = idx.y != LIST_SENTINEL;
-        const uint32_t idx1 = two ? idx.y : idx.x;
-        const Nbhd n0 = load_nbhd(own, oth, idx.x, d.Wp);
-        const Nbhd n1 = load_nbhd(own, oth, idx1, d.Wp);
-        const float hs = st.hd_scale, nlT = st.neg_log2e_over_T;
-        const uint4 x = philox4x32_10(pair, st.t + t_off, 2u + (uint32_t)colour, (uint32_t)g, d.key0, d.key1);
-        uint32_t a0 = 0, a1 = 0;
-        const float2 v0 = update_site<QHALF, ORMODE>(n0, u01_centered(x.x), u01(x.y), hs, nlT, d.bc, d.bs, a0);
-        const float2 v1 = update_site<QHALF, ORMODE>(n1, u01_centered(x.z), u01(x.w), hs, nlT, d.bc, d.bs, a1);
-        own[idx.x & 0x7FFFFFFFu] = v0;
-        if (two) own[idx1 & 0x7FFFFFFFu] = v1;
-        accepted = a0 + (two ? a1 : 0u);
+    if ((flags & PASS_CHECK_DONE) && st.done) return;
+
+    float2*   S  = reinterpret_cast<float2*>(smem_raw);
+    uint32_t* E  = reinterpret_cast<uint32_t*>(S + d.FR * d.FC);
+    uint2*    SP = reinterpret_cast<uint2*>(E + d.max_entries);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = TILE_THREADS / 32;
+    const TileGeom tg = tile_geom(d, tile);
+    const TileMeta& meta = d.tile_meta[(size_t)g * d.ntiles + tile];
+    const int H = d.H, FC = d.FC;
+    const int X = min((int)(2 * K), H);                      // rings of the frame this pass needs
+    const uint32_t src_buf = st.cur ^ flip;
+    const float2* src = cur_vec(d, g, src_buf);
+    float2*       dst = cur_vec(d, g, src_buf ^ 1u);
+
+    if (tid < 2 * (MAX_H + 1)) (&s_cge[0][0])[tid] = (&meta.cge[0][0])[tid];
+    if (tid == 0) s_accepted = 0;
+    const uint32_t nE = meta.cge[0][0] + meta.cge[1][0];
+    {
+        const uint32_t* gE = d.entries + (size_t)g * d.entry_stride + meta.base;
+        for (uint32_t i = tid; i < nE; i += TILE_THREADS) E[i] = gE[i];
     }
-    if (COUNT) {
+    // frame load: out-of-grid sites are zero vectors = open boundary
+    for (int lr = H - X + warp; lr < H + tg.TRc + X; lr += NW) {
+        const int r = tg.r0 - H + lr;
+        const bool rin = r >= 0 && r < d.rows;
+        for (int lc = H - X + lane; lc < H + tg.TCc + X; lc += 32) {
+            const int col = tg.c0 - H + lc;
+            float2 v = make_float2(0.0f, 0.0f);
+            if (rin && col >= 0 && col < d.cols)
+                v = src[(size_t)((r + col) & 1) * d.VS + (uint32_t)(r + 1) * d.Wp + (uint32_t)(col >> 1) + 1u];
+            S[lr * FC + lc] = v;
+        }
+    }
+    __syncthreads();
+
+    const float hs = st.hd_scale, nlT = st.neg_log2e_over_T;
+    const uint32_t t0 = st.t + t_off;
+    const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H), ncorr = d.cols - FC;
+    const bool count = flags & PASS_COUNT;
+    uint32_t accepted = 0;
+
+    for (uint32_t s = 0; s < K; ++s) {
+        const uint32_t t = t0 + s;
+        const bool odd = t & 1u;
+        const bool fresh = !odd || s == 0 || !d.use_spare;           // draw a new Philox block for (site, t >> 1)
+        const bool stash = d.use_spare && !odd && s + 1 < K;        // keep words 2,3 for sweep t + 1
+        const bool renorm = s + 1 == K;
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const int R = (int)(2 * K) - 1 - (int)(2 * s + c);       // rings still needed
+            const uint32_t first = R + 1 <= MAX_H ? s_cge[c][R + 1] : 0u;
+            const uint32_t last = s_cge[c][0], core_from = s_cge[c][1];
+            const uint32_t base = c ? s_cge[0][0] : 0u;
+            for (uint32_t e = first + tid; e < last; e += TILE_THREADS) {
+                const uint32_t ent = E[base + e];
+                const uint32_t off = ent & 0xFFFFu, lr = ent >> 16;
+                const float2 v = S[off], up = S[off - FC], dn = S[off + FC], lf = S[off - 1], rt = S[off + 1];
+                uint32_t w0, w1;
+                if (fresh) {
+                    const uint32_t n = (uint32_t)(nbase + (int)off + (int)lr * ncorr);
+                    const uint4 x = philox4x32_10(n, t >> 1, 2u, (uint32_t)g, d.key0, d.key1);
+                    w0 = odd ? x.z : x.x; w1 = odd ? x.w : x.y;
+                    if (stash) SP[base + e] = make_uint2(x.z, x.w);
+                } else {
+                    const uint2 sp = SP[base + e];
+                    w0 = sp.x; w1 = sp.y;
+                }
+                const float hx = (up.x + dn.x) + (lf.x + rt.x), hy = (up.y + dn.y) + (lf.y + rt.y);
+                uint32_t a = 0;
+                S[off] = update_site<QHALF, ORMODE>(v, hx, hy, up, dn, lf, rt, u01_centered(w0), u01(w1), hs, nlT,
+                                                    d.bc, d.bs, renorm, a);
+                if (count && e >= core_from) accepted += a;
+            }
+            __syncthreads();
+        }
+    }
+
+    // write the core back (both colours, whole rows: coalesced in each colour plane)
+    for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
+        const int r = tg.r0 - H + lr;
+        for (int lc = H + lane; lc < H + tg.TCc; lc += 32) {
+            const int col = tg.c0 - H + lc;
+            dst[(size_t)((r + col) & 1) * d.VS + (uint32_t)(r + 1) * d.Wp + (uint32_t)(col >> 1) + 1u] = S[lr * FC + lc];
+        }
+    }
+    if (flags & PASS_ACCUMULATE) {
+        // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t base = c ? s_cge[0][0] : 0u;
+            float* acc = d.acc + ((size_t)g * 2 + c) * d.VS;
+            for (uint32_t e = s_cge[c][1] + tid; e < s_cge[c][0]; e += TILE_THREADS) {
+                const uint32_t ent = E[base + e];
+                const uint32_t off = ent & 0xFFFFu, lr = ent >> 16, lc = off - lr * FC;
+                const int r = tg.r0 - H + (int)lr, col = tg.c0 - H + (int)lc;
+                acc[(uint32_t)(r + 1) * d.Wp + (uint32_t)(col >> 1) + 1u] += angle_of(S[off], d.inv_q);
+            }
+        }
+    }
+    if (count) {
         accepted = __reduce_add_sync(0xFFFFFFFFu, accepted);
-        if ((threadIdx.x & 31) == 0 && accepted) atomicAdd(&d.states[g].accepted, (unsigned long long)accepted);
+        if (lane == 0 && accepted) atomicAdd(&s_accepted, accepted);
+    }
+    if (flags & PASS_ENERGY) {
+        // a5: H_tile = - sum over the core's colour-1 sites (fixed ones too) of v . h; fixed summation order
+        double sum = 0.0;
+        for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
+            const int r = tg.r0 - H + lr;
+            float row = 0.0f;
+            // first colour-1 column of this row at or after the core's first column
+            for (int lc = H + ((r + tg.c0 + 1) & 1) + 2 * lane; lc < H + tg.TCc; lc += 64) {
+                const int off = lr * FC + lc;
+                const float2 v = S[off], up = S[off - FC], dn = S[off + FC], lf = S[off - 1], rt = S[off + 1];
+                row += fmaf(v.x, (up.x + dn.x) + (lf.x + rt.x), v.y * ((up.y + dn.y) + (lf.y + rt.y)));
+            }
+            sum += (double)row;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+        if (lane == 0) s_red[warp] = sum;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        if (count && s_accepted) atomicAdd(&d.states[g].accepted, (unsigned long long)s_accepted);
+        if (flags & PASS_ENERGY) {
+            double s = 0.0;
+            for (int w = 0; w < NW; ++w) s += s_red[w];
+            d.e_partials[(size_t)g * d.n_partials + tile] = -s;
+        }
     }
 }
 
 // ---------------------------------------------------------------------------
-// a5  energy H = - sum over bonds of cos q(phi_i - phi_j) = - sum over the
+// a5  energy of the current state on demand (mpr_energy): H = - sum over the
 // colour-1 sites i of v_i . h_i (every bond joins the two colours; Eq. 2).
 // Fixed block count and a fixed summation tree: bitwise reproducible.
 // ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(ENERGY_THREADS) k_energy(Dev d, bool check_done)
+__global__ void __launch_bounds__(ENERGY_THREADS) k_energy(Dev d)
 {
     const int g = blockIdx.y;
     __shared__ double warp_sum[ENERGY_THREADS / 32];
-    if (check_done && d.states[g].done) return;
-    const float2* own = d.vec + ((size_t)g * 2 + 1) * d.VS;
-    const float2* oth = d.vec + ((size_t)g * 2 + 0) * d.VS;
+    const float2* own = cur_vec(d, g, d.states[g].cur) + d.VS;
+    const float2* oth = cur_vec(d, g, d.states[g].cur);
     double sum = 0.0;
     for (uint32_t r = blockIdx.x; r < (uint32_t)d.rows; r += gridDim.x) {
         const uint32_t par = (r + 1u) & 1u;
@@ -509,37 +744,38 @@ __global__ void __launch_bounds__(ENERGY_THREADS) k_energy(Dev d, bool check_don
     if (threadIdx.x == 0) {
         double s = 0.0;
         for (int w = 0; w < ENERGY_THREADS / 32; ++w) s += warp_sum[w];
-        d.e_partials[(size_t)g * ENERGY_BLOCKS + blockIdx.x] = -s;
+        d.e_partials[(size_t)g * d.n_partials + blockIdx.x] = -s;
     }
 }
 
-__device__ __forceinline__ double sum_energy_partials(const Dev& d, int g, int n_blocks)
+__device__ __forceinline__ double sum_energy_partials(const Dev& d, int g, int n)
 {
-    const double* p = d.e_partials + (size_t)g * ENERGY_BLOCKS;
+    const double* p = d.e_partials + (size_t)g * d.n_partials;
     double s = 0.0;
-    for (int b = threadIdx.x; b < n_blocks; b += 32) s += p[b];
+    for (int b = threadIdx.x; b < n; b += 32) s += p[b];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
     return s;
 }
 
-__global__ void k_energy_query(Dev d, int n_blocks)
+__global__ void k_energy_query(Dev d, int n_partials)
 {
     const int g = blockIdx.x;
-    const double H = sum_energy_partials(d, g, n_blocks);
+    const double H = sum_energy_partials(d, g, n_partials);
     if (threadIdx.x == 0) d.states[g].e_query = H / d.n_bonds;
 }
 
 // ---------------------------------------------------------------------------
 // a6  equilibration controller: Alg. 2 steps 5.2-5.5 for
-// one grid per warp, after the sweep (5.1) and the energy reduction.
+// one grid per warp, after the sweep (5.1) with its fused energy reduction.
+// Commits the sweep: t += 1 and the vector buffers swap roles.
 // ---------------------------------------------------------------------------
-__global__ void k_controller(Dev d, int n_blocks)
+__global__ void k_controller(Dev d)
 {
     const int g = blockIdx.x;
     GridState& s = d.states[g];
     if (s.done) return;
-    const double H = sum_energy_partials(d, g, n_blocks);
+    const double H = sum_energy_partials(d, g, d.ntiles);
     if (threadIdx.x != 0) return;
     const uint32_t i = s.i;
     const double P = (double)s.n_free[0] + (double)s.n_free[1];
@@ -567,59 +803,46 @@ __global__ void k_controller(Dev d, int n_blocks)
         k = num / den;
     }
     // 5.5
-    s.i = i + 1u; s.t += 1u; s.a = a; s.k = k; s.A_last = A; s.e_last = e; s.accepted = 0ull;
+    s.i = i + 1u; s.t += 1u; s.cur ^= 1u; s.a = a; s.k = k; s.A_last = A; s.e_last = e; s.accepted = 0ull;
     s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F) / a);
     if (!(k < 0.0 && i + 1u < d.equil_cap)) { s.done = 1u; d.done_flags[g] = 1u; }
 }
 
 // scalar state edits ---------------------------------------------------------
 // mode 0: a <- a_value for every grid; mode 1: keep a (refresh the derived scale only)
-__global__ void k_set_a(Dev d, int mode, double a_value)
+__global__ void k_set_a(Dev d, int mode, double a_value, int zero_accepted)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= d.batch) return;
     GridState& s = d.states[g];
     if (mode == 0) s.a = a_value;
     s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F) / s.a);
+    if (zero_accepted) s.accepted = 0ull;
 }
-__global__ void k_advance_t(Dev d, uint32_t n, int set, int zero_accepted)
+// commit passes that ran with (t_off, flip) arguments: t += n_sweeps, swap buffers if the pass count was odd
+__global__ void k_commit(Dev d, uint32_t n_sweeps, uint32_t flip, uint32_t n_realizations)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= d.batch) return;
     GridState& s = d.states[g];
-    s.t = set ? n : s.t + n;
-    if (zero_accepted) s.accepted = 0ull;
+    s.t += n_sweeps; s.cur ^= flip; s.realizations += n_realizations;
+}
+__global__ void k_set_t(Dev d, uint32_t t)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g < d.batch) d.states[g].t = t;
 }
 __global__ void k_begin_run(Dev d, const float* __restrict__ T)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= d.batch) return;
     GridState& s = d.states[g];
-    s.t = 0; s.done = 0; s.i = 0; s.realizations = 0; s.accepted = 0ull;
+    s.t = 0; s.done = 0; s.cur = 0; s.i = 0; s.realizations = 0; s.accepted = 0ull;
     s.a = 1.0; s.k = -1.0; s.A_last = 0.0; s.e_last = 0.0;
     s.T = (double)T[g];
     s.neg_log2e_over_T = (float)(-1.4426950408889634 / (double)T[g]);
     s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F));
     d.done_flags[g] = 0;
-}
-
-// ---------------------------------------------------------------------------
-// a7  realization accumulation (Alg. 2 step 6, L207-211): acc += phi at the
-// prediction sites; the z-space back-transform is linear and applied once in
-// k_predict.  Also advances t by the sweeps of this realization.
-// ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_accumulate(Dev d, uint32_t t_advance, int first)
-{
-    const int g = blockIdx.y, colour = blockIdx.z;
-    const uint32_t o = blockIdx.x * blockDim.x + threadIdx.x;
-    GridState& s = d.states[g];
-    if (o < s.n_free[colour]) {
-        const size_t lo = ((size_t)g * 2 + colour) * d.LC + o;
-        const uint32_t li = d.lists[lo] & 0x7FFFFFFFu;
-        const float p = angle_of(d.vec[((size_t)g * 2 + colour) * d.VS + li], d.inv_q);
-        d.acc[lo] = first ? p : d.acc[lo] + p;
-    }
-    if (o == 0 && colour == 0) { s.t += t_advance; s.realizations = first ? 1u : s.realizations + 1u; }
 }
 
 // ---------------------------------------------------------------------------
@@ -632,10 +855,9 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, float* __restrict__ out)
     const uint32_t o = blockIdx.x * blockDim.x + threadIdx.x;
     const GridState& s = d.states[g];
     if (o >= s.n_free[colour]) return;
-    const size_t lo = ((size_t)g * 2 + colour) * d.LC + o;
-    const uint32_t idx = d.lists[lo], li = idx & 0x7FFFFFFFu, par = idx >> 31;
+    const uint32_t idx = d.lists[((size_t)g * 2 + colour) * d.LC + o], li = idx & 0x7FFFFFFFu, par = idx >> 31;
     const uint32_t r = li / d.Wp - 1u, col = 2u * (li - (r + 1u) * d.Wp - 1u) + par;
-    const double mean_phi = (double)d.acc[lo] / (double)s.realizations;
+    const double mean_phi = (double)d.acc[((size_t)g * 2 + colour) * d.VS + li] / (double)s.realizations;
     const double z = (double)s.zmin + mean_phi * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F;
     out[(size_t)g * d.N + (size_t)r * d.cols + col] = (float)z;
 }
@@ -648,7 +870,8 @@ __global__ void __launch_bounds__(256) k_export_angles(Dev d)
     if (o >= d.states[g].n_free[colour]) return;
     const uint32_t idx = d.lists[((size_t)g * 2 + colour) * d.LC + o], li = idx & 0x7FFFFFFFu, par = idx >> 31;
     const uint32_t r = li / d.Wp - 1u, col = 2u * (li - (r + 1u) * d.Wp - 1u) + par;
-    d.phi[(size_t)g * d.N + (size_t)r * d.cols + col] = angle_of(d.vec[((size_t)g * 2 + colour) * d.VS + li], d.inv_q);
+    const float2 v = cur_vec(d, g, d.states[g].cur)[(size_t)colour * d.VS + li];
+    d.phi[(size_t)g * d.N + (size_t)r * d.cols + col] = angle_of(v, d.inv_q);
 }
 __global__ void __launch_bounds__(256) k_import_angles(Dev d, const float* __restrict__ phi_in)
 {
@@ -664,7 +887,7 @@ __global__ void __launch_bounds__(256) k_import_angles(Dev d, const float* __res
     d.phi[n] = p;
     float sn, cs;
     sincosf(__fmul_rn(d.q, p), &sn, &cs);
-    d.vec[((size_t)g * 2 + colour) * d.VS + li] = make_float2(cs, sn);
+    cur_vec(d, g, d.states[g].cur)[(size_t)colour * d.VS + li] = make_float2(cs, sn);
 }
 
 }  // namespace mpr
