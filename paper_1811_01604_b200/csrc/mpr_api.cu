@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <cudaTypedefs.h>
 #include <new>
 
 using namespace mpr;
@@ -31,49 +32,49 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 struct Geometry {
-    uint32_t N, words, W, Wp, VS, LC;
+    uint32_t N, words, pitch;
+    size_t VG;
     int TR, TC, H, FR, FC, ntx, nty, ntiles;
     uint32_t n_partials;
     size_t entry_stride;
 };
 
 // Tile shape.  A grid that fits one frame is a single tile with a
-// one-site zero border (any number of sweeps per pass); otherwise TR x TC cores with a halo of H
-// (H/2 sweeps per pass).  MPR_TILE="TR,TC,H" overrides the default for experiments.
+// two-site zero border (any number of sweeps per pass); otherwise TR x TC cores with a halo of H
+// (H/2 sweeps per pass).  TC, H and FC are even so that every core row starts on a 16-byte boundary
+// of shared memory (bulk row copies).  MPR_TILE="TR,TC,H" overrides the default for experiments.
 void choose_tiles(int rows, int cols, Geometry* g)
 {
     int TR = 64, TC = 64, H = 8;
     if (const char* e = getenv("MPR_TILE")) {
         int a, b, c;
-        if (sscanf(e, "%d,%d,%d", &a, &b, &c) == 3 && a >= 8 && b >= 8 && c >= 2 && c <= MAX_H && (c & 1) == 0 &&
-            (a + 2 * c) * (b + 2 * c) <= 65536 && a + 2 * c <= 255) { TR = a; TC = b; H = c; }
+        if (sscanf(e, "%d,%d,%d", &a, &b, &c) == 3 && a >= 8 && b >= 8 && (b & 1) == 0 && c >= 2 && c <= MAX_H &&
+            (c & 1) == 0 && (a + 2 * c) * (b + 2 * c) <= 65536 && a + 2 * c <= 255 && b + 2 * c <= 256) { TR = a; TC = b; H = c; }
     }
-    if ((long)rows * cols <= 128L * 128L && rows <= 250 && cols <= 1024) { TR = rows; TC = cols; H = 1; }
-    g->TR = TR; g->TC = TC; g->H = H; g->FR = TR + 2 * H; g->FC = TC + 2 * H;
+    if ((long)rows * cols <= 128L * 128L && rows <= 250 && cols <= 250) { TR = rows; TC = cols; H = 2; }
+    g->TR = TR; g->TC = TC; g->H = H; g->FR = TR + 2 * H; g->FC = (TC + 2 * H + 1) & ~1;
     g->ntx = (cols + TC - 1) / TC; g->nty = (rows + TR - 1) / TR; g->ntiles = g->ntx * g->nty;
     g->n_partials = (uint32_t)(g->ntiles > ENERGY_BLOCKS ? g->ntiles : ENERGY_BLOCKS);
-    g->entry_stride = (size_t)g->ntiles * g->FR * g->FC;
+    g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 3) & ~(size_t)3);
 }
 
 bool make_geometry(int batch, int rows, int cols, Geometry* g)
 {
     if (batch < 1 || batch > 65535 || rows < 2 || cols < 2 || rows > 65534 || cols > 65534) return false;
     const uint64_t N = (uint64_t)rows * (uint64_t)cols;
-    const uint64_t W = ((uint64_t)cols + 1) / 2, Wp = (W + 2 + 1) & ~1ull;   // even pitch
-    const uint64_t VS = ((uint64_t)rows + 2) * Wp;
-    if (N >= (1ull << 31) || VS >= (1ull << 31)) return false;
+    const uint64_t pitch = ((uint64_t)cols + 1) & ~1ull;                      // even: rows start 16-byte aligned
+    if (N >= (1ull << 31) || (uint64_t)rows * pitch >= (1ull << 31)) return false;
     g->N = (uint32_t)N; g->words = (uint32_t)((N + 31) / 32);
-    g->W = (uint32_t)W; g->Wp = (uint32_t)Wp; g->VS = (uint32_t)VS;
-    g->LC = (uint32_t)((((N + 1) / 2 + 1) & ~1ull) + 2);                       // even, >= max count + 2
+    g->pitch = (uint32_t)pitch; g->VG = (size_t)rows * pitch;
     choose_tiles(rows, cols, g);
     return g->entry_stride < (1ull << 32);
 }
 
 struct Layout {
-    size_t states, done, partials, values, phi, bits, vec, lists, acc, rowstart, tile_meta, entries, total;
+    size_t states, done, partials, values, phi, bits, vec, acc, tile_meta, entries, total;
 };
 
-Layout make_layout(int batch, int rows, const Geometry& g)
+Layout make_layout(int batch, const Geometry& g)
 {
     Layout L;
     size_t o = 0;
@@ -85,12 +86,10 @@ Layout make_layout(int batch, int rows, const Geometry& g)
     L.values    = take(B * g.N * sizeof(float));
     L.phi       = take(B * g.N * sizeof(float));
     L.bits      = take(B * g.words * sizeof(uint32_t));
-    L.vec       = take(2 * B * 2 * g.VS * sizeof(float2));
-    L.lists     = take(B * 2 * g.LC * sizeof(uint32_t));
-    L.acc       = take(B * 2 * g.VS * sizeof(float));
-    L.rowstart  = take(B * 2 * ((size_t)rows + 1) * sizeof(uint32_t));
+    L.vec       = take(2 * B * g.VG * sizeof(float2));
+    L.acc       = take(B * g.N * sizeof(float));
     L.tile_meta = take(B * g.ntiles * sizeof(TileMeta));
-    L.entries   = take(B * g.entry_stride * sizeof(uint32_t));
+    L.entries   = take((B * g.entry_stride + 4) * sizeof(uint32_t));
     L.total = o;
     return L;
 }
@@ -100,12 +99,12 @@ enum RunState { CREATED = 0, READY = 1 };
 }  // namespace
 
 struct mpr_ctx {
+    alignas(64) CUtensorMap map[2];   // frame boxes of the two vector buffers (TMA descriptors)
     Dev          d;
     Layout       lay;
     cudaStream_t stream;
     mpr_params   prm;
     RunState     state;
-    uint32_t     max_free[2];     // max over grids of the free count per colour
     int          energy_blocks;
     uint32_t     k_max;           // sweeps per tile pass
     size_t       smem_bytes;      // dynamic shared memory of k_tilepass
@@ -126,20 +125,27 @@ mpr_status fetch_states(mpr_ctx* ctx)
     return MPR_OK;
 }
 
-typedef void (*pass_kernel)(Dev, uint32_t, uint32_t, uint32_t, uint32_t);
+typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t);
 
-pass_kernel pick_pass_kernel(bool qhalf, int or_mode)
+// fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps)
+pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused)
 {
-    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0> : or_mode == 1 ? k_tilepass<true, 1> : k_tilepass<true, 2>;
-    return or_mode == 0 ? k_tilepass<false, 0> : k_tilepass<false, 2>;
+    if (fused) {
+        if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true> : or_mode == 1 ? k_tilepass<true, 1, true> : k_tilepass<true, 2, true>;
+        return or_mode == 0 ? k_tilepass<false, 0, true> : k_tilepass<false, 2, true>;
+    }
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, false> : or_mode == 1 ? k_tilepass<true, 1, false> : k_tilepass<true, 2, false>;
+    return or_mode == 0 ? k_tilepass<false, 0, false> : k_tilepass<false, 2, false>;
 }
 
 // K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile
 mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
 {
     ctx->dirty = true;
-    pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode)
-        <<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(ctx->d, K, t_off, flip, flags);
+    const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
+    pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused)
+        <<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(
+            ctx->map[0], ctx->map[1], ctx->d, K, t_off, flip, flags);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -156,6 +162,36 @@ mpr_status launch_sweeps(mpr_ctx* ctx, uint32_t n, uint32_t* t_off, uint32_t* fl
     return MPR_OK;
 }
 
+// TMA descriptor of one vector buffer: [batch][rows][cols] eight-byte elements with row pitch d.pitch,
+// box = one tile frame; elements outside the grid are delivered as zeros (open boundary)
+mpr_status make_frame_map(mpr_ctx* ctx, int which)
+{
+    static PFN_cuTensorMapEncodeTiled encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (!cuda_ok(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres), "cudaGetDriverEntryPoint") ||
+            qres != cudaDriverEntryPointSuccess || !fn) {
+            snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled not available in this driver");
+            return MPR_ERR_CUDA;
+        }
+        encode = (PFN_cuTensorMapEncodeTiled)fn;
+    }
+    const Dev& d = ctx->d;
+    const cuuint64_t dims[3] = {(cuuint64_t)d.cols, (cuuint64_t)d.rows, (cuuint64_t)d.batch};
+    const cuuint64_t strides[2] = {(cuuint64_t)d.pitch * sizeof(float2), (cuuint64_t)d.VG * sizeof(float2)};
+    const cuuint32_t box[3] = {(cuuint32_t)d.FC, (cuuint32_t)d.FR, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = encode(&ctx->map[which], CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, (void*)(d.vec + (size_t)which * d.VB),
+                              dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        return MPR_ERR_CUDA;
+    }
+    return MPR_OK;
+}
+
 mpr_status launch_energy(mpr_ctx* ctx)
 {
     k_energy<<<dim3(ctx->energy_blocks, ctx->d.batch), ENERGY_THREADS, 0, ctx->stream>>>(ctx->d);
@@ -163,11 +199,7 @@ mpr_status launch_energy(mpr_ctx* ctx)
     return MPR_OK;
 }
 
-dim3 list_grid(const mpr_ctx* ctx)
-{
-    const uint32_t m = ctx->max_free[0] > ctx->max_free[1] ? ctx->max_free[0] : ctx->max_free[1];
-    return dim3(cdiv(m ? m : 1, 256), ctx->d.batch, 2);
-}
+dim3 site_grid(const mpr_ctx* ctx) { return dim3(cdiv(ctx->d.N, 256), ctx->d.batch); }
 
 }  // namespace
 
@@ -206,7 +238,7 @@ mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* bytes)
 {
     Geometry g;
     if (!bytes || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
-    *bytes = make_layout(batch, rows, g).total;
+    *bytes = make_layout(batch, g).total;
     return MPR_OK;
 }
 
@@ -215,7 +247,7 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
 {
     Geometry g;
     if (!out || !d_values || !d_sample_mask || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
-    const Layout lay = make_layout(batch, rows, g);
+    const Layout lay = make_layout(batch, g);
     if (!d_workspace || workspace_bytes < lay.total || ((uintptr_t)d_workspace & 255u)) return MPR_ERR_WORKSPACE;
 
     mpr_ctx* ctx = new (std::nothrow) mpr_ctx();
@@ -240,16 +272,14 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     d.phi = (float*)(base + lay.phi);
     d.bits = (uint32_t*)(base + lay.bits);
     d.vec = (float2*)(base + lay.vec);
-    d.lists = (uint32_t*)(base + lay.lists);
     d.acc = (float*)(base + lay.acc);
-    d.rowstart = (uint32_t*)(base + lay.rowstart);
     d.tile_meta = (TileMeta*)(base + lay.tile_meta);
     d.entries = (uint32_t*)(base + lay.entries);
-    d.VB = (size_t)batch * 2 * g.VS;
+    d.VG = g.VG; d.VB = (size_t)batch * g.VG;
     d.entry_stride = g.entry_stride; d.n_partials = g.n_partials;
     d.TR = g.TR; d.TC = g.TC; d.H = g.H; d.FR = g.FR; d.FC = g.FC; d.ntx = g.ntx; d.nty = g.nty; d.ntiles = g.ntiles;
     d.batch = batch; d.rows = rows; d.cols = cols;
-    d.N = g.N; d.words = g.words; d.W = g.W; d.Wp = g.Wp; d.VS = g.VS; d.LC = g.LC;
+    d.N = g.N; d.words = g.words; d.pitch = g.pitch;
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
     ctx->energy_blocks = rows < ENERGY_BLOCKS ? rows : ENERGY_BLOCKS;
     ctx->h_states = new (std::nothrow) GridState[batch];
@@ -259,21 +289,19 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     if (!cuda_ok(cudaMallocHost((void**)&ctx->h_pinned, sizeof(uint32_t) * batch), "cudaMallocHost")) return fail(MPR_ERR_CUDA);
 
     cudaStream_t s = ctx->stream;
-    // zero pads of the vector arrays = open boundary
+    // the pad column of an odd-width grid stays zero
     if (!cuda_ok(cudaMemsetAsync(d.vec, 0, 2 * d.VB * sizeof(float2), s), "memset vec")) return fail(MPR_ERR_CUDA);
+    for (int w = 0; w < 2; ++w) { st = make_frame_map(ctx, w); if (st != MPR_OK) return fail(st); }
     k_state_reset<<<cdiv(batch, 128), 128, 0, s>>>(d);
     unsigned mm_blocks = cdiv(g.N, 256 * 8);
     if (mm_blocks > 1184) mm_blocks = 1184;
     k_minmax<<<dim3(mm_blocks, batch), 256, 0, s>>>(d, d_values, d_sample_mask);
     k_minmax_finish<<<cdiv(batch, 128), 128, 0, s>>>(d);
     k_transform<<<dim3(cdiv((size_t)g.words * 32, 256), batch), 256, 0, s>>>(d, d_values, d_sample_mask);
-    k_rowcount<<<dim3(cdiv((size_t)rows * 32, 256), batch), 256, 0, s>>>(d);
-    k_rowscan<<<dim3(batch, 2), 32, 0, s>>>(d);
-    k_build_lists<<<dim3(cdiv((size_t)rows * 32, 256), batch), 256, 0, s>>>(d);
     k_tile_count<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
     k_tile_scan<<<batch, 32, 0, s>>>(d);
     k_tile_fill<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
-    ctx->launches += 10;
+    ctx->launches += 7;
     if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
     st = fetch_states(ctx);
     if (st != MPR_OK) return fail(st);
@@ -283,14 +311,12 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
         if (e & ERRF_NONFINITE) return fail(MPR_ERR_NONFINITE);
         if (e & ERRF_DEGENERATE) return fail(MPR_ERR_DEGENERATE_RANGE);
         if (e & ERRF_NO_FREE) return fail(MPR_ERR_NO_FREE);
-        for (int c = 0; c < 2; ++c)
-            if (ctx->h_states[b].n_free[c] > ctx->max_free[c]) ctx->max_free[c] = ctx->h_states[b].n_free[c];
     }
     // shared memory of the tile pass: frame + entries (+ the odd sweeps' random words when they fit)
     uint32_t max_entries = 0;
     for (int b = 0; b < batch; ++b)
         if (ctx->h_states[b].max_tile_entries > max_entries) max_entries = ctx->h_states[b].max_tile_entries;
-    max_entries = (max_entries + 1u) & ~1u;
+    max_entries = (max_entries + 3u) & ~3u;
     d.max_entries = max_entries;
     const size_t frame_bytes = (size_t)g.FR * g.FC * sizeof(float2);
     int smem_max = 0;
@@ -306,11 +332,12 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
         if (k >= 1 && (g.ntiles == 1 || k <= g.H / 2)) ctx->k_max = (uint32_t)k;
     }
     for (int qh = 0; qh < 2; ++qh)
-        for (int om = 0; om < 3; ++om) {
-            if (!qh && om == 1) continue;
-            if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
-        }
+        for (int om = 0; om < 3; ++om)
+            for (int fu = 0; fu < 2; ++fu) {
+                if (!qh && om == 1) continue;
+                if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                  (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
+            }
     *out = ctx;
     return MPR_OK;
 }
@@ -338,7 +365,10 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     ctx->prm = *p;
     ctx->qhalf = p->q == 0.5f;
     Dev& d = ctx->d;
-    d.key0 = (uint32_t)p->seed; d.key1 = (uint32_t)(p->seed >> 32);
+    for (int r = 0; r < PHILOX_ROUNDS; ++r) {          // Philox4x32 key schedule (Weyl sequence)
+        d.rk0[r] = (uint32_t)p->seed + (uint32_t)r * 0x9E3779B9u;
+        d.rk1[r] = (uint32_t)(p->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
     d.q = p->q; d.inv_q = 1.0f / p->q;
     d.bc = (float)cos((double)p->q * (double)TWO_PI_F); d.bs = (float)sin((double)p->q * (double)TWO_PI_F);
     d.n_f = p->n_f; d.n_fit = p->n_fit; d.equil_cap = p->equil_cap;
@@ -347,7 +377,7 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     CU(cudaMemcpyAsync(d.e_partials, h_T, sizeof(float) * d.batch, cudaMemcpyHostToDevice, ctx->stream));
     k_begin_run<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, (const float*)d.e_partials);
     CU_LAUNCH();
-    CU(cudaMemsetAsync(d.acc, 0, (size_t)d.batch * 2 * d.VS * sizeof(float), ctx->stream));
+    CU(cudaMemsetAsync(d.acc, 0, (size_t)d.batch * d.N * sizeof(float), ctx->stream));
     k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d);
     CU_LAUNCH();
     CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
@@ -413,8 +443,7 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out)
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
-    CU(cudaMemcpyAsync(d_out, d.values, sizeof(float) * (size_t)d.N * d.batch, cudaMemcpyDeviceToDevice, ctx->stream));
-    k_predict<<<list_grid(ctx), 256, 0, ctx->stream>>>(d, d_out);
+    k_predict<<<site_grid(ctx), 256, 0, ctx->stream>>>(d, d_out);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -426,7 +455,7 @@ mpr_status mpr_get_angles(mpr_ctx* ctx, float* d_phi)
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
     if (ctx->dirty) {        // otherwise d.phi already holds the state exactly (initial draw or import)
-        k_export_angles<<<list_grid(ctx), 256, 0, ctx->stream>>>(d);
+        k_export_angles<<<site_grid(ctx), 256, 0, ctx->stream>>>(d);
         CU_LAUNCH();
         ctx->dirty = false;
     }
@@ -439,7 +468,7 @@ mpr_status mpr_set_angles(mpr_ctx* ctx, const float* d_phi)
     if (!ctx || !d_phi) return MPR_ERR_ARG;
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
-    k_import_angles<<<list_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, d_phi);
+    k_import_angles<<<site_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, d_phi);
     CU_LAUNCH();
     ctx->dirty = false;
     return MPR_OK;

@@ -12,17 +12,18 @@
 // itself (realization accumulation, export).
 #pragma once
 #include <cstdint>
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 namespace mpr {
 
-constexpr float    TWO_PI_F      = 6.28318530717958647692f;  // float nearest 2 pi; state space [0, TWO_PI_F]
-constexpr int      MAX_NFIT      = 256;
-constexpr uint32_t LIST_SENTINEL = 0xFFFFFFFFu;
-constexpr int      TILE_THREADS  = 512;
-constexpr int      MAX_H         = 16;                       // largest halo: up to 8 sweeps per tile pass
-constexpr int      ENERGY_BLOCKS = 592;                      // 4 x 148 SMs; fixed so the sum order is deterministic
+constexpr float    TWO_PI_F       = 6.28318530717958647692f;  // float nearest 2 pi; state space [0, TWO_PI_F]
+constexpr int      MAX_NFIT       = 256;
+constexpr int      TILE_THREADS   = 256;                      // threads of a tile pass CTA
+constexpr int      MAX_H          = 16;                       // largest halo: up to 8 sweeps per tile pass
+constexpr int      ENERGY_BLOCKS  = 592;                      // 4 x 148 SMs; fixed so the sum order is deterministic
 constexpr int      ENERGY_THREADS = 256;
+constexpr int      PHILOX_ROUNDS  = 10;
 
 enum : uint32_t { ERRF_NO_SAMPLES = 1u, ERRF_NO_FREE = 2u, ERRF_DEGENERATE = 4u, ERRF_NONFINITE = 8u };
 // k_tilepass flags
@@ -54,7 +55,7 @@ struct GridState {
 
 // Free sites of one tile frame (core + halo), see k_tile_fill.
 struct TileMeta {
-    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid)
+    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid), multiple of 4
     uint32_t cge[2][MAX_H + 1];       // cge[c][k] = entries of colour c with ring >= k (ring = distance outside the core)
 };
 
@@ -66,22 +67,21 @@ struct Dev {
     float*     values;         // [batch][N] verbatim copy of the input values
     float*     phi;            // [batch][N] angle view: Eq. 1 at sample sites (never rewritten), export buffer at free sites
     uint32_t*  bits;           // [batch][words] fixed-site bitmask
-    float2*    vec;            // [2 buffers][batch][2 colours][VS] colour-split padded unit vectors; pad = (0,0)
-    uint32_t*  lists;          // [batch][2][LC] padded index | parity<<31 of the free sites, row-major order
-    float*     acc;            // [batch][2][VS] sum over realizations of phi at free sites (same index as vec)
-    uint32_t*  rowstart;       // [batch][2][rows+1] ordinal of the first free site of each row
+    float2*    vec;            // [2 buffers][batch][rows][pitch] row-major unit vectors (pitch = cols rounded up to even)
+    float*     acc;            // [batch][N] sum over realizations of phi at the prediction sites
     TileMeta*  tile_meta;      // [batch][ntiles]
-    uint32_t*  entries;        // [batch][entry_stride] tile frames' free sites: off | local row << 16
+    uint32_t*  entries;        // [batch][entry_stride] tile frames' free sites: frame offset | frame row << 16
     int        batch, rows, cols;
-    uint32_t   N, words, W, Wp, VS, LC;
-    size_t     VB;             // float2 elements per vector buffer = batch * 2 * VS
+    uint32_t   N, words, pitch;
+    size_t     VG;             // float2 elements of one grid in one buffer = rows * pitch
+    size_t     VB;             // float2 elements per vector buffer = batch * VG
     size_t     entry_stride;
     uint32_t   n_partials;
     // tiling
     int        TR, TC, H, FR, FC, ntx, nty, ntiles;
-    uint32_t   max_entries;    // smem capacity for entries (even)
+    uint32_t   max_entries;    // shared-memory capacity for entries (multiple of 4)
     int        use_spare;      // keep the odd sweep's random words in shared memory
-    uint32_t   key0, key1;     // Philox key = (seed lo, seed hi)
+    uint32_t   rk0[PHILOX_ROUNDS], rk1[PHILOX_ROUNDS];   // Philox round keys: (seed lo, seed hi) + r * Weyl constants
     float      q, inv_q;
     float      bc, bs;         // (cos 2 pi q, sin 2 pi q): upper end of the q*phi range
     // Alg. 2 controller constants
@@ -89,47 +89,45 @@ struct Dev {
     double     A_targ, k_a, n_bonds;
 };
 
-__device__ __forceinline__ float2* cur_vec(const Dev& d, int g, uint32_t which)
+__device__ __forceinline__ float2* vec_grid(const Dev& d, int g, uint32_t which)
 {
-    return d.vec + (size_t)which * d.VB + (size_t)g * 2 * d.VS;
+    return d.vec + (size_t)which * d.VB + (size_t)g * d.VG;
 }
 
 // ---------------------------------------------------------------------------
 // Philox4x32-10 (Salmon et al., SC'11), the generator PAPER.md L267 names.
+// The ten round keys are precomputed on the host (Dev::rk0 / rk1).
 // ---------------------------------------------------------------------------
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                               uint32_t k0, uint32_t k1)
+                                               const uint32_t (&rk0)[PHILOX_ROUNDS], const uint32_t (&rk1)[PHILOX_ROUNDS])
 {
 #pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        const uint32_t n0 = hi1 ^ c1 ^ k0;
-        const uint32_t n2 = hi0 ^ c3 ^ k1;
-        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    for (int r = 0; r < PHILOX_ROUNDS; ++r) {
+        const uint64_t p0 = (uint64_t)c0 * 0xD2511F53u;     // IMAD.WIDE: hi and lo in one instruction
+        const uint64_t p1 = (uint64_t)c2 * 0xCD9E8D57u;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk1[r];
+        c0 = n0; c1 = (uint32_t)p1; c2 = n2; c3 = (uint32_t)p0;
     }
     return make_uint4(c0, c1, c2, c3);
 }
 
 // Uniform u = (2 (x >> 9) + 1) 2^-24 in (0,1) (R13), built without
 // an integer->float conversion: f = 1.m in [1,2) with m = x >> 9, so
-// u = (f - 1) + 2^-24 and u - 1/2 = (f - 1.5) + 2^-24, every step exact.
-__device__ __forceinline__ float u01(uint32_t x)
-{
-    const float f = __uint_as_float(0x3F800000u | (x >> 9));
-    return __fadd_rn(__fadd_rn(f, -1.0f), 5.9604644775390625e-08f);
-}
-__device__ __forceinline__ float u01_centered(uint32_t x)
-{
-    const float f = __uint_as_float(0x3F800000u | (x >> 9));
-    return __fadd_rn(__fadd_rn(f, -1.5f), 5.9604644775390625e-08f);
-}
+// u = f - (1 - 2^-24), exact in one subtraction ((2m+1) 2^-24 has 24 bits).
+__device__ __forceinline__ float one_plus_m(uint32_t x) { return __uint_as_float(0x3F800000u | (x >> 9)); }
+__device__ __forceinline__ float u01(uint32_t x) { return __fadd_rn(one_plus_m(x), -0.99999994039535522461f); }
 
 __device__ __forceinline__ float ex2_approx(float x)
 {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
@@ -178,10 +176,9 @@ __device__ __forceinline__ float angle_of(float2 v, float inv_q)
     return p;
 }
 
-// padded colour-split index of site (r, col): colour = (r+col)&1, slot (r+1)*Wp + (col>>1) + 1
-__device__ __forceinline__ uint32_t padded_index(uint32_t r, uint32_t col, uint32_t Wp)
+__device__ __forceinline__ bool is_fixed(const uint32_t* __restrict__ bits, uint32_t n)
 {
-    return (r + 1u) * Wp + (col >> 1) + 1u;
+    return (bits[n >> 5] >> (n & 31)) & 1u;
 }
 
 // ---------------------------------------------------------------------------
@@ -251,7 +248,8 @@ __global__ void k_minmax_finish(Dev d)
 }
 
 // ---------------------------------------------------------------------------
-// a2  Eq. 1 at the sample sites, fixed-site bitmask, verbatim value copy
+// a2  Eq. 1 at the sample sites, fixed-site bitmask, verbatim value copy,
+// prediction-site count per checkerboard colour
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restrict__ values,
                                                    const uint8_t* __restrict__ mask)
@@ -261,98 +259,23 @@ __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restric
     const GridState& s = d.states[g];
     const bool in = n < d.N;
     bool fixed = false;
+    uint32_t colour = 0;
     if (in) {
         const size_t o = (size_t)g * d.N + n;
         const float z = values[o];
         fixed = mask[o] != 0;
         d.values[o] = z;
         d.phi[o] = fixed ? eq1(z, s.zmin, s.zmax) : 0.0f;
+        const uint32_t r = n / d.cols;
+        colour = (r + (n - r * d.cols)) & 1u;
     }
     const uint32_t b = __ballot_sync(0xFFFFFFFFu, fixed);
-    if ((threadIdx.x & 31) == 0 && (n >> 5) < d.words) d.bits[(size_t)g * d.words + (n >> 5)] = b;
-}
-
-// ---------------------------------------------------------------------------
-// a2  checkerboard-split lists of the prediction sites: for
-// each colour, the free sites in row-major order; the position in the list is
-// the site's ordinal o, which keys its random numbers (R13).
-// ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_rowcount(Dev d)
-{
-    const int g = blockIdx.y;
-    const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const uint32_t lane = threadIdx.x & 31;
-    if (r >= (uint32_t)d.rows) return;
-    const uint32_t* bits = d.bits + (size_t)g * d.words;
-    uint32_t cnt0 = 0, cnt1 = 0;
-    for (uint32_t col = lane; col < (uint32_t)d.cols; col += 32) {
-        const uint32_t n = r * d.cols + col;
-        const bool free_ = !((bits[n >> 5] >> (n & 31)) & 1u);
-        const uint32_t colour = (r + col) & 1u;
-        cnt0 += free_ && colour == 0;
-        cnt1 += free_ && colour == 1;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        cnt0 += __shfl_xor_sync(0xFFFFFFFFu, cnt0, o);
-        cnt1 += __shfl_xor_sync(0xFFFFFFFFu, cnt1, o);
-    }
-    if (lane == 0) {
-        d.rowstart[((size_t)g * 2 + 0) * (d.rows + 1) + r] = cnt0;
-        d.rowstart[((size_t)g * 2 + 1) * (d.rows + 1) + r] = cnt1;
-    }
-}
-
-// one warp per (grid, colour): exclusive scan of the row counts in place
-__global__ void k_rowscan(Dev d)
-{
-    const int g = blockIdx.x, colour = blockIdx.y;
-    const uint32_t lane = threadIdx.x;
-    uint32_t* rs = d.rowstart + ((size_t)g * 2 + colour) * (d.rows + 1);
-    uint32_t carry = 0;
-    for (uint32_t base = 0; base < (uint32_t)d.rows; base += 32) {
-        const uint32_t r = base + lane;
-        const uint32_t c = r < (uint32_t)d.rows ? rs[r] : 0u;
-        uint32_t x = c;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, o);
-            if (lane >= (uint32_t)o) x += y;
-        }
-        if (r < (uint32_t)d.rows) rs[r] = carry + x - c;
-        carry += __shfl_sync(0xFFFFFFFFu, x, 31);
-    }
-    if (lane == 0) {
-        rs[d.rows] = carry;
-        d.states[g].n_free[colour] = carry;
-        uint32_t* list = d.lists + ((size_t)g * 2 + colour) * d.LC;
-        list[carry] = LIST_SENTINEL;            // pads an odd count to a whole pair
-        list[carry + 1] = LIST_SENTINEL;
-    }
-}
-
-__global__ void __launch_bounds__(256) k_build_lists(Dev d)
-{
-    const int g = blockIdx.y;
-    const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const uint32_t lane = threadIdx.x & 31;
-    if (r >= (uint32_t)d.rows) return;
-    const uint32_t* bits = d.bits + (size_t)g * d.words;
-    for (uint32_t colour = 0; colour < 2; ++colour) {
-        const uint32_t par = (r + colour) & 1u;                         // parity of this colour's columns in row r
-        uint32_t pos = d.rowstart[((size_t)g * 2 + colour) * (d.rows + 1) + r];
-        uint32_t* list = d.lists + ((size_t)g * 2 + colour) * d.LC;
-        for (uint32_t j0 = 0; j0 < d.W; j0 += 32) {
-            const uint32_t j = j0 + lane, col = 2u * j + par;
-            bool free_ = false;
-            if (col < (uint32_t)d.cols) {
-                const uint32_t n = r * d.cols + col;
-                free_ = !((bits[n >> 5] >> (n & 31)) & 1u);
-            }
-            const uint32_t b = __ballot_sync(0xFFFFFFFFu, free_);
-            if (free_) list[pos + __popc(b & ((1u << lane) - 1u))] = padded_index(r, col, d.Wp) | (par << 31);
-            pos += __popc(b);
-        }
+    const uint32_t f0 = __ballot_sync(0xFFFFFFFFu, in && !fixed && colour == 0);
+    const uint32_t f1 = __ballot_sync(0xFFFFFFFFu, in && !fixed && colour == 1);
+    if ((threadIdx.x & 31) == 0 && (n >> 5) < d.words) {
+        d.bits[(size_t)g * d.words + (n >> 5)] = b;
+        if (f0) atomicAdd(&d.states[g].n_free[0], (uint32_t)__popc(f0));
+        if (f1) atomicAdd(&d.states[g].n_free[1], (uint32_t)__popc(f1));
     }
 }
 
@@ -360,8 +283,14 @@ __global__ void __launch_bounds__(256) k_build_lists(Dev d)
 // a2  tile frames.  The grid is cut into TR x TC core tiles; a tile's frame is
 // its core plus a halo of H sites on every side.  For each tile the free
 // sites of the frame with ring < H (ring = Chebyshev distance outside the
-// core, 0 inside) are listed per colour, outermost ring first, so that the
-// sites a half-sweep of a K-sweep pass still needs are a suffix of the list.
+// core, 0 inside) are listed per colour (checkerboard split),
+// outermost ring first, so that the sites a half-sweep of a K-sweep pass
+// still needs are a suffix of the list.  Within one (colour, ring) class the
+// entries are dealt round-robin over the 16 eight-byte slots of a 128-byte
+// shared-memory line, so that 16 consecutive entries (one half-warp of a
+// 64-bit shared load) hit 16 different bank pairs: the loads of a site, of
+// its four neighbours (the same shift for every lane) and the store are then
+// free of bank conflicts.
 // ---------------------------------------------------------------------------
 struct TileGeom { int r0, c0, TRc, TCc; };
 
@@ -380,8 +309,7 @@ __device__ __forceinline__ bool frame_site_class(const Dev& d, const uint32_t* _
 {
     const int r = t.r0 - d.H + lr, col = t.c0 - d.H + lc;
     if (r < 0 || r >= d.rows || col < 0 || col >= d.cols) return false;
-    const uint32_t n = (uint32_t)r * d.cols + col;
-    if ((bits[n >> 5] >> (n & 31)) & 1u) return false;
+    if (is_fixed(bits, (uint32_t)r * d.cols + col)) return false;
     const int dr = max(max(d.H - lr, lr - (d.H + t.TRc - 1)), 0);
     const int dc = max(max(d.H - lc, lc - (d.H + t.TCc - 1)), 0);
     ring = max(dr, dc);
@@ -411,7 +339,8 @@ __global__ void __launch_bounds__(256) k_tile_count(Dev d)
     }
 }
 
-// one warp per grid: exclusive scan of the tiles' entry counts, and their maximum
+// one warp per grid: exclusive scan of the tiles' entry counts (each rounded up to a multiple of 4
+// so that every tile's list starts on a 16-byte boundary), and their maximum
 __global__ void k_tile_scan(Dev d)
 {
     const int g = blockIdx.x;
@@ -420,7 +349,7 @@ __global__ void k_tile_scan(Dev d)
     uint32_t carry = 0, mx = 0;
     for (int base = 0; base < d.ntiles; base += 32) {
         const int i = base + lane;
-        const uint32_t c = i < d.ntiles ? m[i].cge[0][0] + m[i].cge[1][0] : 0u;
+        const uint32_t c = i < d.ntiles ? (m[i].cge[0][0] + m[i].cge[1][0] + 3u) & ~3u : 0u;
         mx = max(mx, c);
         uint32_t x = c;
 #pragma unroll
@@ -439,8 +368,9 @@ __global__ void k_tile_scan(Dev d)
 __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
 {
     const int tile = blockIdx.x, g = blockIdx.y;
-    __shared__ uint32_t cursor[2][MAX_H + 1];
-    for (int i = threadIdx.x; i < 2 * (MAX_H + 1); i += blockDim.x) (&cursor[0][0])[i] = 0;
+    __shared__ uint32_t cnt[2][MAX_H][16];       // free sites per (colour, ring, slot)
+    __shared__ uint32_t cursor[2][MAX_H][16];
+    for (int i = threadIdx.x; i < 2 * MAX_H * 16; i += blockDim.x) { (&cnt[0][0][0])[i] = 0; (&cursor[0][0][0])[i] = 0; }
     __syncthreads();
     const TileGeom t = tile_geom(d, tile);
     const TileMeta& m = d.tile_meta[(size_t)g * d.ntiles + tile];
@@ -449,9 +379,23 @@ __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
     for (int i = threadIdx.x; i < d.FR * d.FC; i += blockDim.x) {
         const int lr = i / d.FC, lc = i - lr * d.FC;
         int colour, ring;
+        if (frame_site_class(d, bits, t, lr, lc, colour, ring)) atomicAdd(&cnt[colour][ring][i & 15], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < d.FR * d.FC; i += blockDim.x) {
+        const int lr = i / d.FC, lc = i - lr * d.FC;
+        int colour, ring;
         if (frame_site_class(d, bits, t, lr, lc, colour, ring)) {
+            const uint32_t b = i & 15, j = atomicAdd(&cursor[colour][ring][b], 1u);
+            // rank of (round j, slot b) when the class is dealt round-robin over its 16 slots
+            uint32_t pos = 0;
+#pragma unroll
+            for (uint32_t bb = 0; bb < 16; ++bb) {
+                const uint32_t c = cnt[colour][ring][bb];
+                pos += min(c, j) + (bb < b && c > j ? 1u : 0u);
+            }
             // colour 0 first; within a colour the rings in descending order
-            const uint32_t pos = (colour ? m.cge[0][0] : 0u) + m.cge[colour][ring + 1] + atomicAdd(&cursor[colour][ring], 1u);
+            pos += (colour ? m.cge[0][0] : 0u) + m.cge[colour][ring + 1];
             out[pos] = (uint32_t)i | ((uint32_t)lr << 16);
         }
     }
@@ -468,11 +412,10 @@ __global__ void __launch_bounds__(256) k_init_state(Dev d)
     const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= d.N) return;
     const size_t o = (size_t)g * d.N + n;
-    const bool fixed = (d.bits[(size_t)g * d.words + (n >> 5)] >> (n & 31)) & 1u;
     float p;
-    if (fixed) p = d.phi[o];
+    if (is_fixed(d.bits + (size_t)g * d.words, n)) p = d.phi[o];
     else {
-        const uint4 x = philox4x32_10(n >> 2, 0u, 0u, (uint32_t)g, d.key0, d.key1);
+        const uint4 x = philox4x32_10(n >> 2, 0u, 0u, (uint32_t)g, d.rk0, d.rk1);
         const uint32_t w = (n & 3u) == 0 ? x.x : (n & 3u) == 1 ? x.y : (n & 3u) == 2 ? x.z : x.w;
         p = __fmul_rn(TWO_PI_F, u01(w));
         d.phi[o] = p;
@@ -480,26 +423,29 @@ __global__ void __launch_bounds__(256) k_init_state(Dev d)
     const uint32_t r = n / d.cols, col = n - r * d.cols;
     float sn, cs;
     sincosf(__fmul_rn(d.q, p), &sn, &cs);
-    const size_t at = (size_t)((r + col) & 1u) * d.VS + padded_index(r, col, d.Wp);
-    cur_vec(d, g, 0)[at] = make_float2(cs, sn);
-    cur_vec(d, g, 1)[at] = make_float2(cs, sn);
+    const size_t at = (size_t)r * d.pitch + col;
+    vec_grid(d, g, 0)[at] = make_float2(cs, sn);
+    vec_grid(d, g, 1)[at] = make_float2(cs, sn);
 }
 
 // ---------------------------------------------------------------------------
 // a3  UPDATE of one prediction site (Alg. 1) in vector form.
 // v = (cos q phi, sin q phi); (hx, hy) = (C, S) = sum over the neighbours.
+// w0, w1: the two random words of this site and sweep (R13).
 // ---------------------------------------------------------------------------
 template <bool QHALF, int ORMODE>
-__device__ __forceinline__ float2 update_site(float2 v, float hx, float hy, float2 n_up, float2 n_dn, float2 n_lf,
-                                              float2 n_rt, float uc, float r, float hd_scale, float nlT,
-                                              float bc, float bs, bool renorm, uint32_t& accepted)
+__device__ __forceinline__ float2 update_site(float2 v, float2 n_up, float2 n_dn, float2 n_lf, float2 n_rt,
+                                              uint32_t w0, uint32_t w1, float hd_scale, float hd_c1, float nlT,
+                                              float bc, float bs, bool& accepted)
 {
+    const float hx = (n_up.x + n_dn.x) + (n_lf.x + n_rt.x), hy = (n_up.y + n_dn.y) + (n_lf.y + n_rt.y);
     float px = v.x, py = v.y;
     // Alg. 1 line 1: over-relaxation.  Reflect v about h: q phi' = 2 Theta - q phi keeps h.v,
     // i.e. the local energy (L156, L265; R2).  Out of [0, 2 pi]: keep the spin.
     if (ORMODE == 0) {
         const float R2 = fmaf(hx, hx, hy * hy);
-        const float k = __fdividef(2.0f * fmaf(px, hx, py * hy), R2);   // 0/0 -> NaN -> kept below
+        const float dot = fmaf(px, hx, py * hy);
+        const float k = (dot + dot) * rcp_approx(R2);                    // 0 * inf -> NaN -> kept below
         const float fx = fmaf(k, hx, -px), fy = fmaf(k, hy, -py);
         // Theta = atan2(S, C) < 0 when S < 0 (only through sin(q * TWO_PI_F) = -8.7e-8 of a sample at the
         // data maximum, with the other neighbours cancelling): then q phi' = 2 Theta - q phi < 0, out of range (R17)
@@ -519,13 +465,15 @@ __device__ __forceinline__ float2 update_site(float2 v, float hx, float hy, floa
         if (fy < 0.0f) { fx = -fx; fy = -fy; }
         px = fx; py = fy;
     }
-    // lines 2-3: phi'' = phi' + 2 pi (u - 1/2)/a (mod 2 pi): rotate by d = q delta = 2 hd
-    const float hd = uc * hd_scale;
+    // lines 2-3: phi'' = phi' + 2 pi (u - 1/2)/a (mod 2 pi): rotate by d = q delta = 2 hd, with
+    // hd = (u - 1/2) hd_scale = (g + 2^-24) hd_scale, g = 1.m - 1.5 exact, hd_c1 = 2^-24 hd_scale
+    const float hd = fmaf(__fadd_rn(one_plus_m(w0), -1.5f), hd_scale, hd_c1);
     float sh, ch;
     sincos_small(hd, sh, ch);
-    const float sd = 2.0f * sh * ch, omc = 2.0f * sh * sh;               // sin d, 1 - cos d
-    float rx = px - fmaf(omc, px, sd * py);
-    float ry = py - fmaf(omc, py, -sd * px);
+    const float sh2 = sh + sh;
+    const float sd = sh2 * ch, omc = sh2 * sh;                           // sin d, 1 - cos d
+    float rx = fmaf(-sd, py, fmaf(-omc, px, px));
+    float ry = fmaf(sd, px, fmaf(-omc, py, py));
     // line 4: dH = -h.(v'' - v') = (1 - cos d)(h.v') + sin d (h x v'): no cancellation at low T
     const float hdotp = fmaf(hx, px, hy * py);
     const float hcrossp = fmaf(hx, py, -hy * px);
@@ -544,171 +492,223 @@ __device__ __forceinline__ float2 update_site(float2 v, float hx, float hy, floa
         }
     }
     // lines 5-6: AP = min{1, exp(-dH/T)}; accept phi'' if AP > r else keep phi'
-    const bool acc = dH <= 0.0f || ex2_approx(dH * nlT) > r;
-    accepted += acc;
-    float nx = acc ? rx : px, ny = acc ? ry : py;
-    if (renorm) {   // keep |v| = 1 against rounding drift (first-order Newton step of 1/|v|), once per pass
-        const float sc = fmaf(-0.5f, fmaf(nx, nx, ny * ny), 1.5f);
-        nx *= sc; ny *= sc;
-    }
-    return make_float2(nx, ny);
+    accepted = dH <= 0.0f || ex2_approx(dH * nlT) > u01(w1);
+    return make_float2(accepted ? rx : px, accepted ? ry : py);
 }
+
+// ---- TMA / mbarrier PTX (sm_100a) -------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+// frame box (FC x FR x 1 eight-byte elements) of the vector buffer; out-of-grid elements arrive as zeros
+__device__ __forceinline__ void tma_load_frame(void* dst, const CUtensorMap* map, int c, int r, int g, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst)), "l"((uint64_t)map), "r"(c), "r"(r), "r"(g), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"((uint64_t)src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* dst, const void* src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 ::"l"((uint64_t)dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit_wait_read()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------
 // a3/a4  the hot kernel: K whole sweeps (colour 0 then colour 1, L261-265) of
 // one tile, on a copy of its frame in shared memory (temporal blocking).
-// Reads the state from one vector buffer and writes the tile's core to the
-// other, so tiles of one launch never see each other's writes.  Sites of the
-// halo are updated redundantly; they reproduce the neighbouring tiles'
-// results bit for bit because the random numbers are keyed by (site, sweep).
-// After half-sweep number hs (0-based) the frame is valid up to ring
-// 2K-1-hs, so each half-sweep only updates the suffix of the entry list
-// with ring <= 2K-1-hs.  Optionally fused at the end of the pass:
-//   PASS_ENERGY      a5: - sum over the core's colour-1 sites of v.h (each bond once)
-//   PASS_COUNT       a5: accepted proposals of the core sites
+// The frame arrives by one TMA tensor load (out-of-grid sites as zero vectors
+// = open boundary) together with the tile's entry list; the
+// tile's core leaves by one bulk copy per row into the OTHER vector buffer, so
+// tiles of one launch never see each other's writes.  Sites of the halo are
+// updated redundantly; they reproduce the neighbouring tiles' results bit for
+// bit because the random numbers are keyed by (site, sweep).  After half-sweep
+// number hs (0-based) the frame is valid up to ring 2K-1-hs, so each
+// half-sweep only updates the suffix of the entry list with ring <= 2K-1-hs.
+// Every thread keeps two sites in flight.  Optionally fused at the end:
+//   PASS_ENERGY      a5: - sum over the core's colour-1 sites of v.h (each bond once)   [FUSED only]
+//   PASS_COUNT       a5: accepted proposals of the core sites                          [FUSED only]
 //   PASS_ACCUMULATE  a7: acc += phi at the core's prediction sites
 // ---------------------------------------------------------------------------
-template <bool QHALF, int ORMODE>
-__global__ void __launch_bounds__(TILE_THREADS, 2) k_tilepass(Dev d, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
+template <bool QHALF, int ORMODE, bool FUSED>
+__global__ void __launch_bounds__(TILE_THREADS, 2)
+k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
+           uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t s_bar;
     __shared__ uint32_t s_cge[2][MAX_H + 1];
     __shared__ uint32_t s_accepted;
     __shared__ double s_red[TILE_THREADS / 32];
 
+    constexpr int NT = TILE_THREADS, NW = TILE_THREADS / 32;
     const int tile = blockIdx.x, g = blockIdx.y;
     const GridState& st = d.states[g];
-    if ((flags & PASS_CHECK_DONE) && st.done) return;
+    if (FUSED && (flags & PASS_CHECK_DONE) && st.done) return;
 
+    const int H = d.H, FC = d.FC;
     float2*   S  = reinterpret_cast<float2*>(smem_raw);
-    uint32_t* E  = reinterpret_cast<uint32_t*>(S + d.FR * d.FC);
+    uint32_t* E  = reinterpret_cast<uint32_t*>(S + d.FR * FC);
     uint2*    SP = reinterpret_cast<uint2*>(E + d.max_entries);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NW = TILE_THREADS / 32;
     const TileGeom tg = tile_geom(d, tile);
     const TileMeta& meta = d.tile_meta[(size_t)g * d.ntiles + tile];
-    const int H = d.H, FC = d.FC;
-    const int X = min((int)(2 * K), H);                      // rings of the frame this pass needs
     const uint32_t src_buf = st.cur ^ flip;
-    const float2* src = cur_vec(d, g, src_buf);
-    float2*       dst = cur_vec(d, g, src_buf ^ 1u);
+    float2* dst = vec_grid(d, g, src_buf ^ 1u);
 
+    if (tid == 0) { mbar_init(&s_bar, 1); s_accepted = 0; }
     if (tid < 2 * (MAX_H + 1)) (&s_cge[0][0])[tid] = (&meta.cge[0][0])[tid];
-    if (tid == 0) s_accepted = 0;
-    const uint32_t nE = meta.cge[0][0] + meta.cge[1][0];
-    {
-        const uint32_t* gE = d.entries + (size_t)g * d.entry_stride + meta.base;
-        for (uint32_t i = tid; i < nE; i += TILE_THREADS) E[i] = gE[i];
-    }
-    // frame load: out-of-grid sites are zero vectors = open boundary
-    for (int lr = H - X + warp; lr < H + tg.TRc + X; lr += NW) {
-        const int r = tg.r0 - H + lr;
-        const bool rin = r >= 0 && r < d.rows;
-        for (int lc = H - X + lane; lc < H + tg.TCc + X; lc += 32) {
-            const int col = tg.c0 - H + lc;
-            float2 v = make_float2(0.0f, 0.0f);
-            if (rin && col >= 0 && col < d.cols)
-                v = src[(size_t)((r + col) & 1) * d.VS + (uint32_t)(r + 1) * d.Wp + (uint32_t)(col >> 1) + 1u];
-            S[lr * FC + lc] = v;
-        }
-    }
     __syncthreads();
-
-    const float hs = st.hd_scale, nlT = st.neg_log2e_over_T;
+    if (tid == 0) {
+        const uint32_t entry_bytes = ((s_cge[0][0] + s_cge[1][0] + 3u) & ~3u) * (uint32_t)sizeof(uint32_t);
+        mbar_expect_tx(&s_bar, (uint32_t)(d.FR * FC * sizeof(float2)) + entry_bytes);
+        tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar);
+        if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar);
+    }
+    const float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f, nlT = st.neg_log2e_over_T;
     const uint32_t t0 = st.t + t_off;
     const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H), ncorr = d.cols - FC;
-    const bool count = flags & PASS_COUNT;
-    uint32_t accepted = 0;
+    const bool count = FUSED && (flags & PASS_COUNT);
+    uint32_t n_accepted = 0;
+    mbar_wait(&s_bar, 0);
+
+    // |v| = 1 against rounding drift (first-order Newton step of 1/|v|) for entries [from, to)
+    auto renormalise = [&](uint32_t from, uint32_t to) {
+        for (uint32_t e = from + tid; e < to; e += NT) {
+            const uint32_t off = E[e] & 0xFFFFu;
+            const float2 v = S[off];
+            const float sc = fmaf(-0.5f, fmaf(v.x, v.x, v.y * v.y), 1.5f);
+            S[off] = make_float2(v.x * sc, v.y * sc);
+        }
+    };
 
     for (uint32_t s = 0; s < K; ++s) {
         const uint32_t t = t0 + s;
         const bool odd = t & 1u;
-        const bool fresh = !odd || s == 0 || !d.use_spare;           // draw a new Philox block for (site, t >> 1)
+        const bool fresh = !odd || s == 0 || !d.use_spare;          // draw a new Philox block for (site, t >> 1)
         const bool stash = d.use_spare && !odd && s + 1 < K;        // keep words 2,3 for sweep t + 1
-        const bool renorm = s + 1 == K;
 #pragma unroll 1
         for (int c = 0; c < 2; ++c) {
             const int R = (int)(2 * K) - 1 - (int)(2 * s + c);       // rings still needed
             const uint32_t first = R + 1 <= MAX_H ? s_cge[c][R + 1] : 0u;
             const uint32_t last = s_cge[c][0], core_from = s_cge[c][1];
             const uint32_t base = c ? s_cge[0][0] : 0u;
-            for (uint32_t e = first + tid; e < last; e += TILE_THREADS) {
-                const uint32_t ent = E[base + e];
-                const uint32_t off = ent & 0xFFFFu, lr = ent >> 16;
-                const float2 v = S[off], up = S[off - FC], dn = S[off + FC], lf = S[off - 1], rt = S[off + 1];
-                uint32_t w0, w1;
+#pragma unroll 1
+            for (uint32_t eA = first + tid; eA < last; eA += 2 * NT) {
+                const bool hasB = eA + NT < last;
+                const uint32_t eB = hasB ? eA + NT : eA;             // no second site: repeat the first, drop its result
+                const uint32_t entA = E[base + eA], entB = E[base + eB];
+                const uint32_t offA = entA & 0xFFFFu, offB = entB & 0xFFFFu;
+                const float2 vA = S[offA], upA = S[offA - FC], dnA = S[offA + FC], lfA = S[offA - 1], rtA = S[offA + 1];
+                const float2 vB = S[offB], upB = S[offB - FC], dnB = S[offB + FC], lfB = S[offB - 1], rtB = S[offB + 1];
+                uint32_t wA0, wA1, wB0, wB1;
                 if (fresh) {
-                    const uint32_t n = (uint32_t)(nbase + (int)off + (int)lr * ncorr);
-                    const uint4 x = philox4x32_10(n, t >> 1, 2u, (uint32_t)g, d.key0, d.key1);
-                    w0 = odd ? x.z : x.x; w1 = odd ? x.w : x.y;
-                    if (stash) SP[base + e] = make_uint2(x.z, x.w);
+                    const uint32_t nA = (uint32_t)(nbase + (int)offA + (int)(entA >> 16) * ncorr);
+                    const uint32_t nB = (uint32_t)(nbase + (int)offB + (int)(entB >> 16) * ncorr);
+                    const uint4 xA = philox4x32_10(nA, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
+                    const uint4 xB = philox4x32_10(nB, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
+                    wA0 = odd ? xA.z : xA.x; wA1 = odd ? xA.w : xA.y;
+                    wB0 = odd ? xB.z : xB.x; wB1 = odd ? xB.w : xB.y;
+                    if (stash) { SP[base + eA] = make_uint2(xA.z, xA.w); SP[base + eB] = make_uint2(xB.z, xB.w); }
                 } else {
-                    const uint2 sp = SP[base + e];
-                    w0 = sp.x; w1 = sp.y;
+                    const uint2 sA = SP[base + eA], sB = SP[base + eB];
+                    wA0 = sA.x; wA1 = sA.y; wB0 = sB.x; wB1 = sB.y;
                 }
-                const float hx = (up.x + dn.x) + (lf.x + rt.x), hy = (up.y + dn.y) + (lf.y + rt.y);
-                uint32_t a = 0;
-                S[off] = update_site<QHALF, ORMODE>(v, hx, hy, up, dn, lf, rt, u01_centered(w0), u01(w1), hs, nlT,
-                                                    d.bc, d.bs, renorm, a);
-                if (count && e >= core_from) accepted += a;
+                bool accA, accB;
+                const float2 newA = update_site<QHALF, ORMODE>(vA, upA, dnA, lfA, rtA, wA0, wA1, hs, hc1, nlT, d.bc, d.bs, accA);
+                const float2 newB = update_site<QHALF, ORMODE>(vB, upB, dnB, lfB, rtB, wB0, wB1, hs, hc1, nlT, d.bc, d.bs, accB);
+                S[offA] = newA;
+                if (hasB) S[offB] = newB;
+                if (count) n_accepted += (accA && eA >= core_from) + (accB && hasB && eB >= core_from);
             }
             __syncthreads();
         }
-    }
-
-    // write the core back (both colours, whole rows: coalesced in each colour plane)
-    for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
-        const int r = tg.r0 - H + lr;
-        for (int lc = H + lane; lc < H + tg.TCc; lc += 32) {
-            const int col = tg.c0 - H + lc;
-            dst[(size_t)((r + col) & 1) * d.VS + (uint32_t)(r + 1) * d.Wp + (uint32_t)(col >> 1) + 1u] = S[lr * FC + lc];
+        if ((s & 7u) == 7u && s + 1 < K) {       // long single-tile passes: bound the drift of |v|
+            renormalise(0, s_cge[0][0] + s_cge[1][0]);
+            __syncthreads();
         }
     }
+    // the core's prediction sites (ring 0), both colours, before they leave
+    renormalise(s_cge[0][1], s_cge[0][0]);
+    renormalise(s_cge[0][0] + s_cge[1][1], s_cge[0][0] + s_cge[1][0]);
+    fence_proxy_async_smem();
+    __syncthreads();
+
+    // write the core back, one bulk copy per row (an odd last column takes the zero pad column along)
+    const uint32_t row_bytes = (uint32_t)((tg.TCc + 1) & ~1) * (uint32_t)sizeof(float2);
+    for (int lr = tid; lr < tg.TRc; lr += NT)
+        bulk_store(dst + (size_t)(tg.r0 + lr) * d.pitch + tg.c0, S + (H + lr) * FC + H, row_bytes);
+
     if (flags & PASS_ACCUMULATE) {
         // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites
+        float* acc = d.acc + (size_t)g * d.N;
         for (int c = 0; c < 2; ++c) {
             const uint32_t base = c ? s_cge[0][0] : 0u;
-            float* acc = d.acc + ((size_t)g * 2 + c) * d.VS;
-            for (uint32_t e = s_cge[c][1] + tid; e < s_cge[c][0]; e += TILE_THREADS) {
-                const uint32_t ent = E[base + e];
-                const uint32_t off = ent & 0xFFFFu, lr = ent >> 16, lc = off - lr * FC;
-                const int r = tg.r0 - H + (int)lr, col = tg.c0 - H + (int)lc;
-                acc[(uint32_t)(r + 1) * d.Wp + (uint32_t)(col >> 1) + 1u] += angle_of(S[off], d.inv_q);
+            for (uint32_t e = s_cge[c][1] + tid; e < s_cge[c][0]; e += NT) {
+                const uint32_t ent = E[base + e], off = ent & 0xFFFFu;
+                acc[nbase + (int)off + (int)(ent >> 16) * ncorr] += angle_of(S[off], d.inv_q);
             }
         }
     }
-    if (count) {
-        accepted = __reduce_add_sync(0xFFFFFFFFu, accepted);
-        if (lane == 0 && accepted) atomicAdd(&s_accepted, accepted);
-    }
-    if (flags & PASS_ENERGY) {
-        // a5: H_tile = - sum over the core's colour-1 sites (fixed ones too) of v . h; fixed summation order
-        double sum = 0.0;
-        for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
-            const int r = tg.r0 - H + lr;
-            float row = 0.0f;
-            // first colour-1 column of this row at or after the core's first column
-            for (int lc = H + ((r + tg.c0 + 1) & 1) + 2 * lane; lc < H + tg.TCc; lc += 64) {
-                const int off = lr * FC + lc;
-                const float2 v = S[off], up = S[off - FC], dn = S[off + FC], lf = S[off - 1], rt = S[off + 1];
-                row += fmaf(v.x, (up.x + dn.x) + (lf.x + rt.x), v.y * ((up.y + dn.y) + (lf.y + rt.y)));
-            }
-            sum += (double)row;
+    if (FUSED) {
+        if (count) {
+            n_accepted = __reduce_add_sync(0xFFFFFFFFu, n_accepted);
+            if (lane == 0 && n_accepted) atomicAdd(&s_accepted, n_accepted);
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
-        if (lane == 0) s_red[warp] = sum;
-    }
-    __syncthreads();
-    if (tid == 0) {
-        if (count && s_accepted) atomicAdd(&d.states[g].accepted, (unsigned long long)s_accepted);
         if (flags & PASS_ENERGY) {
-            double s = 0.0;
-            for (int w = 0; w < NW; ++w) s += s_red[w];
-            d.e_partials[(size_t)g * d.n_partials + tile] = -s;
+            // a5: H_tile = - sum over the core's colour-1 sites (fixed ones too) of v . h; fixed summation order
+            double sum = 0.0;
+            for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
+                const int r = tg.r0 - H + lr;
+                float row = 0.0f;
+                // first colour-1 column of this row at or after the core's first column
+                for (int lc = H + ((r + tg.c0 + 1) & 1) + 2 * lane; lc < H + tg.TCc; lc += 64) {
+                    const int off = lr * FC + lc;
+                    const float2 v = S[off], up = S[off - FC], dn = S[off + FC], lf = S[off - 1], rt = S[off + 1];
+                    row += fmaf(v.x, (up.x + dn.x) + (lf.x + rt.x), v.y * ((up.y + dn.y) + (lf.y + rt.y)));
+                }
+                sum += (double)row;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+            if (lane == 0) s_red[warp] = sum;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            if (count && s_accepted) atomicAdd(&d.states[g].accepted, (unsigned long long)s_accepted);
+            if (flags & PASS_ENERGY) {
+                double s = 0.0;
+                for (int w = 0; w < NW; ++w) s += s_red[w];
+                d.e_partials[(size_t)g * d.n_partials + tile] = -s;
+            }
         }
     }
+    bulk_commit_wait_read();      // shared memory must stay until the row copies have read it
 }
 
 // ---------------------------------------------------------------------------
@@ -720,22 +720,21 @@ __global__ void __launch_bounds__(ENERGY_THREADS) k_energy(Dev d)
 {
     const int g = blockIdx.y;
     __shared__ double warp_sum[ENERGY_THREADS / 32];
-    const float2* own = cur_vec(d, g, d.states[g].cur) + d.VS;
-    const float2* oth = cur_vec(d, g, d.states[g].cur);
+    const float2* v = vec_grid(d, g, d.states[g].cur);
+    const float2 zero = make_float2(0.0f, 0.0f);
     double sum = 0.0;
-    for (uint32_t r = blockIdx.x; r < (uint32_t)d.rows; r += gridDim.x) {
-        const uint32_t par = (r + 1u) & 1u;
-        float row = 0.0f;
+    for (int r = blockIdx.x; r < d.rows; r += gridDim.x) {
+        const float2* row = v + (size_t)r * d.pitch;
+        float part = 0.0f;
         int cnt = 0;
-        for (uint32_t j = threadIdx.x; j < d.W; j += ENERGY_THREADS) {
-            const uint32_t li = (r + 1u) * d.Wp + j + 1u;
-            const float2 v = own[li];
-            const float2 up = oth[li - d.Wp], dn = oth[li + d.Wp], lf = oth[li - 1u + par], rt = oth[li + par];
-            const float hx = (up.x + dn.x) + (lf.x + rt.x), hy = (up.y + dn.y) + (lf.y + rt.y);
-            row += fmaf(v.x, hx, v.y * hy);
-            if (++cnt == 8) { sum += (double)row; row = 0.0f; cnt = 0; }
+        for (int col = ((r + 1) & 1) + 2 * (int)threadIdx.x; col < d.cols; col += 2 * ENERGY_THREADS) {
+            const float2 c = row[col];
+            const float2 up = r > 0 ? row[col - (int)d.pitch] : zero, dn = r + 1 < d.rows ? row[col + d.pitch] : zero;
+            const float2 lf = col > 0 ? row[col - 1] : zero, rt = col + 1 < d.cols ? row[col + 1] : zero;
+            part += fmaf(c.x, (up.x + dn.x) + (lf.x + rt.x), c.y * ((up.y + dn.y) + (lf.y + rt.y)));
+            if (++cnt == 8) { sum += (double)part; part = 0.0f; cnt = 0; }
         }
-        sum += (double)row;
+        sum += (double)part;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
@@ -846,48 +845,47 @@ __global__ void k_begin_run(Dev d, const float* __restrict__ T)
 }
 
 // ---------------------------------------------------------------------------
-// a8  prediction (Alg. 2 step 7, L148, L212) at the free sites; the caller
-// has already copied the input values (sample sites bit for bit) into out.
+// a8  prediction (Alg. 2 step 7, L148, L212): mean angle over the realizations,
+// back-transformed by the inverse of Eq. 1 at the prediction sites; sample
+// sites return the input value bit for bit.
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_predict(Dev d, float* __restrict__ out)
 {
-    const int g = blockIdx.y, colour = blockIdx.z;
-    const uint32_t o = blockIdx.x * blockDim.x + threadIdx.x;
+    const int g = blockIdx.y;
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N) return;
+    const size_t o = (size_t)g * d.N + n;
+    if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = d.values[o]; return; }
     const GridState& s = d.states[g];
-    if (o >= s.n_free[colour]) return;
-    const uint32_t idx = d.lists[((size_t)g * 2 + colour) * d.LC + o], li = idx & 0x7FFFFFFFu, par = idx >> 31;
-    const uint32_t r = li / d.Wp - 1u, col = 2u * (li - (r + 1u) * d.Wp - 1u) + par;
-    const double mean_phi = (double)d.acc[((size_t)g * 2 + colour) * d.VS + li] / (double)s.realizations;
+    const double mean_phi = (double)d.acc[o] / (double)s.realizations;
     const double z = (double)s.zmin + mean_phi * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F;
-    out[(size_t)g * d.N + (size_t)r * d.cols + col] = (float)z;
+    out[o] = (float)z;
 }
 
-// angle import / export at the free sites -----------------------------------
+// angle import / export at the prediction sites ------------------------------
 __global__ void __launch_bounds__(256) k_export_angles(Dev d)
 {
-    const int g = blockIdx.y, colour = blockIdx.z;
-    const uint32_t o = blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= d.states[g].n_free[colour]) return;
-    const uint32_t idx = d.lists[((size_t)g * 2 + colour) * d.LC + o], li = idx & 0x7FFFFFFFu, par = idx >> 31;
-    const uint32_t r = li / d.Wp - 1u, col = 2u * (li - (r + 1u) * d.Wp - 1u) + par;
-    const float2 v = cur_vec(d, g, d.states[g].cur)[(size_t)colour * d.VS + li];
-    d.phi[(size_t)g * d.N + (size_t)r * d.cols + col] = angle_of(v, d.inv_q);
+    const int g = blockIdx.y;
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N || is_fixed(d.bits + (size_t)g * d.words, n)) return;
+    const uint32_t r = n / d.cols, col = n - r * d.cols;
+    const float2 v = vec_grid(d, g, d.states[g].cur)[(size_t)r * d.pitch + col];
+    d.phi[(size_t)g * d.N + n] = angle_of(v, d.inv_q);
 }
 __global__ void __launch_bounds__(256) k_import_angles(Dev d, const float* __restrict__ phi_in)
 {
-    const int g = blockIdx.y, colour = blockIdx.z;
-    const uint32_t o = blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= d.states[g].n_free[colour]) return;
-    const uint32_t idx = d.lists[((size_t)g * 2 + colour) * d.LC + o], li = idx & 0x7FFFFFFFu, par = idx >> 31;
-    const uint32_t r = li / d.Wp - 1u, col = 2u * (li - (r + 1u) * d.Wp - 1u) + par;
-    const size_t n = (size_t)g * d.N + (size_t)r * d.cols + col;
-    float p = phi_in[n];
+    const int g = blockIdx.y;
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N || is_fixed(d.bits + (size_t)g * d.words, n)) return;
+    const uint32_t r = n / d.cols, col = n - r * d.cols;
+    const size_t o = (size_t)g * d.N + n;
+    float p = phi_in[o];
     p = p < 0.0f ? 0.0f : p;
     p = p > TWO_PI_F ? TWO_PI_F : p;
-    d.phi[n] = p;
+    d.phi[o] = p;
     float sn, cs;
     sincosf(__fmul_rn(d.q, p), &sn, &cs);
-    cur_vec(d, g, d.states[g].cur)[(size_t)colour * d.VS + li] = make_float2(cs, sn);
+    vec_grid(d, g, d.states[g].cur)[(size_t)r * d.pitch + col] = make_float2(cs, sn);
 }
 
 }  // namespace mpr

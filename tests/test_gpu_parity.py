@@ -289,7 +289,8 @@ def test_equilibration_controller_follows_the_oracle(torch_cuda, mpr, orc):
     assert 0.5 * st["sweeps"] <= g.equil_sweeps <= 2.0 * st["sweeps"]
     assert g.a == pytest.approx(st["a"], rel=0.3)
     assert g.e_last == pytest.approx(st["e_hist"][-1], abs=3e-4)
-    assert ctx.energy()[0] == pytest.approx(g.e_last, abs=1e-12)
+    # the fused per-tile reduction and mpr_energy add the same fp32 bond terms in different orders
+    assert ctx.energy()[0] == pytest.approx(g.e_last, abs=1e-8)
     ctx.close()
 
 
