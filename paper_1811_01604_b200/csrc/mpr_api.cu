@@ -49,13 +49,14 @@ void choose_tiles(int rows, int cols, Geometry* g)
     if (const char* e = getenv("MPR_TILE")) {
         int a, b, c;
         if (sscanf(e, "%d,%d,%d", &a, &b, &c) == 3 && a >= 8 && b >= 8 && (b & 1) == 0 && c >= 2 && c <= MAX_H &&
-            (c & 1) == 0 && (a + 2 * c) * (b + 2 * c) <= 65536 && a + 2 * c <= 255 && b + 2 * c <= 256) { TR = a; TC = b; H = c; }
+            (c & 1) == 0 && (a + 2 * c) * (b + 2 * c + 2) <= 65535 && a + 2 * c <= 255 && b + 2 * c <= 252) { TR = a; TC = b; H = c; }
     }
     if ((long)rows * cols <= 128L * 128L && rows <= 250 && cols <= 250) { TR = rows; TC = cols; H = 2; }
-    g->TR = TR; g->TC = TC; g->H = H; g->FR = TR + 2 * H; g->FC = (TC + 2 * H + 1) & ~1;
+    g->TR = TR; g->TC = TC; g->H = H; g->FR = TR + 2 * H;
+    g->FC = ((TC + 2 * H + 1) & ~3) + 2;        // >= TC + 2H and = 2 (mod 4): a column's rows spread over the banks
     g->ntx = (cols + TC - 1) / TC; g->nty = (rows + TR - 1) / TR; g->ntiles = g->ntx * g->nty;
     g->n_partials = (uint32_t)(g->ntiles > ENERGY_BLOCKS ? g->ntiles : ENERGY_BLOCKS);
-    g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 3) & ~(size_t)3);
+    g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 7) & ~(size_t)7);
 }
 
 bool make_geometry(int batch, int rows, int cols, Geometry* g)
@@ -89,7 +90,7 @@ Layout make_layout(int batch, const Geometry& g)
     L.vec       = take(2 * B * g.VG * sizeof(float2));
     L.acc       = take(B * g.N * sizeof(float));
     L.tile_meta = take(B * g.ntiles * sizeof(TileMeta));
-    L.entries   = take((B * g.entry_stride + 4) * sizeof(uint32_t));
+    L.entries   = take((B * g.entry_stride + 8) * sizeof(uint16_t));
     L.total = o;
     return L;
 }
@@ -274,9 +275,10 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     d.vec = (float2*)(base + lay.vec);
     d.acc = (float*)(base + lay.acc);
     d.tile_meta = (TileMeta*)(base + lay.tile_meta);
-    d.entries = (uint32_t*)(base + lay.entries);
+    d.entries = (uint16_t*)(base + lay.entries);
     d.VG = g.VG; d.VB = (size_t)batch * g.VG;
     d.entry_stride = g.entry_stride; d.n_partials = g.n_partials;
+    d.fc_inv = (uint32_t)(((1u << 24) + (uint32_t)g.FC - 1u) / (uint32_t)g.FC);
     d.TR = g.TR; d.TC = g.TC; d.H = g.H; d.FR = g.FR; d.FC = g.FC; d.ntx = g.ntx; d.nty = g.nty; d.ntiles = g.ntiles;
     d.batch = batch; d.rows = rows; d.cols = cols;
     d.N = g.N; d.words = g.words; d.pitch = g.pitch;
@@ -316,15 +318,15 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     uint32_t max_entries = 0;
     for (int b = 0; b < batch; ++b)
         if (ctx->h_states[b].max_tile_entries > max_entries) max_entries = ctx->h_states[b].max_tile_entries;
-    max_entries = (max_entries + 3u) & ~3u;
+    max_entries = (max_entries + 7u) & ~7u;
     d.max_entries = max_entries;
     const size_t frame_bytes = (size_t)g.FR * g.FC * sizeof(float2);
     int smem_max = 0;
     if (!cuda_ok(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device), "smem attr")) return fail(MPR_ERR_CUDA);
     const size_t budget = (size_t)smem_max - 2048;               // static shared memory of the kernel
     d.use_spare = g.ntiles == 1 || g.H >= 4;                       // pointless when every pass is a single sweep
-    if (frame_bytes + 12ull * max_entries > budget) d.use_spare = 0;
-    ctx->smem_bytes = frame_bytes + (d.use_spare ? 12ull : 4ull) * max_entries;
+    if (frame_bytes + 10ull * max_entries > budget) d.use_spare = 0;
+    ctx->smem_bytes = frame_bytes + (d.use_spare ? 10ull : 2ull) * max_entries;
     if (ctx->smem_bytes > budget) return fail(MPR_ERR_WORKSPACE);
     ctx->k_max = g.ntiles == 1 ? 1024u : (uint32_t)(g.H / 2);
     if (const char* e = getenv("MPR_KMAX")) {

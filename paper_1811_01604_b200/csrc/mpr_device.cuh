@@ -55,7 +55,7 @@ struct GridState {
 
 // Free sites of one tile frame (core + halo), see k_tile_fill.
 struct TileMeta {
-    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid), multiple of 4
+    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid), multiple of 8
     uint32_t cge[2][MAX_H + 1];       // cge[c][k] = entries of colour c with ring >= k (ring = distance outside the core)
 };
 
@@ -70,7 +70,7 @@ struct Dev {
     float2*    vec;            // [2 buffers][batch][rows][pitch] row-major unit vectors (pitch = cols rounded up to even)
     float*     acc;            // [batch][N] sum over realizations of phi at the prediction sites
     TileMeta*  tile_meta;      // [batch][ntiles]
-    uint32_t*  entries;        // [batch][entry_stride] tile frames' free sites: frame offset | frame row << 16
+    uint16_t*  entries;        // [batch][entry_stride] tile frames' free sites: offset in the frame (row * FC + col)
     int        batch, rows, cols;
     uint32_t   N, words, pitch;
     size_t     VG;             // float2 elements of one grid in one buffer = rows * pitch
@@ -79,7 +79,8 @@ struct Dev {
     uint32_t   n_partials;
     // tiling
     int        TR, TC, H, FR, FC, ntx, nty, ntiles;
-    uint32_t   max_entries;    // shared-memory capacity for entries (multiple of 4)
+    uint32_t   max_entries;    // shared-memory capacity for entries (multiple of 8)
+    uint32_t   fc_inv;         // ceil(2^24 / FC): frame row of offset o = (o * fc_inv) >> 24, exact for o < 2^16
     int        use_spare;      // keep the odd sweep's random words in shared memory
     uint32_t   rk0[PHILOX_ROUNDS], rk1[PHILOX_ROUNDS];   // Philox round keys: (seed lo, seed hi) + r * Weyl constants
     float      q, inv_q;
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(256) k_tile_count(Dev d)
     }
 }
 
-// one warp per grid: exclusive scan of the tiles' entry counts (each rounded up to a multiple of 4
+// one warp per grid: exclusive scan of the tiles' entry counts (each rounded up to a multiple of 8
 // so that every tile's list starts on a 16-byte boundary), and their maximum
 __global__ void k_tile_scan(Dev d)
 {
@@ -349,7 +350,7 @@ __global__ void k_tile_scan(Dev d)
     uint32_t carry = 0, mx = 0;
     for (int base = 0; base < d.ntiles; base += 32) {
         const int i = base + lane;
-        const uint32_t c = i < d.ntiles ? (m[i].cge[0][0] + m[i].cge[1][0] + 3u) & ~3u : 0u;
+        const uint32_t c = i < d.ntiles ? (m[i].cge[0][0] + m[i].cge[1][0] + 7u) & ~7u : 0u;
         mx = max(mx, c);
         uint32_t x = c;
 #pragma unroll
@@ -375,7 +376,7 @@ __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
     const TileGeom t = tile_geom(d, tile);
     const TileMeta& m = d.tile_meta[(size_t)g * d.ntiles + tile];
     const uint32_t* bits = d.bits + (size_t)g * d.words;
-    uint32_t* out = d.entries + (size_t)g * d.entry_stride + m.base;
+    uint16_t* out = d.entries + (size_t)g * d.entry_stride + m.base;
     for (int i = threadIdx.x; i < d.FR * d.FC; i += blockDim.x) {
         const int lr = i / d.FC, lc = i - lr * d.FC;
         int colour, ring;
@@ -396,7 +397,7 @@ __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
             }
             // colour 0 first; within a colour the rings in descending order
             pos += (colour ? m.cge[0][0] : 0u) + m.cge[colour][ring + 1];
-            out[pos] = (uint32_t)i | ((uint32_t)lr << 16);
+            out[pos] = (uint16_t)i;
         }
     }
 }
@@ -572,8 +573,8 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 
     const int H = d.H, FC = d.FC;
     float2*   S  = reinterpret_cast<float2*>(smem_raw);
-    uint32_t* E  = reinterpret_cast<uint32_t*>(S + d.FR * FC);
-    uint2*    SP = reinterpret_cast<uint2*>(E + d.max_entries);
+    uint2*    SP = reinterpret_cast<uint2*>(S + d.FR * FC);
+    uint16_t* E  = reinterpret_cast<uint16_t*>(SP + (d.use_spare ? d.max_entries : 0u));
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const TileGeom tg = tile_geom(d, tile);
@@ -585,7 +586,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     if (tid < 2 * (MAX_H + 1)) (&s_cge[0][0])[tid] = (&meta.cge[0][0])[tid];
     __syncthreads();
     if (tid == 0) {
-        const uint32_t entry_bytes = ((s_cge[0][0] + s_cge[1][0] + 3u) & ~3u) * (uint32_t)sizeof(uint32_t);
+        const uint32_t entry_bytes = ((s_cge[0][0] + s_cge[1][0] + 7u) & ~7u) * (uint32_t)sizeof(uint16_t);
         mbar_expect_tx(&s_bar, (uint32_t)(d.FR * FC * sizeof(float2)) + entry_bytes);
         tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar);
         if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar);
@@ -600,7 +601,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     // |v| = 1 against rounding drift (first-order Newton step of 1/|v|) for entries [from, to)
     auto renormalise = [&](uint32_t from, uint32_t to) {
         for (uint32_t e = from + tid; e < to; e += NT) {
-            const uint32_t off = E[e] & 0xFFFFu;
+            const uint32_t off = E[e];
             const float2 v = S[off];
             const float sc = fmaf(-0.5f, fmaf(v.x, v.x, v.y * v.y), 1.5f);
             S[off] = make_float2(v.x * sc, v.y * sc);
@@ -618,18 +619,24 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             const uint32_t first = R + 1 <= MAX_H ? s_cge[c][R + 1] : 0u;
             const uint32_t last = s_cge[c][0], core_from = s_cge[c][1];
             const uint32_t base = c ? s_cge[0][0] : 0u;
+            // every thread takes the entries eA and eB = eA + stride; the last round splits what is left
+            // into two halves of whole warps, so that no warp runs a round for a missing second site
 #pragma unroll 1
-            for (uint32_t eA = first + tid; eA < last; eA += 2 * NT) {
-                const bool hasB = eA + NT < last;
-                const uint32_t eB = hasB ? eA + NT : eA;             // no second site: repeat the first, drop its result
-                const uint32_t entA = E[base + eA], entB = E[base + eB];
-                const uint32_t offA = entA & 0xFFFFu, offB = entB & 0xFFFFu;
+            for (uint32_t pos = first; pos < last;) {
+                const uint32_t rem = last - pos;
+                const uint32_t stride = rem >= 2u * NT ? (uint32_t)NT : ((rem + 63u) >> 6) << 5;
+                const uint32_t eA = pos + tid;
+                pos += 2u * stride;
+                if ((uint32_t)tid >= stride || eA >= last) continue;
+                const bool hasB = eA + stride < last;
+                const uint32_t eB = hasB ? eA + stride : eA;         // no second site: repeat the first, drop its result
+                const uint32_t offA = E[base + eA], offB = E[base + eB];
                 const float2 vA = S[offA], upA = S[offA - FC], dnA = S[offA + FC], lfA = S[offA - 1], rtA = S[offA + 1];
                 const float2 vB = S[offB], upB = S[offB - FC], dnB = S[offB + FC], lfB = S[offB - 1], rtB = S[offB + 1];
                 uint32_t wA0, wA1, wB0, wB1;
                 if (fresh) {
-                    const uint32_t nA = (uint32_t)(nbase + (int)offA + (int)(entA >> 16) * ncorr);
-                    const uint32_t nB = (uint32_t)(nbase + (int)offB + (int)(entB >> 16) * ncorr);
+                    const uint32_t nA = (uint32_t)(nbase + (int)offA + (int)((offA * d.fc_inv) >> 24) * ncorr);
+                    const uint32_t nB = (uint32_t)(nbase + (int)offB + (int)((offB * d.fc_inv) >> 24) * ncorr);
                     const uint4 xA = philox4x32_10(nA, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
                     const uint4 xB = philox4x32_10(nB, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
                     wA0 = odd ? xA.z : xA.x; wA1 = odd ? xA.w : xA.y;
@@ -670,8 +677,8 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         for (int c = 0; c < 2; ++c) {
             const uint32_t base = c ? s_cge[0][0] : 0u;
             for (uint32_t e = s_cge[c][1] + tid; e < s_cge[c][0]; e += NT) {
-                const uint32_t ent = E[base + e], off = ent & 0xFFFFu;
-                acc[nbase + (int)off + (int)(ent >> 16) * ncorr] += angle_of(S[off], d.inv_q);
+                const uint32_t off = E[base + e];
+                acc[nbase + (int)off + (int)((off * d.fc_inv) >> 24) * ncorr] += angle_of(S[off], d.inv_q);
             }
         }
     }
