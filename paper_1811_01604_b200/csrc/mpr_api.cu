@@ -128,15 +128,21 @@ mpr_status fetch_states(mpr_ctx* ctx)
 
 typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t);
 
-// fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps)
-pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused)
+// fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps);
+// std_fc = the frame pitch is the compile-time STD_FC (standard tile shape)
+template <int FCT>
+pass_kernel pick_pass_kernel_fc(bool qhalf, int or_mode, bool fused)
 {
     if (fused) {
-        if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true> : or_mode == 1 ? k_tilepass<true, 1, true> : k_tilepass<true, 2, true>;
-        return or_mode == 0 ? k_tilepass<false, 0, true> : k_tilepass<false, 2, true>;
+        if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true, FCT> : or_mode == 1 ? k_tilepass<true, 1, true, FCT> : k_tilepass<true, 2, true, FCT>;
+        return or_mode == 0 ? k_tilepass<false, 0, true, FCT> : k_tilepass<false, 2, true, FCT>;
     }
-    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, false> : or_mode == 1 ? k_tilepass<true, 1, false> : k_tilepass<true, 2, false>;
-    return or_mode == 0 ? k_tilepass<false, 0, false> : k_tilepass<false, 2, false>;
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, false, FCT> : or_mode == 1 ? k_tilepass<true, 1, false, FCT> : k_tilepass<true, 2, false, FCT>;
+    return or_mode == 0 ? k_tilepass<false, 0, false, FCT> : k_tilepass<false, 2, false, FCT>;
+}
+pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused, bool std_fc)
+{
+    return std_fc ? pick_pass_kernel_fc<STD_FC>(qhalf, or_mode, fused) : pick_pass_kernel_fc<0>(qhalf, or_mode, fused);
 }
 
 // K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile
@@ -144,7 +150,7 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
 {
     ctx->dirty = true;
     const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
-    pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused)
+    pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC)
         <<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(
             ctx->map[0], ctx->map[1], ctx->d, K, t_off, flip, flags);
     CU_LAUNCH();
@@ -337,7 +343,7 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
         for (int om = 0; om < 3; ++om)
             for (int fu = 0; fu < 2; ++fu) {
                 if (!qh && om == 1) continue;
-                if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, g.FC == STD_FC), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                   (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
             }
     *out = ctx;

@@ -21,6 +21,7 @@ constexpr float    TWO_PI_F       = 6.28318530717958647692f;  // float nearest 2
 constexpr int      MAX_NFIT       = 256;
 constexpr int      TILE_THREADS   = 256;                      // threads of a tile pass CTA
 constexpr int      MAX_H          = 16;                       // largest halo: up to 8 sweeps per tile pass
+constexpr int      STD_FC         = 82;                       // frame pitch of the standard 64 x 64 tile with halo 8 (compile-time in k_tilepass)
 constexpr int      ENERGY_BLOCKS  = 592;                      // 4 x 148 SMs; fixed so the sum order is deterministic
 constexpr int      ENERGY_THREADS = 256;
 constexpr int      PHILOX_ROUNDS  = 10;
@@ -146,6 +147,29 @@ __device__ __forceinline__ void sincos_small(float x, float& s, float& c)
     pc = fmaf(x2, pc, 4.16666667e-2f);
     pc = fmaf(x2, pc, -0.5f);
     c = fmaf(x2, pc, 1.0f);
+}
+
+// Packed fp32 pairs (sm_100a FFMA2 / FADD2 / FMUL2: two fp32 operations per issued instruction).
+// In update_pair the two lanes of a pair are the two sites a thread has in flight.
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
+
+// sincos_small on a pair
+__device__ __forceinline__ void sincos_small2(float2 x, float2& s, float2& c)
+{
+    const float2 x2 = mul2(x, x);
+    float2 ps = fma2(x2, bc2(2.75573192e-6f), bc2(-1.98412698e-4f));
+    ps = fma2(x2, ps, bc2(8.33333333e-3f));
+    ps = fma2(x2, ps, bc2(-1.66666667e-1f));
+    s = fma2(mul2(x, x2), ps, x);
+    float2 pc = fma2(x2, bc2(-2.75573192e-7f), bc2(2.48015873e-5f));
+    pc = fma2(x2, pc, bc2(-1.38888889e-3f));
+    pc = fma2(x2, pc, bc2(4.16666667e-2f));
+    pc = fma2(x2, pc, bc2(-0.5f));
+    c = fma2(x2, pc, bc2(1.0f));
 }
 
 __device__ __forceinline__ uint32_t enc_ordered(float f)
@@ -497,6 +521,100 @@ __device__ __forceinline__ float2 update_site(float2 v, float2 n_up, float2 n_dn
     return make_float2(accepted ? rx : px, accepted ? ry : py);
 }
 
+// The same UPDATE for the two sites A and B a thread has in flight, with the fp32 arithmetic of both packed
+// into f32x2 instructions (lane x = site A, lane y = site B).  Identities used on top of update_site:
+// the reflection keeps h.v, so h.v' = h.v, and turns h x v into -(h x v); both are taken from the stored v,
+// which is what the oracle's exact arithmetic does (it does not round v' before the Metropolis step).
+// exp(-dH/T) > r already accepts every dH <= 0 because r < 1.
+template <bool QHALF, int ORMODE>
+__device__ __forceinline__ void update_pair(float2& vA, float2 upA, float2 dnA, float2 lfA, float2 rtA,
+                                            float2& vB, float2 upB, float2 dnB, float2 lfB, float2 rtB,
+                                            uint32_t wA0, uint32_t wA1, uint32_t wB0, uint32_t wB1,
+                                            float hd_scale, float hd_c1, float nlT, float bc, float bs, bool renorm,
+                                            bool& accA, bool& accB)
+{
+    if (ORMODE == 1) {      // Eq. 6 as printed: comparison mode, not packed
+        vA = update_site<QHALF, ORMODE>(vA, upA, dnA, lfA, rtA, wA0, wA1, hd_scale, hd_c1, nlT, bc, bs, accA);
+        vB = update_site<QHALF, ORMODE>(vB, upB, dnB, lfB, rtB, wB0, wB1, hd_scale, hd_c1, nlT, bc, bs, accB);
+        if (renorm) {
+            const float sA = fmaf(-0.5f, fmaf(vA.x, vA.x, vA.y * vA.y), 1.5f), sB = fmaf(-0.5f, fmaf(vB.x, vB.x, vB.y * vB.y), 1.5f);
+            vA = make_float2(vA.x * sA, vA.y * sA); vB = make_float2(vB.x * sB, vB.y * sB);
+        }
+        return;
+    }
+    // Two packings are used so that no register moves are needed: (x, y) of ONE site for what is linear in
+    // the vectors (the registers a 64-bit shared load fills), and (site A, site B) for the scalar chain.
+    // (C, S) = h per site
+    const float2 hA = add2(add2(upA, dnA), add2(lfA, rtA));
+    const float2 hB = add2(add2(upB, dnB), add2(lfB, rtB));
+    const float2 hvA = mul2(hA, vA), hvB = mul2(hB, vB);
+    const float2 dot = make_float2(hvA.x + hvA.y, hvB.x + hvB.y);            // h . v  (= h . v')
+    float2 crs = make_float2(fmaf(hA.x, vA.y, -hA.y * vA.x), fmaf(hB.x, vB.y, -hB.y * vB.x));   // h x v
+    float2 pA = vA, pB = vB;
+    if (ORMODE == 0) {
+        // Alg. 1 line 1: over-relaxation, v' = 2 (h.v)/(h.h) h - v; out of [0, 2 pi]: keep the spin (R2, R17);
+        // h x v' = -(h x v)
+        const float2 hhA = mul2(hA, hA), hhB = mul2(hB, hB);
+        const float2 R2 = make_float2(hhA.x + hhA.y, hhB.x + hhB.y);
+        const float2 rinv = make_float2(rcp_approx(R2.x), rcp_approx(R2.y));      // 0 * inf -> NaN -> kept
+        const float2 t = mul2(dot, rinv);
+        const float2 k = add2(t, t);
+        const float2 fA = fma2(hA, bc2(k.x), neg2(vA)), fB = fma2(hB, bc2(k.y), neg2(vB));
+        bool inA = fA.y >= 0.0f && hA.y >= 0.0f, inB = fB.y >= 0.0f && hB.y >= 0.0f;
+        if (!QHALF) {
+            inA = inA && fmaf(fA.x, bs, -fA.y * bc) >= 0.0f;
+            inB = inB && fmaf(fB.x, bs, -fB.y * bc) >= 0.0f;
+        }
+        pA = make_float2(inA ? fA.x : vA.x, inA ? fA.y : vA.y);
+        pB = make_float2(inB ? fB.x : vB.x, inB ? fB.y : vB.y);
+        crs = make_float2(inA ? -crs.x : crs.x, inB ? -crs.y : crs.y);
+    }
+    // lines 2-3: rotate v' by d = q delta = 2 hd, hd = (u - 1/2) hd_scale = (g + 2^-24) hd_scale,
+    // g = 1.m - 1.5 exact, hd_c1 = 2^-24 hd_scale
+    const float2 hd = fma2(add2(make_float2(one_plus_m(wA0), one_plus_m(wB0)), bc2(-1.5f)), bc2(hd_scale), bc2(hd_c1));
+    float2 sh, ch;
+    sincos_small2(hd, sh, ch);
+    const float2 sh2 = add2(sh, sh);
+    const float2 sd = mul2(sh2, ch), omc = mul2(sh2, sh);       // sin d, 1 - cos d
+    const float2 tA = fma2(pA, bc2(-omc.x), pA), tB = fma2(pB, bc2(-omc.y), pB);
+    float rxA = fmaf(-sd.x, pA.y, tA.x), ryA = fmaf(sd.x, pA.x, tA.y);
+    float rxB = fmaf(-sd.y, pB.y, tB.x), ryB = fmaf(sd.y, pB.x, tB.y);
+    // line 4: dH = -h.(v'' - v') = (1 - cos d)(h.v') + sin d (h x v')
+    float2 dH = fma2(omc, dot, mul2(sd, crs));
+    if (QHALF) {
+        // q = 1/2: q phi in [0, pi]; leaving it <=> sin < 0; phi -/+ 2 pi <=> v -> -v
+        if (ryA < 0.0f) { rxA = -rxA; ryA = -ryA; dH.x = fmaf(2.0f, dot.x, -dH.x); }
+        if (ryB < 0.0f) { rxB = -rxB; ryB = -ryB; dH.y = fmaf(2.0f, dot.y, -dH.y); }
+    } else {
+        const bool underA = hd.x < 0.0f && ryA < 0.0f, overA = hd.x > 0.0f && !(ryA >= 0.0f && fmaf(rxA, bs, -ryA * bc) >= 0.0f);
+        const bool underB = hd.y < 0.0f && ryB < 0.0f, overB = hd.y > 0.0f && !(ryB >= 0.0f && fmaf(rxB, bs, -ryB * bc) >= 0.0f);
+        if (underA || overA) {
+            const float s2 = underA ? bs : -bs;
+            const float wx = fmaf(rxA, bc, -ryA * s2), wy = fmaf(rxA, s2, ryA * bc);
+            rxA = wx; ryA = wy;
+            dH.x = dot.x - fmaf(hA.x, wx, hA.y * wy);
+        }
+        if (underB || overB) {
+            const float s2 = underB ? bs : -bs;
+            const float wx = fmaf(rxB, bc, -ryB * s2), wy = fmaf(rxB, s2, ryB * bc);
+            rxB = wx; ryB = wy;
+            dH.y = dot.y - fmaf(hB.x, wx, hB.y * wy);
+        }
+    }
+    // lines 5-6: AP = min{1, exp(-dH/T)}; accept phi'' if AP > r else keep phi'
+    const float2 arg = mul2(dH, bc2(nlT));
+    const float2 r = add2(make_float2(one_plus_m(wA1), one_plus_m(wB1)), bc2(-0.99999994039535522461f));
+    accA = ex2_approx(arg.x) > r.x;
+    accB = ex2_approx(arg.y) > r.y;
+    vA = make_float2(accA ? rxA : pA.x, accA ? ryA : pA.y);
+    vB = make_float2(accB ? rxB : pB.x, accB ? ryB : pB.y);
+    if (renorm) {           // first-order Newton step of 1/|v|
+        const float2 nA = mul2(vA, vA), nB = mul2(vB, vB);
+        vA = mul2(vA, bc2(fmaf(-0.5f, nA.x + nA.y, 1.5f)));
+        vB = mul2(vB, bc2(fmaf(-0.5f, nB.x + nB.y, 1.5f)));
+    }
+}
+
 // ---- TMA / mbarrier PTX (sm_100a) -------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
@@ -555,8 +673,10 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 //   PASS_COUNT       a5: accepted proposals of the core sites                          [FUSED only]
 //   PASS_ACCUMULATE  a7: acc += phi at the core's prediction sites
 // ---------------------------------------------------------------------------
-template <bool QHALF, int ORMODE, bool FUSED>
-__global__ void __launch_bounds__(TILE_THREADS, 2)
+template <bool B> struct FreshTag { static constexpr bool value = B; };
+
+template <bool QHALF, int ORMODE, bool FUSED, int FCT>
+__global__ void __launch_bounds__(TILE_THREADS, 3)
 k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
            uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
 {
@@ -571,7 +691,9 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     const GridState& st = d.states[g];
     if (FUSED && (flags & PASS_CHECK_DONE) && st.done) return;
 
-    const int H = d.H, FC = d.FC;
+    // frame pitch: a compile-time constant for the standard tile shape (neighbour offsets become immediates)
+    const int H = d.H, FC = FCT ? FCT : d.FC;
+    const uint32_t fc_inv = FCT ? (uint32_t)(((1u << 24) + (uint32_t)(FCT ? FCT : 1) - 1u) / (uint32_t)(FCT ? FCT : 1)) : d.fc_inv;
     float2*   S  = reinterpret_cast<float2*>(smem_raw);
     uint2*    SP = reinterpret_cast<uint2*>(S + d.FR * FC);
     uint16_t* E  = reinterpret_cast<uint16_t*>(SP + (d.use_spare ? d.max_entries : 0u));
@@ -595,74 +717,69 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     const uint32_t t0 = st.t + t_off;
     const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H), ncorr = d.cols - FC;
     const bool count = FUSED && (flags & PASS_COUNT);
+    const bool use_spare = d.use_spare;
     uint32_t n_accepted = 0;
     mbar_wait(&s_bar, 0);
 
-    // |v| = 1 against rounding drift (first-order Newton step of 1/|v|) for entries [from, to)
-    auto renormalise = [&](uint32_t from, uint32_t to) {
-        for (uint32_t e = from + tid; e < to; e += NT) {
-            const uint32_t off = E[e];
-            const float2 v = S[off];
-            const float sc = fmaf(-0.5f, fmaf(v.x, v.x, v.y * v.y), 1.5f);
-            S[off] = make_float2(v.x * sc, v.y * sc);
-        }
-    };
-
-    for (uint32_t s = 0; s < K; ++s) {
-        const uint32_t t = t0 + s;
+    // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1)
+#pragma unroll 1
+    for (uint32_t j = 0; j < 2u * K; ++j) {
+        const uint32_t s = j >> 1, c = j & 1u, t = t0 + s;
         const bool odd = t & 1u;
-        const bool fresh = !odd || s == 0 || !d.use_spare;          // draw a new Philox block for (site, t >> 1)
-        const bool stash = d.use_spare && !odd && s + 1 < K;        // keep words 2,3 for sweep t + 1
-#pragma unroll 1
-        for (int c = 0; c < 2; ++c) {
-            const int R = (int)(2 * K) - 1 - (int)(2 * s + c);       // rings still needed
-            const uint32_t first = R + 1 <= MAX_H ? s_cge[c][R + 1] : 0u;
-            const uint32_t last = s_cge[c][0], core_from = s_cge[c][1];
-            const uint32_t base = c ? s_cge[0][0] : 0u;
-            // every thread takes the entries eA and eB = eA + stride; the last round splits what is left
-            // into two halves of whole warps, so that no warp runs a round for a missing second site
-#pragma unroll 1
-            for (uint32_t pos = first; pos < last;) {
-                const uint32_t rem = last - pos;
-                const uint32_t stride = rem >= 2u * NT ? (uint32_t)NT : ((rem + 63u) >> 6) << 5;
-                const uint32_t eA = pos + tid;
-                pos += 2u * stride;
-                if ((uint32_t)tid >= stride || eA >= last) continue;
-                const bool hasB = eA + stride < last;
-                const uint32_t eB = hasB ? eA + stride : eA;         // no second site: repeat the first, drop its result
-                const uint32_t offA = E[base + eA], offB = E[base + eB];
-                const float2 vA = S[offA], upA = S[offA - FC], dnA = S[offA + FC], lfA = S[offA - 1], rtA = S[offA + 1];
-                const float2 vB = S[offB], upB = S[offB - FC], dnB = S[offB + FC], lfB = S[offB - 1], rtB = S[offB + 1];
-                uint32_t wA0, wA1, wB0, wB1;
-                if (fresh) {
-                    const uint32_t nA = (uint32_t)(nbase + (int)offA + (int)((offA * d.fc_inv) >> 24) * ncorr);
-                    const uint32_t nB = (uint32_t)(nbase + (int)offB + (int)((offB * d.fc_inv) >> 24) * ncorr);
-                    const uint4 xA = philox4x32_10(nA, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
-                    const uint4 xB = philox4x32_10(nB, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
-                    wA0 = odd ? xA.z : xA.x; wA1 = odd ? xA.w : xA.y;
-                    wB0 = odd ? xB.z : xB.x; wB1 = odd ? xB.w : xB.y;
-                    if (stash) { SP[base + eA] = make_uint2(xA.z, xA.w); SP[base + eB] = make_uint2(xB.z, xB.w); }
-                } else {
-                    const uint2 sA = SP[base + eA], sB = SP[base + eB];
-                    wA0 = sA.x; wA1 = sA.y; wB0 = sB.x; wB1 = sB.y;
-                }
-                bool accA, accB;
-                const float2 newA = update_site<QHALF, ORMODE>(vA, upA, dnA, lfA, rtA, wA0, wA1, hs, hc1, nlT, d.bc, d.bs, accA);
-                const float2 newB = update_site<QHALF, ORMODE>(vB, upB, dnB, lfB, rtB, wB0, wB1, hs, hc1, nlT, d.bc, d.bs, accB);
-                S[offA] = newA;
-                if (hasB) S[offB] = newB;
-                if (count) n_accepted += (accA && eA >= core_from) + (accB && hasB && eB >= core_from);
+        const bool fresh = !odd || s == 0 || !use_spare;            // draw a new Philox block for (site, t >> 1)
+        const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
+        // |v| = 1 against rounding drift: in the sweep whose result leaves the tile, and every 8th sweep of a long pass
+        const bool renorm = s + 1 == K || (s & 7u) == 7u;
+        const uint32_t R = 2u * K - 1u - j;                          // rings still needed
+        const uint32_t first = R + 1 <= MAX_H ? s_cge[c][R + 1] : 0u;
+        const uint32_t last = s_cge[c][0], core_from = s_cge[c][1];
+        const uint16_t* Ec = E + (c ? s_cge[0][0] : 0u);
+        uint2* SPc = SP + (c ? s_cge[0][0] : 0u);
+
+        // the sites eA and eB of this colour's list (eB == eA: no second site, its result is dropped).
+        // FRESH is a compile-time tag so that the Philox rounds and the update arithmetic of a drawing
+        // sweep sit in one basic block (independent instruction streams for the scheduler to interleave).
+        auto update_two = [&](auto fresh_tag, uint32_t eA, uint32_t eB) {
+            constexpr bool FRESH = decltype(fresh_tag)::value;
+            const uint32_t offA = Ec[eA], offB = Ec[eB];
+            float2 vA = S[offA], vB = S[offB];
+            const float2 upA = S[offA - FC], dnA = S[offA + FC], lfA = S[offA - 1], rtA = S[offA + 1];
+            const float2 upB = S[offB - FC], dnB = S[offB + FC], lfB = S[offB - 1], rtB = S[offB + 1];
+            uint32_t wA0, wA1, wB0, wB1;
+            if (FRESH) {
+                const uint32_t nA = (uint32_t)(nbase + (int)offA + (int)((offA * fc_inv) >> 24) * ncorr);
+                const uint32_t nB = (uint32_t)(nbase + (int)offB + (int)((offB * fc_inv) >> 24) * ncorr);
+                const uint4 xA = philox4x32_10(nA, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
+                const uint4 xB = philox4x32_10(nB, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
+                wA0 = odd ? xA.z : xA.x; wA1 = odd ? xA.w : xA.y;
+                wB0 = odd ? xB.z : xB.x; wB1 = odd ? xB.w : xB.y;
+                if (stash) { SPc[eA] = make_uint2(xA.z, xA.w); SPc[eB] = make_uint2(xB.z, xB.w); }
+            } else {
+                const uint2 sA = SPc[eA], sB = SPc[eB];
+                wA0 = sA.x; wA1 = sA.y; wB0 = sB.x; wB1 = sB.y;
             }
-            __syncthreads();
-        }
-        if ((s & 7u) == 7u && s + 1 < K) {       // long single-tile passes: bound the drift of |v|
-            renormalise(0, s_cge[0][0] + s_cge[1][0]);
-            __syncthreads();
-        }
+            bool accA, accB;
+            update_pair<QHALF, ORMODE>(vA, upA, dnA, lfA, rtA, vB, upB, dnB, lfB, rtB, wA0, wA1, wB0, wB1,
+                                       hs, hc1, nlT, d.bc, d.bs, renorm, accA, accB);
+            S[offA] = vA;
+            if (eB != eA) S[offB] = vB;
+            if (count) n_accepted += (accA && eA >= core_from) + (accB && eB != eA && eB >= core_from);
+        };
+        // full rounds: thread tid takes the entries pos + tid and pos + NT + tid; the last round splits what
+        // is left into two halves of whole warps, so that no warp runs a round for a missing second site
+        auto half_sweep = [&](auto fresh_tag) {
+            uint32_t pos = first;
+#pragma unroll 1
+            for (; pos + 2u * NT <= last; pos += 2u * NT) update_two(fresh_tag, pos + tid, pos + NT + tid);
+            if (pos < last) {
+                const uint32_t stride = ((last - pos + 63u) >> 6) << 5;
+                const uint32_t eA = pos + tid;
+                if ((uint32_t)tid < stride && eA < last) update_two(fresh_tag, eA, eA + stride < last ? eA + stride : eA);
+            }
+        };
+        if (fresh) half_sweep(FreshTag<true>{}); else half_sweep(FreshTag<false>{});
+        __syncthreads();
     }
-    // the core's prediction sites (ring 0), both colours, before they leave
-    renormalise(s_cge[0][1], s_cge[0][0]);
-    renormalise(s_cge[0][0] + s_cge[1][1], s_cge[0][0] + s_cge[1][0]);
     fence_proxy_async_smem();
     __syncthreads();
 
@@ -678,7 +795,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             const uint32_t base = c ? s_cge[0][0] : 0u;
             for (uint32_t e = s_cge[c][1] + tid; e < s_cge[c][0]; e += NT) {
                 const uint32_t off = E[base + e];
-                acc[nbase + (int)off + (int)((off * d.fc_inv) >> 24) * ncorr] += angle_of(S[off], d.inv_q);
+                acc[nbase + (int)off + (int)((off * fc_inv) >> 24) * ncorr] += angle_of(S[off], d.inv_q);
             }
         }
     }
