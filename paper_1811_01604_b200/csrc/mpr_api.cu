@@ -56,7 +56,7 @@ void choose_tiles(int rows, int cols, Geometry* g)
     g->FC = ((TC + 2 * H + 1) & ~3) + 2;        // >= TC + 2H and = 2 (mod 4): a column's rows spread over the banks
     g->ntx = (cols + TC - 1) / TC; g->nty = (rows + TR - 1) / TR; g->ntiles = g->ntx * g->nty;
     g->n_partials = (uint32_t)(g->ntiles > ENERGY_BLOCKS ? g->ntiles : ENERGY_BLOCKS);
-    g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 7) & ~(size_t)7);
+    g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 31) & ~(size_t)15);   // two 16-aligned lists per tile
 }
 
 bool make_geometry(int batch, int rows, int cols, Geometry* g)
@@ -90,7 +90,7 @@ Layout make_layout(int batch, const Geometry& g)
     L.vec       = take(2 * B * g.VG * sizeof(float2));
     L.acc       = take(B * g.N * sizeof(float));
     L.tile_meta = take(B * g.ntiles * sizeof(TileMeta));
-    L.entries   = take((B * g.entry_stride + 8) * sizeof(uint16_t));
+    L.entries   = take((B * g.entry_stride + 16) * sizeof(uint16_t));
     L.total = o;
     return L;
 }
@@ -308,7 +308,11 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     k_transform<<<dim3(cdiv((size_t)g.words * 32, 256), batch), 256, 0, s>>>(d, d_values, d_sample_mask);
     k_tile_count<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
     k_tile_scan<<<batch, 32, 0, s>>>(d);
-    k_tile_fill<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
+    const size_t fill_smem = (size_t)g.FR * g.FC * sizeof(uint16_t);
+    if (fill_smem > 40960 &&
+        !cuda_ok(cudaFuncSetAttribute((const void*)k_tile_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fill_smem), "k_tile_fill smem"))
+        return fail(MPR_ERR_CUDA);
+    k_tile_fill<<<dim3(g.ntiles, batch), 256, fill_smem, s>>>(d);
     ctx->launches += 7;
     if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
     st = fetch_states(ctx);
@@ -324,7 +328,7 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     uint32_t max_entries = 0;
     for (int b = 0; b < batch; ++b)
         if (ctx->h_states[b].max_tile_entries > max_entries) max_entries = ctx->h_states[b].max_tile_entries;
-    max_entries = (max_entries + 7u) & ~7u;
+    max_entries = (max_entries + 15u) & ~15u;
     d.max_entries = max_entries;
     const size_t frame_bytes = (size_t)g.FR * g.FC * sizeof(float2);
     int smem_max = 0;

@@ -56,9 +56,11 @@ struct GridState {
 
 // Free sites of one tile frame (core + halo), see k_tile_fill.
 struct TileMeta {
-    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid), multiple of 8
-    uint32_t cge[2][MAX_H + 1];       // cge[c][k] = entries of colour c with ring >= k (ring = distance outside the core)
+    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid), multiple of 16
+    uint32_t cle[2][MAX_H];           // cle[c][k] = entries of colour c with ring <= k (ring = distance outside the core)
 };
+// colour 1's list starts on a 16-entry boundary after colour 0's
+__host__ __device__ __forceinline__ uint32_t colour1_base(uint32_t n0) { return (n0 + 15u) & ~15u; }
 
 // Device view of one context (passed by value to kernels).
 struct Dev {
@@ -309,13 +311,13 @@ __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restric
 // its core plus a halo of H sites on every side.  For each tile the free
 // sites of the frame with ring < H (ring = Chebyshev distance outside the
 // core, 0 inside) are listed per colour (checkerboard split),
-// outermost ring first, so that the sites a half-sweep of a K-sweep pass
-// still needs are a suffix of the list.  Within one (colour, ring) class the
-// entries are dealt round-robin over the 16 eight-byte slots of a 128-byte
-// shared-memory line, so that 16 consecutive entries (one half-warp of a
-// 64-bit shared load) hit 16 different bank pairs: the loads of a site, of
-// its four neighbours (the same shift for every lane) and the store are then
-// free of bank conflicts.
+// core first, then ring 1, 2, ..., so that the sites a half-sweep of a
+// K-sweep pass still needs are a prefix of the list.  A half-warp of a
+// 64-bit shared-memory access is served in one wavefront when its 16 lanes
+// fall into 16 different eight-byte slots of a 128-byte line (slot = frame
+// offset mod 16; the four neighbours shift every lane's slot alike).  The
+// list is therefore built 16 entries at a time, each group taking sites of
+// slots it does not hold yet, fullest slot first (k_tile_fill).
 // ---------------------------------------------------------------------------
 struct TileGeom { int r0, c0, TRc, TCc; };
 
@@ -345,8 +347,8 @@ __device__ __forceinline__ bool frame_site_class(const Dev& d, const uint32_t* _
 __global__ void __launch_bounds__(256) k_tile_count(Dev d)
 {
     const int tile = blockIdx.x, g = blockIdx.y;
-    __shared__ uint32_t hist[2][MAX_H + 1];
-    for (int i = threadIdx.x; i < 2 * (MAX_H + 1); i += blockDim.x) (&hist[0][0])[i] = 0;
+    __shared__ uint32_t hist[2][MAX_H];
+    for (int i = threadIdx.x; i < 2 * MAX_H; i += blockDim.x) (&hist[0][0])[i] = 0;
     __syncthreads();
     const TileGeom t = tile_geom(d, tile);
     const uint32_t* bits = d.bits + (size_t)g * d.words;
@@ -360,12 +362,12 @@ __global__ void __launch_bounds__(256) k_tile_count(Dev d)
         TileMeta& m = d.tile_meta[(size_t)g * d.ntiles + tile];
         const int c = threadIdx.x;
         uint32_t run = 0;
-        for (int k = MAX_H; k >= 0; --k) { run += hist[c][k]; m.cge[c][k] = run; }
+        for (int k = 0; k < MAX_H; ++k) { run += hist[c][k]; m.cle[c][k] = run; }
     }
 }
 
-// one warp per grid: exclusive scan of the tiles' entry counts (each rounded up to a multiple of 8
-// so that every tile's list starts on a 16-byte boundary), and their maximum
+// one warp per grid: exclusive scan of the tiles' entry counts (each rounded up to a multiple of 16
+// so that every tile's list starts on a 32-byte boundary), and their maximum
 __global__ void k_tile_scan(Dev d)
 {
     const int g = blockIdx.x;
@@ -374,7 +376,7 @@ __global__ void k_tile_scan(Dev d)
     uint32_t carry = 0, mx = 0;
     for (int base = 0; base < d.ntiles; base += 32) {
         const int i = base + lane;
-        const uint32_t c = i < d.ntiles ? (m[i].cge[0][0] + m[i].cge[1][0] + 7u) & ~7u : 0u;
+        const uint32_t c = i < d.ntiles ? (colour1_base(m[i].cle[0][MAX_H - 1]) + m[i].cle[1][MAX_H - 1] + 15u) & ~15u : 0u;
         mx = max(mx, c);
         uint32_t x = c;
 #pragma unroll
@@ -390,10 +392,13 @@ __global__ void k_tile_scan(Dev d)
     if (lane == 0) d.states[g].max_tile_entries = mx;
 }
 
+// dynamic shared memory: FR * FC uint16 (the frame's free sites bucketed by colour, ring, slot)
 __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
 {
     const int tile = blockIdx.x, g = blockIdx.y;
+    extern __shared__ uint16_t bucketed[];
     __shared__ uint32_t cnt[2][MAX_H][16];       // free sites per (colour, ring, slot)
+    __shared__ uint32_t start[2][MAX_H][16];     // bucket offsets in bucketed[]
     __shared__ uint32_t cursor[2][MAX_H][16];
     for (int i = threadIdx.x; i < 2 * MAX_H * 16; i += blockDim.x) { (&cnt[0][0][0])[i] = 0; (&cursor[0][0][0])[i] = 0; }
     __syncthreads();
@@ -407,21 +412,40 @@ __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
         if (frame_site_class(d, bits, t, lr, lc, colour, ring)) atomicAdd(&cnt[colour][ring][i & 15], 1u);
     }
     __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = 0;
+        for (int i = 0; i < 2 * MAX_H * 16; ++i) { (&start[0][0][0])[i] = run; run += (&cnt[0][0][0])[i]; }
+    }
+    __syncthreads();
     for (int i = threadIdx.x; i < d.FR * d.FC; i += blockDim.x) {
         const int lr = i / d.FC, lc = i - lr * d.FC;
         int colour, ring;
         if (frame_site_class(d, bits, t, lr, lc, colour, ring)) {
-            const uint32_t b = i & 15, j = atomicAdd(&cursor[colour][ring][b], 1u);
-            // rank of (round j, slot b) when the class is dealt round-robin over its 16 slots
-            uint32_t pos = 0;
-#pragma unroll
-            for (uint32_t bb = 0; bb < 16; ++bb) {
-                const uint32_t c = cnt[colour][ring][bb];
-                pos += min(c, j) + (bb < b && c > j ? 1u : 0u);
+            const uint32_t b = i & 15;
+            bucketed[start[colour][ring][b] + atomicAdd(&cursor[colour][ring][b], 1u)] = (uint16_t)i;
+        }
+    }
+    __syncthreads();
+    // warp c builds colour c's list: lane b < 16 owns slot b.  Every position takes the site of the slot
+    // that occurs least in the current group of 16, fullest slot first.
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (c >= 2) return;
+    uint32_t pos = c ? colour1_base(m.cle[0][MAX_H - 1]) : 0u;
+    uint32_t in_group = 0;                        // how often this lane's slot occurs in the current group
+    for (int ring = 0; ring < d.H; ++ring) {
+        uint32_t rem = lane < 16 ? cnt[c][ring][lane] : 0u;
+        const uint32_t from = lane < 16 ? start[c][ring][lane] : 0u;
+        uint32_t taken = 0;
+        for (;;) {
+            if ((pos & 15u) == 0u) in_group = 0;  // a new group starts
+            const uint32_t key = rem ? ((15u - min(in_group, 15u)) << 24) | (min(rem, 0xFFFFFu) << 4) | (uint32_t)lane : 0u;
+            const uint32_t best = __reduce_max_sync(0xFFFFFFFFu, key);
+            if (best == 0u) break;
+            if (lane == (int)(best & 15u)) {
+                out[pos] = bucketed[from + taken];
+                ++taken; --rem; ++in_group;
             }
-            // colour 0 first; within a colour the rings in descending order
-            pos += (colour ? m.cge[0][0] : 0u) + m.cge[colour][ring + 1];
-            out[pos] = (uint16_t)i;
+            ++pos;
         }
     }
 }
@@ -682,7 +706,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar;
-    __shared__ uint32_t s_cge[2][MAX_H + 1];
+    __shared__ uint32_t s_cle[2][MAX_H];
     __shared__ uint32_t s_accepted;
     __shared__ double s_red[TILE_THREADS / 32];
 
@@ -705,10 +729,10 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     float2* dst = vec_grid(d, g, src_buf ^ 1u);
 
     if (tid == 0) { mbar_init(&s_bar, 1); s_accepted = 0; }
-    if (tid < 2 * (MAX_H + 1)) (&s_cge[0][0])[tid] = (&meta.cge[0][0])[tid];
+    if (tid < 2 * MAX_H) (&s_cle[0][0])[tid] = (&meta.cle[0][0])[tid];
     __syncthreads();
     if (tid == 0) {
-        const uint32_t entry_bytes = ((s_cge[0][0] + s_cge[1][0] + 7u) & ~7u) * (uint32_t)sizeof(uint16_t);
+        const uint32_t entry_bytes = ((colour1_base(s_cle[0][MAX_H - 1]) + s_cle[1][MAX_H - 1] + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
         mbar_expect_tx(&s_bar, (uint32_t)(d.FR * FC * sizeof(float2)) + entry_bytes);
         tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar);
         if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar);
@@ -730,11 +754,11 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
         // |v| = 1 against rounding drift: in the sweep whose result leaves the tile, and every 8th sweep of a long pass
         const bool renorm = s + 1 == K || (s & 7u) == 7u;
-        const uint32_t R = 2u * K - 1u - j;                          // rings still needed
-        const uint32_t first = R + 1 <= MAX_H ? s_cge[c][R + 1] : 0u;
-        const uint32_t last = s_cge[c][0], core_from = s_cge[c][1];
-        const uint16_t* Ec = E + (c ? s_cge[0][0] : 0u);
-        uint2* SPc = SP + (c ? s_cge[0][0] : 0u);
+        const uint32_t R = 2u * K - 1u - j;                          // rings still needed: 0 .. R
+        const uint32_t n = s_cle[c][R < (uint32_t)MAX_H ? R : (uint32_t)MAX_H - 1u], n_core = s_cle[c][0];
+        const uint32_t cbase = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
+        const uint16_t* Ec = E + cbase;
+        uint2* SPc = SP + cbase;
 
         // the sites eA and eB of this colour's list (eB == eA: no second site, its result is dropped).
         // FRESH is a compile-time tag so that the Philox rounds and the update arithmetic of a drawing
@@ -763,18 +787,18 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
                                        hs, hc1, nlT, d.bc, d.bs, renorm, accA, accB);
             S[offA] = vA;
             if (eB != eA) S[offB] = vB;
-            if (count) n_accepted += (accA && eA >= core_from) + (accB && eB != eA && eB >= core_from);
+            if (count) n_accepted += (accA && eA < n_core) + (accB && eB != eA && eB < n_core);
         };
         // full rounds: thread tid takes the entries pos + tid and pos + NT + tid; the last round splits what
         // is left into two halves of whole warps, so that no warp runs a round for a missing second site
         auto half_sweep = [&](auto fresh_tag) {
-            uint32_t pos = first;
+            uint32_t pos = 0;
 #pragma unroll 1
-            for (; pos + 2u * NT <= last; pos += 2u * NT) update_two(fresh_tag, pos + tid, pos + NT + tid);
-            if (pos < last) {
-                const uint32_t stride = ((last - pos + 63u) >> 6) << 5;
+            for (; pos + 2u * NT <= n; pos += 2u * NT) update_two(fresh_tag, pos + tid, pos + NT + tid);
+            if (pos < n) {
+                const uint32_t stride = ((n - pos + 63u) >> 6) << 5;
                 const uint32_t eA = pos + tid;
-                if ((uint32_t)tid < stride && eA < last) update_two(fresh_tag, eA, eA + stride < last ? eA + stride : eA);
+                if ((uint32_t)tid < stride && eA < n) update_two(fresh_tag, eA, eA + stride < n ? eA + stride : eA);
             }
         };
         if (fresh) half_sweep(FreshTag<true>{}); else half_sweep(FreshTag<false>{});
@@ -792,8 +816,8 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites
         float* acc = d.acc + (size_t)g * d.N;
         for (int c = 0; c < 2; ++c) {
-            const uint32_t base = c ? s_cge[0][0] : 0u;
-            for (uint32_t e = s_cge[c][1] + tid; e < s_cge[c][0]; e += NT) {
+            const uint32_t base = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
+            for (uint32_t e = tid; e < s_cle[c][0]; e += NT) {
                 const uint32_t off = E[base + e];
                 acc[nbase + (int)off + (int)((off * fc_inv) >> 24) * ncorr] += angle_of(S[off], d.inv_q);
             }
