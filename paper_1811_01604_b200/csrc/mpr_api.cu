@@ -115,6 +115,8 @@ struct mpr_ctx {
     bool         qhalf;
     bool         dirty;           // vectors changed since d.phi was last written at the free sites
     int          device;          // device the workspace lives on
+    uint32_t     cur;             // vector buffer holding the current state, the same for every grid outside mpr_equilibrate
+    uint32_t     pf_dist;         // tile passes resident on the device at once (L2 prefetch distance), 0 = not yet known
 };
 
 namespace {
@@ -126,7 +128,7 @@ mpr_status fetch_states(mpr_ctx* ctx)
     return MPR_OK;
 }
 
-typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t);
+typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t);
 
 // fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps);
 // std_fc = the frame pitch is the compile-time STD_FC (standard tile shape)
@@ -145,14 +147,23 @@ pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused, bool std_fc)
     return std_fc ? pick_pass_kernel_fc<STD_FC>(qhalf, or_mode, fused) : pick_pass_kernel_fc<0>(qhalf, or_mode, fused);
 }
 
-// K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile
+// K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile.
+// flip = 0 / 1: read buffer ctx->cur ^ flip (known to the host); PER_GRID: each grid reads its own GridState::cur
+enum : uint32_t { PER_GRID = 2u };
 mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
 {
     ctx->dirty = true;
     const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
-    pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC)
-        <<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(
-            ctx->map[0], ctx->map[1], ctx->d, K, t_off, flip, flags);
+    const pass_kernel kern = pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC);
+    if (!ctx->pf_dist) {
+        int per_sm = 0, sms = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)kern, TILE_THREADS, ctx->smem_bytes));
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
+        ctx->pf_dist = (uint32_t)(per_sm > 0 ? per_sm * sms : sms);
+    }
+    const uint32_t src_sel = flip == PER_GRID ? PER_GRID : (ctx->cur ^ flip);
+    kern<<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(
+        ctx->map[0], ctx->map[1], ctx->d, K, t_off, src_sel, flags, ctx->pf_dist);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -395,6 +406,7 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
     ctx->state = READY;
     ctx->dirty = false;
+    ctx->cur = 0;
     return MPR_OK;
 }
 
@@ -413,7 +425,7 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
         for (uint32_t j = 0; j < chunk; ++j) {
             // 5.1 one sweep with the energy (5.3) and the accepted count fused; the controller does
             // 5.2, 5.4, 5.5 and commits the sweep (t, buffer swap) for the grids still running
-            mpr_status s = launch_pass(ctx, 1, 0, 0, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
+            mpr_status s = launch_pass(ctx, 1, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
             if (s != MPR_OK) return s;
             k_controller<<<d.batch, 32, 0, ctx->stream>>>(d);
             CU_LAUNCH();
@@ -426,6 +438,18 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
         if (all) break;
         chunk = ctx->prm.n_f;
     }
+    // the grids stopped after different numbers of sweeps: bring every state into the same vector buffer
+    mpr_status fs = fetch_states(ctx);
+    if (fs != MPR_OK) return fs;
+    bool any0 = false, any1 = false;
+    for (int b = 0; b < d.batch; ++b) (ctx->h_states[b].cur ? any1 : any0) = true;
+    if (any0 && any1) {
+        k_unify_cur<<<dim3(cdiv(d.VG, 256), d.batch), 256, 0, ctx->stream>>>(d);
+        CU_LAUNCH();
+        k_set_cur<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0u);
+        CU_LAUNCH();
+        ctx->cur = 0;
+    } else ctx->cur = any1 ? 1u : 0u;
     return MPR_OK;
 }
 
@@ -446,6 +470,7 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
     }
     k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, t_off, flip, ctx->prm.M);
     CU_LAUNCH();
+    ctx->cur ^= flip;
     return MPR_OK;
 }
 
@@ -509,6 +534,7 @@ mpr_status mpr_sweep(mpr_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_acce
     if (rs != MPR_OK) return rs;
     k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, t_off, flip, 0);
     CU_LAUNCH();
+    ctx->cur ^= flip;
     if (h_accepted) {
         mpr_status s = fetch_states(ctx);
         if (s != MPR_OK) return s;

@@ -664,6 +664,16 @@ __device__ __forceinline__ void tma_load_frame(void* dst, const CUtensorMap* map
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                  ::"r"(smem_u32(dst)), "l"((uint64_t)map), "r"(c), "r"(r), "r"(g), "r"(smem_u32(bar)) : "memory");
 }
+// L2 prefetch of a frame box / of a byte range (no shared-memory destination, no completion to wait for)
+__device__ __forceinline__ void tma_prefetch_frame(const CUtensorMap* map, int c, int r, int g)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                 ::"l"((uint64_t)map), "r"(c), "r"(r), "r"(g) : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch(const void* src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"((uint64_t)src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -700,12 +710,12 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 template <bool B> struct FreshTag { static constexpr bool value = B; };
 
 template <bool QHALF, int ORMODE, bool FUSED, int FCT>
-__global__ void __launch_bounds__(TILE_THREADS, 3)
+__global__ void __launch_bounds__(TILE_THREADS, TILE_THREADS >= 384 ? 2 : 3)
 k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
-           uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
+           uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t s_bar;
+    __shared__ __align__(8) uint64_t s_bar[2];       // [0] frame, [1] entry list
     __shared__ uint32_t s_cle[2][MAX_H];
     __shared__ uint32_t s_accepted;
     __shared__ double s_red[TILE_THREADS / 32];
@@ -725,25 +735,37 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const TileGeom tg = tile_geom(d, tile);
     const TileMeta& meta = d.tile_meta[(size_t)g * d.ntiles + tile];
-    const uint32_t src_buf = st.cur ^ flip;
+    // src_sel 0 / 1: the source buffer is known to the host (every grid alike); 2: per grid, from its state
+    const uint32_t src_buf = src_sel < 2u ? src_sel : st.cur;
     float2* dst = vec_grid(d, g, src_buf ^ 1u);
 
-    if (tid == 0) { mbar_init(&s_bar, 1); s_accepted = 0; }
-    if (tid < 2 * MAX_H) (&s_cle[0][0])[tid] = (&meta.cle[0][0])[tid];
-    __syncthreads();
+    // three warps start the tile: warp 0 the frame (before anything else is known about the tile), warp 1 the
+    // entry list (needs the tile's counts from global memory first), warp 2 the L2 prefetch
     if (tid == 0) {
-        const uint32_t entry_bytes = ((colour1_base(s_cle[0][MAX_H - 1]) + s_cle[1][MAX_H - 1] + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
-        mbar_expect_tx(&s_bar, (uint32_t)(d.FR * FC * sizeof(float2)) + entry_bytes);
-        tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar);
-        if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar);
+        mbar_init(&s_bar[0], 1); s_accepted = 0;
+        mbar_expect_tx(&s_bar[0], (uint32_t)(d.FR * FC * sizeof(float2)));
+        tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar[0]);
+    } else if (tid == 32) {
+        mbar_init(&s_bar[1], 1);
+        const uint32_t n0 = meta.cle[0][MAX_H - 1], n1 = meta.cle[1][MAX_H - 1];
+        const uint32_t entry_bytes = ((colour1_base(n0) + n1 + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
+        mbar_expect_tx(&s_bar[1], entry_bytes);
+        if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar[1]);
+    } else if (tid == 64 && pf_dist && tile + (int)pf_dist < d.ntiles) {
+        // pull the frame of the tile that will run in this slot next towards L2
+        const TileGeom tn = tile_geom(d, tile + (int)pf_dist);
+        tma_prefetch_frame(src_buf ? &map1 : &map0, tn.c0 - H, tn.r0 - H, g);
     }
+    if (tid >= 96 && tid < 96 + 2 * MAX_H) (&s_cle[0][0])[tid - 96] = (&meta.cle[0][0])[tid - 96];
     const float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f, nlT = st.neg_log2e_over_T;
     const uint32_t t0 = st.t + t_off;
     const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H), ncorr = d.cols - FC;
     const bool count = FUSED && (flags & PASS_COUNT);
     const bool use_spare = d.use_spare;
     uint32_t n_accepted = 0;
-    mbar_wait(&s_bar, 0);
+    __syncthreads();
+    mbar_wait(&s_bar[1], 0);
+    mbar_wait(&s_bar[0], 0);
 
     // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1)
 #pragma unroll 1
@@ -809,8 +831,9 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 
     // write the core back, one bulk copy per row (an odd last column takes the zero pad column along)
     const uint32_t row_bytes = (uint32_t)((tg.TCc + 1) & ~1) * (uint32_t)sizeof(float2);
-    for (int lr = tid; lr < tg.TRc; lr += NT)
-        bulk_store(dst + (size_t)(tg.r0 + lr) * d.pitch + tg.c0, S + (H + lr) * FC + H, row_bytes);
+    if (lane == 0)          // one issuing lane per warp: the copy engine takes its operands from uniform registers
+        for (int lr = warp; lr < tg.TRc; lr += NW)
+            bulk_store(dst + (size_t)(tg.r0 + lr) * d.pitch + tg.c0, S + (H + lr) * FC + H, row_bytes);
 
     if (flags & PASS_ACCUMULATE) {
         // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites
@@ -973,6 +996,18 @@ __global__ void k_commit(Dev d, uint32_t n_sweeps, uint32_t flip, uint32_t n_rea
     if (g >= d.batch) return;
     GridState& s = d.states[g];
     s.t += n_sweeps; s.cur ^= flip; s.realizations += n_realizations;
+}
+// after equilibration: grids whose state sits in buffer 1 are copied into buffer 0 (then k_set_cur(0))
+__global__ void __launch_bounds__(256) k_unify_cur(Dev d)
+{
+    const int g = blockIdx.y;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < d.VG && d.states[g].cur == 1u) vec_grid(d, g, 0)[i] = vec_grid(d, g, 1)[i];
+}
+__global__ void k_set_cur(Dev d, uint32_t cur)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g < d.batch) d.states[g].cur = cur;
 }
 __global__ void k_set_t(Dev d, uint32_t t)
 {
