@@ -115,6 +115,8 @@ struct mpr_ctx {
     bool         qhalf;
     bool         dirty;           // vectors changed since d.phi was last written at the free sites
     int          device;          // device the workspace lives on
+    double       a_min;           // smallest proposal-width parameter a over the grids, as far as the host knows it (0 = unknown)
+    bool         small_d;         // every grid's proposal half-rotation q pi / (2 a) is below SMALL_HD (host knowledge of a)
     uint32_t     cur;             // vector buffer holding the current state, the same for every grid outside mpr_equilibrate
     uint32_t     pf_dist;         // tile passes resident on the device at once (L2 prefetch distance), 0 = not yet known
 };
@@ -132,19 +134,30 @@ typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uin
 
 // fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps);
 // std_fc = the frame pitch is the compile-time STD_FC (standard tile shape)
-template <int FCT>
-pass_kernel pick_pass_kernel_fc(bool qhalf, int or_mode, bool fused)
+// small_d = every proposal half-rotation is below SMALL_HD (short sin / cos polynomials); only without the fused tails
+template <int FCT, bool SMALLD>
+pass_kernel pick_pass_kernel_fc(bool qhalf, int or_mode)
 {
-    if (fused) {
-        if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true, FCT> : or_mode == 1 ? k_tilepass<true, 1, true, FCT> : k_tilepass<true, 2, true, FCT>;
-        return or_mode == 0 ? k_tilepass<false, 0, true, FCT> : k_tilepass<false, 2, true, FCT>;
-    }
-    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, false, FCT> : or_mode == 1 ? k_tilepass<true, 1, false, FCT> : k_tilepass<true, 2, false, FCT>;
-    return or_mode == 0 ? k_tilepass<false, 0, false, FCT> : k_tilepass<false, 2, false, FCT>;
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, false, FCT, SMALLD> : or_mode == 1 ? k_tilepass<true, 1, false, FCT, SMALLD> : k_tilepass<true, 2, false, FCT, SMALLD>;
+    return or_mode == 0 ? k_tilepass<false, 0, false, FCT, SMALLD> : k_tilepass<false, 2, false, FCT, SMALLD>;
 }
-pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused, bool std_fc)
+template <int FCT>
+pass_kernel pick_fused_kernel_fc(bool qhalf, int or_mode)
 {
-    return std_fc ? pick_pass_kernel_fc<STD_FC>(qhalf, or_mode, fused) : pick_pass_kernel_fc<0>(qhalf, or_mode, fused);
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true, FCT, false> : or_mode == 1 ? k_tilepass<true, 1, true, FCT, false> : k_tilepass<true, 2, true, FCT, false>;
+    return or_mode == 0 ? k_tilepass<false, 0, true, FCT, false> : k_tilepass<false, 2, true, FCT, false>;
+}
+pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused, bool std_fc, bool small_d)
+{
+    if (fused) return std_fc ? pick_fused_kernel_fc<STD_FC>(qhalf, or_mode) : pick_fused_kernel_fc<0>(qhalf, or_mode);
+    if (small_d) return std_fc ? pick_pass_kernel_fc<STD_FC, true>(qhalf, or_mode) : pick_pass_kernel_fc<0, true>(qhalf, or_mode);
+    return std_fc ? pick_pass_kernel_fc<STD_FC, false>(qhalf, or_mode) : pick_pass_kernel_fc<0, false>(qhalf, or_mode);
+}
+
+void note_a(mpr_ctx* ctx, double a_min)
+{
+    ctx->a_min = a_min;
+    ctx->small_d = a_min > 0.0 && (double)ctx->prm.q * 3.14159265358979323846 / (2.0 * a_min) <= (double)SMALL_HD;
 }
 
 // K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile.
@@ -154,7 +167,7 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
 {
     ctx->dirty = true;
     const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
-    const pass_kernel kern = pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC);
+    const pass_kernel kern = pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC, ctx->small_d);
     if (!ctx->pf_dist) {
         int per_sm = 0, sms = 0;
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)kern, TILE_THREADS, ctx->smem_bytes));
@@ -356,11 +369,12 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     }
     for (int qh = 0; qh < 2; ++qh)
         for (int om = 0; om < 3; ++om)
-            for (int fu = 0; fu < 2; ++fu) {
-                if (!qh && om == 1) continue;
-                if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, g.FC == STD_FC), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                  (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
-            }
+            for (int fu = 0; fu < 2; ++fu)
+                for (int sd = 0; sd < 2; ++sd) {
+                    if (!qh && om == 1) continue;
+                    if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, g.FC == STD_FC, sd), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                      (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
+                }
     *out = ctx;
     return MPR_OK;
 }
@@ -407,6 +421,7 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     ctx->state = READY;
     ctx->dirty = false;
     ctx->cur = 0;
+    note_a(ctx, 1.0);
     return MPR_OK;
 }
 
@@ -442,7 +457,12 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
     mpr_status fs = fetch_states(ctx);
     if (fs != MPR_OK) return fs;
     bool any0 = false, any1 = false;
-    for (int b = 0; b < d.batch; ++b) (ctx->h_states[b].cur ? any1 : any0) = true;
+    double a_min = ctx->h_states[0].a;
+    for (int b = 0; b < d.batch; ++b) {
+        (ctx->h_states[b].cur ? any1 : any0) = true;
+        if (ctx->h_states[b].a < a_min) a_min = ctx->h_states[b].a;
+    }
+    note_a(ctx, a_min);
     if (any0 && any1) {
         k_unify_cur<<<dim3(cdiv(d.VG, 256), d.batch), 256, 0, ctx->stream>>>(d);
         CU_LAUNCH();
@@ -462,6 +482,7 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
     const uint32_t s_per = ctx->prm.sweeps_per_real;
     k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, ctx->prm.a_eq_mode == 1 ? 0 : 1, 1.0, 0);
     CU_LAUNCH();
+    if (ctx->prm.a_eq_mode == 1) note_a(ctx, 1.0);
     uint32_t t_off = 0, flip = 0;
     for (uint32_t j = 0; j < ctx->prm.M; ++j) {
         // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
@@ -529,6 +550,7 @@ mpr_status mpr_sweep(mpr_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_acce
     const Dev& d = ctx->d;
     k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, a, 1);       // also zeroes the accepted counters
     CU_LAUNCH();
+    note_a(ctx, a);
     uint32_t t_off = 0, flip = 0;
     mpr_status rs = launch_sweeps(ctx, n_sweeps, &t_off, &flip, h_accepted ? PASS_COUNT : 0u, 0);
     if (rs != MPR_OK) return rs;

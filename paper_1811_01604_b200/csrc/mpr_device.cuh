@@ -174,6 +174,18 @@ __device__ __forceinline__ void sincos_small2(float2 x, float2& s, float2& c)
     c = fma2(x2, pc, bc2(1.0f));
 }
 
+// the same for |x| <= SMALL_HD (proposal windows a >= q pi / (2 SMALL_HD)): sin to x^5 (truncation x^6/5040 < 2e-10
+// relative), cos to x^4 (x^6/720 < 1.4e-9)
+constexpr float SMALL_HD = 0.1f;
+__device__ __forceinline__ void sincos_tiny2(float2 x, float2& s, float2& c)
+{
+    const float2 x2 = mul2(x, x);
+    const float2 ps = fma2(x2, bc2(8.33333333e-3f), bc2(-1.66666667e-1f));
+    s = fma2(mul2(x, x2), ps, x);
+    const float2 pc = fma2(x2, bc2(4.16666667e-2f), bc2(-0.5f));
+    c = fma2(x2, pc, bc2(1.0f));
+}
+
 __device__ __forceinline__ uint32_t enc_ordered(float f)
 {
     const uint32_t b = __float_as_uint(f);
@@ -550,7 +562,7 @@ __device__ __forceinline__ float2 update_site(float2 v, float2 n_up, float2 n_dn
 // the reflection keeps h.v, so h.v' = h.v, and turns h x v into -(h x v); both are taken from the stored v,
 // which is what the oracle's exact arithmetic does (it does not round v' before the Metropolis step).
 // exp(-dH/T) > r already accepts every dH <= 0 because r < 1.
-template <bool QHALF, int ORMODE>
+template <bool QHALF, int ORMODE, bool SMALLD>
 __device__ __forceinline__ void update_pair(float2& vA, float2 upA, float2 dnA, float2 lfA, float2 rtA,
                                             float2& vB, float2 upB, float2 dnB, float2 lfB, float2 rtB,
                                             uint32_t wA0, uint32_t wA1, uint32_t wB0, uint32_t wB1,
@@ -597,7 +609,7 @@ __device__ __forceinline__ void update_pair(float2& vA, float2 upA, float2 dnA, 
     // g = 1.m - 1.5 exact, hd_c1 = 2^-24 hd_scale
     const float2 hd = fma2(add2(make_float2(one_plus_m(wA0), one_plus_m(wB0)), bc2(-1.5f)), bc2(hd_scale), bc2(hd_c1));
     float2 sh, ch;
-    sincos_small2(hd, sh, ch);
+    if (SMALLD) sincos_tiny2(hd, sh, ch); else sincos_small2(hd, sh, ch);
     const float2 sh2 = add2(sh, sh);
     const float2 sd = mul2(sh2, ch), omc = mul2(sh2, sh);       // sin d, 1 - cos d
     const float2 tA = fma2(pA, bc2(-omc.x), pA), tB = fma2(pB, bc2(-omc.y), pB);
@@ -709,7 +721,7 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // ---------------------------------------------------------------------------
 template <bool B> struct FreshTag { static constexpr bool value = B; };
 
-template <bool QHALF, int ORMODE, bool FUSED, int FCT>
+template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD>
 __global__ void __launch_bounds__(TILE_THREADS, TILE_THREADS >= 384 ? 2 : 3)
 k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
            uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist)
@@ -805,7 +817,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
                 wA0 = sA.x; wA1 = sA.y; wB0 = sB.x; wB1 = sB.y;
             }
             bool accA, accB;
-            update_pair<QHALF, ORMODE>(vA, upA, dnA, lfA, rtA, vB, upB, dnB, lfB, rtB, wA0, wA1, wB0, wB1,
+            update_pair<QHALF, ORMODE, SMALLD>(vA, upA, dnA, lfA, rtA, vB, upB, dnB, lfB, rtB, wA0, wA1, wB0, wB1,
                                        hs, hc1, nlT, d.bc, d.bs, renorm, accA, accB);
             S[offA] = vA;
             if (eB != eA) S[offB] = vB;
