@@ -245,16 +245,89 @@ def test_t2_full_size_cfg4_shape_one_sweep(torch_cuda, mpr, orc):
     z = synth.grf(L, L, 64.0, "gaussian", 1004)
     m = synth.bernoulli_mask(L, L, 0.33, 2004)
     T = synth.choose_T(z, m)
-    zmin, zmax, _ = orc.minmax(z, m)
-    rng = np.random.default_rng(8)
-    phi = ((z.astype(np.float64) - zmin) / (float(zmax) - float(zmin)) * TWO_PI_F
-           + math.sqrt(T) * rng.standard_normal(z.shape)).clip(0.0, TWO_PI_F).astype(np.float32)
-    ref0, _, _ = orc.transform(z, m, 3004)
-    phi[m == 1] = ref0[m == 1]
+    phi = _generator_state(orc, z, m, T, 3004, 8)
     ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
     ctx.set_params(T, seed=3004)
     res = _compare_one_sweep(orc, ctx, phi[None], m[None], 0.5, [T], 40.0, 3004, 123, 0)
     assert res[0][2] <= TOL_RAD
+    ctx.close()
+
+
+def _generator_state(orc, z, m, T, seed, rng_seed, g=0):
+    """A stand-in for an equilibrated state at sizes the oracle cannot equilibrate in seconds:
+    the truth field's own angles plus thermal-size noise at the prediction sites."""
+    zmin, zmax, _ = orc.minmax(z, m)
+    rng = np.random.default_rng(rng_seed)
+    phi = ((z.astype(np.float64) - zmin) / (float(zmax) - float(zmin)) * TWO_PI_F
+           + math.sqrt(T) * rng.standard_normal(z.shape)).clip(0.0, TWO_PI_F).astype(np.float32)
+    ref0, _, _ = orc.transform(z, m, seed, g)
+    phi[m == 1] = ref0[m == 1]
+    return phi
+
+
+def test_t2_full_size_cfg3_shape_one_sweep(torch_cuda, mpr, orc):
+    """BASELINE configs[2] at full size: 1024 x 1024, exponential covariance + 5 % noise, 50 % removed
+    at random plus 20 holes of 64 x 64 (tiles without any sample site, tiles that are one hole)."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg3")
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    phi = _generator_state(orc, z, m, T, w.seed, 9)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=w.seed)
+    res = _compare_one_sweep(orc, ctx, phi[None], m[None], 0.5, [T], 6.0, w.seed, 77, 0)
+    assert res[0][2] <= TOL_RAD
+    ctx.close()
+
+
+def test_t2_cfg5_shape_batch_one_sweep(torch_cuda, mpr, orc):
+    """BASELINE configs[4] shape: a batch of 2048 x 2048 grids (here 3 of the 32) with their own
+    correlation length, seed offset and temperature, 66 % removed, one launch for the batch."""
+    torch = torch_cuda
+    L, B, seed = 2048, 3, 3005
+    zs, ms, Ts, phis = [], [], [], []
+    for g, ell in enumerate((8.0, 47.0, 128.0)):
+        z = synth.grf(L, L, ell, "gaussian", 1005 + 100 * g)
+        m = synth.bernoulli_mask(L, L, 0.66, 2005 + 100 * g)
+        T = synth.choose_T(z, m)
+        zs.append(z); ms.append(m); Ts.append(T)
+        phis.append(_generator_state(orc, z, m, T, seed, 10 + g, g))
+    z, m, phi = np.stack(zs), np.stack(ms), np.stack(phis)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(Ts, seed=seed)
+    res = _compare_one_sweep(orc, ctx, phi, m, 0.5, Ts, 12.0, seed, 200, 0, g_list=range(B))
+    assert max(r[2] for r in res) <= TOL_RAD
+    ctx.close()
+
+
+def test_t2_after_batch_equilibration_grids_share_one_buffer(torch_cuda, mpr, orc):
+    """Grids of a batch stop equilibrating after different numbers of sweeps, so their states end in
+    different vector buffers; mpr_equilibrate brings them into one (the tile pass then reads the buffer
+    the host names).  One sweep from oracle-made states afterwards must still match for every grid."""
+    torch = torch_cuda
+    B, L, seed = 4, 160, 4242
+    zs, ms, Ts = [], [], []
+    for g in range(B):
+        z, m = _field(L, L, 3.0 + 4.0 * g, 0.5, 700 + 10 * g)
+        zs.append(z); ms.append(m); Ts.append(synth.choose_T(z, m))
+    z, m = np.stack(zs), np.stack(ms)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(Ts, seed=seed, equil_cap=300).equilibrate()
+    st = ctx.get_stats()
+    assert all(s.equilibrated for s in st)
+    assert len({s.equil_sweeps & 1 for s in st}) == 2, [s.equil_sweeps for s in st]   # both buffers were in use
+    phis = []
+    for g in range(B):
+        phi, _, _ = orc.transform(z[g], m[g], seed, g)
+        orc.equilibrate(phi, m[g], Ts[g], orc.Params(seed=seed, equil_cap=40), g=g)
+        phis.append(phi)
+    _compare_one_sweep(orc, ctx, np.stack(phis), m, 0.5, Ts, 5.0, seed, 40, 0, g_list=range(B))
+    # and the realization loop runs on from there for every grid
+    ctx.set_params(Ts, seed=seed, equil_cap=300, M=3, sweeps_per_real=4).equilibrate().simulate()
+    pred = ctx.predict().cpu().numpy()
+    for g in range(B):
+        s = m[g].astype(bool)
+        assert np.array_equal(pred[g][s], z[g][s])
+        assert synth.validation_measures(z[g], pred[g], m[g])["rmse"] < 0.5 * float(z[g].std())
     ctx.close()
 
 
