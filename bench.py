@@ -114,6 +114,24 @@ def algorithmic_bytes_per_sweep(N: int, P: int) -> float:
     return 4.0 * N + 4.0 * P + N / 8.0
 
 
+def algorithmic_mufu_per_sweep(N: int, P: int) -> float:
+    """SURVEY.md 8(d), angle formulation: 6P + 2N special-function results per sweep."""
+    return 6.0 * P + 2.0 * N
+
+
+# Special-function (MUFU) peak: 4 lanes / clk / SM sub-partition, measured on this pool's B200 with a
+# dependent-free ex2.approx loop (0.124 warp instructions / clk / sub-partition, DESIGN.md section 6):
+# 148 SMs x 16 results / clk x 1.965 GHz.
+SFU_PEAK_PER_S = 148 * 16 * 1.965e9
+# Issue peak: one warp instruction / clk / sub-partition = 148 x 4 x 32 thread instructions / clk.
+ISSUE_PEAK_PER_S = 148 * 4 * 32 * 1.965e9
+# Instructions one UPDATE needs at the least (DESIGN.md section 6): Philox4x32-10 is 40 per call and serves two
+# updates (20), about 40 fp32 / compare / select for Alg. 1 lines 1-6, 8 shared-memory accesses and addresses.
+ALGORITHMIC_INSTR_PER_UPDATE = 68.0
+# DRAM bytes of one 4-sweep tile-pass launch on cfg4 from the committed ncu capture (profiles/r01d_*.md)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4": 243.9e6}
+
+
 # ---------------------------------------------------------------------------
 # reference arm: the CPU oracle, as it stands, on the host cores
 # ---------------------------------------------------------------------------
@@ -280,6 +298,9 @@ def run_b200(args, w):
         bytes_per_launch = algorithmic_bytes_per_sweep(N_sites, P_sites) * sweeps_per_launch
         launch_s = sweep_s * sweeps_per_launch
         achieved = bytes_per_launch / launch_s / 1e9
+        t_hbm = algorithmic_bytes_per_sweep(N_sites, P_sites) / (peak * 1e9)
+        t_sfu = algorithmic_mufu_per_sweep(N_sites, P_sites) / SFU_PEAK_PER_S
+        t_roof = max(t_hbm, t_sfu)
         out = {
             "metric": METRIC, "value": updates / secs / 1e9, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
@@ -297,10 +318,20 @@ def run_b200(args, w):
             "gpu_launches": int(launches),
             "clocks": clk.summary(),
             "roofline": {"bound": "hbm", "kernel": "k_tilepass", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w.name) if sweeps_per_launch == 4.0 else None,
+                         "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": bytes_per_launch, "sweeps_per_launch": sweeps_per_launch,
                          "us_per_launch": launch_s * 1e6, "us_per_sweep": sweep_s * 1e6,
-                         "gupdates_per_s_kernel_only": P_sites / sweep_s / 1e9},
+                         "gupdates_per_s_kernel_only": P_sites / sweep_s / 1e9,
+                         # north_star's roofline: the slower of the bytes at HBM peak and the special-function work at SFU peak
+                         "us_per_sweep_hbm_roof": t_hbm * 1e6, "us_per_sweep_sfu_roof": t_sfu * 1e6,
+                         "frac_of_slower_roof": t_roof / sweep_s,
+                         # what the kernel is bound by in fact: instruction issue
+                         "issue": {"algorithmic_instr_per_update": ALGORITHMIC_INSTR_PER_UPDATE,
+                                   "achieved_tinstr_per_s": ALGORITHMIC_INSTR_PER_UPDATE * P_sites / sweep_s / 1e12,
+                                   "peak_tinstr_per_s": ISSUE_PEAK_PER_S / 1e12,
+                                   "frac": ALGORITHMIC_INSTR_PER_UPDATE * P_sites / sweep_s / ISSUE_PEAK_PER_S}},
         }
         if not args.no_cpu_baseline and world == 1:
             n_sweeps = oracle_sweeps_for(w)
