@@ -719,6 +719,11 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 //   PASS_COUNT       a5: accepted proposals of the core sites                          [FUSED only]
 //   PASS_ACCUMULATE  a7: acc += phi at the core's prediction sites
 // ---------------------------------------------------------------------------
+// what one half-sweep of a tile pass needs to know (tabulated per CTA, see k_tilepass)
+struct __align__(16) HalfSweep { uint32_t n, cbase, c1, flags; };   // entries to walk, list offset, Philox counter word 1, HS_*
+enum : uint32_t { HS_ODD = 1u, HS_FRESH = 2u, HS_STASH = 4u, HS_RENORM = 8u };
+constexpr int HS_CHUNK = 16;
+
 template <bool B> struct FreshTag { static constexpr bool value = B; };
 
 template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD>
@@ -729,6 +734,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar[2];       // [0] frame, [1] entry list
     __shared__ uint32_t s_cle[2][MAX_H];
+    __shared__ HalfSweep s_hs[HS_CHUNK];
     __shared__ uint32_t s_accepted;
     __shared__ double s_red[TILE_THREADS / 32];
 
@@ -779,20 +785,35 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     mbar_wait(&s_bar[1], 0);
     mbar_wait(&s_bar[0], 0);
 
-    // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1)
+    // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1).  What a half-sweep needs to
+    // know is tabulated by one warp for 16 half-sweeps at a time (HalfSweep), so that the other warps do not redo it.
 #pragma unroll 1
-    for (uint32_t j = 0; j < 2u * K; ++j) {
-        const uint32_t s = j >> 1, c = j & 1u, t = t0 + s;
-        const bool odd = t & 1u;
-        const bool fresh = !odd || s == 0 || !use_spare;            // draw a new Philox block for (site, t >> 1)
-        const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
-        // |v| = 1 against rounding drift: in the sweep whose result leaves the tile, and every 8th sweep of a long pass
-        const bool renorm = s + 1 == K || (s & 7u) == 7u;
-        const uint32_t R = 2u * K - 1u - j;                          // rings still needed: 0 .. R
-        const uint32_t n = s_cle[c][R < (uint32_t)MAX_H ? R : (uint32_t)MAX_H - 1u], n_core = s_cle[c][0];
-        const uint32_t cbase = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
-        const uint16_t* Ec = E + cbase;
-        uint2* SPc = SP + cbase;
+    for (uint32_t j0 = 0; j0 < 2u * K; j0 += HS_CHUNK) {
+        if (tid < HS_CHUNK && j0 + tid < 2u * K) {
+            const uint32_t j = j0 + tid, s = j >> 1, c = j & 1u, t = t0 + s;
+            const bool odd = t & 1u;
+            const bool fresh = !odd || s == 0 || !use_spare;            // draw a new Philox block for (site, t >> 1)
+            const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
+            // |v| = 1 against rounding drift: in the sweep whose result leaves the tile, and every 8th sweep of a long pass
+            const bool renorm = s + 1 == K || (s & 7u) == 7u;
+            const uint32_t R = 2u * K - 1u - j;                          // rings still needed: 0 .. R
+            HalfSweep h;
+            h.n = s_cle[c][R < (uint32_t)MAX_H ? R : (uint32_t)MAX_H - 1u];
+            h.cbase = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
+            h.c1 = t >> 1;
+            h.flags = (odd ? HS_ODD : 0u) | (fresh ? HS_FRESH : 0u) | (stash ? HS_STASH : 0u) | (renorm ? HS_RENORM : 0u) | (c << 8);
+            s_hs[tid] = h;
+        }
+        __syncthreads();
+        const uint32_t j_end = min(2u * K - j0, (uint32_t)HS_CHUNK);
+#pragma unroll 1
+      for (uint32_t jj = 0; jj < j_end; ++jj) {
+        const HalfSweep h = s_hs[jj];
+        const bool odd = h.flags & HS_ODD, fresh = h.flags & HS_FRESH, stash = h.flags & HS_STASH, renorm = h.flags & HS_RENORM;
+        const uint32_t n = h.n, tc1 = h.c1;
+        const uint32_t n_core = count ? s_cle[h.flags >> 8][0] : 0u;
+        const uint16_t* Ec = E + h.cbase;
+        uint2* SPc = SP + h.cbase;
 
         // the sites eA and eB of this colour's list (eB == eA: no second site, its result is dropped).
         // FRESH is a compile-time tag so that the Philox rounds and the update arithmetic of a drawing
@@ -807,8 +828,8 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             if (FRESH) {
                 const uint32_t nA = (uint32_t)(nbase + (int)offA + (int)((offA * fc_inv) >> 24) * ncorr);
                 const uint32_t nB = (uint32_t)(nbase + (int)offB + (int)((offB * fc_inv) >> 24) * ncorr);
-                const uint4 xA = philox4x32_10(nA, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
-                const uint4 xB = philox4x32_10(nB, t >> 1, 2u, (uint32_t)g, d.rk0, d.rk1);
+                const uint4 xA = philox4x32_10(nA, tc1, 2u, (uint32_t)g, d.rk0, d.rk1);
+                const uint4 xB = philox4x32_10(nB, tc1, 2u, (uint32_t)g, d.rk0, d.rk1);
                 wA0 = odd ? xA.z : xA.x; wA1 = odd ? xA.w : xA.y;
                 wB0 = odd ? xB.z : xB.x; wB1 = odd ? xB.w : xB.y;
                 if (stash) { SPc[eA] = make_uint2(xA.z, xA.w); SPc[eB] = make_uint2(xB.z, xB.w); }
@@ -837,6 +858,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         };
         if (fresh) half_sweep(FreshTag<true>{}); else half_sweep(FreshTag<false>{});
         __syncthreads();
+      }
     }
     fence_proxy_async_smem();
     __syncthreads();
