@@ -182,6 +182,28 @@ def run_reference(args, w):
 
 
 # ---------------------------------------------------------------------------
+# rank plumbing (one process per GPU, replicas only: DESIGN.md section 10)
+# ---------------------------------------------------------------------------
+def replica_seed(base_seed: int, rank: int) -> int:
+    """Every rank interpolates its own independent grid batch: same fields, own simulation seed."""
+    return base_seed + 7919 * rank
+
+
+def combine_over_ranks(times, counts, device=None):
+    """Whole-job numbers from per-rank ones: the MAX over ranks of every time, the SUM of every count.
+    Works on any initialised process group (nccl on the GPUs, gloo in the CPU tests); no group = one rank."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(x) for x in times], [float(x) for x in counts]
+    t = torch.tensor([float(x) for x in times], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([float(x) for x in counts], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t.cpu()], [float(x) for x in u.cpu()]
+
+
+# ---------------------------------------------------------------------------
 # the CUDA path
 # ---------------------------------------------------------------------------
 def run_b200(args, w):
@@ -200,7 +222,7 @@ def run_b200(args, w):
         dist.init_process_group("nccl", device_id=dev)
 
     # one independent unit (grid batch) per rank, no data-path collective: replicas, weak scaling
-    seed = w.seed + 7919 * rank
+    seed = replica_seed(w.seed, rank)
     h_values = torch.from_numpy(w.truth).pin_memory()
     h_mask = torch.from_numpy(w.mask).pin_memory()
     h_out = torch.empty(w.truth.shape, dtype=torch.float32).pin_memory()
@@ -284,13 +306,8 @@ def run_b200(args, w):
     equil_sweeps = [s.equil_sweeps for s in st]
     ctx.close()
 
-    if world > 1:
-        t = torch.tensor([secs, secs_e2e, sweep_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        secs, secs_e2e, sweep_s = (float(x) for x in t.cpu())
-        u = torch.tensor([updates, updates_e2e, launches], dtype=torch.float64, device=dev)
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        updates, updates_e2e, launches = (float(x) for x in u.cpu())
+    (secs, secs_e2e, sweep_s), (updates, updates_e2e, launches) = combine_over_ranks(
+        [secs, secs_e2e, sweep_s], [updates, updates_e2e, launches], dev)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
