@@ -25,7 +25,8 @@
  *   - Grids are row-major, [batch][rows][cols]; rectangular grids are allowed
  *     (PAPER.md L261).  2 <= rows, cols <= 65534; rows*cols < 2^31.
  *   - Random numbers: Philox4x32-10 keyed by `seed`, counter
- *     (ordinal pair, global sweep index t, 2 + colour, grid) for the sweeps and
+ *     (site = row*cols + col, t >> 1, 2, grid) for the sweeps -- words 0,1 give
+ *     (u, r) of the even global sweep index t, words 2,3 of the odd one -- and
  *     (site >> 2, 0, 0, grid) for the initial state (reading R13).
  *     t counts sweeps from mpr_set_params on, through equilibration and every
  *     realization.

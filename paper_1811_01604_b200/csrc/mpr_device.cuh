@@ -739,6 +739,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     __shared__ double s_red[TILE_THREADS / 32];
 
     constexpr int NT = TILE_THREADS, NW = TILE_THREADS / 32;
+    static_assert(TILE_THREADS >= 96 + 2 * MAX_H && TILE_THREADS >= HS_CHUNK, "the prologue gives warps 0-3 their own jobs");
     const int tile = blockIdx.x, g = blockIdx.y;
     const GridState& st = d.states[g];
     if (FUSED && (flags & PASS_CHECK_DONE) && st.done) return;
