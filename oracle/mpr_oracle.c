@@ -20,7 +20,9 @@
  * fixed sites bit-identical, Metropolis/Boltzmann chi-square against
  * quadrature, Philox against the cuRAND host generator, uniform lattice,
  * OLS slope closed forms, transform closed forms, unconditional equipartition
- * energy, and the paper's Table 3 validation measures.
+ * energy, the sample specific energy of hand-built grids, the unconditional
+ * energy of a 2 x 2 grid against 4-D quadrature, and the paper's Table 3
+ * validation measures.
  * Parity unpinned (nothing printed in the paper can tell the readings apart):
  * the value of `a` used in equilibrium (R10), the SG filter degree (R9), the
  * defaults of n_f, n_fit, A_targ, k_a (R7).
@@ -289,6 +291,30 @@ double orc_energy(const float *phi, int rows, int cols, double q)
     for (int r = 0; r < rows; ++r) H += row_sum[r];
     free(row_sum);
     return H;
+}
+
+/* ------------------------------------------------------------------------
+ * Alg. 2 step 4.1, PAPER.md L101-104 (Eq. 4): sample specific energy
+ *   e_s = -(1/N_SP) sum over nearest-neighbour pairs of SAMPLE sites of
+ *         cos q(phi_i - phi_j),
+ * every unordered pair once, N_SP their number (reading R1).
+ * Returns e_s (0 when there is no such pair) and N_SP through n_pairs.
+ * ---------------------------------------------------------------------- */
+double orc_sample_energy(const float *phi, const uint8_t *mask, int rows, int cols,
+                         double q, int64_t *n_pairs)
+{
+    double sum = 0.0;
+    int64_t n_sp = 0;
+    for (int r = 0; r < rows; ++r)
+        for (int c = 0; c < cols; ++c) {
+            int64_t n = (int64_t)r * cols + c;
+            if (!mask[n]) continue;
+            double p = (double)phi[n];
+            if (c < cols - 1 && mask[n + 1]) { sum += cos(q * (p - (double)phi[n + 1])); ++n_sp; }
+            if (r < rows - 1 && mask[n + cols]) { sum += cos(q * (p - (double)phi[n + cols])); ++n_sp; }
+        }
+    *n_pairs = n_sp;
+    return n_sp ? -sum / (double)n_sp : 0.0;
 }
 
 /* ------------------------------------------------------------------------

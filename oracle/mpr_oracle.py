@@ -63,6 +63,8 @@ def lib():
         L.orc_n_bonds.restype = C.c_int64
         L.orc_energy.argtypes = [f32p, C.c_int, C.c_int, C.c_double]
         L.orc_energy.restype = C.c_double
+        L.orc_sample_energy.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int64)]
+        L.orc_sample_energy.restype = C.c_double
         L.orc_sg_slope.argtypes = [f64p, C.c_int]
         L.orc_sg_slope.restype = C.c_double
         L.orc_equilibrate.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_double, C.c_double,
@@ -230,6 +232,50 @@ def run(z, mask, T, p: Params, g=0):
     st.update(t_end=t_end, a_eq=a_eq, zmin=zmin, zmax=zmax,
               e_final=energy_per_bond(phi, p.q))
     return {"pred": pred, "phi": phi, "stats": st}
+
+
+# ---------------------------------------------------------------------------
+# Alg. 2 step 4: parameter inference
+# ---------------------------------------------------------------------------
+def sample_energy(phi: np.ndarray, mask: np.ndarray, q=0.5):
+    """Step 4.1, Eq. 4: (e_s, N_SP) over the nearest-neighbour pairs of sample sites (reading R1)."""
+    rows, cols = phi.shape
+    n = C.c_int64()
+    e = lib().orc_sample_energy(np.ascontiguousarray(phi, dtype=np.float32),
+                                np.ascontiguousarray(mask, dtype=np.uint8), rows, cols, float(q), C.byref(n))
+    return float(e), int(n.value)
+
+
+def energy_table(rows: int, cols: int, Ts, p: Params, n_meas: int):
+    """e(T_k, L) of Eq. 5 (L105-109): one unconditional chain per ladder temperature T_k (every node free,
+    L109 "the values of the spins can be varied at every grid node"), chain k with Philox grid index k.
+    Reading R23: the chain starts from the ordered state phi = pi (the paper does not say; a uniform start
+    freezes vortices in at low T), is relaxed by the step-5 loop of Alg. 2 (same stopping rule and
+    a-control) and then averaged over n_meas further UPDATE sweeps at the a reached, e after every sweep."""
+    mask = np.zeros((rows, cols), dtype=np.uint8)
+    out = []
+    for k, T in enumerate(Ts):
+        phi = np.full((rows, cols), np.float32(np.pi), dtype=np.float32)
+        st = equilibrate(phi, mask, float(T), p, g=k, t0=0)
+        t, acc = st["t"], 0.0
+        for _ in range(n_meas):
+            sweep(phi, mask, p.q, float(T), st["a"], p.seed, k, t, p.or_mode)
+            t += 1
+            acc += energy_per_bond(phi, p.q)
+        out.append(acc / n_meas)
+    return np.array(out)
+
+
+def infer_T(e_s: float, Ts, es) -> float:
+    """Step 4.2, T = argmin_T |e_s - e(T, L)| (L111) with e(T, L) the piecewise-linear interpolant of the
+    ladder (T_k ascending): the first segment that brackets e_s, else the nearer end (reading R24)."""
+    Ts = [float(x) for x in Ts]; es = [float(x) for x in es]
+    for k in range(len(Ts) - 1):
+        lo, hi = es[k], es[k + 1]
+        if min(lo, hi) <= e_s <= max(lo, hi) and hi != lo:
+            return Ts[k] + (e_s - lo) / (hi - lo) * (Ts[k + 1] - Ts[k])
+    k = min(range(len(Ts)), key=lambda i: abs(es[i] - e_s))
+    return Ts[k]
 
 
 def num_threads() -> int:

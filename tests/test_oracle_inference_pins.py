@@ -1,0 +1,116 @@
+"""Pins of the oracle's Alg. 2 step 4 (parameter inference) against what the
+paper and the mathematics fix: closed-form sample specific energies of hand-built grids (Eq. 4), the
+relation e_s = H / N_GP when every site is a sample (Eq. 2 / Eq. 5), the unconditional energy of a
+2 x 2 grid against 4-D Gauss-Legendre quadrature of the Boltzmann average (Eq. 3, Eq. 5), the low-T
+equipartition form of e(T, L), and the inversion on an exactly linear ladder."""
+import math
+
+import numpy as np
+import pytest
+
+PI = math.pi
+TWO_PI_F = float(np.float32(2.0 * math.pi))
+
+
+def test_sample_energy_hand_built(orc):
+    ones = np.ones((2, 2), dtype=np.uint8)
+    # every bond differs by pi: cos(pi/2) = 0
+    e, n = orc.sample_energy(np.array([[0, PI], [PI, 2 * PI]], dtype=np.float32), ones)
+    assert n == 4 and abs(e) < 1e-6
+    # two bonds cos 0 = +1, two bonds cos(+-pi) = -1: 0 and 2 pi are opposite states
+    e, n = orc.sample_energy(np.array([[0, 0], [0, TWO_PI_F]], dtype=np.float32), ones)
+    assert n == 4 and abs(e) < 1e-6
+    # aligned spins, centre missing: the 4 bonds of the centre do not count (N_SP = 12 - 4)
+    m = np.ones((3, 3), dtype=np.uint8); m[1, 1] = 0
+    phi = np.full((3, 3), 1.25, dtype=np.float32); phi[1, 1] = 5.0      # value at a non-sample site is ignored
+    e, n = orc.sample_energy(phi, m)
+    assert n == 8 and e == pytest.approx(-1.0, abs=1e-12)
+    # phi_ij = i + j, q = 1/2: every bond differs by 1 -> e_s = -cos(1/2), whatever the mask
+    phi = np.add.outer(np.arange(4), np.arange(5)).astype(np.float32)
+    m = np.ones((4, 5), dtype=np.uint8); m[0, 0] = m[2, 3] = m[3, 4] = 0
+    e, n = orc.sample_energy(phi, m)
+    assert n == 31 - 2 - 4 - 2 and e == pytest.approx(-math.cos(0.5), abs=1e-12)
+    # q enters: q = 0.25
+    e, _ = orc.sample_energy(phi, m, q=0.25)
+    assert e == pytest.approx(-math.cos(0.25), abs=1e-12)
+    # isolated samples only: no pair
+    m = np.zeros((3, 3), dtype=np.uint8); m[0, 0] = m[2, 2] = m[0, 2] = 1
+    assert orc.sample_energy(phi[:3, :3].copy(), m) == (0.0, 0)
+
+
+def test_sample_energy_equals_energy_per_bond_when_every_site_is_a_sample(orc):
+    rng = np.random.default_rng(5)
+    phi = (rng.random((17, 23)) * TWO_PI_F).astype(np.float32)
+    e, n = orc.sample_energy(phi, np.ones_like(phi, dtype=np.uint8))
+    assert n == orc.n_bonds(17, 23)
+    assert e == pytest.approx(orc.energy_per_bond(phi), abs=1e-12)
+
+
+def test_sample_energy_brute_force_on_random_mask(orc):
+    rng = np.random.default_rng(6)
+    phi = (rng.random((9, 11)) * TWO_PI_F).astype(np.float32)
+    m = (rng.random((9, 11)) < 0.6).astype(np.uint8)
+    tot, cnt = 0.0, 0
+    for r in range(9):
+        for c in range(11):
+            for dr, dc in ((0, 1), (1, 0), (0, -1), (-1, 0)):          # Eq. 4's double sum: ordered pairs
+                rr, cc = r + dr, c + dc
+                if 0 <= rr < 9 and 0 <= cc < 11 and m[r, c] and m[rr, cc]:
+                    tot += math.cos(0.5 * (float(phi[r, c]) - float(phi[rr, cc]))); cnt += 1
+    e, n = orc.sample_energy(phi, m)
+    assert 2 * n == cnt and e == pytest.approx(-tot / cnt, abs=1e-12)
+
+
+def _quadrature_energy_2x2(T, q=0.5, order=24):
+    """<H> / N_GP of the 2 x 2 grid with open boundaries by Gauss-Legendre quadrature over [0, 2 pi]^4."""
+    x, w = np.polynomial.legendre.leggauss(order)
+    x = PI * (x + 1.0); w = PI * w
+    a, b, c, d = np.meshgrid(x, x, x, x, indexing="ij")              # a b / c d
+    H = -(np.cos(q * (a - b)) + np.cos(q * (c - d)) + np.cos(q * (a - c)) + np.cos(q * (b - d)))
+    W = np.einsum("i,j,k,l->ijkl", w, w, w, w) * np.exp(-H / T)
+    return float((H * W).sum() / W.sum()) / 4.0
+
+
+def test_unconditional_energy_of_the_2x2_grid_matches_quadrature(orc):
+    T = 0.5
+    want = _quadrature_energy_2x2(T)
+    assert abs(_quadrature_energy_2x2(T, order=16) - want) < 1e-6     # the quadrature itself has converged
+    phi = np.full((2, 2), PI, dtype=np.float32)
+    mask = np.zeros((2, 2), dtype=np.uint8)
+    es = []
+    for t in range(42000):
+        orc.sweep(phi, mask, 0.5, T, 1.0, 99, 0, t, 0)
+        if t >= 2000:
+            es.append(orc.energy_per_bond(phi))
+    es = np.array(es)
+    blocks = es.reshape(100, -1).mean(axis=1)
+    err = blocks.std(ddof=1) / math.sqrt(len(blocks))
+    assert abs(es.mean() - want) < 4.0 * err + 1e-3, (es.mean(), want, err)
+    assert err < 0.01
+
+
+def test_energy_table_follows_equipartition_at_low_T_and_is_monotone(orc):
+    L = 32
+    Ts = [0.004, 0.008, 0.016, 0.032]
+    p = orc.Params(seed=21, equil_cap=400)
+    es = orc.energy_table(L, L, Ts, p, n_meas=300)
+    want = [-1.0 + (L + 1) * T / (4 * L) for T in Ts]
+    for got, w in zip(es, want):
+        assert (1 + got) == pytest.approx(1 + w, rel=0.03), (es, want)
+    assert np.all(np.diff(es) > 0)
+    # chains differ by their Philox grid index: same T twice gives two different (but close) averages
+    e2 = orc.energy_table(L, L, [0.016, 0.016], p, n_meas=50)
+    assert e2[0] != e2[1] and (1 + e2[0]) == pytest.approx(1 + e2[1], rel=0.05)
+
+
+def test_infer_T_on_ladders(orc):
+    Ts = [0.01, 0.02, 0.04, 0.08]
+    es = [-1 + T / 4 for T in Ts]                                    # exactly linear ladder
+    for T in (0.01, 0.013, 0.02, 0.05, 0.08):
+        assert orc.infer_T(-1 + T / 4, Ts, es) == pytest.approx(T, rel=1e-12)
+    assert orc.infer_T(-1.5, Ts, es) == Ts[0] and orc.infer_T(0.3, Ts, es) == Ts[-1]   # outside: the nearer end
+    # curved ladder: the interpolant is used, not the nearest point
+    es = [-0.99, -0.98, -0.95, -0.85]
+    assert orc.infer_T(-0.965, Ts, es) == pytest.approx(0.03, rel=1e-12)
+    # a noisy, non-monotone ladder: the first bracketing segment
+    assert orc.infer_T(-0.975, [1, 2, 3, 4], [-0.99, -0.97, -0.98, -0.96]) == pytest.approx(1.75)
