@@ -134,6 +134,41 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out);
 
 mpr_status mpr_destroy(mpr_ctx* ctx);
 
+/* ---- Alg. 2 step 4: parameter inference ---- */
+
+/* Step 4.1, Eq. 4 (L101-104): sample specific energy e_s = -(1/N_SP) sum over the nearest-neighbour
+ * pairs of SAMPLE sites of cos q(phi_i - phi_j), every unordered pair once (reading R1), with
+ * q of the last mpr_set_params (1/2 before the first).  h_e_s host double [batch], h_n_pairs host
+ * uint64 [batch] (N_SP; e_s = 0 where N_SP = 0).  Needs only mpr_create.  Synchronises. */
+mpr_status mpr_sample_energy(mpr_ctx* ctx, double* h_e_s, uint64_t* h_n_pairs);
+
+/* A context of `batch` unconditional grids (L109: "the values of the spins can be varied at every grid
+ * node"): no data, every node a prediction site, Eq. 1 the identity on [0, 2 pi].  mpr_set_params starts
+ * each grid from the ordered state phi = pi instead of the uniform draw (reading R23); everything else
+ * (mpr_equilibrate, mpr_sweep, mpr_measure_energy, mpr_energy, ...) works as on a conditional context.
+ * Workspace as mpr_query_workspace(batch, rows, cols).  Errors: ARG, WORKSPACE, CUDA. */
+mpr_status mpr_create_unconditional(mpr_ctx** out, int batch, int rows, int cols,
+                                    void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* n_sweeps further UPDATE sweeps of every grid at its current a, the energy per bond taken after each
+ * (the fused reduction of the equilibration pass); h_e_mean host double [batch] receives the mean over
+ * these sweeps: <H> / N_GP of Eq. 5 (L105-109) for an equilibrated chain.  t advances by n_sweeps.
+ * Synchronises.  Errors: ARG (n_sweeps = 0), STATE, CUDA. */
+mpr_status mpr_measure_energy(mpr_ctx* ctx, uint32_t n_sweeps, double* h_e_mean);
+
+/* Step 4.2, Eq. 5: e(T_k, L) for a ladder of n_T temperatures h_T (host float, > 0) on a rows x cols
+ * grid: one unconditional chain per temperature (chain k = grid k of one batch), mpr_set_params(h_params,
+ * h_T), mpr_equilibrate, mpr_measure_energy(n_meas).  h_e host double [n_T].  d_workspace: at least
+ * mpr_query_workspace(n_T, rows, cols) bytes.  Synchronises. */
+mpr_status mpr_energy_table(int rows, int cols, const mpr_params* h_params, const float* h_T, int n_T,
+                            uint32_t n_meas, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                            double* h_e);
+
+/* Step 4.2, T = argmin_T |e_s - e(T, L)| (L111) over the piecewise-linear interpolant of the ladder
+ * (h_T ascending): the first segment that brackets e_s, else the ladder point nearest in energy (reading
+ * R24).  Host arithmetic on n_T numbers.  Errors: ARG. */
+mpr_status mpr_infer_temperature(const float* h_T, const double* h_e, int n_T, double e_s, double* h_T_hat);
+
 /* ---- diagnostic / test / checkpoint surface ---- */
 
 /* Current angles phi in [0, 2 pi], device float [batch][rows][cols]. Sample

@@ -115,6 +115,7 @@ struct mpr_ctx {
     bool         qhalf;
     bool         dirty;           // vectors changed since d.phi was last written at the free sites
     int          device;          // device the workspace lives on
+    bool         unconditional;   // no data: every node free, ordered start (Alg. 2 step 4.2)
     double       a_min;           // smallest proposal-width parameter a over the grids, as far as the host knows it (0 = unknown)
     bool         small_d;         // every grid's proposal half-rotation q pi / (2 a) is below SMALL_HD (host knowledge of a)
     uint32_t     cur;             // vector buffer holding the current state, the same for every grid outside mpr_equilibrate
@@ -273,11 +274,17 @@ mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* bytes)
     return MPR_OK;
 }
 
-mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float* d_values,
-                      const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+}  // extern "C"
+
+namespace {
+
+// mpr_create (data given) and mpr_create_unconditional (d_values = d_sample_mask = nullptr)
+mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float* d_values,
+                       const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
+    const bool unconditional = !d_values && !d_sample_mask;
     Geometry g;
-    if (!out || !d_values || !d_sample_mask || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
+    if (!out || (!unconditional && (!d_values || !d_sample_mask)) || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
     const Layout lay = make_layout(batch, g);
     if (!d_workspace || workspace_bytes < lay.total || ((uintptr_t)d_workspace & 255u)) return MPR_ERR_WORKSPACE;
 
@@ -294,6 +301,8 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
         if (!cuda_ok(cudaSetDevice(ctx->device), "cudaSetDevice")) { delete ctx; return MPR_ERR_CUDA; }
     }
     ctx->state = CREATED;
+    ctx->unconditional = unconditional;
+    ctx->prm.q = 0.5f; ctx->d.q = 0.5f; ctx->d.inv_q = 2.0f;      // until mpr_set_params says otherwise (L89)
     char* base = (char*)d_workspace;
     Dev& d = ctx->d;
     d.states = (GridState*)(base + lay.states);
@@ -327,8 +336,11 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     k_state_reset<<<cdiv(batch, 128), 128, 0, s>>>(d);
     unsigned mm_blocks = cdiv(g.N, 256 * 8);
     if (mm_blocks > 1184) mm_blocks = 1184;
-    k_minmax<<<dim3(mm_blocks, batch), 256, 0, s>>>(d, d_values, d_sample_mask);
-    k_minmax_finish<<<cdiv(batch, 128), 128, 0, s>>>(d);
+    if (unconditional) k_state_unconditional<<<cdiv(batch, 128), 128, 0, s>>>(d);
+    else {
+        k_minmax<<<dim3(mm_blocks, batch), 256, 0, s>>>(d, d_values, d_sample_mask);
+        k_minmax_finish<<<cdiv(batch, 128), 128, 0, s>>>(d);
+    }
     k_transform<<<dim3(cdiv((size_t)g.words * 32, 256), batch), 256, 0, s>>>(d, d_values, d_sample_mask);
     k_tile_count<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
     k_tile_scan<<<batch, 32, 0, s>>>(d);
@@ -379,6 +391,23 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
     return MPR_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float* d_values,
+                      const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!d_values || !d_sample_mask) return MPR_ERR_ARG;
+    return create_impl(out, batch, rows, cols, d_values, d_sample_mask, d_workspace, workspace_bytes, cuda_stream);
+}
+
+mpr_status mpr_create_unconditional(mpr_ctx** out, int batch, int rows, int cols,
+                                    void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    return create_impl(out, batch, rows, cols, nullptr, nullptr, d_workspace, workspace_bytes, cuda_stream);
+}
+
 mpr_status mpr_destroy(mpr_ctx* ctx)
 {
     if (!ctx) return MPR_ERR_ARG;
@@ -415,7 +444,7 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     k_begin_run<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, (const float*)d.e_partials);
     CU_LAUNCH();
     CU(cudaMemsetAsync(d.acc, 0, (size_t)d.batch * d.N * sizeof(float), ctx->stream));
-    k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d);
+    k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d, ctx->unconditional ? 1 : 0);
     CU_LAUNCH();
     CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
     ctx->state = READY;
@@ -503,6 +532,78 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out)
     const Dev& d = ctx->d;
     k_predict<<<site_grid(ctx), 256, 0, ctx->stream>>>(d, d_out);
     CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr_sample_energy(mpr_ctx* ctx, double* h_e_s, uint64_t* h_n_pairs)
+{
+    if (!ctx || !h_e_s || !h_n_pairs) return MPR_ERR_ARG;
+    ENTER(ctx);
+    const Dev& d = ctx->d;
+    k_zero_pairs<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d);
+    CU_LAUNCH();
+    k_sample_energy<<<dim3(ctx->energy_blocks, d.batch), ENERGY_THREADS, 0, ctx->stream>>>(d);
+    CU_LAUNCH();
+    k_sample_energy_finish<<<d.batch, 32, 0, ctx->stream>>>(d, ctx->energy_blocks);
+    CU_LAUNCH();
+    mpr_status s = fetch_states(ctx);
+    if (s != MPR_OK) return s;
+    for (int b = 0; b < d.batch; ++b) { h_e_s[b] = ctx->h_states[b].e_query; h_n_pairs[b] = ctx->h_states[b].n_pairs; }
+    return MPR_OK;
+}
+
+mpr_status mpr_measure_energy(mpr_ctx* ctx, uint32_t n_sweeps, double* h_e_mean)
+{
+    if (!ctx || !h_e_mean || n_sweeps == 0) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const Dev& d = ctx->d;
+    k_measure_begin<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d);
+    CU_LAUNCH();
+    for (uint32_t j = 0; j < n_sweeps; ++j) {
+        // one sweep with the energy reduction fused; k_measure adds e and commits the sweep (t, buffer swap)
+        mpr_status s = launch_pass(ctx, 1, 0, PER_GRID, PASS_ENERGY);
+        if (s != MPR_OK) return s;
+        k_measure<<<d.batch, 32, 0, ctx->stream>>>(d);
+        CU_LAUNCH();
+    }
+    ctx->cur ^= n_sweeps & 1u;          // every grid swapped buffers n_sweeps times
+    mpr_status s = fetch_states(ctx);
+    if (s != MPR_OK) return s;
+    for (int b = 0; b < d.batch; ++b) h_e_mean[b] = ctx->h_states[b].e_sum / (double)ctx->h_states[b].n_meas;
+    return MPR_OK;
+}
+
+mpr_status mpr_energy_table(int rows, int cols, const mpr_params* h_params, const float* h_T, int n_T,
+                            uint32_t n_meas, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                            double* h_e)
+{
+    if (!h_params || !h_T || !h_e || n_T < 1 || n_meas == 0) return MPR_ERR_ARG;
+    mpr_ctx* ctx = nullptr;
+    mpr_status s = mpr_create_unconditional(&ctx, n_T, rows, cols, d_workspace, workspace_bytes, cuda_stream);
+    if (s != MPR_OK) return s;
+    s = mpr_set_params(ctx, h_params, h_T);
+    if (s == MPR_OK) s = mpr_equilibrate(ctx);
+    if (s == MPR_OK) s = mpr_measure_energy(ctx, n_meas, h_e);
+    mpr_destroy(ctx);
+    return s;
+}
+
+mpr_status mpr_infer_temperature(const float* h_T, const double* h_e, int n_T, double e_s, double* h_T_hat)
+{
+    if (!h_T || !h_e || !h_T_hat || n_T < 1 || !std::isfinite(e_s)) return MPR_ERR_ARG;
+    for (int k = 0; k + 1 < n_T; ++k) {
+        if (!(h_T[k + 1] > h_T[k])) return MPR_ERR_ARG;
+        const double lo = h_e[k], hi = h_e[k + 1];
+        if (hi != lo && e_s >= (lo < hi ? lo : hi) && e_s <= (lo < hi ? hi : lo)) {
+            *h_T_hat = (double)h_T[k] + (e_s - lo) / (hi - lo) * ((double)h_T[k + 1] - (double)h_T[k]);
+            return MPR_OK;
+        }
+    }
+    int best = 0;
+    for (int k = 1; k < n_T; ++k)
+        if (std::fabs(h_e[k] - e_s) < std::fabs(h_e[best] - e_s)) best = k;
+    *h_T_hat = (double)h_T[best];
     return MPR_OK;
 }
 

@@ -50,7 +50,10 @@ struct GridState {
     uint32_t realizations;
     double   a, k, A_last, e_last, T;
     float    zmin, zmax;
-    double   e_query;            // result slot of mpr_energy
+    double   e_query;            // result slot of mpr_energy / mpr_sample_energy
+    double   e_sum;              // mpr_measure_energy: sum over the measured sweeps of e
+    uint32_t n_meas;             //   and their number
+    unsigned long long n_pairs;  // N_SP of Eq. 4 (mpr_sample_energy)
     double   e_ring[MAX_NFIT];   // e(i) at slot i % n_fit
 };
 
@@ -234,7 +237,7 @@ __global__ void k_state_reset(Dev d)
     s.zmin_enc = 0xFFFFFFFFu; s.zmax_enc = 0u;
     s.n_samples = 0; s.err_flags = 0; s.i = 0; s.realizations = 0;
     s.a = 1.0; s.k = -1.0; s.A_last = 0.0; s.e_last = 0.0; s.T = 0.0;
-    s.zmin = 0.f; s.zmax = 0.f; s.e_query = 0.0;
+    s.zmin = 0.f; s.zmax = 0.f; s.e_query = 0.0; s.e_sum = 0.0; s.n_meas = 0; s.n_pairs = 0ull;
     d.done_flags[g] = 0;
 }
 
@@ -286,6 +289,14 @@ __global__ void k_minmax_finish(Dev d)
     s.err_flags = err;
 }
 
+// unconditional grids (Alg. 2 step 4.2: every node free, no data): the angle is its own value
+__global__ void k_state_unconditional(Dev d)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= d.batch) return;
+    d.states[g].zmin = 0.0f; d.states[g].zmax = TWO_PI_F;
+}
+
 // ---------------------------------------------------------------------------
 // a2  Eq. 1 at the sample sites, fixed-site bitmask, verbatim value copy,
 // prediction-site count per checkerboard colour
@@ -301,8 +312,8 @@ __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restric
     uint32_t colour = 0;
     if (in) {
         const size_t o = (size_t)g * d.N + n;
-        const float z = values[o];
-        fixed = mask[o] != 0;
+        const float z = values ? values[o] : 0.0f;           // no inputs: an unconditional grid
+        fixed = mask ? mask[o] != 0 : false;
         d.values[o] = z;
         d.phi[o] = fixed ? eq1(z, s.zmin, s.zmax) : 0.0f;
         const uint32_t r = n / d.cols;
@@ -467,7 +478,7 @@ __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
 // sites from the INIT stream; every site's unit vector (cos q phi, sin q phi)
 // into BOTH vector buffers (sample sites are never written again).
 // ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_init_state(Dev d)
+__global__ void __launch_bounds__(256) k_init_state(Dev d, int ordered)
 {
     const int g = blockIdx.y;
     const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
@@ -476,9 +487,12 @@ __global__ void __launch_bounds__(256) k_init_state(Dev d)
     float p;
     if (is_fixed(d.bits + (size_t)g * d.words, n)) p = d.phi[o];
     else {
-        const uint4 x = philox4x32_10(n >> 2, 0u, 0u, (uint32_t)g, d.rk0, d.rk1);
-        const uint32_t w = (n & 3u) == 0 ? x.x : (n & 3u) == 1 ? x.y : (n & 3u) == 2 ? x.z : x.w;
-        p = __fmul_rn(TWO_PI_F, u01(w));
+        if (ordered) p = 3.14159274101257324f;          // unconditional chains start from phi = pi (reading R23)
+        else {
+            const uint4 x = philox4x32_10(n >> 2, 0u, 0u, (uint32_t)g, d.rk0, d.rk1);
+            const uint32_t w = (n & 3u) == 0 ? x.x : (n & 3u) == 1 ? x.y : (n & 3u) == 2 ? x.z : x.w;
+            p = __fmul_rn(TWO_PI_F, u01(w));
+        }
         d.phi[o] = p;
     }
     const uint32_t r = n / d.cols, col = n - r * d.cols;
@@ -812,7 +826,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         const HalfSweep h = s_hs[jj];
         const bool odd = h.flags & HS_ODD, fresh = h.flags & HS_FRESH, stash = h.flags & HS_STASH, renorm = h.flags & HS_RENORM;
         const uint32_t n = h.n, tc1 = h.c1;
-        const uint32_t n_core = count ? s_cle[h.flags >> 8][0] : 0u;
+        const uint32_t n_core = FUSED ? s_cle[h.flags >> 8][0] : 0u;
         const uint16_t* Ec = E + h.cbase;
         uint2* SPc = SP + h.cbase;
 
@@ -843,7 +857,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
                                        hs, hc1, nlT, d.bc, d.bs, renorm, accA, accB);
             S[offA] = vA;
             if (eB != eA) S[offB] = vB;
-            if (count) n_accepted += (accA && eA < n_core) + (accB && eB != eA && eB < n_core);
+            if constexpr (FUSED) { if (count) n_accepted += (accA && eA < n_core) + (accB && eB != eA && eB < n_core); }
         };
         // full rounds: thread tid takes the entries pos + tid and pos + NT + tid; the last round splits what
         // is left into two halves of whole warps, so that no warp runs a round for a missing second site
@@ -968,6 +982,73 @@ __global__ void k_energy_query(Dev d, int n_partials)
     const int g = blockIdx.x;
     const double H = sum_energy_partials(d, g, n_partials);
     if (threadIdx.x == 0) d.states[g].e_query = H / d.n_bonds;
+}
+
+// ---------------------------------------------------------------------------
+// Alg. 2 step 4.1 (Eq. 4): sample specific energy.  Block b sums -cos q(phi_i - phi_j)
+// over the bonds (right, down) between SAMPLE sites of its rows in double (fixed order: reproducible);
+// the pair count goes through an integer atomic.  k_sample_energy_finish divides.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(ENERGY_THREADS) k_sample_energy(Dev d)
+{
+    const int g = blockIdx.y;
+    __shared__ double warp_sum[ENERGY_THREADS / 32];
+    const float* phi = d.phi + (size_t)g * d.N;
+    const uint32_t* bits = d.bits + (size_t)g * d.words;
+    const double q = (double)d.q;
+    double sum = 0.0;
+    unsigned long long cnt = 0ull;
+    for (int r = blockIdx.x; r < d.rows; r += gridDim.x)
+        for (int col = threadIdx.x; col < d.cols; col += ENERGY_THREADS) {
+            const uint32_t n = (uint32_t)r * d.cols + col;
+            if (!is_fixed(bits, n)) continue;
+            const double p = (double)phi[n];
+            if (col + 1 < d.cols && is_fixed(bits, n + 1)) { sum -= cos(q * (p - (double)phi[n + 1])); ++cnt; }
+            if (r + 1 < d.rows && is_fixed(bits, n + d.cols)) { sum -= cos(q * (p - (double)phi[n + d.cols])); ++cnt; }
+        }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+        cnt += __shfl_xor_sync(0xFFFFFFFFu, cnt, o);
+    }
+    if ((threadIdx.x & 31) == 0) { warp_sum[threadIdx.x >> 5] = sum; if (cnt) atomicAdd(&d.states[g].n_pairs, cnt); }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < ENERGY_THREADS / 32; ++w) s += warp_sum[w];
+        d.e_partials[(size_t)g * d.n_partials + blockIdx.x] = s;
+    }
+}
+__global__ void k_zero_pairs(Dev d)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g < d.batch) d.states[g].n_pairs = 0ull;
+}
+
+// ---------------------------------------------------------------------------
+// Alg. 2 step 4.2 (Eq. 5): energy averaged over the sweeps of a chain.  After each
+// K = 1 pass with the fused energy reduction: e_sum += H / N_GP, and the sweep is committed.
+// ---------------------------------------------------------------------------
+__global__ void k_measure_begin(Dev d)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g < d.batch) { d.states[g].e_sum = 0.0; d.states[g].n_meas = 0u; }
+}
+__global__ void k_measure(Dev d)
+{
+    const int g = blockIdx.x;
+    GridState& s = d.states[g];
+    const double H = sum_energy_partials(d, g, d.ntiles);
+    if (threadIdx.x != 0) return;
+    s.e_last = H / d.n_bonds;
+    s.e_sum += s.e_last; s.n_meas += 1u;
+    s.t += 1u; s.cur ^= 1u;
+}
+__global__ void k_sample_energy_finish(Dev d, int n_partials)
+{
+    const int g = blockIdx.x;
+    const double sum = sum_energy_partials(d, g, n_partials);
+    if (threadIdx.x == 0) d.states[g].e_query = d.states[g].n_pairs ? sum / (double)d.states[g].n_pairs : 0.0;
 }
 
 // ---------------------------------------------------------------------------

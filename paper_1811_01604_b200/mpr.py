@@ -31,6 +31,8 @@ EXPORTS = (
     "mpr_simulate", "mpr_predict", "mpr_destroy", "mpr_get_angles", "mpr_set_angles",
     "mpr_set_sweep_index", "mpr_sweep", "mpr_energy", "mpr_get_transform", "mpr_get_mask_bits",
     "mpr_get_stats", "mpr_get_launch_count", "mpr_status_string", "mpr_last_cuda_error",
+    "mpr_sample_energy", "mpr_create_unconditional", "mpr_measure_energy", "mpr_energy_table",
+    "mpr_infer_temperature",
 )
 
 
@@ -89,6 +91,13 @@ def lib():
         L.mpr_get_mask_bits.argtypes = [vp, vp]
         L.mpr_get_stats.argtypes = [vp, C.POINTER(mpr_stats)]
         L.mpr_get_launch_count.argtypes = [vp, C.POINTER(u64)]
+        L.mpr_sample_energy.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(u64)]
+        L.mpr_create_unconditional.argtypes = [C.POINTER(vp), i, i, i, vp, sz, vp]
+        L.mpr_measure_energy.argtypes = [vp, u32, C.POINTER(C.c_double)]
+        L.mpr_energy_table.argtypes = [i, i, C.POINTER(mpr_params), C.POINTER(C.c_float), i, u32, vp, sz, vp,
+                                       C.POINTER(C.c_double)]
+        L.mpr_infer_temperature.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_double), i, C.c_double,
+                                            C.POINTER(C.c_double)]
         for name in EXPORTS:
             getattr(L, name).restype = C.c_int
         L.mpr_default_params.restype = None
@@ -144,8 +153,21 @@ class Mpr:
     sample_mask: uint8 CUDA tensor of the same shape, 1 = sample (fixed).
     """
 
-    def __init__(self, values, sample_mask, stream=None):
+    def __init__(self, values, sample_mask, stream=None, unconditional=None):
         import torch
+        if unconditional is not None:
+            # (batch, rows, cols, device): mpr_create_unconditional, every node free, no data
+            self.batch, self.rows, self.cols, self.device = unconditional
+            self._torch = torch
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            nbytes = mpr_query_workspace(self.batch, self.rows, self.cols)
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._ctx = C.c_void_p()
+            _check(lib().mpr_create_unconditional(C.byref(self._ctx), self.batch, self.rows, self.cols,
+                                                  self.workspace.data_ptr(), nbytes, self._stream.cuda_stream),
+                   "mpr_create_unconditional")
+            self.params = None
+            return
         if not values.is_cuda or not sample_mask.is_cuda:
             raise ValueError("values and sample_mask must be CUDA tensors (there is no CPU path)")
         if values.dim() == 2:
@@ -208,6 +230,22 @@ class Mpr:
         _check(lib().mpr_predict(self._ctx, out.data_ptr()), "mpr_predict")
         return out
 
+    # -- Alg. 2 step 4 -------------------------------------------------------
+    @classmethod
+    def unconditional(cls, batch: int, rows: int, cols: int, device, stream=None):
+        return cls(None, None, stream=stream, unconditional=(int(batch), int(rows), int(cols), device))
+
+    def sample_energy(self):
+        """(e_s, N_SP) per grid: Eq. 4."""
+        e, n = (C.c_double * self.batch)(), (C.c_uint64 * self.batch)()
+        _check(lib().mpr_sample_energy(self._ctx, e, n), "mpr_sample_energy")
+        return [float(x) for x in e], [int(x) for x in n]
+
+    def measure_energy(self, n_sweeps: int):
+        e = (C.c_double * self.batch)()
+        _check(lib().mpr_measure_energy(self._ctx, int(n_sweeps), e), "mpr_measure_energy")
+        return [float(x) for x in e]
+
     # -- diagnostics -------------------------------------------------------
     def get_angles(self, out=None):
         torch = self._torch
@@ -261,6 +299,30 @@ class Mpr:
         n = C.c_uint64()
         _check(lib().mpr_get_launch_count(self._ctx, C.byref(n)), "mpr_get_launch_count")
         return int(n.value)
+
+
+def energy_table(rows: int, cols: int, Ts, n_meas: int, device, params: mpr_params | None = None, **overrides):
+    """mpr_energy_table: e(T_k, L) of Eq. 5 for the ladder Ts from unconditional chains.  Returns a list."""
+    import torch
+    p = params if params is not None else default_params(**overrides)
+    n_T = len(Ts)
+    nbytes = mpr_query_workspace(n_T, rows, cols)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    arr = (C.c_float * n_T)(*[float(x) for x in Ts])
+    e = (C.c_double * n_T)()
+    stream = torch.cuda.current_stream(device)
+    _check(lib().mpr_energy_table(int(rows), int(cols), C.byref(p), arr, n_T, int(n_meas), ws.data_ptr(), nbytes,
+                                  stream.cuda_stream, e), "mpr_energy_table")
+    return [float(x) for x in e]
+
+
+def infer_temperature(Ts, es, e_s: float) -> float:
+    """mpr_infer_temperature: the ladder's interpolant inverted at e_s."""
+    n = len(Ts)
+    out = C.c_double()
+    _check(lib().mpr_infer_temperature((C.c_float * n)(*[float(x) for x in Ts]), (C.c_double * n)(*[float(x) for x in es]),
+                                       n, float(e_s), C.byref(out)), "mpr_infer_temperature")
+    return float(out.value)
 
 
 def interpolate(values, sample_mask, T, **params):

@@ -1,0 +1,110 @@
+"""Parity of Alg. 2 step 4 (parameter inference) on the GPU against the oracle:
+Eq. 4's sample specific energy, unconditional chains (Eq. 5) and the inferred temperature."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1811_01604_b200 import synth
+from test_gpu_parity import _compare_one_sweep, _dev, _field, mpr, torch_cuda   # noqa: F401  (fixtures)
+
+pytestmark = pytest.mark.gpu
+PI_F = np.float32(np.pi)
+
+
+def test_sample_energy_matches_eq4(torch_cuda, mpr, orc):
+    torch = torch_cuda
+    zs, ms = [], []
+    for g, (ell, p) in enumerate(((6.0, 0.33), (20.0, 0.66), (3.0, 0.9))):
+        z, m = _field(150, 197, ell, p, 40 + g)
+        zs.append(z); ms.append(m)
+    m_none = np.zeros((150, 197), dtype=np.uint8); m_none[::3, ::3] = 1     # samples, but no two adjacent
+    zs.append(zs[0]); ms.append(m_none)
+    z, m = np.stack(zs), np.stack(ms)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    e_gpu, n_gpu = ctx.sample_energy()                                      # before mpr_set_params: q = 1/2
+    for g in range(4):
+        phi, _, _ = orc.transform(z[g], m[g], 0, g)
+        e_ref, n_ref = orc.sample_energy(phi, m[g])
+        assert n_gpu[g] == n_ref
+        assert e_gpu[g] == pytest.approx(e_ref, abs=1e-12)
+    assert n_gpu[3] == 0 and e_gpu[3] == 0.0
+    ctx.set_params([0.1] * 4, q=0.25)
+    e_q, _ = ctx.sample_energy()
+    phi, _, _ = orc.transform(z[1], m[1], 0, 1)
+    assert e_q[1] == pytest.approx(orc.sample_energy(phi, m[1], q=0.25)[0], abs=1e-12)
+    ctx.close()
+
+
+def test_unconditional_context_ordered_start_and_one_sweep(torch_cuda, mpr, orc):
+    torch = torch_cuda
+    B, rows, cols, seed = 2, 150, 131, 88
+    ctx = mpr.Mpr.unconditional(B, rows, cols, torch.device("cuda:0"))
+    Ts = [0.05, 0.4]
+    ctx.set_params(Ts, seed=seed)
+    st = ctx.get_stats()
+    assert all(s.n_samples == 0 and s.n_free == rows * cols for s in st)
+    start = ctx.get_angles().cpu().numpy()
+    assert np.array_equal(start, np.full((B, rows, cols), PI_F))           # reading R23
+    assert ctx.energy() == pytest.approx([-1.0, -1.0], abs=1e-6)
+    # one sweep from oracle-made unconditional states (every node free)
+    mask = np.zeros((B, rows, cols), dtype=np.uint8)
+    phis = []
+    for g in range(B):
+        phi = np.full((rows, cols), PI_F, dtype=np.float32)
+        orc.equilibrate(phi, mask[g], Ts[g], orc.Params(seed=seed, equil_cap=60), g=g)
+        phis.append(phi)
+    _compare_one_sweep(orc, ctx, np.stack(phis), mask, 0.5, Ts, 3.0, seed, 60, 0, g_list=range(B))
+    # the identity transform: the prediction is the mean angle
+    ctx.set_params(Ts, seed=seed, M=2, sweeps_per_real=1).simulate()
+    pred = ctx.predict().cpu().numpy()
+    assert pred.min() >= 0.0 and pred.max() <= 2 * math.pi + 1e-6 and abs(float(pred.mean()) - math.pi) < 0.2
+    ctx.close()
+
+
+def test_measure_energy_is_the_mean_of_the_energies_after_each_sweep(torch_cuda, mpr, orc):
+    torch = torch_cuda
+    L, seed, T, a, t0 = 96, 5, 0.3, 2.0, 40
+    ctx = mpr.Mpr.unconditional(1, L, L, torch.device("cuda:0"))
+    ctx.set_params(T, seed=seed)
+    mask = np.zeros((L, L), dtype=np.uint8)
+    phi = np.full((L, L), PI_F, dtype=np.float32)
+    for t in range(t0):
+        orc.sweep(phi, mask, 0.5, T, a, seed, 0, t)
+    ctx.set_angles(torch.from_numpy(phi)[None].cuda())
+    ctx.set_sweep_index(t0)
+    ctx.sweep(0, a)                                                        # sets a (no sweep)
+    n = 3
+    got = ctx.measure_energy(n)[0]
+    es = []
+    for t in range(t0, t0 + n):
+        orc.sweep(phi, mask, 0.5, T, a, seed, 0, t)
+        es.append(orc.energy_per_bond(phi))
+    # a decision flip in an early sweep moves one site's later energies: a few 1e-5 at most at this size
+    assert got == pytest.approx(float(np.mean(es)), abs=5e-5)
+    assert ctx.get_stats()[0].t == t0 + n
+    assert ctx.energy()[0] == pytest.approx(es[-1], abs=1e-4)
+    ctx.close()
+
+
+def test_energy_table_and_inferred_temperature(torch_cuda, mpr, orc):
+    """Step 4.2 on a 160 x 160 grid (3 x 3 tiles): the ladder's energies agree with the oracle's within the
+    chains' noise, and the temperature inferred for a cfg1-like sample set agrees between the two tables
+    and with the low-T closed form the harness uses (reading R15)."""
+    torch = torch_cuda
+    L = 160
+    Ts = [0.005, 0.01, 0.02, 0.04, 0.08]
+    n_meas = 150
+    p = orc.Params(seed=31, equil_cap=300)
+    e_gpu = mpr.energy_table(L, L, Ts, n_meas, torch.device("cuda:0"), seed=31, equil_cap=300)
+    e_ref = orc.energy_table(L, L, Ts, p, n_meas)
+    for g, r in zip(e_gpu, e_ref):
+        assert (1 + g) == pytest.approx(1 + r, rel=0.02), (e_gpu, list(e_ref))
+    z, m = _field(L, L, 8.0, 0.33, 77)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    e_s = ctx.sample_energy()[0][0]
+    ctx.close()
+    T_gpu = mpr.infer_temperature(Ts, e_gpu, e_s)
+    T_ref = orc.infer_T(e_s, Ts, e_ref)
+    assert T_gpu == pytest.approx(T_ref, rel=0.03)
+    assert T_gpu == pytest.approx(synth.choose_T(z, m), rel=0.05)

@@ -85,3 +85,16 @@ def test_no_cpu_fallback_in_the_product():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 assert not pat.search(open(os.path.join(dirpath, f)).read()), f
+
+
+def test_infer_temperature_is_host_arithmetic_and_matches_the_oracle(lib, orc):
+    """mpr_infer_temperature (Alg. 2 step 4.2, L111) needs no device: same ladders as the oracle's pins."""
+    cases = [([0.01, 0.02, 0.04, 0.08], [-1 + T / 4 for T in (0.01, 0.02, 0.04, 0.08)], [-0.9975, -0.99675, -0.995, -0.9875, -0.98, -1.5, 0.3]),
+             ([0.01, 0.02, 0.04, 0.08], [-0.99, -0.98, -0.95, -0.85], [-0.965, -0.99, -0.85, -0.9]),
+             ([1, 2, 3, 4], [-0.99, -0.97, -0.98, -0.96], [-0.975, -0.965, -0.5])]
+    for Ts, es, queries in cases:
+        for e_s in queries:
+            assert mpr.infer_temperature(Ts, es, e_s) == pytest.approx(orc.infer_T(e_s, Ts, es), rel=1e-6)
+    with pytest.raises(mpr.MprError) as e:
+        mpr.infer_temperature([2, 1], [-0.9, -0.8], -0.85)          # ladder not ascending
+    assert e.value.name == "MPR_ERR_ARG"
