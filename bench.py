@@ -43,6 +43,7 @@ def parse_args():
     ap.add_argument("--L", type=int, default=None, help="override the grid side (debugging only)")
     ap.add_argument("--batch", type=int, default=None, help="override the batch of cfg5 (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-inference", action="store_true", help="skip the Alg. 2 step 4 timing (extra key, not in the step)")
     return ap.parse_args()
 
 
@@ -301,6 +302,22 @@ def run_b200(args, w):
     e1.synchronize()
     probe_launches = ctx.launch_count() - l0 - 2          # minus the two scalar kernels around the passes
     sweep_s = e0.elapsed_time(e1) / 1e3 / n_probe
+    # Alg. 2 step 4 (parameter inference) timed on its own: it is not part of the step, whose T is an input
+    inference = None
+    if not args.no_inference and world == 1:
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record(stream)
+        e_s, n_sp = ctx.sample_energy()
+        ev[1].record(stream)
+        T_cf = float(w.T[0])
+        ladder = [T_cf * f for f in (0.25, 0.5, 1.0, 2.0, 4.0)]
+        table = mpr.energy_table(w.rows, w.cols, ladder, 100, dev, seed=seed, q=w.q, equil_cap=500)
+        ev[2].record(stream)
+        ev[2].synchronize()
+        inference = {"e_s": e_s[0], "n_sample_pairs": n_sp[0], "ladder_T": ladder, "ladder_e": table,
+                     "T_hat": mpr.infer_temperature(ladder, table, e_s[0]), "T_closed_form_R15": T_cf,
+                     "ms_sample_energy": ev[0].elapsed_time(ev[1]), "ms_energy_table": ev[1].elapsed_time(ev[2]),
+                     "table": f"5 unconditional {w.rows}x{w.cols} chains, 500 burn-in + 100 measured sweeps each"}
     N_sites = w.rows * w.cols * w.batch
     P_sites = sum(s.n_free for s in st)
     equil_sweeps = [s.equil_sweeps for s in st]
@@ -350,6 +367,8 @@ def run_b200(args, w):
                                    "peak_tinstr_per_s": ISSUE_PEAK_PER_S / 1e12,
                                    "frac": ALGORITHMIC_INSTR_PER_UPDATE * P_sites / sweep_s / ISSUE_PEAK_PER_S}},
         }
+        if inference is not None:
+            out["temperature_inference"] = inference
         if not args.no_cpu_baseline and world == 1:
             n_sweeps = oracle_sweeps_for(w)
             rate, dt, cores = oracle_sample(w, n_sweeps)

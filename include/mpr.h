@@ -144,8 +144,10 @@ mpr_status mpr_sample_energy(mpr_ctx* ctx, double* h_e_s, uint64_t* h_n_pairs);
 
 /* A context of `batch` unconditional grids (L109: "the values of the spins can be varied at every grid
  * node"): no data, every node a prediction site, Eq. 1 the identity on [0, 2 pi].  mpr_set_params starts
- * each grid from the ordered state phi = pi instead of the uniform draw (reading R23); everything else
- * (mpr_equilibrate, mpr_sweep, mpr_measure_energy, mpr_energy, ...) works as on a conditional context.
+ * each grid from the ordered state phi = pi instead of the uniform draw, and mpr_equilibrate burns in for
+ * exactly equil_cap sweeps with the a-control of step 5.2 but without the slope stop (from the ordered state
+ * the energy rises, so k >= 0 holds at the first check; reading R23); everything else (mpr_sweep,
+ * mpr_measure_energy, mpr_energy, ...) works as on a conditional context.
  * Workspace as mpr_query_workspace(batch, rows, cols).  Errors: ARG, WORKSPACE, CUDA. */
 mpr_status mpr_create_unconditional(mpr_ctx** out, int batch, int rows, int cols,
                                     void* d_workspace, size_t workspace_bytes, void* cuda_stream);

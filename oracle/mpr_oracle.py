@@ -249,17 +249,25 @@ def sample_energy(phi: np.ndarray, mask: np.ndarray, q=0.5):
 def energy_table(rows: int, cols: int, Ts, p: Params, n_meas: int):
     """e(T_k, L) of Eq. 5 (L105-109): one unconditional chain per ladder temperature T_k (every node free,
     L109 "the values of the spins can be varied at every grid node"), chain k with Philox grid index k.
-    Reading R23: the chain starts from the ordered state phi = pi (the paper does not say; a uniform start
-    freezes vortices in at low T), is relaxed by the step-5 loop of Alg. 2 (same stopping rule and
-    a-control) and then averaged over n_meas further UPDATE sweeps at the a reached, e after every sweep."""
+    Reading R23 (the paper does not describe these runs): the chain starts from the ordered state phi = pi
+    (a uniform start freezes vortices in at low T); burn-in is exactly p.equil_cap sweeps of Alg. 2 steps
+    5.1-5.2 (sweep, then a = 1 + (i+1)/k_a while A < A_targ) -- the slope criterion of step 5.4 is not used,
+    because from the ordered state the energy RISES towards equilibrium and k >= 0 holds at the first check;
+    then n_meas further UPDATE sweeps at the a reached, e = H / N_GP after every sweep, averaged."""
     mask = np.zeros((rows, cols), dtype=np.uint8)
+    P = rows * cols
     out = []
     for k, T in enumerate(Ts):
         phi = np.full((rows, cols), np.float32(np.pi), dtype=np.float32)
-        st = equilibrate(phi, mask, float(T), p, g=k, t0=0)
-        t, acc = st["t"], 0.0
+        a, t = 1.0, 0
+        for i in range(p.equil_cap):
+            accepted = sweep(phi, mask, p.q, float(T), a, p.seed, k, t, p.or_mode)
+            t += 1
+            if accepted / P < p.A_targ:
+                a = 1.0 + (i + 1) / p.k_a
+        acc = 0.0
         for _ in range(n_meas):
-            sweep(phi, mask, p.q, float(T), st["a"], p.seed, k, t, p.or_mode)
+            sweep(phi, mask, p.q, float(T), a, p.seed, k, t, p.or_mode)
             t += 1
             acc += energy_per_bond(phi, p.q)
         out.append(acc / n_meas)

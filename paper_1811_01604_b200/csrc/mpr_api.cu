@@ -322,6 +322,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float
     d.batch = batch; d.rows = rows; d.cols = cols;
     d.N = g.N; d.words = g.words; d.pitch = g.pitch;
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
+    d.burn_in_only = unconditional ? 1 : 0;
     ctx->energy_blocks = rows < ENERGY_BLOCKS ? rows : ENERGY_BLOCKS;
     ctx->h_states = new (std::nothrow) GridState[batch];
     mpr_status st = MPR_OK;

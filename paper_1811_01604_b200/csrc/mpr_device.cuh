@@ -93,6 +93,7 @@ struct Dev {
     float      bc, bs;         // (cos 2 pi q, sin 2 pi q): upper end of the q*phi range
     // Alg. 2 controller constants
     uint32_t   n_f, n_fit, equil_cap;
+    int        burn_in_only;   // unconditional context: no slope stop
     double     A_targ, k_a, n_bonds;
 };
 
@@ -1091,7 +1092,10 @@ __global__ void k_controller(Dev d)
     // 5.5
     s.i = i + 1u; s.t += 1u; s.cur ^= 1u; s.a = a; s.k = k; s.A_last = A; s.e_last = e; s.accepted = 0ull;
     s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F) / a);
-    if (!(k < 0.0 && i + 1u < d.equil_cap)) { s.done = 1u; d.done_flags[g] = 1u; }
+    // unconditional chains burn in for exactly equil_cap sweeps: from their ordered start the energy rises, so the
+    // slope criterion would stop them at its first check (reading R23)
+    const bool go_on = d.burn_in_only ? i + 1u < d.equil_cap : (k < 0.0 && i + 1u < d.equil_cap);
+    if (!go_on) { s.done = 1u; d.done_flags[g] = 1u; }
 }
 
 // scalar state edits ---------------------------------------------------------

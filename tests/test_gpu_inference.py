@@ -52,7 +52,8 @@ def test_unconditional_context_ordered_start_and_one_sweep(torch_cuda, mpr, orc)
     phis = []
     for g in range(B):
         phi = np.full((rows, cols), PI_F, dtype=np.float32)
-        orc.equilibrate(phi, mask[g], Ts[g], orc.Params(seed=seed, equil_cap=60), g=g)
+        for t in range(60):
+            orc.sweep(phi, mask[g], 0.5, Ts[g], 3.0, seed, g, t)
         phis.append(phi)
     _compare_one_sweep(orc, ctx, np.stack(phis), mask, 0.5, Ts, 3.0, seed, 60, 0, g_list=range(B))
     # the identity transform: the prediction is the mean angle
@@ -93,7 +94,7 @@ def test_energy_table_and_inferred_temperature(torch_cuda, mpr, orc):
     and with the low-T closed form the harness uses (reading R15)."""
     torch = torch_cuda
     L = 160
-    Ts = [0.005, 0.01, 0.02, 0.04, 0.08]
+    Ts = [0.0008, 0.005, 0.01, 0.02, 0.04, 0.08]
     n_meas = 150
     p = orc.Params(seed=31, equil_cap=300)
     e_gpu = mpr.energy_table(L, L, Ts, n_meas, torch.device("cuda:0"), seed=31, equil_cap=300)
