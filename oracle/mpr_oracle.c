@@ -25,7 +25,8 @@
  * validation measures.
  * Parity unpinned (nothing printed in the paper can tell the readings apart):
  * the value of `a` used in equilibrium (R10), the SG filter degree (R9), the
- * defaults of n_f, n_fit, A_targ, k_a (R7).
+ * defaults of n_f, n_fit, A_targ, k_a (R7), the start and burn-in of the
+ * unconditional chains of step 4.2 (R23; their result is pinned).
  *
  * OpenMP (optional, -fopenmp): only over the rows of ONE colour inside a
  * half-sweep and over rows of the energy sum; sites of one colour are
