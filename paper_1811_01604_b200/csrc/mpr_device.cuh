@@ -739,7 +739,10 @@ struct __align__(16) HalfSweep { uint32_t n, cbase, c1, flags; };   // entries t
 enum : uint32_t { HS_ODD = 1u, HS_FRESH = 2u, HS_STASH = 4u, HS_RENORM = 8u };
 constexpr int HS_CHUNK = 16;
 
-template <bool B> struct FreshTag { static constexpr bool value = B; };
+// how a half-sweep gets its random words: the stored second pair, a Philox draw of an even sweep whose second pair is
+// stored (the usual drawing sweep), or a draw in general (odd sweep at the start of a pass, no room for stored words)
+enum { DRAW_STORED = 0, DRAW_EVEN_STORE = 1, DRAW_ANY = 2 };
+template <int M> struct DrawTag { static constexpr int value = M; };
 
 template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD>
 __global__ void __launch_bounds__(TILE_THREADS, TILE_THREADS >= 384 ? 2 : 3)
@@ -832,23 +835,28 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         uint2* SPc = SP + h.cbase;
 
         // the sites eA and eB of this colour's list (eB == eA: no second site, its result is dropped).
-        // FRESH is a compile-time tag so that the Philox rounds and the update arithmetic of a drawing
+        // The draw mode is a compile-time tag so that the Philox rounds and the update arithmetic of a drawing
         // sweep sit in one basic block (independent instruction streams for the scheduler to interleave).
-        auto update_two = [&](auto fresh_tag, uint32_t eA, uint32_t eB) {
-            constexpr bool FRESH = decltype(fresh_tag)::value;
+        auto update_two = [&](auto draw_tag, uint32_t eA, uint32_t eB) {
+            constexpr int DRAW = decltype(draw_tag)::value;
             const uint32_t offA = Ec[eA], offB = Ec[eB];
             float2 vA = S[offA], vB = S[offB];
             const float2 upA = S[offA - FC], dnA = S[offA + FC], lfA = S[offA - 1], rtA = S[offA + 1];
             const float2 upB = S[offB - FC], dnB = S[offB + FC], lfB = S[offB - 1], rtB = S[offB + 1];
             uint32_t wA0, wA1, wB0, wB1;
-            if (FRESH) {
+            if (DRAW != DRAW_STORED) {
                 const uint32_t nA = (uint32_t)(nbase + (int)offA + (int)((offA * fc_inv) >> 24) * ncorr);
                 const uint32_t nB = (uint32_t)(nbase + (int)offB + (int)((offB * fc_inv) >> 24) * ncorr);
                 const uint4 xA = philox4x32_10(nA, tc1, 2u, (uint32_t)g, d.rk0, d.rk1);
                 const uint4 xB = philox4x32_10(nB, tc1, 2u, (uint32_t)g, d.rk0, d.rk1);
-                wA0 = odd ? xA.z : xA.x; wA1 = odd ? xA.w : xA.y;
-                wB0 = odd ? xB.z : xB.x; wB1 = odd ? xB.w : xB.y;
-                if (stash) { SPc[eA] = make_uint2(xA.z, xA.w); SPc[eB] = make_uint2(xB.z, xB.w); }
+                if (DRAW == DRAW_EVEN_STORE) {
+                    wA0 = xA.x; wA1 = xA.y; wB0 = xB.x; wB1 = xB.y;
+                    SPc[eA] = make_uint2(xA.z, xA.w); SPc[eB] = make_uint2(xB.z, xB.w);
+                } else {
+                    wA0 = odd ? xA.z : xA.x; wA1 = odd ? xA.w : xA.y;
+                    wB0 = odd ? xB.z : xB.x; wB1 = odd ? xB.w : xB.y;
+                    if (stash) { SPc[eA] = make_uint2(xA.z, xA.w); SPc[eB] = make_uint2(xB.z, xB.w); }
+                }
             } else {
                 const uint2 sA = SPc[eA], sB = SPc[eB];
                 wA0 = sA.x; wA1 = sA.y; wB0 = sB.x; wB1 = sB.y;
@@ -862,17 +870,19 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         };
         // full rounds: thread tid takes the entries pos + tid and pos + NT + tid; the last round splits what
         // is left into two halves of whole warps, so that no warp runs a round for a missing second site
-        auto half_sweep = [&](auto fresh_tag) {
+        auto half_sweep = [&](auto draw_tag) {
             uint32_t pos = 0;
 #pragma unroll 1
-            for (; pos + 2u * NT <= n; pos += 2u * NT) update_two(fresh_tag, pos + tid, pos + NT + tid);
+            for (; pos + 2u * NT <= n; pos += 2u * NT) update_two(draw_tag, pos + tid, pos + NT + tid);
             if (pos < n) {
                 const uint32_t stride = ((n - pos + 63u) >> 6) << 5;
                 const uint32_t eA = pos + tid;
-                if ((uint32_t)tid < stride && eA < n) update_two(fresh_tag, eA, eA + stride < n ? eA + stride : eA);
+                if ((uint32_t)tid < stride && eA < n) update_two(draw_tag, eA, eA + stride < n ? eA + stride : eA);
             }
         };
-        if (fresh) half_sweep(FreshTag<true>{}); else half_sweep(FreshTag<false>{});
+        if (!fresh) half_sweep(DrawTag<DRAW_STORED>{});
+        else if (!odd && stash) half_sweep(DrawTag<DRAW_EVEN_STORE>{});
+        else half_sweep(DrawTag<DRAW_ANY>{});
         __syncthreads();
       }
     }
