@@ -391,9 +391,11 @@ int orc_equilibrate(float *phi, const uint8_t *mask, int rows, int cols,
  * paper has s = 1 (L210); BASELINE.json's configurations set s = 100 (R11).
  * acc: double [rows*cols], caller-zeroed; only prediction sites are touched.
  * ---------------------------------------------------------------------- */
-void orc_simulate(float *phi, const uint8_t *mask, int rows, int cols,
-                  double q, double T, double a_eq, uint64_t seed, uint32_t g,
-                  int or_mode, int M, int s, uint32_t *t_io, double *acc)
+/* acc2 (may be NULL): sum over the realizations of phi^2, for the spread of the realizations
+ * ("Statistics of M realizations"). */
+void orc_simulate2(float *phi, const uint8_t *mask, int rows, int cols,
+                   double q, double T, double a_eq, uint64_t seed, uint32_t g,
+                   int or_mode, int M, int s, uint32_t *t_io, double *acc, double *acc2)
 {
     uint32_t t = *t_io;
     int64_t N = (int64_t)rows * cols;
@@ -402,9 +404,20 @@ void orc_simulate(float *phi, const uint8_t *mask, int rows, int cols,
             orc_sweep(phi, mask, rows, cols, q, T, a_eq, seed, g, t, or_mode, NULL, NULL, NULL);
             ++t;
         }
-        for (int64_t n = 0; n < N; ++n) if (!mask[n]) acc[n] += (double)phi[n];
+        for (int64_t n = 0; n < N; ++n)
+            if (!mask[n]) {
+                acc[n] += (double)phi[n];
+                if (acc2) acc2[n] += (double)phi[n] * (double)phi[n];
+            }
     }
     *t_io = t;
+}
+
+void orc_simulate(float *phi, const uint8_t *mask, int rows, int cols,
+                  double q, double T, double a_eq, uint64_t seed, uint32_t g,
+                  int or_mode, int M, int s, uint32_t *t_io, double *acc)
+{
+    orc_simulate2(phi, mask, rows, cols, q, T, a_eq, seed, g, or_mode, M, s, t_io, acc, NULL);
 }
 
 /* ------------------------------------------------------------------------
@@ -421,6 +434,23 @@ void orc_predict(const double *acc, int M, const float *z, const uint8_t *mask,
         if (mask[n]) { out[n] = z[n]; continue; }
         double mean_phi = acc[n] / (double)M;
         out[n] = (float)((double)zmin + mean_phi * ((double)zmax - (double)zmin) / TWO_PI);
+    }
+}
+
+/* ------------------------------------------------------------------------
+ * Spread of the M realizations at every prediction site (Alg. 2 step 7 "Statistics of M
+ * realizations"; L148: the realizations sample the conditional distribution): the unbiased sample standard
+ * deviation of the back-transformed values, s_z = sqrt((sum phi^2 - (sum phi)^2 / M) / (M - 1)) (zmax - zmin) / (2 pi),
+ * M >= 2; 0 at sample sites (their value is data).
+ * ---------------------------------------------------------------------- */
+void orc_predict_std(const double *acc, const double *acc2, int M, const uint8_t *mask,
+                     int64_t n_sites, float zmin, float zmax, float *out)
+{
+    for (int64_t n = 0; n < n_sites; ++n) {
+        if (mask[n]) { out[n] = 0.0f; continue; }
+        double var = (acc2[n] - acc[n] * acc[n] / (double)M) / (double)(M - 1);
+        if (var < 0.0) var = 0.0;
+        out[n] = (float)(sqrt(var) * ((double)zmax - (double)zmin) / TWO_PI);
     }
 }
 

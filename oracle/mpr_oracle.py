@@ -77,6 +77,12 @@ def lib():
                                    C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_int,
                                    C.POINTER(C.c_uint32), f64p]
         L.orc_simulate.restype = None
+        L.orc_simulate2.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                    C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_int,
+                                    C.POINTER(C.c_uint32), f64p, f64p]
+        L.orc_simulate2.restype = None
+        L.orc_predict_std.argtypes = [f64p, f64p, C.c_int, u8p, C.c_int64, C.c_float, C.c_float, f32p]
+        L.orc_predict_std.restype = None
         L.orc_predict.argtypes = [f64p, C.c_int, f32p, u8p, C.c_int64, C.c_float, C.c_float, f32p]
         L.orc_predict.restype = None
         L.orc_num_threads.restype = C.c_int
@@ -210,6 +216,28 @@ def simulate(phi, mask, T, a_eq, p: Params, g=0, t0=0):
     lib().orc_simulate(phi, m, rows, cols, p.q, float(T), float(a_eq), p.seed, g, p.or_mode,
                        p.M, p.sweeps_per_real, C.byref(t), acc.reshape(-1))
     return acc, int(t.value)
+
+
+def simulate_stats(phi, mask, T, a_eq, p: Params, g=0, t0=0):
+    """Step 6 with the sums of phi and of phi^2 over the realizations: (acc, acc2, t)."""
+    rows, cols = phi.shape
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    t = C.c_uint32(t0)
+    acc = np.zeros((rows, cols), dtype=np.float64)
+    acc2 = np.zeros((rows, cols), dtype=np.float64)
+    lib().orc_simulate2(phi, m, rows, cols, p.q, float(T), float(a_eq), p.seed, g, p.or_mode,
+                        p.M, p.sweeps_per_real, C.byref(t), acc.reshape(-1), acc2.reshape(-1))
+    return acc, acc2, int(t.value)
+
+
+def predict_std(acc, acc2, M, mask, zmin, zmax) -> np.ndarray:
+    """Sample standard deviation of the M back-transformed realizations at the prediction sites (L212)."""
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    out = np.empty(m.shape, dtype=np.float32)
+    lib().orc_predict_std(np.ascontiguousarray(acc, dtype=np.float64).reshape(-1),
+                          np.ascontiguousarray(acc2, dtype=np.float64).reshape(-1), M, m.reshape(-1), m.size,
+                          float(zmin), float(zmax), out.reshape(-1))
+    return out
 
 
 def predict(acc, M, z, mask, zmin, zmax) -> np.ndarray:

@@ -503,3 +503,46 @@ def test_sweep_independent_of_thread_count(orc):
         outs.append((phi, acc, orc.energy(phi)))
     orc.set_num_threads(nthr)
     assert np.array_equal(outs[0][0], outs[1][0]) and outs[0][1] == outs[1][1] and outs[0][2] == outs[1][2]
+
+
+# ---------------------------------------------------------------------------
+# spread of the realizations, PAPER.md L212 ("Statistics of M realizations")
+# ---------------------------------------------------------------------------
+def test_predict_std_closed_forms(orc):
+    mask = np.array([[1, 0, 0, 0]], dtype=np.uint8)
+    seqs = [[0.0, 0.0, 0.0], [1.0, 2.0, 3.0], [2.5, 2.5, 2.5], [0.0, TWO_PI_F, 0.0]]    # the realizations of 4 sites
+    acc = np.array([[sum(s) for s in seqs]]); acc2 = np.array([[sum(x * x for x in s) for s in seqs]])
+    zmin, zmax = 10.0, 30.0
+    out = orc.predict_std(acc, acc2, 3, mask, zmin, zmax)
+    scale = (zmax - zmin) / TWO_PI_F
+    assert out[0, 0] == 0.0                                             # a sample site: its value is data
+    assert out[0, 1] == pytest.approx(1.0 * scale, rel=1e-6)            # sample s.d. of 1, 2, 3 is 1
+    assert out[0, 2] == 0.0                                             # constant chain
+    assert out[0, 3] == pytest.approx(math.sqrt(TWO_PI_F ** 2 * (2 / 3) / 2) * scale, rel=1e-6)
+    # cancellation below zero is clamped
+    assert orc.predict_std(np.array([[0.0, 3.0]]), np.array([[0.0, 3.0 - 1e-12]]), 3, mask[:, :2], 0, 1)[0, 1] == 0.0
+
+
+def test_simulate_stats_sums_follow_the_chain(orc):
+    """acc and acc2 are the sums of phi and phi^2 over the states after every s-th sweep of the chain."""
+    rng = np.random.default_rng(12)
+    z = rng.standard_normal((12, 9)).astype(np.float32)
+    mask = (rng.random((12, 9)) < 0.5).astype(np.uint8); mask[0, 0] = 1; mask[-1, -1] = 0
+    p = orc.Params(seed=5, M=4, sweeps_per_real=3)
+    phi, _, _ = orc.transform(z, mask, p.seed)
+    ref = phi.copy()
+    acc, acc2, t_end = orc.simulate_stats(phi, mask, 0.2, 2.0, p, t0=7)
+    s1 = np.zeros(ref.shape); s2 = np.zeros(ref.shape); t = 7
+    for _ in range(p.M):
+        for _ in range(p.sweeps_per_real):
+            orc.sweep(ref, mask, p.q, 0.2, 2.0, p.seed, 0, t); t += 1
+        s1 += ref.astype(np.float64); s2 += ref.astype(np.float64) ** 2
+    free = mask == 0
+    assert t_end == t and np.array_equal(ref, phi)
+    assert np.array_equal(acc[free], s1[free]) and np.array_equal(acc2[free], s2[free])
+    assert np.all(acc[~free] == 0) and np.all(acc2[~free] == 0)
+    assert np.all(acc2[free] * p.M >= acc[free] ** 2 * (1 - 1e-12))      # Cauchy-Schwarz
+    # the mean-only entry point is the same chain
+    phi2, _, _ = orc.transform(z, mask, p.seed)
+    acc_only, _ = orc.simulate(phi2, mask, 0.2, 2.0, p, t0=7)
+    assert np.array_equal(acc_only, acc)
