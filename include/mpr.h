@@ -132,6 +132,13 @@ mpr_status mpr_simulate(mpr_ctx* ctx);
  * value bit for bit.  Asynchronous. */
 mpr_status mpr_predict(mpr_ctx* ctx, float* d_out);
 
+/* "Statistics of M realizations" (Alg. 2 step 7, L212; L148: the realizations sample the conditional
+ * distribution): d_out device float [batch][rows][cols] receives, at prediction sites, the unbiased sample
+ * standard deviation of the M back-transformed realizations accumulated so far,
+ * sqrt(sum_k (phi_k - mean)^2 / (M - 1)) (z_max - z_min) / (2 pi), and 0 at sample sites.  Needs M >= 2
+ * realizations (else MPR_ERR_STATE).  Synchronises. */
+mpr_status mpr_predict_std(mpr_ctx* ctx, float* d_out);
+
 mpr_status mpr_destroy(mpr_ctx* ctx);
 
 /* ---- Alg. 2 step 4: parameter inference ---- */

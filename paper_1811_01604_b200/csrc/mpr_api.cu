@@ -72,7 +72,7 @@ bool make_geometry(int batch, int rows, int cols, Geometry* g)
 }
 
 struct Layout {
-    size_t states, done, partials, values, phi, bits, vec, acc, tile_meta, entries, total;
+    size_t states, done, partials, values, phi, bits, vec, acc, m2, tile_meta, entries, total;
 };
 
 Layout make_layout(int batch, const Geometry& g)
@@ -89,6 +89,7 @@ Layout make_layout(int batch, const Geometry& g)
     L.bits      = take(B * g.words * sizeof(uint32_t));
     L.vec       = take(2 * B * g.VG * sizeof(float2));
     L.acc       = take(B * g.N * sizeof(float));
+    L.m2        = take(B * g.N * sizeof(float));
     L.tile_meta = take(B * g.ntiles * sizeof(TileMeta));
     L.entries   = take((B * g.entry_stride + 16) * sizeof(uint16_t));
     L.total = o;
@@ -131,7 +132,7 @@ mpr_status fetch_states(mpr_ctx* ctx)
     return MPR_OK;
 }
 
-typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t);
+typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t);
 
 // fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps);
 // std_fc = the frame pitch is the compile-time STD_FC (standard tile shape)
@@ -164,7 +165,7 @@ void note_a(mpr_ctx* ctx, double a_min)
 // K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile.
 // flip = 0 / 1: read buffer ctx->cur ^ flip (known to the host); PER_GRID: each grid reads its own GridState::cur
 enum : uint32_t { PER_GRID = 2u };
-mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags)
+mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags, uint32_t real_no = 0)
 {
     ctx->dirty = true;
     const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
@@ -177,17 +178,18 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
     }
     const uint32_t src_sel = flip == PER_GRID ? PER_GRID : (ctx->cur ^ flip);
     kern<<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(
-        ctx->map[0], ctx->map[1], ctx->d, K, t_off, src_sel, flags, ctx->pf_dist);
+        ctx->map[0], ctx->map[1], ctx->d, K, t_off, src_sel, flags, ctx->pf_dist, real_no);
     CU_LAUNCH();
     return MPR_OK;
 }
 
 // n sweeps at the current a as passes of at most k_max sweeps; *t_off and *flip carry the uncommitted progress
-mpr_status launch_sweeps(mpr_ctx* ctx, uint32_t n, uint32_t* t_off, uint32_t* flip, uint32_t flags, uint32_t last_flags)
+mpr_status launch_sweeps(mpr_ctx* ctx, uint32_t n, uint32_t* t_off, uint32_t* flip, uint32_t flags, uint32_t last_flags,
+                         uint32_t real_no = 0)
 {
     while (n) {
         const uint32_t K = n < ctx->k_max ? n : ctx->k_max;
-        mpr_status s = launch_pass(ctx, K, *t_off, *flip, flags | (n == K ? last_flags : 0u));
+        mpr_status s = launch_pass(ctx, K, *t_off, *flip, flags | (n == K ? last_flags : 0u), real_no);
         if (s != MPR_OK) return s;
         *t_off += K; *flip ^= 1u; n -= K;
     }
@@ -313,6 +315,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float
     d.bits = (uint32_t*)(base + lay.bits);
     d.vec = (float2*)(base + lay.vec);
     d.acc = (float*)(base + lay.acc);
+    d.m2 = (float*)(base + lay.m2);
     d.tile_meta = (TileMeta*)(base + lay.tile_meta);
     d.entries = (uint16_t*)(base + lay.entries);
     d.VG = g.VG; d.VB = (size_t)batch * g.VG;
@@ -445,6 +448,7 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     k_begin_run<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, (const float*)d.e_partials);
     CU_LAUNCH();
     CU(cudaMemsetAsync(d.acc, 0, (size_t)d.batch * d.N * sizeof(float), ctx->stream));
+    CU(cudaMemsetAsync(d.m2, 0, (size_t)d.batch * d.N * sizeof(float), ctx->stream));
     k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d, ctx->unconditional ? 1 : 0);
     CU_LAUNCH();
     CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
@@ -516,7 +520,7 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
     uint32_t t_off = 0, flip = 0;
     for (uint32_t j = 0; j < ctx->prm.M; ++j) {
         // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
-        mpr_status s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE);
+        mpr_status s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE, j + 1u);   // realization number: realizations so far + j + 1
         if (s != MPR_OK) return s;
     }
     k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, t_off, flip, ctx->prm.M);
@@ -532,6 +536,20 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out)
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
     k_predict<<<site_grid(ctx), 256, 0, ctx->stream>>>(d, d_out);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr_predict_std(mpr_ctx* ctx, float* d_out)
+{
+    if (!ctx || !d_out) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr_status s = fetch_states(ctx);
+    if (s != MPR_OK) return s;
+    for (int b = 0; b < ctx->d.batch; ++b)
+        if (ctx->h_states[b].realizations < 2u) return MPR_ERR_STATE;
+    k_predict_std<<<site_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, d_out);
     CU_LAUNCH();
     return MPR_OK;
 }

@@ -75,6 +75,7 @@ struct Dev {
     uint32_t*  bits;           // [batch][words] fixed-site bitmask
     float2*    vec;            // [2 buffers][batch][rows][pitch] row-major unit vectors (pitch = cols rounded up to even)
     float*     acc;            // [batch][N] sum over realizations of phi at the prediction sites
+    float*     m2;             // [batch][N] sum of squared deviations from the running mean (Welford), for the spread (L212)
     TileMeta*  tile_meta;      // [batch][ntiles]
     uint16_t*  entries;        // [batch][entry_stride] tile frames' free sites: offset in the frame (row * FC + col)
     int        batch, rows, cols;
@@ -747,7 +748,7 @@ template <int M> struct DrawTag { static constexpr int value = M; };
 template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD>
 __global__ void __launch_bounds__(TILE_THREADS, TILE_THREADS >= 384 ? 2 : 3)
 k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
-           uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist)
+           uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist, uint32_t real_no)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar[2];       // [0] frame, [1] entry list
@@ -896,13 +897,21 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             bulk_store(dst + (size_t)(tg.r0 + lr) * d.pitch + tg.c0, S + (H + lr) * FC + H, row_bytes);
 
     if (flags & PASS_ACCUMULATE) {
-        // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites
+        // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites; and for the spread of the
+        // realizations (L212) the sum of squared deviations, updated from the running mean so that nothing cancels:
+        // m2 += (phi - mean_{k-1}) (phi - mean_k), k = number of this realization
         float* acc = d.acc + (size_t)g * d.N;
+        float* m2 = d.m2 + (size_t)g * d.N;
+        const uint32_t k = st.realizations + real_no;
+        const float inv_km1 = k > 1u ? 1.0f / (float)(k - 1u) : 0.0f, inv_k = 1.0f / (float)k;
         for (int c = 0; c < 2; ++c) {
             const uint32_t base = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
             for (uint32_t e = tid; e < s_cle[c][0]; e += NT) {
                 const uint32_t off = E[base + e];
-                acc[nbase + (int)off + (int)((off * fc_inv) >> 24) * ncorr] += angle_of(S[off], d.inv_q);
+                const int idx = nbase + (int)off + (int)((off * fc_inv) >> 24) * ncorr;
+                const float phi = angle_of(S[off], d.inv_q), before = acc[idx], after = before + phi;
+                acc[idx] = after;
+                if (k > 1u) m2[idx] += (phi - before * inv_km1) * (phi - after * inv_k);
             }
         }
     }
@@ -1173,6 +1182,19 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, float* __restrict__ out)
     const double mean_phi = (double)d.acc[o] / (double)s.realizations;
     const double z = (double)s.zmin + mean_phi * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F;
     out[o] = (float)z;
+}
+
+// spread of the realizations (L212): sample standard deviation of the back-transformed values, 0 at sample sites
+__global__ void __launch_bounds__(256) k_predict_std(Dev d, float* __restrict__ out)
+{
+    const int g = blockIdx.y;
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N) return;
+    const size_t o = (size_t)g * d.N + n;
+    if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = 0.0f; return; }
+    const GridState& s = d.states[g];
+    const double var = s.realizations > 1u ? fmax((double)d.m2[o], 0.0) / (double)(s.realizations - 1u) : 0.0;
+    out[o] = (float)(sqrt(var) * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F);
 }
 
 // angle import / export at the prediction sites ------------------------------

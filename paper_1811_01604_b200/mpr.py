@@ -32,7 +32,7 @@ EXPORTS = (
     "mpr_set_sweep_index", "mpr_sweep", "mpr_energy", "mpr_get_transform", "mpr_get_mask_bits",
     "mpr_get_stats", "mpr_get_launch_count", "mpr_status_string", "mpr_last_cuda_error",
     "mpr_sample_energy", "mpr_create_unconditional", "mpr_measure_energy", "mpr_energy_table",
-    "mpr_infer_temperature",
+    "mpr_infer_temperature", "mpr_predict_std",
 )
 
 
@@ -91,6 +91,7 @@ def lib():
         L.mpr_get_mask_bits.argtypes = [vp, vp]
         L.mpr_get_stats.argtypes = [vp, C.POINTER(mpr_stats)]
         L.mpr_get_launch_count.argtypes = [vp, C.POINTER(u64)]
+        L.mpr_predict_std.argtypes = [vp, vp]
         L.mpr_sample_energy.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(u64)]
         L.mpr_create_unconditional.argtypes = [C.POINTER(vp), i, i, i, vp, sz, vp]
         L.mpr_measure_energy.argtypes = [vp, u32, C.POINTER(C.c_double)]
@@ -228,6 +229,13 @@ class Mpr:
         if out is None:
             out = torch.empty((self.batch, self.rows, self.cols), dtype=torch.float32, device=self.device)
         _check(lib().mpr_predict(self._ctx, out.data_ptr()), "mpr_predict")
+        return out
+
+    def predict_std(self, out=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty((self.batch, self.rows, self.cols), dtype=torch.float32, device=self.device)
+        _check(lib().mpr_predict_std(self._ctx, out.data_ptr()), "mpr_predict_std")
         return out
 
     # -- Alg. 2 step 4 -------------------------------------------------------

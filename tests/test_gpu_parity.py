@@ -487,3 +487,68 @@ def test_same_seed_same_result_bitwise(torch_cuda, mpr):
         outs.append((pred.cpu().numpy(), st[0].equil_sweeps, st[0].e_last))
     assert np.array_equal(outs[0][0].view(np.uint32), outs[1][0].view(np.uint32))
     assert outs[0][1:] == outs[1][1:]
+
+
+# ---------------------------------------------------------------------------
+# spread of the realizations
+# ---------------------------------------------------------------------------
+def test_predict_std_against_oracle_chain(torch_cuda, mpr, orc):
+    """The same short chain on both sides from an identical oracle-made state (M = 4 realizations of 2 sweeps):
+    the sample standard deviation per prediction site agrees except where a near-threshold decision fell the
+    other way in one of the 8 sweeps."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg2", L=192)
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    p = orc.Params(seed=w.seed, equil_cap=80, M=4, sweeps_per_real=2)
+    phi, zmin, zmax = orc.transform(z, m, p.seed)
+    st = orc.equilibrate(phi, m, T, p)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=p.seed, M=p.M, sweeps_per_real=p.sweeps_per_real)
+    with pytest.raises(mpr.MprError) as e:
+        ctx.predict_std()                                   # no realization yet
+    assert e.value.name == "MPR_ERR_STATE"
+    ctx.set_angles(torch.from_numpy(phi)[None].cuda())
+    ctx.set_sweep_index(st["t"])
+    ctx.sweep(0, st["a"])                                   # sets a, no sweep
+    ctx.simulate()
+    got = ctx.predict_std().cpu().numpy()[0]
+    mean_gpu = ctx.predict().cpu().numpy()[0]
+    acc, acc2, _ = orc.simulate_stats(phi, m, T, st["a"], p, t0=st["t"])
+    ref = orc.predict_std(acc, acc2, p.M, m, zmin, zmax)
+    mean_ref = orc.predict(acc, p.M, z, m, zmin, zmax)
+    free = m == 0
+    assert np.all(got[~free] == 0.0)
+    scale = (float(zmax) - float(zmin)) / TWO_PI_F
+    bad = free & (np.abs(got - ref) > 2e-5 * scale + 1e-3 * ref)
+    assert bad.sum() <= max(2, 1e-3 * free.sum()), (int(bad.sum()), int(free.sum()))
+    assert np.abs(mean_gpu - mean_ref)[free & ~bad].max() < 2e-5 * scale
+    assert float(got[free].mean()) == pytest.approx(float(ref[free].mean()), rel=2e-3)
+    ctx.close()
+
+
+def test_predict_std_full_run_and_running_update_has_no_cancellation(torch_cuda, mpr, orc):
+    """cfg1 full run (M = 10 x 100 sweeps): the mean spread over the prediction sites agrees with the oracle's
+    (mean over seeds); and a frozen chain (T -> 0, huge a, no over-relaxation) has spread ~ 0 although phi^2 ~ 10."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    free = m == 0
+    g_means, o_means = [], []
+    for seed in range(6000, 6006):
+        ctx.set_params(T, seed=seed, equil_cap=w.equil_cap, sweeps_per_real=w.sweeps_per_real, M=w.M).equilibrate().simulate()
+        g_means.append(float(ctx.predict_std().cpu().numpy()[0][free].mean()))
+        p = orc.Params(seed=seed, equil_cap=w.equil_cap, sweeps_per_real=w.sweeps_per_real, M=w.M)
+        phi, zmin, zmax = orc.transform(z, m, seed)
+        st = orc.equilibrate(phi, m, T, p)
+        acc, acc2, _ = orc.simulate_stats(phi, m, T, st["a"], p, t0=st["t"])
+        o_means.append(float(orc.predict_std(acc, acc2, p.M, m, zmin, zmax)[free].mean()))
+    assert np.mean(g_means) == pytest.approx(np.mean(o_means), rel=0.03), (g_means, o_means)
+    # frozen chain
+    ctx.set_params(1e-9, seed=1, M=50, sweeps_per_real=1, or_mode=2)
+    ctx.sweep(0, 1e6)
+    ctx.simulate()
+    s = ctx.predict_std().cpu().numpy()[0]
+    zmin, zmax, _ = orc.minmax(z, m)
+    assert s[free].max() < 1e-4 * (float(zmax) - float(zmin))
+    ctx.close()

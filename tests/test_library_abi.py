@@ -50,10 +50,10 @@ def test_workspace_query_validates_and_scales(lib):
     big = mpr.mpr_query_workspace(1, 4096, 4096)
     batch = mpr.mpr_query_workspace(32, 2048, 2048)
     assert small < 1 << 20
-    # about 31.3 bytes per site: 16 (two buffers of unit vectors) + 4 + 4 (values, angles) + 4 (accumulator)
-    # + 1/8 (bitmask) + 3.2 (tile-frame entries, 2 bytes each, worst case) + padding
-    assert 29 * 4096 ** 2 < big < 34 * 4096 ** 2
-    assert 29 * 32 * 2048 ** 2 < batch < 34 * 32 * 2048 ** 2
+    # about 35.3 bytes per site: 16 (two buffers of unit vectors) + 4 + 4 (values, angles) + 4 + 4 (sum and squared
+    # deviations over the realizations) + 1/8 (bitmask) + 3.2 (tile-frame entries, 2 bytes each, worst case) + padding
+    assert 33 * 4096 ** 2 < big < 38 * 4096 ** 2
+    assert 33 * 32 * 2048 ** 2 < batch < 38 * 32 * 2048 ** 2
     assert mpr.mpr_query_workspace(3, 37, 53) % 256 == 0
 
 
