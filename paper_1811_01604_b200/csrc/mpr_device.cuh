@@ -789,10 +789,16 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         const uint32_t entry_bytes = ((colour1_base(n0) + n1 + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
         mbar_expect_tx(&s_bar[1], entry_bytes);
         if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar[1]);
-    } else if (tid == 64 && pf_dist && tile + (int)pf_dist < d.ntiles) {
-        // pull the frame of the tile that will run in this slot next towards L2
+    }
+    // warp 2 pulls what the tile that will run in this CTA slot next needs towards L2: its frame now, its entry
+    // list (whose place and size are in its TileMeta, read here, used after the waits below) a little later
+    const bool prefetcher = tid == 64 && pf_dist && tile + (int)pf_dist < d.ntiles;
+    uint32_t pf_base = 0, pf_n0 = 0, pf_n1 = 0;
+    if (prefetcher) {
         const TileGeom tn = tile_geom(d, tile + (int)pf_dist);
         tma_prefetch_frame(src_buf ? &map1 : &map0, tn.c0 - H, tn.r0 - H, g);
+        const TileMeta& mn = d.tile_meta[(size_t)g * d.ntiles + tile + pf_dist];
+        pf_base = mn.base; pf_n0 = mn.cle[0][MAX_H - 1]; pf_n1 = mn.cle[1][MAX_H - 1];
     }
     if (tid >= 96 && tid < 96 + 2 * MAX_H) (&s_cle[0][0])[tid - 96] = (&meta.cle[0][0])[tid - 96];
     const float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f, nlT = st.neg_log2e_over_T;
@@ -804,6 +810,10 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     __syncthreads();
     mbar_wait(&s_bar[1], 0);
     mbar_wait(&s_bar[0], 0);
+    if (prefetcher) {
+        const uint32_t bytes = ((colour1_base(pf_n0) + pf_n1 + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
+        if (bytes) bulk_prefetch(d.entries + (size_t)g * d.entry_stride + pf_base, bytes);
+    }
 
     // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1).  What a half-sweep needs to
     // know is tabulated by one warp for 16 half-sweeps at a time (HalfSweep), so that the other warps do not redo it.
