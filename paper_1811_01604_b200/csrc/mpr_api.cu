@@ -125,6 +125,7 @@ struct mpr_ctx {
     bool         qhalf;
     bool         dirty;           // vectors changed since d.phi was last written at the free sites
     int          device;          // device the workspace lives on
+    bool         no_pdl;          // MPR_NO_PDL=1: launch the tile passes without programmatic stream serialization (experiments)
     bool         unconditional;   // no data: every node free, ordered start (Alg. 2 step 4.2)
     double       a_min;           // smallest proposal-width parameter a over the grids, as far as the host knows it (0 = unknown)
     bool         small_d;         // every grid's proposal half-rotation q pi / (2 a) is below SMALL_HD (host knowledge of a)
@@ -186,9 +187,18 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
         ctx->pf_dist = (uint32_t)(per_sm > 0 ? per_sm * sms : sms);
     }
     const uint32_t src_sel = flip == PER_GRID ? PER_GRID : (ctx->cur ^ flip);
-    kern<<<dim3(ctx->d.ntiles, ctx->d.batch), TILE_THREADS, ctx->smem_bytes, ctx->stream>>>(
-        ctx->map[0], ctx->map[1], ctx->d, K, t_off, src_sel, flags, ctx->pf_dist, real_no);
-    CU_LAUNCH();
+    // programmatic stream serialization: this pass's CTAs may start (and load their tile lists) while the last
+    // CTAs of the previous kernel still run; k_tilepass waits for that kernel before it reads any result of it
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ctx->d.ntiles, ctx->d.batch); cfg.blockDim = dim3(TILE_THREADS);
+    cfg.dynamicSmemBytes = ctx->smem_bytes; cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = ctx->no_pdl ? 0 : 1;
+    ++ctx->launches;
+    if (!cuda_ok(cudaLaunchKernelEx(&cfg, kern, ctx->map[0], ctx->map[1], ctx->d, K, t_off, src_sel, flags, ctx->pf_dist, real_no),
+                 "tile pass launch")) return MPR_ERR_CUDA;
     return MPR_OK;
 }
 
@@ -313,6 +323,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float
     }
     ctx->state = CREATED;
     ctx->unconditional = unconditional;
+    ctx->no_pdl = getenv("MPR_NO_PDL") != nullptr;
     ctx->prm.q = 0.5f; ctx->d.q = 0.5f; ctx->d.inv_q = 2.0f;      // until mpr_set_params says otherwise (L89)
     char* base = (char*)d_workspace;
     Dev& d = ctx->d;

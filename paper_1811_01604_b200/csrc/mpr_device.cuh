@@ -717,6 +717,9 @@ __device__ __forceinline__ void bulk_commit_wait_read()
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
+// programmatic dependent launch (no-ops in a kernel launched without the attribute)
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------
@@ -761,7 +764,10 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     static_assert(TILE_THREADS >= 96 + 2 * MAX_H && TILE_THREADS >= HS_CHUNK, "the prologue gives warps 0-3 their own jobs");
     const int tile = blockIdx.x, g = blockIdx.y;
     const GridState& st = d.states[g];
-    if (FUSED && (flags & PASS_CHECK_DONE) && st.done) return;
+    // Programmatic dependent launch: the next kernel of the stream may start its CTAs while the last of this
+    // one still run.  What a tile pass does before its own griddep_wait() touches only data no kernel of a run
+    // writes (tile lists) and its own shared memory.
+    griddep_launch_dependents();
 
     // frame pitch: a compile-time constant for the standard tile shape (neighbour offsets become immediates)
     const int H = d.H, FC = FCT ? FCT : d.FC;
@@ -773,22 +779,31 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const TileGeom tg = tile_geom(d, tile);
     const TileMeta& meta = d.tile_meta[(size_t)g * d.ntiles + tile];
-    // src_sel 0 / 1: the source buffer is known to the host (every grid alike); 2: per grid, from its state
-    const uint32_t src_buf = src_sel < 2u ? src_sel : st.cur;
-    float2* dst = vec_grid(d, g, src_buf ^ 1u);
 
-    // three warps start the tile: warp 0 the frame (before anything else is known about the tile), warp 1 the
-    // entry list (needs the tile's counts from global memory first), warp 2 the L2 prefetch
-    if (tid == 0) {
-        mbar_init(&s_bar[0], 1); s_accepted = 0;
-        mbar_expect_tx(&s_bar[0], (uint32_t)(d.FR * FC * sizeof(float2)));
-        tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar[0]);
-    } else if (tid == 32) {
+    // three warps start the tile: warp 1 the entry list (needs the tile's counts from global memory first), and,
+    // once the previous kernel's results are visible, warp 0 the frame and warp 2 the L2 prefetch
+    if (tid == 0) { mbar_init(&s_bar[0], 1); s_accepted = 0; }
+    else if (tid == 32) {
         mbar_init(&s_bar[1], 1);
         const uint32_t n0 = meta.cle[0][MAX_H - 1], n1 = meta.cle[1][MAX_H - 1];
         const uint32_t entry_bytes = ((colour1_base(n0) + n1 + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
         mbar_expect_tx(&s_bar[1], entry_bytes);
         if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar[1]);
+    }
+    if (tid >= 96 && tid < 96 + 2 * MAX_H) (&s_cle[0][0])[tid - 96] = (&meta.cle[0][0])[tid - 96];
+
+    griddep_wait();         // from here on: the vector buffers and the grids' states as the previous kernels left them
+    if (FUSED && (flags & PASS_CHECK_DONE) && st.done) {        // this grid's equilibration has stopped
+        __syncthreads();
+        mbar_wait(&s_bar[1], 0);                                 // no copy into this CTA's shared memory is left in flight
+        return;
+    }
+    // src_sel 0 / 1: the source buffer is known to the host (every grid alike); 2: per grid, from its state
+    const uint32_t src_buf = src_sel < 2u ? src_sel : st.cur;
+    float2* dst = vec_grid(d, g, src_buf ^ 1u);
+    if (tid == 0) {
+        mbar_expect_tx(&s_bar[0], (uint32_t)(d.FR * FC * sizeof(float2)));
+        tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar[0]);
     }
     // warp 2 pulls what the tile that will run in this CTA slot next needs towards L2: its frame now, its entry
     // list (whose place and size are in its TileMeta, read here, used after the waits below) a little later
@@ -800,7 +815,6 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         const TileMeta& mn = d.tile_meta[(size_t)g * d.ntiles + tile + pf_dist];
         pf_base = mn.base; pf_n0 = mn.cle[0][MAX_H - 1]; pf_n1 = mn.cle[1][MAX_H - 1];
     }
-    if (tid >= 96 && tid < 96 + 2 * MAX_H) (&s_cle[0][0])[tid - 96] = (&meta.cle[0][0])[tid - 96];
     const float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f, nlT = st.neg_log2e_over_T;
     const uint32_t t0 = st.t + t_off;
     const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H), ncorr = d.cols - FC;
