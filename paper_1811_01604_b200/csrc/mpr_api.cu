@@ -340,6 +340,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float
     d.entries = (uint16_t*)(base + lay.entries);
     d.VG = g.VG; d.VB = (size_t)batch * g.VG;
     d.entry_stride = g.entry_stride; d.n_partials = g.n_partials;
+    d.tile_entries = (uint32_t)(g.entry_stride / (size_t)g.ntiles);
     d.fc_inv = (uint32_t)(((1u << 24) + (uint32_t)g.FC - 1u) / (uint32_t)g.FC);
     d.TR = g.TR; d.TC = g.TC; d.H = g.H; d.FR = g.FR; d.FC = g.FC; d.ntx = g.ntx; d.nty = g.nty; d.ntiles = g.ntiles;
     d.batch = batch; d.rows = rows; d.cols = cols;

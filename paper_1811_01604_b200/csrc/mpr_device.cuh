@@ -59,7 +59,6 @@ struct GridState {
 
 // Free sites of one tile frame (core + halo), see k_tile_fill.
 struct TileMeta {
-    uint32_t base;                    // offset of the tile's entries in Dev::entries (per grid), multiple of 16
     uint32_t cle[2][MAX_H];           // cle[c][k] = entries of colour c with ring <= k (ring = distance outside the core)
 };
 // colour 1's list starts on a 16-entry boundary after colour 0's
@@ -82,7 +81,9 @@ struct Dev {
     uint32_t   N, words, pitch;
     size_t     VG;             // float2 elements of one grid in one buffer = rows * pitch
     size_t     VB;             // float2 elements per vector buffer = batch * VG
-    size_t     entry_stride;
+    size_t     entry_stride;   // entries per grid = ntiles * tile_entries
+    uint32_t   tile_entries;   // room of one tile's lists (worst case: every frame site free), multiple of 16; tile i's
+                               // lists start at i * tile_entries, so that loading them needs nothing read first
     uint32_t   n_partials;
     // tiling
     int        TR, TC, H, FR, FC, ntx, nty, ntiles;
@@ -391,27 +392,16 @@ __global__ void __launch_bounds__(256) k_tile_count(Dev d)
     }
 }
 
-// one warp per grid: exclusive scan of the tiles' entry counts (each rounded up to a multiple of 16
-// so that every tile's list starts on a 32-byte boundary), and their maximum
+// one warp per grid: the largest entry count of a tile (two 16-aligned lists), which sizes the tile pass's
+// shared memory and its entry-list copy
 __global__ void k_tile_scan(Dev d)
 {
     const int g = blockIdx.x;
     const uint32_t lane = threadIdx.x;
-    TileMeta* m = d.tile_meta + (size_t)g * d.ntiles;
-    uint32_t carry = 0, mx = 0;
-    for (int base = 0; base < d.ntiles; base += 32) {
-        const int i = base + lane;
-        const uint32_t c = i < d.ntiles ? (colour1_base(m[i].cle[0][MAX_H - 1]) + m[i].cle[1][MAX_H - 1] + 15u) & ~15u : 0u;
-        mx = max(mx, c);
-        uint32_t x = c;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, o);
-            if (lane >= (uint32_t)o) x += y;
-        }
-        if (i < d.ntiles) m[i].base = carry + x - c;
-        carry += __shfl_sync(0xFFFFFFFFu, x, 31);
-    }
+    const TileMeta* m = d.tile_meta + (size_t)g * d.ntiles;
+    uint32_t mx = 0;
+    for (int i = lane; i < d.ntiles; i += 32)
+        mx = max(mx, (colour1_base(m[i].cle[0][MAX_H - 1]) + m[i].cle[1][MAX_H - 1] + 15u) & ~15u);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
     if (lane == 0) d.states[g].max_tile_entries = mx;
@@ -430,7 +420,7 @@ __global__ void __launch_bounds__(256) k_tile_fill(Dev d)
     const TileGeom t = tile_geom(d, tile);
     const TileMeta& m = d.tile_meta[(size_t)g * d.ntiles + tile];
     const uint32_t* bits = d.bits + (size_t)g * d.words;
-    uint16_t* out = d.entries + (size_t)g * d.entry_stride + m.base;
+    uint16_t* out = d.entries + (size_t)g * d.entry_stride + (size_t)tile * d.tile_entries;
     for (int i = threadIdx.x; i < d.FR * d.FC; i += blockDim.x) {
         const int lr = i / d.FC, lc = i - lr * d.FC;
         int colour, ring;
@@ -784,11 +774,12 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     // once the previous kernel's results are visible, warp 0 the frame and warp 2 the L2 prefetch
     if (tid == 0) { mbar_init(&s_bar[0], 1); s_accepted = 0; }
     else if (tid == 32) {
+        // the entry list: always the size of the largest tile's (the rest of this tile's room is never indexed),
+        // from a place that depends on the tile number only -- nothing has to be read first
         mbar_init(&s_bar[1], 1);
-        const uint32_t n0 = meta.cle[0][MAX_H - 1], n1 = meta.cle[1][MAX_H - 1];
-        const uint32_t entry_bytes = ((colour1_base(n0) + n1 + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
+        const uint32_t entry_bytes = d.max_entries * (uint32_t)sizeof(uint16_t);
         mbar_expect_tx(&s_bar[1], entry_bytes);
-        if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + meta.base, entry_bytes, &s_bar[1]);
+        if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + (size_t)tile * d.tile_entries, entry_bytes, &s_bar[1]);
     }
     if (tid >= 96 && tid < 96 + 2 * MAX_H) (&s_cle[0][0])[tid - 96] = (&meta.cle[0][0])[tid - 96];
 
@@ -805,15 +796,13 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         mbar_expect_tx(&s_bar[0], (uint32_t)(d.FR * FC * sizeof(float2)));
         tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar[0]);
     }
-    // warp 2 pulls what the tile that will run in this CTA slot next needs towards L2: its frame now, its entry
-    // list (whose place and size are in its TileMeta, read here, used after the waits below) a little later
-    const bool prefetcher = tid == 64 && pf_dist && tile + (int)pf_dist < d.ntiles;
-    uint32_t pf_base = 0, pf_n0 = 0, pf_n1 = 0;
-    if (prefetcher) {
+    // warp 2 pulls what the tile that will run in this CTA slot next needs towards L2: its frame and its entry list
+    if (tid == 64 && pf_dist && tile + (int)pf_dist < d.ntiles) {
         const TileGeom tn = tile_geom(d, tile + (int)pf_dist);
         tma_prefetch_frame(src_buf ? &map1 : &map0, tn.c0 - H, tn.r0 - H, g);
-        const TileMeta& mn = d.tile_meta[(size_t)g * d.ntiles + tile + pf_dist];
-        pf_base = mn.base; pf_n0 = mn.cle[0][MAX_H - 1]; pf_n1 = mn.cle[1][MAX_H - 1];
+        if (d.max_entries)
+            bulk_prefetch(d.entries + (size_t)g * d.entry_stride + (size_t)(tile + pf_dist) * d.tile_entries,
+                          d.max_entries * (uint32_t)sizeof(uint16_t));
     }
     const float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f, nlT = st.neg_log2e_over_T;
     const uint32_t t0 = st.t + t_off;
@@ -824,10 +813,6 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     __syncthreads();
     mbar_wait(&s_bar[1], 0);
     mbar_wait(&s_bar[0], 0);
-    if (prefetcher) {
-        const uint32_t bytes = ((colour1_base(pf_n0) + pf_n1 + 15u) & ~15u) * (uint32_t)sizeof(uint16_t);
-        if (bytes) bulk_prefetch(d.entries + (size_t)g * d.entry_stride + pf_base, bytes);
-    }
 
     // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1).  What a half-sweep needs to
     // know is tabulated by one warp for 16 half-sweeps at a time (HalfSweep), so that the other warps do not redo it.
