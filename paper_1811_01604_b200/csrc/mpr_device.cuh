@@ -901,9 +901,10 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 
     // write the core back, one bulk copy per row (an odd last column takes the zero pad column along)
     const uint32_t row_bytes = (uint32_t)((tg.TCc + 1) & ~1) * (uint32_t)sizeof(float2);
-    if (lane == 0)          // one issuing lane per warp: the copy engine takes its operands from uniform registers
-        for (int lr = warp; lr < tg.TRc; lr += NW)
-            bulk_store(dst + (size_t)(tg.r0 + lr) * d.pitch + tg.c0, S + (H + lr) * FC + H, row_bytes);
+    // rows dealt over the warps first, then over a warp's lanes: the copy engine takes its operands from uniform
+    // registers, one issuing lane after the other, so every warp issues its few copies at the same time
+    for (int lr = warp + NW * lane; lr < tg.TRc; lr += NW * 32)
+        bulk_store(dst + (size_t)(tg.r0 + lr) * d.pitch + tg.c0, S + (H + lr) * FC + H, row_bytes);
 
     if (flags & PASS_ACCUMULATE) {
         // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites; and for the spread of the
