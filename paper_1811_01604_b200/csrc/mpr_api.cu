@@ -185,6 +185,7 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)kern, TILE_THREADS, ctx->smem_bytes));
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
         ctx->pf_dist = (uint32_t)(per_sm > 0 ? per_sm * sms : sms);
+        if (const char* e = getenv("MPR_PF_DIST")) ctx->pf_dist = (uint32_t)atoi(e) ? (uint32_t)atoi(e) : ctx->pf_dist;   // experiments
     }
     const uint32_t src_sel = flip == PER_GRID ? PER_GRID : (ctx->cur ^ flip);
     // programmatic stream serialization: this pass's CTAs may start (and load their tile lists) while the last
