@@ -722,11 +722,12 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // updated redundantly; they reproduce the neighbouring tiles' results bit for
 // bit because the random numbers are keyed by (site, sweep).  After half-sweep
 // number hs (0-based) the frame is valid up to ring 2K-1-hs, so each
-// half-sweep only updates the suffix of the entry list with ring <= 2K-1-hs.
-// Every thread keeps two sites in flight.  Optionally fused at the end:
+// half-sweep only updates the prefix of the entry list with ring <= 2K-1-hs.
+// Every thread keeps two sites in flight and their arithmetic shares f32x2
+// instructions (update_pair).  Optionally fused at the end:
 //   PASS_ENERGY      a5: - sum over the core's colour-1 sites of v.h (each bond once)   [FUSED only]
 //   PASS_COUNT       a5: accepted proposals of the core sites                          [FUSED only]
-//   PASS_ACCUMULATE  a7: acc += phi at the core's prediction sites
+//   PASS_ACCUMULATE  a7: acc += phi at the core's prediction sites (and the squared deviations for L212)
 // ---------------------------------------------------------------------------
 // what one half-sweep of a tile pass needs to know (tabulated per CTA, see k_tilepass)
 struct __align__(16) HalfSweep { uint32_t n, cbase, c1, flags; };   // entries to walk, list offset, Philox counter word 1, HS_*
