@@ -375,6 +375,15 @@ def run_b200(args, w):
             out["cpu_baseline"] = {
                 "value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
                 "sample": f"{n_sweeps} UPDATE sweeps of grid 0 of {w.name} ({w.rows}x{w.cols}) from the initial state"}
+            # the same oracle on ONE thread (a shorter sample), the arm the paper's speedups are quoted against
+            from oracle import mpr_oracle as orc
+            orc.set_num_threads(1)
+            rate1, dt1, _ = oracle_sample(w, max(2, n_sweeps // 16))
+            orc.set_num_threads(cores)
+            out["cpu_baseline"].update({
+                "value_1_thread": rate1 / 1e9, "seconds_1_thread": dt1,
+                "paper_context": "paper (BASELINE.md): 166x-306x end to end at 1024^2 and 'almost 500 times' at 2048^2, "
+                                 "GTX 980 against one i5-4440 core, single precision; another machine, context only"})
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
