@@ -411,6 +411,21 @@ def test_t3_full_run_cfg2_shape(torch_cuda, mpr, orc):
     assert (1.0 + e_g) == pytest.approx(1.0 + e_o, rel=0.01)
 
 
+def test_t3_full_run_cfg3_and_cfg4_at_full_size_short_chains(torch_cuda, mpr, orc):
+    """configs[2] (1024 x 1024 with holes) and configs[3] (4096 x 4096) at full size, whole path on both sides,
+    with one sweep per realization so that the oracle's ~200-300 sweeps stay within seconds (the
+    full-length oracle run is infeasible there).  One seed: at these sizes the seed-to-seed noise is far below 1 %."""
+    for name in ("cfg3", "cfg4"):
+        w = synth.make_workload(name)
+        r = _full_run_scores(orc, mpr, torch_cuda, w, seeds=[w.seed], s=1, M=100)[0]
+        mae_g, mae_o, rmse_g, rmse_o, e_g, e_o, sw_g, sw_o = r
+        assert mae_g == pytest.approx(mae_o, rel=0.01), name
+        assert rmse_g == pytest.approx(rmse_o, rel=0.01), name
+        assert e_g == pytest.approx(e_o, rel=0.01), name
+        assert (1.0 + e_g) == pytest.approx(1.0 + e_o, rel=0.01), name
+        assert abs(sw_g - sw_o) <= 10, (name, sw_g, sw_o)
+
+
 def test_accumulate_and_predict_against_oracle_back_transform(torch_cuda, mpr, orc):
     """Step 6-7 alone, deterministic: import an oracle state, accumulate it
     M times with sweeps that cannot move (over-relaxation off, T so low and a
