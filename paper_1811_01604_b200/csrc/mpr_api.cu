@@ -498,7 +498,7 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
             // 5.2, 5.4, 5.5 and commits the sweep (t, buffer swap) for the grids still running
             mpr_status s = launch_pass(ctx, 1, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
             if (s != MPR_OK) return s;
-            k_controller<<<d.batch, 32, 0, ctx->stream>>>(d);
+            k_controller<<<d.batch, REDUCE_THREADS, 0, ctx->stream>>>(d);
             CU_LAUNCH();
         }
         issued += chunk;
@@ -585,7 +585,7 @@ mpr_status mpr_sample_energy(mpr_ctx* ctx, double* h_e_s, uint64_t* h_n_pairs)
     CU_LAUNCH();
     k_sample_energy<<<dim3(ctx->energy_blocks, d.batch), ENERGY_THREADS, 0, ctx->stream>>>(d);
     CU_LAUNCH();
-    k_sample_energy_finish<<<d.batch, 32, 0, ctx->stream>>>(d, ctx->energy_blocks);
+    k_sample_energy_finish<<<d.batch, REDUCE_THREADS, 0, ctx->stream>>>(d, ctx->energy_blocks);
     CU_LAUNCH();
     mpr_status s = fetch_states(ctx);
     if (s != MPR_OK) return s;
@@ -605,7 +605,7 @@ mpr_status mpr_measure_energy(mpr_ctx* ctx, uint32_t n_sweeps, double* h_e_mean)
         // one sweep with the energy reduction fused; k_measure adds e and commits the sweep (t, buffer swap)
         mpr_status s = launch_pass(ctx, 1, 0, PER_GRID, PASS_ENERGY);
         if (s != MPR_OK) return s;
-        k_measure<<<d.batch, 32, 0, ctx->stream>>>(d);
+        k_measure<<<d.batch, REDUCE_THREADS, 0, ctx->stream>>>(d);
         CU_LAUNCH();
     }
     ctx->cur ^= n_sweeps & 1u;          // every grid swapped buffers n_sweeps times
@@ -714,7 +714,7 @@ mpr_status mpr_energy(mpr_ctx* ctx, double* h_e)
     if (ctx->state != READY) return MPR_ERR_STATE;
     mpr_status s = launch_energy(ctx);
     if (s != MPR_OK) return s;
-    k_energy_query<<<ctx->d.batch, 32, 0, ctx->stream>>>(ctx->d, ctx->energy_blocks);
+    k_energy_query<<<ctx->d.batch, REDUCE_THREADS, 0, ctx->stream>>>(ctx->d, ctx->energy_blocks);
     CU_LAUNCH();
     s = fetch_states(ctx);
     if (s != MPR_OK) return s;

@@ -325,11 +325,17 @@ __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restric
     const uint32_t b = __ballot_sync(0xFFFFFFFFu, fixed);
     const uint32_t f0 = __ballot_sync(0xFFFFFFFFu, in && !fixed && colour == 0);
     const uint32_t f1 = __ballot_sync(0xFFFFFFFFu, in && !fixed && colour == 1);
+    // counts: per block in shared memory, then one global atomic per block and colour
+    __shared__ uint32_t s_free[2];
+    if (threadIdx.x < 2) s_free[threadIdx.x] = 0;
+    __syncthreads();
     if ((threadIdx.x & 31) == 0 && (n >> 5) < d.words) {
         d.bits[(size_t)g * d.words + (n >> 5)] = b;
-        if (f0) atomicAdd(&d.states[g].n_free[0], (uint32_t)__popc(f0));
-        if (f1) atomicAdd(&d.states[g].n_free[1], (uint32_t)__popc(f1));
+        if (f0) atomicAdd(&s_free[0], (uint32_t)__popc(f0));
+        if (f1) atomicAdd(&s_free[1], (uint32_t)__popc(f1));
     }
+    __syncthreads();
+    if (threadIdx.x < 2 && s_free[threadIdx.x]) atomicAdd(&d.states[g].n_free[threadIdx.x], s_free[threadIdx.x]);
 }
 
 // ---------------------------------------------------------------------------
@@ -998,14 +1004,23 @@ __global__ void __launch_bounds__(ENERGY_THREADS) k_energy(Dev d)
     }
 }
 
+// Sum of a grid's n partials by one block of REDUCE_THREADS threads in a fixed order (strided per thread, shuffle
+// tree per warp, warps in order): bitwise reproducible.  Every thread of the block must call it; thread 0 gets the sum.
+constexpr int REDUCE_THREADS = 256;
 __device__ __forceinline__ double sum_energy_partials(const Dev& d, int g, int n)
 {
+    __shared__ double warp_part[REDUCE_THREADS / 32];
     const double* p = d.e_partials + (size_t)g * d.n_partials;
     double s = 0.0;
-    for (int b = threadIdx.x; b < n; b += 32) s += p[b];
+    for (int b = threadIdx.x; b < n; b += REDUCE_THREADS) s += p[b];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
-    return s;
+    if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    double total = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < REDUCE_THREADS / 32; ++w) total += warp_part[w];
+    return total;
 }
 
 __global__ void k_energy_query(Dev d, int n_partials)
@@ -1084,7 +1099,7 @@ __global__ void k_sample_energy_finish(Dev d, int n_partials)
 
 // ---------------------------------------------------------------------------
 // a6  equilibration controller: Alg. 2 steps 5.2-5.5 for
-// one grid per warp, after the sweep (5.1) with its fused energy reduction.
+// one grid per block, after the sweep (5.1) with its fused energy reduction.
 // Commits the sweep: t += 1 and the vector buffers swap roles.
 // ---------------------------------------------------------------------------
 __global__ void k_controller(Dev d)
