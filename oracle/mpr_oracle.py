@@ -230,6 +230,32 @@ def simulate_stats(phi, mask, T, a_eq, p: Params, g=0, t0=0):
     return acc, acc2, int(t.value)
 
 
+def chains_realizations(M: int, chains: int) -> int:
+    """Realizations per chain when M are asked of `chains` chains: ceil(M / chains) (reading R25)."""
+    return -(-int(M) // int(chains))
+
+
+def simulate_chains(phi, mask, T, a_eq, p: Params, chains: int, g=0, batch=1, t0=0):
+    """Step 6 run as `chains` independent chains (reading R25; a variant of the paper's single
+    chain): every chain starts from the same equilibrated state `phi` (left untouched) at the same sweep index t0,
+    chain c draws from the Philox grid word g + c * batch, and each makes ceil(M / chains) realizations of s sweeps.
+    The sums of phi and phi^2 are pooled.  Returns (acc, acc2, M_total, t_end, final states [chains][rows][cols])."""
+    import dataclasses
+    Mc = chains_realizations(p.M, chains)
+    pc = dataclasses.replace(p, M=Mc)
+    acc = np.zeros(phi.shape, dtype=np.float64)
+    acc2 = np.zeros(phi.shape, dtype=np.float64)
+    finals = []
+    t_end = t0
+    for c in range(chains):
+        state = phi.copy()
+        a1, a2, t_end = simulate_stats(state, mask, T, a_eq, pc, g=g + c * batch, t0=t0)
+        acc += a1
+        acc2 += a2
+        finals.append(state)
+    return acc, acc2, chains * Mc, t_end, np.stack(finals)
+
+
 def predict_std(acc, acc2, M, mask, zmin, zmax) -> np.ndarray:
     """Sample standard deviation of the M back-transformed realizations at the prediction sites (L212)."""
     m = np.ascontiguousarray(mask, dtype=np.uint8)

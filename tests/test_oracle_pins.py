@@ -546,3 +546,74 @@ def test_simulate_stats_sums_follow_the_chain(orc):
     phi2, _, _ = orc.transform(z, mask, p.seed)
     acc_only, _ = orc.simulate(phi2, mask, 0.2, 2.0, p, t0=7)
     assert np.array_equal(acc_only, acc)
+
+
+# ---------------------------------------------------------------------------
+# chain parallelism (reading R25): the M realizations
+# made by several chains forked from the equilibrated state
+# ---------------------------------------------------------------------------
+def test_chains_one_chain_is_step_6(orc):
+    rng = np.random.default_rng(31)
+    z = rng.standard_normal((10, 13)).astype(np.float32)
+    mask = (rng.random((10, 13)) < 0.4).astype(np.uint8); mask[0, 0] = 1; mask[-1, -1] = 0
+    p = orc.Params(seed=9, M=5, sweeps_per_real=2)
+    phi, _, _ = orc.transform(z, mask, p.seed)
+    start = phi.copy()
+    acc, acc2, M_tot, t_end, finals = orc.simulate_chains(start, mask, 0.3, 1.5, p, chains=1, t0=4)
+    a1, a2, t1 = orc.simulate_stats(phi, mask, 0.3, 1.5, p, t0=4)
+    assert M_tot == 5 and t_end == t1 == 4 + 10
+    assert np.array_equal(acc, a1) and np.array_equal(acc2, a2) and np.array_equal(finals[0], phi)
+
+
+def test_chains_pool_the_hand_swept_realizations(orc):
+    """Mean and spread of simulate_chains are numpy's mean and sample s.d. over the realizations of every chain,
+    each swept by hand from a copy of the start state with the chain's own Philox grid word g + c * batch."""
+    rng = np.random.default_rng(32)
+    z = rng.standard_normal((9, 11)).astype(np.float32)
+    mask = (rng.random((9, 11)) < 0.5).astype(np.uint8); mask[0, 0] = 1; mask[-1, -1] = 0
+    p = orc.Params(seed=21, M=7, sweeps_per_real=2)           # 3 chains -> ceil(7 / 3) = 3 realizations each
+    phi, zmin, zmax = orc.transform(z, mask, p.seed, g=2)
+    start = phi.copy()
+    acc, acc2, M_tot, t_end, finals = orc.simulate_chains(phi, mask, 0.25, 2.0, p, chains=3, g=2, batch=5, t0=6)
+    assert np.array_equal(phi, start)                           # the start state is not advanced
+    assert orc.chains_realizations(7, 3) == 3 and M_tot == 9 and t_end == 6 + 3 * 2
+    reals = []
+    for c in range(3):
+        state = start.copy(); t = 6
+        for _ in range(3):
+            for _ in range(2):
+                orc.sweep(state, mask, p.q, 0.25, 2.0, p.seed, 2 + 5 * c, t); t += 1
+            reals.append(state.astype(np.float64))
+        assert np.array_equal(state, finals[c])
+    reals = np.stack(reals)
+    free = mask == 0
+    assert not np.array_equal(finals[0], finals[1])             # the chains do differ
+    pred = orc.predict(acc, M_tot, z, mask, zmin, zmax)
+    std = orc.predict_std(acc, acc2, M_tot, mask, zmin, zmax)
+    scale = (float(zmax) - float(zmin)) / TWO_PI_F
+    assert np.allclose(pred[free], float(zmin) + reals.mean(axis=0)[free] * scale, rtol=1e-6, atol=1e-6)
+    assert np.allclose(std[free], reals.std(axis=0, ddof=1)[free] * scale, rtol=1e-5, atol=1e-6)
+
+
+def test_chains_pooled_moments_match_boltzmann(orc):
+    """One free site between four fixed neighbours: the first two moments pooled over 40 chains forked from a
+    burnt-in state equal those of the Gibbs density (Eq. 3) by quadrature, within the chains' own sampling error."""
+    nbrs, T, q = (1.0, 2.5, 4.0, 5.5), 0.5, 0.5
+    phi = np.zeros((3, 3), dtype=np.float32)
+    phi[0, 0], phi[0, 2], phi[2, 0], phi[2, 2] = 0.3, 5.9, 4.4, 2.2
+    phi[0, 1], phi[2, 1], phi[1, 0], phi[1, 2] = nbrs
+    phi[1, 1] = 3.0
+    mask = np.ones((3, 3), dtype=np.uint8); mask[1, 1] = 0
+    for t in range(50):
+        orc.sweep(phi, mask, q, T, 1.0, 123, 0, t)
+    p = orc.Params(seed=123, M=40 * 500, sweeps_per_real=8)
+    acc, acc2, M_tot, _, _ = orc.simulate_chains(phi, mask, T, 1.0, p, chains=40, t0=50)
+    dens = lambda x: math.exp(sum(math.cos(q * (x - pj)) for pj in nbrs) / T)
+    Z = integrate.quad(dens, 0, TWO_PI_F, epsabs=1e-13)[0]
+    m1 = integrate.quad(lambda x: x * dens(x), 0, TWO_PI_F, epsabs=1e-13)[0] / Z
+    m2 = integrate.quad(lambda x: x * x * dens(x), 0, TWO_PI_F, epsabs=1e-13)[0] / Z
+    m4 = integrate.quad(lambda x: x ** 4 * dens(x), 0, TWO_PI_F, epsabs=1e-13)[0] / Z
+    # realizations 8 sweeps apart are nearly independent; allow 4.5 standard errors at an effective size of M / 2
+    n_eff = M_tot / 2
+    assert abs(acc[1, 1] / M_tot - m1) < 4.5 * math.sqrt((m2 - m1 * m1) / n_eff)
+    assert abs(acc2[1, 1] / M_tot - m2) < 4.5 * math.sqrt((m4 - m2 * m2) / n_eff)
