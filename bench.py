@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--L", type=int, default=None, help="override the grid side (debugging only)")
     ap.add_argument("--batch", type=int, default=None, help="override the batch of cfg5 (debugging only)")
+    ap.add_argument("--chains", type=int, default=1,
+                    help="chains per grid in step 6 (DESIGN.md reading R25); 1 = the paper's single chain")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-inference", action="store_true", help="skip the Alg. 2 step 4 timing (extra key, not in the step)")
     return ap.parse_args()
@@ -240,7 +242,7 @@ def run_b200(args, w):
         torch.cuda.synchronize(dev)
 
     def one_pass(values, mask):
-        ctx = mpr.Mpr(values, mask)
+        ctx = mpr.Mpr(values, mask, chains=args.chains)
         ctx.set_params(T, **prm).equilibrate().simulate()
         ctx.predict(d_out)
         return ctx
@@ -270,7 +272,8 @@ def run_b200(args, w):
             e1.synchronize()
             total_ms += e0.elapsed_time(e1)
             st = ctx.get_stats()
-            updates += sum(s.n_free * s.t for s in st)
+            # sweeps of a grid = its equilibration + (realizations over all of its chains) x s
+            updates += sum(s.n_free * (s.equil_sweeps + s.realizations * w.sweeps_per_real) for s in st)
             launches += ctx.launch_count()
             ctx.close()
         return total_ms / 1e3, updates, launches
@@ -341,7 +344,7 @@ def run_b200(args, w):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "rows": w.rows, "cols": w.cols, "batch": w.batch,
                        "n_free_per_rank": int(P_sites), "equil_cap": w.equil_cap, "M": w.M,
-                       "sweeps_per_real": w.sweeps_per_real, "equil_sweeps": equil_sweeps,
+                       "sweeps_per_real": w.sweeps_per_real, "chains": args.chains, "equil_sweeps": equil_sweeps,
                        "parallelism": f"replicas x{world}", "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)",
                        "step": "mpr_create+set_params+equilibrate+simulate+predict"},
             "ms_per_grid": 1e3 * secs / args.steps / w.batch,

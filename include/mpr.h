@@ -139,6 +139,21 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out);
  * realizations (else MPR_ERR_STATE).  Synchronises. */
 mpr_status mpr_predict_std(mpr_ctx* ctx, float* d_out);
 
+/* ---- chain parallelism (a variant of the paper's single chain, reading R25) ----
+ * The M realizations of step 6 ("Statistics of M realizations") made by `chains` independent
+ * chains per grid instead of one, so that small grids fill the device: mpr_equilibrate runs one chain per grid
+ * as Alg. 2 step 5 says; mpr_simulate then starts chains 1 .. chains-1 from a copy of that equilibrated state
+ * (same sweep index t), chain c of grid g drawing from the Philox grid word g + c * batch, and every chain makes
+ * ceil(M / chains) realizations of sweeps_per_real sweeps, all in the same launches.  mpr_predict and
+ * mpr_predict_std pool the realizations of a grid's chains; mpr_stats.realizations is their total.  The
+ * diagnostic calls (get/set_angles, sweep, energy, measure_energy) act on chain 0; after any of them, and after
+ * mpr_equilibrate, the next mpr_simulate forks again (accumulators are kept).  chains = 1 is mpr_create.
+ * batch * chains <= 65535.  Workspace: mpr_query_workspace_chains bytes. */
+mpr_status mpr_query_workspace_chains(int batch, int chains, int rows, int cols, size_t* h_bytes);
+mpr_status mpr_create_chains(mpr_ctx** out, int batch, int chains, int rows, int cols,
+                             const float* d_values, const uint8_t* d_sample_mask,
+                             void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
 mpr_status mpr_destroy(mpr_ctx* ctx);
 
 /* ---- Alg. 2 step 4: parameter inference ---- */

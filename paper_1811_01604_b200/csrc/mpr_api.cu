@@ -68,15 +68,15 @@ void choose_tiles(int batch, int rows, int cols, Geometry* g)
     g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 31) & ~(size_t)15);   // two 16-aligned lists per tile
 }
 
-bool make_geometry(int batch, int rows, int cols, Geometry* g)
+bool make_geometry(int batch, int chains, int rows, int cols, Geometry* g)
 {
-    if (batch < 1 || batch > 65535 || rows < 2 || cols < 2 || rows > 65534 || cols > 65534) return false;
+    if (batch < 1 || chains < 1 || (long)batch * chains > 65535 || rows < 2 || cols < 2 || rows > 65534 || cols > 65534) return false;
     const uint64_t N = (uint64_t)rows * (uint64_t)cols;
     const uint64_t pitch = ((uint64_t)cols + 1) & ~1ull;                      // even: rows start 16-byte aligned
     if (N >= (1ull << 31) || (uint64_t)rows * pitch >= (1ull << 31)) return false;
     g->N = (uint32_t)N; g->words = (uint32_t)((N + 31) / 32);
     g->pitch = (uint32_t)pitch; g->VG = (size_t)rows * pitch;
-    choose_tiles(batch, rows, cols, g);
+    choose_tiles(batch * chains, rows, cols, g);        // step 6 runs every chain of every grid at once
     return g->entry_stride < (1ull << 32);
 }
 
@@ -84,21 +84,22 @@ struct Layout {
     size_t states, done, partials, values, phi, bits, vec, acc, m2, tile_meta, entries, total;
 };
 
-Layout make_layout(int batch, const Geometry& g)
+// B grids with data of their own, V = B * chains states (vectors, accumulators, Alg. 2 scalars)
+Layout make_layout(int batch, int chains, const Geometry& g)
 {
     Layout L;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
-    const size_t B = (size_t)batch;
-    L.states    = take(B * sizeof(GridState));
-    L.done      = take(B * sizeof(uint32_t));
+    const size_t B = (size_t)batch, V = B * (size_t)chains;
+    L.states    = take(V * sizeof(GridState));
+    L.done      = take(V * sizeof(uint32_t));
     L.partials  = take(B * g.n_partials * sizeof(double));
     L.values    = take(B * g.N * sizeof(float));
     L.phi       = take(B * g.N * sizeof(float));
     L.bits      = take(B * g.words * sizeof(uint32_t));
-    L.vec       = take(2 * B * g.VG * sizeof(float2));
-    L.acc       = take(B * g.N * sizeof(float));
-    L.m2        = take(B * g.N * sizeof(float));
+    L.vec       = take(2 * V * g.VG * sizeof(float2));
+    L.acc       = take(V * g.N * sizeof(float));
+    L.m2        = take(V * g.N * sizeof(float));
     L.tile_meta = take(B * g.ntiles * sizeof(TileMeta));
     L.entries   = take((B * g.entry_stride + 16) * sizeof(uint16_t));
     L.total = o;
@@ -131,13 +132,15 @@ struct mpr_ctx {
     bool         small_d;         // every grid's proposal half-rotation q pi / (2 a) is below SMALL_HD (host knowledge of a)
     uint32_t     cur;             // vector buffer holding the current state, the same for every grid outside mpr_equilibrate
     uint32_t     pf_dist;         // tile passes resident on the device at once (L2 prefetch distance), 0 = not yet known
+    int          active;          // states the tile passes cover: the grids (chain 0), or every chain inside mpr_simulate
+    bool         forked;          // chains >= 1 hold a copy of their grid's state (until chain 0 alone moves again)
 };
 
 namespace {
 
 mpr_status fetch_states(mpr_ctx* ctx)
 {
-    CU(cudaMemcpyAsync(ctx->h_states, ctx->d.states, sizeof(GridState) * ctx->d.batch, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_states, ctx->d.states, sizeof(GridState) * ctx->d.nv, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MPR_OK;
 }
@@ -191,7 +194,7 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
     // programmatic stream serialization: this pass's CTAs may start (and load their tile lists) while the last
     // CTAs of the previous kernel still run; k_tilepass waits for that kernel before it reads any result of it
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(ctx->d.ntiles, ctx->d.batch); cfg.blockDim = dim3(TILE_THREADS);
+    cfg.gridDim = dim3(ctx->d.ntiles, ctx->active); cfg.blockDim = dim3(TILE_THREADS);
     cfg.dynamicSmemBytes = ctx->smem_bytes; cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -232,7 +235,7 @@ mpr_status make_frame_map(mpr_ctx* ctx, int which)
         encode = (PFN_cuTensorMapEncodeTiled)fn;
     }
     const Dev& d = ctx->d;
-    const cuuint64_t dims[3] = {(cuuint64_t)d.cols, (cuuint64_t)d.rows, (cuuint64_t)d.batch};
+    const cuuint64_t dims[3] = {(cuuint64_t)d.cols, (cuuint64_t)d.rows, (cuuint64_t)d.nv};
     const cuuint64_t strides[2] = {(cuuint64_t)d.pitch * sizeof(float2), (cuuint64_t)d.VG * sizeof(float2)};
     const cuuint32_t box[3] = {(cuuint32_t)d.FC, (cuuint32_t)d.FR, 1u};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
@@ -288,12 +291,17 @@ void mpr_default_params(mpr_params* p)
     p->or_mode = 0; p->a_eq_mode = 0; p->seed = 0;
 }
 
-mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* bytes)
+mpr_status mpr_query_workspace_chains(int batch, int chains, int rows, int cols, size_t* bytes)
 {
     Geometry g;
-    if (!bytes || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
-    *bytes = make_layout(batch, g).total;
+    if (!bytes || !make_geometry(batch, chains, rows, cols, &g)) return MPR_ERR_ARG;
+    *bytes = make_layout(batch, chains, g).total;
     return MPR_OK;
+}
+
+mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* bytes)
+{
+    return mpr_query_workspace_chains(batch, 1, rows, cols, bytes);
 }
 
 }  // extern "C"
@@ -301,13 +309,13 @@ mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* bytes)
 namespace {
 
 // mpr_create (data given) and mpr_create_unconditional (d_values = d_sample_mask = nullptr)
-mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float* d_values,
+mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols, const float* d_values,
                        const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
     const bool unconditional = !d_values && !d_sample_mask;
     Geometry g;
-    if (!out || (!unconditional && (!d_values || !d_sample_mask)) || !make_geometry(batch, rows, cols, &g)) return MPR_ERR_ARG;
-    const Layout lay = make_layout(batch, g);
+    if (!out || (!unconditional && (!d_values || !d_sample_mask)) || !make_geometry(batch, chains, rows, cols, &g)) return MPR_ERR_ARG;
+    const Layout lay = make_layout(batch, chains, g);
     if (!d_workspace || workspace_bytes < lay.total || ((uintptr_t)d_workspace & 255u)) return MPR_ERR_WORKSPACE;
 
     mpr_ctx* ctx = new (std::nothrow) mpr_ctx();
@@ -339,7 +347,8 @@ mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float
     d.m2 = (float*)(base + lay.m2);
     d.tile_meta = (TileMeta*)(base + lay.tile_meta);
     d.entries = (uint16_t*)(base + lay.entries);
-    d.VG = g.VG; d.VB = (size_t)batch * g.VG;
+    d.chains = chains; d.nv = batch * chains;
+    d.VG = g.VG; d.VB = (size_t)d.nv * g.VG;
     d.entry_stride = g.entry_stride; d.n_partials = g.n_partials;
     d.tile_entries = (uint32_t)(g.entry_stride / (size_t)g.ntiles);
     d.fc_inv = (uint32_t)(((1u << 24) + (uint32_t)g.FC - 1u) / (uint32_t)g.FC);
@@ -349,7 +358,8 @@ mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
     d.burn_in_only = unconditional ? 1 : 0;
     ctx->energy_blocks = rows < ENERGY_BLOCKS ? rows : ENERGY_BLOCKS;
-    ctx->h_states = new (std::nothrow) GridState[batch];
+    ctx->active = batch;
+    ctx->h_states = new (std::nothrow) GridState[d.nv];
     mpr_status st = MPR_OK;
     auto fail = [&](mpr_status s) { mpr_destroy(ctx); return s; };
     if (!ctx->h_states) return fail(MPR_ERR_ARG);
@@ -359,7 +369,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int rows, int cols, const float
     // the pad column of an odd-width grid stays zero
     if (!cuda_ok(cudaMemsetAsync(d.vec, 0, 2 * d.VB * sizeof(float2), s), "memset vec")) return fail(MPR_ERR_CUDA);
     for (int w = 0; w < 2; ++w) { st = make_frame_map(ctx, w); if (st != MPR_OK) return fail(st); }
-    k_state_reset<<<cdiv(batch, 128), 128, 0, s>>>(d);
+    k_state_reset<<<cdiv(d.nv, 128), 128, 0, s>>>(d);
     unsigned mm_blocks = cdiv(g.N, 256 * 8);
     if (mm_blocks > 1184) mm_blocks = 1184;
     if (unconditional) k_state_unconditional<<<cdiv(batch, 128), 128, 0, s>>>(d);
@@ -425,13 +435,20 @@ mpr_status mpr_create(mpr_ctx** out, int batch, int rows, int cols, const float*
                       const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
     if (!d_values || !d_sample_mask) return MPR_ERR_ARG;
-    return create_impl(out, batch, rows, cols, d_values, d_sample_mask, d_workspace, workspace_bytes, cuda_stream);
+    return create_impl(out, batch, 1, rows, cols, d_values, d_sample_mask, d_workspace, workspace_bytes, cuda_stream);
+}
+
+mpr_status mpr_create_chains(mpr_ctx** out, int batch, int chains, int rows, int cols, const float* d_values,
+                             const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!d_values || !d_sample_mask) return MPR_ERR_ARG;
+    return create_impl(out, batch, chains, rows, cols, d_values, d_sample_mask, d_workspace, workspace_bytes, cuda_stream);
 }
 
 mpr_status mpr_create_unconditional(mpr_ctx** out, int batch, int rows, int cols,
                                     void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
-    return create_impl(out, batch, rows, cols, nullptr, nullptr, d_workspace, workspace_bytes, cuda_stream);
+    return create_impl(out, batch, 1, rows, cols, nullptr, nullptr, d_workspace, workspace_bytes, cuda_stream);
 }
 
 mpr_status mpr_destroy(mpr_ctx* ctx)
@@ -467,16 +484,17 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     d.A_targ = (double)p->A_targ; d.k_a = (double)p->k_a;
     // per-grid temperatures: staged through the energy partials (free between calls)
     CU(cudaMemcpyAsync(d.e_partials, h_T, sizeof(float) * d.batch, cudaMemcpyHostToDevice, ctx->stream));
-    k_begin_run<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, (const float*)d.e_partials);
+    k_begin_run<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, (const float*)d.e_partials);
     CU_LAUNCH();
-    CU(cudaMemsetAsync(d.acc, 0, (size_t)d.batch * d.N * sizeof(float), ctx->stream));
-    CU(cudaMemsetAsync(d.m2, 0, (size_t)d.batch * d.N * sizeof(float), ctx->stream));
+    CU(cudaMemsetAsync(d.acc, 0, (size_t)d.nv * d.N * sizeof(float), ctx->stream));
+    CU(cudaMemsetAsync(d.m2, 0, (size_t)d.nv * d.N * sizeof(float), ctx->stream));
     k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d, ctx->unconditional ? 1 : 0);
     CU_LAUNCH();
     CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
     ctx->state = READY;
     ctx->dirty = false;
     ctx->cur = 0;
+    ctx->forked = false;
     note_a(ctx, 1.0);
     return MPR_OK;
 }
@@ -487,6 +505,7 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
+    ctx->forked = false;           // chain 0 of every grid moves alone (Alg. 2 step 5 is one chain per grid)
     const uint32_t cap = ctx->prm.equil_cap;
     uint32_t issued = 0;
     // the first slope check happens at i = n_fit, then every n_f sweeps (Alg. 2 step 5.4)
@@ -536,16 +555,29 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
     const uint32_t s_per = ctx->prm.sweeps_per_real;
-    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, ctx->prm.a_eq_mode == 1 ? 0 : 1, 1.0, 0);
+    k_set_a<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, ctx->prm.a_eq_mode == 1 ? 0 : 1, 1.0, 0);
     CU_LAUNCH();
     if (ctx->prm.a_eq_mode == 1) note_a(ctx, 1.0);
-    uint32_t t_off = 0, flip = 0;
-    for (uint32_t j = 0; j < ctx->prm.M; ++j) {
-        // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
-        mpr_status s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE, j + 1u);   // realization number: realizations so far + j + 1
-        if (s != MPR_OK) return s;
+    // several chains per grid (reading R25): the others start from a copy of chain 0's state, every chain makes
+    // ceil(M / chains) realizations, all chains of all grids in the same launches
+    uint32_t n_real = ctx->prm.M;
+    if (d.chains > 1) {
+        if (!ctx->forked) {
+            k_fork_chains<<<dim3(cdiv(d.VG, 256), d.nv - d.batch), 256, 0, ctx->stream>>>(d, ctx->cur);
+            CU_LAUNCH();
+            ctx->forked = true;
+        }
+        n_real = (ctx->prm.M + (uint32_t)d.chains - 1u) / (uint32_t)d.chains;
+        ctx->active = d.nv;
     }
-    k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, t_off, flip, ctx->prm.M);
+    uint32_t t_off = 0, flip = 0;
+    mpr_status s = MPR_OK;
+    for (uint32_t j = 0; j < n_real && s == MPR_OK; ++j)
+        // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
+        s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE, j + 1u);   // realization number: realizations so far + j + 1
+    ctx->active = d.batch;
+    if (s != MPR_OK) return s;
+    k_commit<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, d.chains > 1 ? d.nv : d.batch, t_off, flip, n_real);
     CU_LAUNCH();
     ctx->cur ^= flip;
     return MPR_OK;
@@ -569,8 +601,11 @@ mpr_status mpr_predict_std(mpr_ctx* ctx, float* d_out)
     if (ctx->state != READY) return MPR_ERR_STATE;
     mpr_status s = fetch_states(ctx);
     if (s != MPR_OK) return s;
-    for (int b = 0; b < ctx->d.batch; ++b)
-        if (ctx->h_states[b].realizations < 2u) return MPR_ERR_STATE;
+    for (int b = 0; b < ctx->d.batch; ++b) {
+        uint32_t n = 0;
+        for (int c = 0; c < ctx->d.chains; ++c) n += ctx->h_states[b + c * ctx->d.batch].realizations;
+        if (n < 2u) return MPR_ERR_STATE;
+    }
     k_predict_std<<<site_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, d_out);
     CU_LAUNCH();
     return MPR_OK;
@@ -599,6 +634,7 @@ mpr_status mpr_measure_energy(mpr_ctx* ctx, uint32_t n_sweeps, double* h_e_mean)
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
+    ctx->forked = false;
     k_measure_begin<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d);
     CU_LAUNCH();
     for (uint32_t j = 0; j < n_sweeps; ++j) {
@@ -671,6 +707,7 @@ mpr_status mpr_set_angles(mpr_ctx* ctx, const float* d_phi)
     k_import_angles<<<site_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, d_phi);
     CU_LAUNCH();
     ctx->dirty = false;
+    ctx->forked = false;
     return MPR_OK;
 }
 
@@ -681,6 +718,7 @@ mpr_status mpr_set_sweep_index(mpr_ctx* ctx, uint32_t t)
     if (ctx->state != READY) return MPR_ERR_STATE;
     k_set_t<<<cdiv(ctx->d.batch, 128), 128, 0, ctx->stream>>>(ctx->d, t);
     CU_LAUNCH();
+    ctx->forked = false;
     return MPR_OK;
 }
 
@@ -690,13 +728,14 @@ mpr_status mpr_sweep(mpr_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_acce
     ENTER(ctx);
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
-    k_set_a<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, a, 1);       // also zeroes the accepted counters
+    k_set_a<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, 0, a, 1);       // also zeroes the accepted counters
     CU_LAUNCH();
     note_a(ctx, a);
+    ctx->forked = false;
     uint32_t t_off = 0, flip = 0;
     mpr_status rs = launch_sweeps(ctx, n_sweeps, &t_off, &flip, h_accepted ? PASS_COUNT : 0u, 0);
     if (rs != MPR_OK) return rs;
-    k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, t_off, flip, 0);
+    k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, d.batch, t_off, flip, 0);
     CU_LAUNCH();
     ctx->cur ^= flip;
     if (h_accepted) {
@@ -747,7 +786,9 @@ mpr_status mpr_get_stats(mpr_ctx* ctx, mpr_stats* h_out)
     for (int b = 0; b < ctx->d.batch; ++b) {
         const GridState& g = ctx->h_states[b];
         mpr_stats& o = h_out[b];
-        o.equil_sweeps = g.i; o.t = g.t; o.equilibrated = g.done; o.realizations = g.realizations;
+        o.equil_sweeps = g.i; o.t = g.t; o.equilibrated = g.done;
+        o.realizations = 0;            // pooled over the grid's chains
+        for (int c = 0; c < ctx->d.chains; ++c) o.realizations += ctx->h_states[b + c * ctx->d.batch].realizations;
         o.n_free = (uint64_t)g.n_free[0] + g.n_free[1];
         o.n_samples = g.n_samples;
         o.n_bonds = (uint64_t)ctx->d.n_bonds;

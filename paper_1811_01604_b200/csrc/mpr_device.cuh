@@ -66,21 +66,23 @@ __host__ __device__ __forceinline__ uint32_t colour1_base(uint32_t n0) { return 
 
 // Device view of one context (passed by value to kernels).
 struct Dev {
-    GridState* states;
+    GridState* states;         // [nv]
     uint32_t*  done_flags;     // [batch] copy of GridState::done for cheap host polling
     double*    e_partials;     // [batch][n_partials]
     float*     values;         // [batch][N] verbatim copy of the input values
     float*     phi;            // [batch][N] angle view: Eq. 1 at sample sites (never rewritten), export buffer at free sites
     uint32_t*  bits;           // [batch][words] fixed-site bitmask
-    float2*    vec;            // [2 buffers][batch][rows][pitch] row-major unit vectors (pitch = cols rounded up to even)
-    float*     acc;            // [batch][N] sum over realizations of phi at the prediction sites
-    float*     m2;             // [batch][N] sum of squared deviations from the running mean (Welford), for the spread (L212)
+    float2*    vec;            // [2 buffers][nv][rows][pitch] row-major unit vectors (pitch = cols rounded up to even)
+    float*     acc;            // [nv][N] sum over realizations of phi at the prediction sites
+    float*     m2;             // [nv][N] sum of squared deviations from the running mean (Welford), for the spread (L212)
     TileMeta*  tile_meta;      // [batch][ntiles]
     uint16_t*  entries;        // [batch][entry_stride] tile frames' free sites: offset in the frame (row * FC + col)
-    int        batch, rows, cols;
+    int        batch, rows, cols;   // batch = grids with data of their own
+    int        chains, nv;          // chains per grid (reading R25) and nv = batch * chains states: chain c of grid g is
+                                    // state v = g + c * batch; it shares grid g's values, mask and tile lists
     uint32_t   N, words, pitch;
     size_t     VG;             // float2 elements of one grid in one buffer = rows * pitch
-    size_t     VB;             // float2 elements per vector buffer = batch * VG
+    size_t     VB;             // float2 elements per vector buffer = nv * VG
     size_t     entry_stride;   // entries per grid = ntiles * tile_entries
     uint32_t   tile_entries;   // room of one tile's lists (worst case: every frame site free), multiple of 16; tile i's
                                // lists start at i * tile_entries, so that loading them needs nothing read first
@@ -232,7 +234,7 @@ __device__ __forceinline__ bool is_fixed(const uint32_t* __restrict__ bits, uint
 __global__ void k_state_reset(Dev d)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= d.batch) return;
+    if (g >= d.nv) return;
     GridState& s = d.states[g];
     s.t = 0; s.done = 0; s.cur = 0; s.hd_scale = 0.f; s.neg_log2e_over_T = 0.f;
     s.n_free[0] = s.n_free[1] = 0; s.max_tile_entries = 0;
@@ -759,7 +761,8 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 
     constexpr int NT = TILE_THREADS, NW = TILE_THREADS / 32;
     static_assert(TILE_THREADS >= 96 + 2 * MAX_H && TILE_THREADS >= HS_CHUNK, "the prologue gives warps 0-3 their own jobs");
-    const int tile = blockIdx.x, g = blockIdx.y;
+    const int tile = blockIdx.x, g = blockIdx.y;            // g: state (grid and chain), gd: the grid whose data it shares
+    const int gd = g < d.batch ? g : g % d.batch;
     const GridState& st = d.states[g];
     // Programmatic dependent launch: the next kernel of the stream may start its CTAs while the last of this
     // one still run.  What a tile pass does before its own griddep_wait() touches only data no kernel of a run
@@ -775,7 +778,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const TileGeom tg = tile_geom(d, tile);
-    const TileMeta& meta = d.tile_meta[(size_t)g * d.ntiles + tile];
+    const TileMeta& meta = d.tile_meta[(size_t)gd * d.ntiles + tile];
 
     // three warps start the tile: warp 1 the entry list (needs the tile's counts from global memory first), and,
     // once the previous kernel's results are visible, warp 0 the frame and warp 2 the L2 prefetch
@@ -786,7 +789,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         mbar_init(&s_bar[1], 1);
         const uint32_t entry_bytes = d.max_entries * (uint32_t)sizeof(uint16_t);
         mbar_expect_tx(&s_bar[1], entry_bytes);
-        if (entry_bytes) bulk_load(E, d.entries + (size_t)g * d.entry_stride + (size_t)tile * d.tile_entries, entry_bytes, &s_bar[1]);
+        if (entry_bytes) bulk_load(E, d.entries + (size_t)gd * d.entry_stride + (size_t)tile * d.tile_entries, entry_bytes, &s_bar[1]);
     }
     if (tid >= 96 && tid < 96 + 2 * MAX_H) (&s_cle[0][0])[tid - 96] = (&meta.cle[0][0])[tid - 96];
 
@@ -808,7 +811,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         const TileGeom tn = tile_geom(d, tile + (int)pf_dist);
         tma_prefetch_frame(src_buf ? &map1 : &map0, tn.c0 - H, tn.r0 - H, g);
         if (d.max_entries)
-            bulk_prefetch(d.entries + (size_t)g * d.entry_stride + (size_t)(tile + pf_dist) * d.tile_entries,
+            bulk_prefetch(d.entries + (size_t)gd * d.entry_stride + (size_t)(tile + pf_dist) * d.tile_entries,
                           d.max_entries * (uint32_t)sizeof(uint16_t));
     }
     const float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f, nlT = st.neg_log2e_over_T;
@@ -1148,17 +1151,17 @@ __global__ void k_controller(Dev d)
 __global__ void k_set_a(Dev d, int mode, double a_value, int zero_accepted)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= d.batch) return;
+    if (g >= d.nv) return;
     GridState& s = d.states[g];
     if (mode == 0) s.a = a_value;
     s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F) / s.a);
     if (zero_accepted) s.accepted = 0ull;
 }
 // commit passes that ran with (t_off, flip) arguments: t += n_sweeps, swap buffers if the pass count was odd
-__global__ void k_commit(Dev d, uint32_t n_sweeps, uint32_t flip, uint32_t n_realizations)
+__global__ void k_commit(Dev d, int n_states, uint32_t n_sweeps, uint32_t flip, uint32_t n_realizations)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= d.batch) return;
+    if (g >= n_states) return;
     GridState& s = d.states[g];
     s.t += n_sweeps; s.cur ^= flip; s.realizations += n_realizations;
 }
@@ -1179,15 +1182,31 @@ __global__ void k_set_t(Dev d, uint32_t t)
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g < d.batch) d.states[g].t = t;
 }
+// Chain parallelism (reading R25): chain c >= 1 of grid g (state v = g + c * batch) starts step 6 from a copy
+// of grid g's equilibrated state: vectors (buffer cur) and the scalars of Alg. 2; it keeps its own realization count.
+__global__ void __launch_bounds__(256) k_fork_chains(Dev d, uint32_t cur)
+{
+    const int v = d.batch + blockIdx.y, g = v % d.batch;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < d.VG) vec_grid(d, v, cur)[i] = vec_grid(d, g, cur)[i];
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        GridState& s = d.states[v];
+        const GridState& o = d.states[g];
+        s.t = o.t; s.done = o.done; s.cur = cur; s.hd_scale = o.hd_scale; s.neg_log2e_over_T = o.neg_log2e_over_T;
+        s.i = o.i; s.a = o.a; s.k = o.k; s.A_last = o.A_last; s.e_last = o.e_last; s.T = o.T;
+        s.zmin = o.zmin; s.zmax = o.zmax; s.accepted = 0ull;
+    }
+}
 __global__ void k_begin_run(Dev d, const float* __restrict__ T)
 {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= d.batch) return;
+    if (g >= d.nv) return;
     GridState& s = d.states[g];
     s.t = 0; s.done = 0; s.cur = 0; s.i = 0; s.realizations = 0; s.accepted = 0ull;
     s.a = 1.0; s.k = -1.0; s.A_last = 0.0; s.e_last = 0.0;
-    s.T = (double)T[g];
-    s.neg_log2e_over_T = (float)(-1.4426950408889634 / (double)T[g]);
+    const double Tg = (double)T[g % d.batch];
+    s.T = Tg;
+    s.neg_log2e_over_T = (float)(-1.4426950408889634 / Tg);
     s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F));
     d.done_flags[g] = 0;
 }
@@ -1205,7 +1224,13 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, float* __restrict__ out)
     const size_t o = (size_t)g * d.N + n;
     if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = d.values[o]; return; }
     const GridState& s = d.states[g];
-    const double mean_phi = (double)d.acc[o] / (double)s.realizations;
+    // the realizations of every chain of the grid are pooled (one chain: the paper's step 7)
+    double sum = 0.0, count = 0.0;
+    for (int c = 0; c < d.chains; ++c) {
+        const int v = g + c * d.batch;
+        sum += (double)d.acc[(size_t)v * d.N + n]; count += (double)d.states[v].realizations;
+    }
+    const double mean_phi = sum / count;
     const double z = (double)s.zmin + mean_phi * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F;
     out[o] = (float)z;
 }
@@ -1219,7 +1244,23 @@ __global__ void __launch_bounds__(256) k_predict_std(Dev d, float* __restrict__ 
     const size_t o = (size_t)g * d.N + n;
     if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = 0.0f; return; }
     const GridState& s = d.states[g];
-    const double var = s.realizations > 1u ? fmax((double)d.m2[o], 0.0) / (double)(s.realizations - 1u) : 0.0;
+    // pooled over the chains: sum of squared deviations from the pooled mean =
+    // sum over the chains of [their own m2 + n_c (mean_c - mean)^2]
+    double sum = 0.0, count = 0.0;
+    for (int c = 0; c < d.chains; ++c) {
+        const int v = g + c * d.batch;
+        sum += (double)d.acc[(size_t)v * d.N + n]; count += (double)d.states[v].realizations;
+    }
+    const double mean = sum / count;
+    double ssd = 0.0;
+    for (int c = 0; c < d.chains; ++c) {
+        const int v = g + c * d.batch;
+        const double nc = (double)d.states[v].realizations;
+        if (nc == 0.0) continue;
+        const double dev = (double)d.acc[(size_t)v * d.N + n] / nc - mean;
+        ssd += fmax((double)d.m2[(size_t)v * d.N + n], 0.0) + nc * dev * dev;
+    }
+    const double var = count > 1.0 ? ssd / (count - 1.0) : 0.0;
     out[o] = (float)(sqrt(var) * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F);
 }
 

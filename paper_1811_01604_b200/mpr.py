@@ -32,7 +32,7 @@ EXPORTS = (
     "mpr_set_sweep_index", "mpr_sweep", "mpr_energy", "mpr_get_transform", "mpr_get_mask_bits",
     "mpr_get_stats", "mpr_get_launch_count", "mpr_status_string", "mpr_last_cuda_error",
     "mpr_sample_energy", "mpr_create_unconditional", "mpr_measure_energy", "mpr_energy_table",
-    "mpr_infer_temperature", "mpr_predict_std",
+    "mpr_infer_temperature", "mpr_predict_std", "mpr_query_workspace_chains", "mpr_create_chains",
 )
 
 
@@ -77,6 +77,8 @@ def lib():
         L.mpr_default_params.argtypes = [C.POINTER(mpr_params)]; L.mpr_default_params.restype = None
         L.mpr_query_workspace.argtypes = [i, i, i, C.POINTER(sz)]
         L.mpr_create.argtypes = [C.POINTER(vp), i, i, i, vp, vp, vp, sz, vp]
+        L.mpr_query_workspace_chains.argtypes = [i, i, i, i, C.POINTER(sz)]
+        L.mpr_create_chains.argtypes = [C.POINTER(vp), i, i, i, i, vp, vp, vp, sz, vp]
         L.mpr_set_params.argtypes = [vp, C.POINTER(mpr_params), C.POINTER(C.c_float)]
         L.mpr_equilibrate.argtypes = [vp]
         L.mpr_simulate.argtypes = [vp]
@@ -130,6 +132,12 @@ def mpr_query_workspace(batch: int, rows: int, cols: int) -> int:
     return int(n.value)
 
 
+def mpr_query_workspace_chains(batch: int, chains: int, rows: int, cols: int) -> int:
+    n = C.c_size_t()
+    _check(lib().mpr_query_workspace_chains(batch, chains, rows, cols, C.byref(n)), "mpr_query_workspace_chains")
+    return int(n.value)
+
+
 @dataclass
 class Stats:
     equil_sweeps: int
@@ -154,8 +162,9 @@ class Mpr:
     sample_mask: uint8 CUDA tensor of the same shape, 1 = sample (fixed).
     """
 
-    def __init__(self, values, sample_mask, stream=None, unconditional=None):
+    def __init__(self, values, sample_mask, stream=None, unconditional=None, chains: int = 1):
         import torch
+        self.chains = int(chains)
         if unconditional is not None:
             # (batch, rows, cols, device): mpr_create_unconditional, every node free, no data
             self.batch, self.rows, self.cols, self.device = unconditional
@@ -180,13 +189,18 @@ class Mpr:
         self.batch, self.rows, self.cols = (int(x) for x in values.shape)
         self._torch = torch
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        nbytes = mpr_query_workspace(self.batch, self.rows, self.cols)
+        nbytes = mpr_query_workspace_chains(self.batch, self.chains, self.rows, self.cols)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         assert self.workspace.data_ptr() % 256 == 0
         self._ctx = C.c_void_p()
-        _check(lib().mpr_create(C.byref(self._ctx), self.batch, self.rows, self.cols,
-                                values.data_ptr(), sample_mask.data_ptr(),
-                                self.workspace.data_ptr(), nbytes, self._stream.cuda_stream), "mpr_create")
+        if self.chains == 1:
+            _check(lib().mpr_create(C.byref(self._ctx), self.batch, self.rows, self.cols,
+                                    values.data_ptr(), sample_mask.data_ptr(),
+                                    self.workspace.data_ptr(), nbytes, self._stream.cuda_stream), "mpr_create")
+        else:
+            _check(lib().mpr_create_chains(C.byref(self._ctx), self.batch, self.chains, self.rows, self.cols,
+                                           values.data_ptr(), sample_mask.data_ptr(),
+                                           self.workspace.data_ptr(), nbytes, self._stream.cuda_stream), "mpr_create_chains")
         self.params = None
 
     # -- lifecycle ---------------------------------------------------------
@@ -333,10 +347,10 @@ def infer_temperature(Ts, es, e_s: float) -> float:
     return float(out.value)
 
 
-def interpolate(values, sample_mask, T, **params):
+def interpolate(values, sample_mask, T, chains: int = 1, **params):
     """The whole path for a batch of grids: create, set_params, equilibrate,
     simulate, predict.  Returns (prediction tensor, list of Stats)."""
-    m = Mpr(values, sample_mask)
+    m = Mpr(values, sample_mask, chains=chains)
     try:
         m.set_params(T, **params).equilibrate().simulate()
         out = m.predict()

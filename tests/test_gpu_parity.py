@@ -567,3 +567,80 @@ def test_predict_std_full_run_and_running_update_has_no_cancellation(torch_cuda,
     zmin, zmax, _ = orc.minmax(z, m)
     assert s[free].max() < 1e-4 * (float(zmax) - float(zmin))
     ctx.close()
+
+
+# ---------------------------------------------------------------------------
+# chain parallelism (reading R25)
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("batch,chains,M", [(1, 3, 7), (2, 4, 8)])
+def test_chains_against_oracle_chains_from_identical_state(torch_cuda, mpr, orc, batch, chains, M):
+    """Step 6 with several chains per grid, from identical oracle-made equilibrated states: ceil(M / chains)
+    realizations of 2 sweeps per chain; pooled mean and spread per prediction site agree except where a
+    near-threshold decision fell the other way in one of the sweeps."""
+    torch = torch_cuda
+    L = 160
+    fields = [_field(L, L, 12.0, 0.6, 700 + 10 * g) for g in range(batch)]
+    zs = np.stack([f[0] for f in fields]); ms = np.stack([f[1] for f in fields])
+    Ts = [0.01 * (1 + g) for g in range(batch)]
+    p = orc.Params(seed=77, equil_cap=60, M=M, sweeps_per_real=2)
+    phis, a_list, t_list, tr = [], [], [], []
+    for g in range(batch):
+        phi, zmin, zmax = orc.transform(zs[g], ms[g], p.seed, g)
+        st = orc.equilibrate(phi, ms[g], Ts[g], orc.Params(seed=p.seed, equil_cap=60, n_fit=200), g=g)   # exactly 60 sweeps
+        assert st["sweeps"] == 60
+        phis.append(phi); a_list.append(st["a"]); t_list.append(st["t"]); tr.append((zmin, zmax))
+    a = float(np.mean(a_list))          # one proposal width for the batch (mpr_sweep sets one a)
+    ctx = mpr.Mpr(_dev(torch, zs), _dev(torch, ms), chains=chains)
+    ctx.set_params(Ts, seed=p.seed, M=M, sweeps_per_real=2)
+    ctx.set_angles(torch.from_numpy(np.stack(phis)).cuda())
+    ctx.set_sweep_index(60)
+    ctx.sweep(0, a)
+    ctx.simulate()
+    mean_g = ctx.predict().cpu().numpy(); std_g = ctx.predict_std().cpu().numpy()
+    stats = ctx.get_stats()
+    Mc = orc.chains_realizations(M, chains)
+    for g in range(batch):
+        acc, acc2, M_tot, t_end, _ = orc.simulate_chains(phis[g], ms[g], Ts[g], a, p, chains, g=g, batch=batch, t0=60)
+        assert M_tot == chains * Mc and stats[g].realizations == M_tot and stats[g].t == t_end
+        zmin, zmax = tr[g]
+        mean_o = orc.predict(acc, M_tot, zs[g], ms[g], zmin, zmax)
+        std_o = orc.predict_std(acc, acc2, M_tot, ms[g], zmin, zmax)
+        free = ms[g] == 0
+        scale = (float(zmax) - float(zmin)) / TWO_PI_F
+        assert np.array_equal(mean_g[g][~free], zs[g][~free]) and np.all(std_g[g][~free] == 0.0)
+        bad = free & ((np.abs(mean_g[g] - mean_o) > 2e-5 * scale) | (np.abs(std_g[g] - std_o) > 2e-5 * scale + 1e-3 * std_o))
+        assert bad.sum() <= max(2, 1e-3 * free.sum()), (g, int(bad.sum()), int(free.sum()))
+        assert float(std_g[g][free].mean()) == pytest.approx(float(std_o[free].mean()), rel=2e-3)
+    # a second mpr_simulate continues every chain (no new fork): realization counts add up
+    ctx.simulate()
+    assert ctx.get_stats()[0].realizations == 2 * chains * Mc
+    ctx.close()
+
+
+def test_chains_full_run_cfg1_and_one_chain_is_the_plain_context(torch_cuda, mpr, orc):
+    """cfg1 whole path with 4 chains: MAE / RMSE against the withheld truth agree with the oracle's chains run
+    (means over seeds); a context made with chains = 1 gives bitwise the result of mpr_create."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    chains, M, s = 4, 12, 25
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m), chains=chains)
+    rows = []
+    for seed in range(7000, 7024):
+        ctx.set_params(T, seed=seed, equil_cap=w.equil_cap, sweeps_per_real=s, M=M).equilibrate().simulate()
+        vg = synth.validation_measures(z, ctx.predict().cpu().numpy()[0], m)
+        p = orc.Params(seed=seed, equil_cap=w.equil_cap, sweeps_per_real=s, M=M)
+        phi, zmin, zmax = orc.transform(z, m, seed)
+        st = orc.equilibrate(phi, m, T, p)
+        acc, _, M_tot, _, _ = orc.simulate_chains(phi, m, T, st["a"], p, chains, t0=st["t"])
+        vo = synth.validation_measures(z, orc.predict(acc, M_tot, z, m, zmin, zmax), m)
+        rows.append((vg["mae"], vo["mae"], vg["rmse"], vo["rmse"]))
+    ctx.close()
+    r = np.array(rows).mean(axis=0)
+    assert r[0] == pytest.approx(r[1], rel=0.01) and r[2] == pytest.approx(r[3], rel=0.01)
+    outs = []
+    for ch in (None, 1):
+        c = mpr.Mpr(_dev(torch, z), _dev(torch, m)) if ch is None else mpr.Mpr(_dev(torch, z), _dev(torch, m), chains=1)
+        c.set_params(T, seed=5, equil_cap=200, sweeps_per_real=3, M=5).equilibrate().simulate()
+        outs.append(c.predict().cpu().numpy()); c.close()
+    assert np.array_equal(outs[0], outs[1])

@@ -55,6 +55,16 @@ def test_workspace_query_validates_and_scales(lib):
     assert 33 * 4096 ** 2 < big < 38 * 4096 ** 2
     assert 33 * 32 * 2048 ** 2 < batch < 38 * 32 * 2048 ** 2
     assert mpr.mpr_query_workspace(3, 37, 53) % 256 == 0
+    # chains (reading R25): every further chain adds its vectors and accumulators, 24 bytes per site, nothing else
+    # (the tile shape, and with it the size of the tile lists, follows the number of chains)
+    one = mpr.mpr_query_workspace_chains(1, 1, 1024, 1024)
+    assert one == mpr.mpr_query_workspace(1, 1024, 1024)
+    four = mpr.mpr_query_workspace_chains(1, 4, 1024, 1024)
+    assert 3 * 23.5 * 1024 ** 2 < four - one < 3 * 24.5 * 1024 ** 2
+    for bad in [(1, 0, 8, 8), (2, 40000, 8, 8), (0, 2, 8, 8)]:
+        with pytest.raises(mpr.MprError) as e:
+            mpr.mpr_query_workspace_chains(*bad)
+        assert e.value.name == "MPR_ERR_ARG"
 
 
 def test_null_and_misuse_are_errors_not_crashes(lib):
