@@ -454,6 +454,39 @@ void orc_predict_std(const double *acc, const double *acc2, int M, const uint8_t
     }
 }
 
+/* ------------------------------------------------------------------------
+ * Quantiles of the conditional distribution at the prediction sites from the first two moments of the M
+ * realizations ("Statistics of M realizations"; SURVEY 8(f) NEXT-2 "quantiles from sum phi^2";
+ * DESIGN.md reading R26): the Gaussian quantile z_p = mean_z + Phi^-1(p) s_z, clamped to the data range
+ * [zmin, zmax] that the state space [0, 2 pi] maps to.  Phi^-1 by bisection on Phi(x) = erfc(-x / sqrt 2) / 2.
+ * Sample sites return their input value.  0 < p < 1, M >= 2.
+ * ---------------------------------------------------------------------- */
+double orc_inv_norm_cdf(double p)
+{
+    double lo = -40.0, hi = 40.0;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (0.5 * erfc(-mid / sqrt(2.0)) < p) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+void orc_predict_quantile(const double *acc, const double *acc2, int M, double p, const float *z,
+                          const uint8_t *mask, int64_t n_sites, float zmin, float zmax, float *out)
+{
+    const double xp = orc_inv_norm_cdf(p);
+    const double scale = ((double)zmax - (double)zmin) / TWO_PI;
+    for (int64_t n = 0; n < n_sites; ++n) {
+        if (mask[n]) { out[n] = z[n]; continue; }
+        double var = (acc2[n] - acc[n] * acc[n] / (double)M) / (double)(M - 1);
+        if (var < 0.0) var = 0.0;
+        double zq = (double)zmin + (acc[n] / (double)M) * scale + xp * sqrt(var) * scale;
+        if (zq < (double)zmin) zq = (double)zmin;
+        if (zq > (double)zmax) zq = (double)zmax;
+        out[n] = (float)zq;
+    }
+}
+
 int orc_num_threads(void)
 {
 #ifdef _OPENMP

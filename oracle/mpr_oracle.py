@@ -83,6 +83,10 @@ def lib():
         L.orc_simulate2.restype = None
         L.orc_predict_std.argtypes = [f64p, f64p, C.c_int, u8p, C.c_int64, C.c_float, C.c_float, f32p]
         L.orc_predict_std.restype = None
+        L.orc_inv_norm_cdf.argtypes = [C.c_double]
+        L.orc_inv_norm_cdf.restype = C.c_double
+        L.orc_predict_quantile.argtypes = [f64p, f64p, C.c_int, C.c_double, f32p, u8p, C.c_int64, C.c_float, C.c_float, f32p]
+        L.orc_predict_quantile.restype = None
         L.orc_predict.argtypes = [f64p, C.c_int, f32p, u8p, C.c_int64, C.c_float, C.c_float, f32p]
         L.orc_predict.restype = None
         L.orc_num_threads.restype = C.c_int
@@ -263,6 +267,21 @@ def predict_std(acc, acc2, M, mask, zmin, zmax) -> np.ndarray:
     lib().orc_predict_std(np.ascontiguousarray(acc, dtype=np.float64).reshape(-1),
                           np.ascontiguousarray(acc2, dtype=np.float64).reshape(-1), M, m.reshape(-1), m.size,
                           float(zmin), float(zmax), out.reshape(-1))
+    return out
+
+
+def inv_norm_cdf(p: float) -> float:
+    return float(lib().orc_inv_norm_cdf(float(p)))
+
+
+def predict_quantile(acc, acc2, M, p, z, mask, zmin, zmax) -> np.ndarray:
+    """Gaussian p-quantile of the conditional distribution from mean and spread of the M realizations (R26)."""
+    zf = np.ascontiguousarray(z, dtype=np.float32)
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    out = np.empty_like(zf)
+    lib().orc_predict_quantile(np.ascontiguousarray(acc, dtype=np.float64).reshape(-1),
+                               np.ascontiguousarray(acc2, dtype=np.float64).reshape(-1), M, float(p), zf.reshape(-1),
+                               m.reshape(-1), zf.size, float(zmin), float(zmax), out.reshape(-1))
     return out
 
 

@@ -617,3 +617,36 @@ def test_chains_pooled_moments_match_boltzmann(orc):
     n_eff = M_tot / 2
     assert abs(acc[1, 1] / M_tot - m1) < 4.5 * math.sqrt((m2 - m1 * m1) / n_eff)
     assert abs(acc2[1, 1] / M_tot - m2) < 4.5 * math.sqrt((m4 - m2 * m2) / n_eff)
+
+
+# ---------------------------------------------------------------------------
+# quantiles from the first two moments of the realizations (reading R26)
+# ---------------------------------------------------------------------------
+def test_inverse_normal_cdf_against_scipy_and_closed_forms(orc):
+    assert orc.inv_norm_cdf(0.5) == pytest.approx(0.0, abs=1e-12)
+    assert orc.inv_norm_cdf(0.8413447460685429) == pytest.approx(1.0, abs=1e-10)      # Phi(1)
+    assert orc.inv_norm_cdf(0.975) == pytest.approx(1.959963984540054, abs=1e-10)
+    for p in (1e-9, 1e-3, 0.05, 0.3, 0.7, 0.999, 1 - 1e-9):
+        assert orc.inv_norm_cdf(p) == pytest.approx(stats.norm.ppf(p), abs=1e-8)
+        assert orc.inv_norm_cdf(p) == pytest.approx(-orc.inv_norm_cdf(1 - p), abs=1e-6)
+
+
+def test_predict_quantile_closed_forms(orc):
+    mask = np.array([[1, 0, 0, 0]], dtype=np.uint8)
+    z = np.array([[17.0, np.nan, np.nan, np.nan]], dtype=np.float32)
+    seqs = [[0.0] * 3, [1.0, 2.0, 3.0], [2.5, 2.5, 2.5], [0.0, TWO_PI_F, 0.0]]
+    acc = np.array([[sum(s) for s in seqs]]); acc2 = np.array([[sum(x * x for x in s) for s in seqs]])
+    zmin, zmax = 10.0, 30.0
+    scale = (zmax - zmin) / TWO_PI_F
+    med = orc.predict_quantile(acc, acc2, 3, 0.5, z, mask, zmin, zmax)
+    assert med[0, 0] == np.float32(17.0)                                               # a sample site returns its datum
+    assert np.array_equal(med[0, 1:], orc.predict(acc, 3, z, mask, zmin, zmax)[0, 1:]) # the median is the mean
+    up = orc.predict_quantile(acc, acc2, 3, 0.8413447460685429, z, mask, zmin, zmax)
+    assert up[0, 1] == pytest.approx(zmin + (2.0 + 1.0) * scale, rel=1e-6)             # mean 2, s.d. 1: one s.d. up
+    assert up[0, 2] == pytest.approx(zmin + 2.5 * scale, rel=1e-6)                     # no spread: every quantile is the value
+    lo = orc.predict_quantile(acc, acc2, 3, 0.001, z, mask, zmin, zmax)
+    assert lo[0, 3] == np.float32(zmin)                                                # clamped to the data range
+    assert orc.predict_quantile(acc, acc2, 3, 0.999, z, mask, zmin, zmax)[0, 3] == pytest.approx(zmax)
+    qs = [orc.predict_quantile(acc, acc2, 3, p, z, mask, zmin, zmax)[0, 1] for p in (0.1, 0.3, 0.5, 0.7, 0.9)]
+    assert all(a < b for a, b in zip(qs, qs[1:]))
+    assert qs[0] + qs[4] == pytest.approx(2 * qs[2], rel=1e-6)                          # symmetric about the mean
