@@ -139,6 +139,13 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out);
  * realizations (else MPR_ERR_STATE).  Synchronises. */
 mpr_status mpr_predict_std(mpr_ctx* ctx, float* d_out);
 
+/* Quantiles from the first two moments of the realizations (L212; reading R26):
+ * d_out device float [batch][rows][cols] receives, at prediction sites, the Gaussian p-quantile
+ * mean + Phi^-1(p) * (standard deviation of mpr_predict_std), clamped to the data range [z_min, z_max] that the
+ * state space [0, 2 pi] maps to; sample sites = the input value.  0 < p < 1 (else MPR_ERR_ARG), needs >= 2
+ * realizations (else MPR_ERR_STATE).  p = 0.5 is mpr_predict.  Synchronises. */
+mpr_status mpr_predict_quantile(mpr_ctx* ctx, double p, float* d_out);
+
 /* ---- chain parallelism (a variant of the paper's single chain, reading R25) ----
  * The M realizations of step 6 ("Statistics of M realizations") made by `chains` independent
  * chains per grid instead of one, so that small grids fill the device: mpr_equilibrate runs one chain per grid

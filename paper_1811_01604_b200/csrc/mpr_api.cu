@@ -611,6 +611,29 @@ mpr_status mpr_predict_std(mpr_ctx* ctx, float* d_out)
     return MPR_OK;
 }
 
+mpr_status mpr_predict_quantile(mpr_ctx* ctx, double p, float* d_out)
+{
+    if (!ctx || !d_out || !(p > 0.0 && p < 1.0)) return MPR_ERR_ARG;
+    ENTER(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr_status s = fetch_states(ctx);
+    if (s != MPR_OK) return s;
+    for (int b = 0; b < ctx->d.batch; ++b) {
+        uint32_t n = 0;
+        for (int c = 0; c < ctx->d.chains; ++c) n += ctx->h_states[b + c * ctx->d.batch].realizations;
+        if (n < 2u) return MPR_ERR_STATE;
+    }
+    // x_p = Phi^-1(p): the root of erfc(-x / sqrt 2) / 2 = p by bisection (host, once per call)
+    double lo = -40.0, hi = 40.0;
+    for (int it = 0; it < 200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        (0.5 * std::erfc(-mid / std::sqrt(2.0)) < p ? lo : hi) = mid;
+    }
+    k_predict_quantile<<<site_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, 0.5 * (lo + hi), d_out);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
 mpr_status mpr_sample_energy(mpr_ctx* ctx, double* h_e_s, uint64_t* h_n_pairs)
 {
     if (!ctx || !h_e_s || !h_n_pairs) return MPR_ERR_ARG;

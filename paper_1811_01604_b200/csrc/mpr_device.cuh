@@ -1264,6 +1264,36 @@ __global__ void __launch_bounds__(256) k_predict_std(Dev d, float* __restrict__ 
     out[o] = (float)(sqrt(var) * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F);
 }
 
+// Gaussian p-quantile of the conditional distribution from the pooled mean and spread (reading R26):
+// z_p = mean_z + x_p s_z with x_p = Phi^-1(p) computed on the host, clamped to the data range; sample sites = input
+__global__ void __launch_bounds__(256) k_predict_quantile(Dev d, double x_p, float* __restrict__ out)
+{
+    const int g = blockIdx.y;
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N) return;
+    const size_t o = (size_t)g * d.N + n;
+    if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = d.values[o]; return; }
+    const GridState& s = d.states[g];
+    double sum = 0.0, count = 0.0;
+    for (int c = 0; c < d.chains; ++c) {
+        const int v = g + c * d.batch;
+        sum += (double)d.acc[(size_t)v * d.N + n]; count += (double)d.states[v].realizations;
+    }
+    const double mean = sum / count;
+    double ssd = 0.0;
+    for (int c = 0; c < d.chains; ++c) {
+        const int v = g + c * d.batch;
+        const double nc = (double)d.states[v].realizations;
+        if (nc == 0.0) continue;
+        const double dev = (double)d.acc[(size_t)v * d.N + n] / nc - mean;
+        ssd += fmax((double)d.m2[(size_t)v * d.N + n], 0.0) + nc * dev * dev;
+    }
+    const double sd = count > 1.0 ? sqrt(ssd / (count - 1.0)) : 0.0;
+    const double scale = ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F;
+    const double z = (double)s.zmin + mean * scale + x_p * sd * scale;
+    out[o] = (float)fmin(fmax(z, (double)s.zmin), (double)s.zmax);
+}
+
 // angle import / export at the prediction sites ------------------------------
 __global__ void __launch_bounds__(256) k_export_angles(Dev d)
 {

@@ -33,6 +33,7 @@ EXPORTS = (
     "mpr_get_stats", "mpr_get_launch_count", "mpr_status_string", "mpr_last_cuda_error",
     "mpr_sample_energy", "mpr_create_unconditional", "mpr_measure_energy", "mpr_energy_table",
     "mpr_infer_temperature", "mpr_predict_std", "mpr_query_workspace_chains", "mpr_create_chains",
+    "mpr_predict_quantile",
 )
 
 
@@ -94,6 +95,7 @@ def lib():
         L.mpr_get_stats.argtypes = [vp, C.POINTER(mpr_stats)]
         L.mpr_get_launch_count.argtypes = [vp, C.POINTER(u64)]
         L.mpr_predict_std.argtypes = [vp, vp]
+        L.mpr_predict_quantile.argtypes = [vp, C.c_double, vp]
         L.mpr_sample_energy.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(u64)]
         L.mpr_create_unconditional.argtypes = [C.POINTER(vp), i, i, i, vp, sz, vp]
         L.mpr_measure_energy.argtypes = [vp, u32, C.POINTER(C.c_double)]
@@ -250,6 +252,13 @@ class Mpr:
         if out is None:
             out = torch.empty((self.batch, self.rows, self.cols), dtype=torch.float32, device=self.device)
         _check(lib().mpr_predict_std(self._ctx, out.data_ptr()), "mpr_predict_std")
+        return out
+
+    def predict_quantile(self, p: float, out=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty((self.batch, self.rows, self.cols), dtype=torch.float32, device=self.device)
+        _check(lib().mpr_predict_quantile(self._ctx, float(p), out.data_ptr()), "mpr_predict_quantile")
         return out
 
     # -- Alg. 2 step 4 -------------------------------------------------------

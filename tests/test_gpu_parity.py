@@ -538,6 +538,17 @@ def test_predict_std_against_oracle_chain(torch_cuda, mpr, orc):
     assert bad.sum() <= max(2, 1e-3 * free.sum()), (int(bad.sum()), int(free.sum()))
     assert np.abs(mean_gpu - mean_ref)[free & ~bad].max() < 2e-5 * scale
     assert float(got[free].mean()) == pytest.approx(float(ref[free].mean()), rel=2e-3)
+    # quantiles from the same two moments (reading R26): median = mean bit for bit, 5 % / 95 % against the oracle
+    assert np.array_equal(ctx.predict_quantile(0.5).cpu().numpy()[0], mean_gpu)
+    for pq in (0.05, 0.95):
+        q_gpu = ctx.predict_quantile(pq).cpu().numpy()[0]
+        q_ref = orc.predict_quantile(acc, acc2, p.M, pq, z, m, zmin, zmax)
+        assert np.array_equal(q_gpu[~free], z[~free])
+        assert np.abs(q_gpu - q_ref)[free & ~bad].max() < 6e-5 * scale + 2e-3 * float(ref[free].max())
+        assert q_gpu.min() >= float(zmin) and q_gpu.max() <= float(zmax)
+    with pytest.raises(mpr.MprError) as e:
+        ctx.predict_quantile(1.0)
+    assert e.value.name == "MPR_ERR_ARG"
     ctx.close()
 
 
