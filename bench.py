@@ -131,7 +131,7 @@ ISSUE_PEAK_PER_S = 148 * 4 * 32 * 1.965e9
 # Instructions one UPDATE needs at the least: Philox4x32-10 is 40 per call and serves two
 # updates (20), about 40 fp32 / compare / select for Alg. 1 lines 1-6, 8 shared-memory accesses and addresses.
 ALGORITHMIC_INSTR_PER_UPDATE = 68.0
-# DRAM bytes of one 4-sweep tile-pass launch on cfg4 from the committed ncu capture (profiles/r01f_tilepass_v6.md)
+# DRAM bytes of one 4-sweep tile-pass launch on cfg4 from the committed ncu capture (profiles/r01g_tilepass_v7.md)
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4": 244.9e6}
 
 
