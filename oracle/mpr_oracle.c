@@ -8,9 +8,10 @@
  * must never be imported by it.  Only tests/, __graft_entry__.smoke() and the
  * cpu_baseline / --impl reference legs of bench.py may call it.
  *
- * Arithmetic: the spin state is stored in float (as on the GPU); everything
+ * Arithmetic: the spin state is stored in float (as on the GPU; with
+ * -DORC_F64 in double, see real_t below); everything
  * inside one site update is done in double from that state and rounded ONCE
- * to float when stored.  The data->angle transform (Eq. 1) alone is done in
+ * to the storage type when stored.  The data->angle transform (Eq. 1) alone is done in
  * float with a fixed operation order because the GPU must match it bit for
  * bit.  "2 pi" is the float nearest to 2 pi, TWO_PI = 6.2831854820251465,
  * everywhere (state space [0, TWO_PI]; reading R4).
@@ -41,8 +42,19 @@
 #include <omp.h>
 #endif
 
+/* Storage type of data and spin state.  Default float: the configurations of BASELINE.json and the paper's
+ * single-precision program (Table 3).  -DORC_F64 builds the same source with double storage (the paper's
+ * double-precision program, Table 2): "2 pi" is then the double nearest 2 pi, Eq. 1 is the
+ * same pinned operation order in double, and a site update computes in double from the double state. */
+#ifdef ORC_F64
+typedef double real_t;
+#define ORC_TWO_PI_F 6.28318530717958647692
+#else
+typedef float real_t;
 #define ORC_TWO_PI_F 6.28318530717958647692f
+#endif
 static const double TWO_PI = (double)ORC_TWO_PI_F;
+int orc_real_bytes(void) { return (int)sizeof(real_t); }
 
 /* ------------------------------------------------------------------------
  * Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), the generator the paper
@@ -98,10 +110,10 @@ static void sweep_uniforms(uint64_t seed, uint32_t g, uint32_t t, uint32_t n,
  * step 3).  Minimum and maximum over SAMPLE values only.
  * Returns the number of sample sites.
  * ---------------------------------------------------------------------- */
-int64_t orc_minmax(const float *z, const uint8_t *mask, int64_t n, float *zmin, float *zmax)
+int64_t orc_minmax(const real_t *z, const uint8_t *mask, int64_t n, real_t *zmin, real_t *zmax)
 {
     int64_t count = 0;
-    float lo = INFINITY, hi = -INFINITY;
+    real_t lo = INFINITY, hi = -INFINITY;
     for (int64_t i = 0; i < n; ++i) {
         if (!mask[i]) continue;
         if (z[i] < lo) lo = z[i];
@@ -115,13 +127,13 @@ int64_t orc_minmax(const float *z, const uint8_t *mask, int64_t n, float *zmin, 
 /* Eq. 1 in float, pinned order (no FMA contraction: build with
  * -ffp-contract=off): scale = TWO_PI_F / (zmax - zmin);
  * phi = (z - zmin) * scale, clamped to [0, TWO_PI_F]. */
-float orc_eq1(float z, float zmin, float zmax)
+real_t orc_eq1(real_t z, real_t zmin, real_t zmax)
 {
-    volatile float range = zmax - zmin;
-    volatile float scale = ORC_TWO_PI_F / range;
-    volatile float d = z - zmin;
-    float phi = d * scale;
-    if (phi < 0.0f) phi = 0.0f;
+    volatile real_t range = zmax - zmin;
+    volatile real_t scale = ORC_TWO_PI_F / range;
+    volatile real_t d = z - zmin;
+    real_t phi = d * scale;
+    if (phi < 0) phi = 0;
     if (phi > ORC_TWO_PI_F) phi = ORC_TWO_PI_F;
     return phi;
 }
@@ -129,8 +141,8 @@ float orc_eq1(float z, float zmin, float zmax)
 /* O1 + O2: sample sites by Eq. 1; prediction sites ~ U(0, 2 pi) from the INIT
  * stream (Alg. 2 step 2.2): phi = TWO_PI_F * u in float (u is
  * exact in float, one rounding). */
-void orc_transform(const float *z, const uint8_t *mask, int rows, int cols,
-                   uint64_t seed, uint32_t g, float zmin, float zmax, float *phi)
+void orc_transform(const real_t *z, const uint8_t *mask, int rows, int cols,
+                   uint64_t seed, uint32_t g, real_t zmin, real_t zmax, real_t *phi)
 {
     uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
     for (int64_t n = 0; n < (int64_t)rows * cols; ++n) {
@@ -140,8 +152,8 @@ void orc_transform(const float *z, const uint8_t *mask, int rows, int cols,
             uint32_t ctr[4] = { (uint32_t)(n >> 2), 0u, 0u, g };
             uint32_t x[4];
             orc_philox4x32_10(ctr, key, x);
-            float u = (float)orc_u01(x[n & 3]);
-            volatile float p = ORC_TWO_PI_F * u;
+            real_t u = (real_t)orc_u01(x[n & 3]);
+            volatile real_t p = ORC_TWO_PI_F * u;
             phi[n] = p;
         }
     }
@@ -207,7 +219,7 @@ static double dist_to_ends(double x)
     return a < b ? a : b;
 }
 
-uint64_t orc_sweep(float *phi, const uint8_t *mask, int rows, int cols,
+uint64_t orc_sweep(real_t *phi, const uint8_t *mask, int rows, int cols,
                    double q, double T, double a, uint64_t seed, uint32_t g,
                    uint32_t t, int or_mode,
                    double *d_margin, double *d_edge, double *d_R)
@@ -248,7 +260,7 @@ uint64_t orc_sweep(float *phi, const uint8_t *mask, int rows, int cols,
                 /* lines 6-6.2 */
                 double p_new;
                 if (AP > rr) { p_new = p2; ++accepted; } else { p_new = p1; }
-                phi[n] = (float)p_new;
+                phi[n] = (real_t)p_new;
                 if (d_margin) d_margin[n] = fabs(AP - rr);
                 if (d_edge) {
                     double e1 = (or_mode == 0) ? dist_to_ends(p_raw) : 1e30;
@@ -272,7 +284,7 @@ int64_t orc_n_bonds(int rows, int cols)
     return (int64_t)rows * (cols - 1) + (int64_t)cols * (rows - 1);
 }
 
-double orc_energy(const float *phi, int rows, int cols, double q)
+double orc_energy(const real_t *phi, int rows, int cols, double q)
 {
     double *row_sum = (double *)malloc(sizeof(double) * (size_t)rows);
 #ifdef _OPENMP
@@ -301,7 +313,7 @@ double orc_energy(const float *phi, int rows, int cols, double q)
  * every unordered pair once, N_SP their number (reading R1).
  * Returns e_s (0 when there is no such pair) and N_SP through n_pairs.
  * ---------------------------------------------------------------------- */
-double orc_sample_energy(const float *phi, const uint8_t *mask, int rows, int cols,
+double orc_sample_energy(const real_t *phi, const uint8_t *mask, int rows, int cols,
                          double q, int64_t *n_pairs)
 {
     double sum = 0.0;
@@ -356,7 +368,7 @@ static int64_t count_free(const uint8_t *mask, int64_t n)
  * a_hist[i+1] = a after step 5.2.  *t_io is the global sweep index.
  * Returns i = number of sweeps done.
  * ---------------------------------------------------------------------- */
-int orc_equilibrate(float *phi, const uint8_t *mask, int rows, int cols,
+int orc_equilibrate(real_t *phi, const uint8_t *mask, int rows, int cols,
                     double q, double T, uint64_t seed, uint32_t g, int or_mode,
                     int cap, int n_f, int n_fit, double A_targ, double k_a,
                     uint32_t *t_io, double *a_out, double *k_out,
@@ -393,7 +405,7 @@ int orc_equilibrate(float *phi, const uint8_t *mask, int rows, int cols,
  * ---------------------------------------------------------------------- */
 /* acc2 (may be NULL): sum over the realizations of phi^2, for the spread of the realizations
  * ("Statistics of M realizations"). */
-void orc_simulate2(float *phi, const uint8_t *mask, int rows, int cols,
+void orc_simulate2(real_t *phi, const uint8_t *mask, int rows, int cols,
                    double q, double T, double a_eq, uint64_t seed, uint32_t g,
                    int or_mode, int M, int s, uint32_t *t_io, double *acc, double *acc2)
 {
@@ -413,7 +425,7 @@ void orc_simulate2(float *phi, const uint8_t *mask, int rows, int cols,
     *t_io = t;
 }
 
-void orc_simulate(float *phi, const uint8_t *mask, int rows, int cols,
+void orc_simulate(real_t *phi, const uint8_t *mask, int rows, int cols,
                   double q, double T, double a_eq, uint64_t seed, uint32_t g,
                   int or_mode, int M, int s, uint32_t *t_io, double *acc)
 {
@@ -427,13 +439,13 @@ void orc_simulate(float *phi, const uint8_t *mask, int rows, int cols,
  * back-transform of the mean angle: z = zmin + mean(phi) (zmax-zmin)/(2 pi).
  * Sample sites return their input value unchanged.
  * ---------------------------------------------------------------------- */
-void orc_predict(const double *acc, int M, const float *z, const uint8_t *mask,
-                 int64_t n_sites, float zmin, float zmax, float *out)
+void orc_predict(const double *acc, int M, const real_t *z, const uint8_t *mask,
+                 int64_t n_sites, real_t zmin, real_t zmax, real_t *out)
 {
     for (int64_t n = 0; n < n_sites; ++n) {
         if (mask[n]) { out[n] = z[n]; continue; }
         double mean_phi = acc[n] / (double)M;
-        out[n] = (float)((double)zmin + mean_phi * ((double)zmax - (double)zmin) / TWO_PI);
+        out[n] = (real_t)((double)zmin + mean_phi * ((double)zmax - (double)zmin) / TWO_PI);
     }
 }
 
@@ -444,13 +456,13 @@ void orc_predict(const double *acc, int M, const float *z, const uint8_t *mask,
  * M >= 2; 0 at sample sites (their value is data).
  * ---------------------------------------------------------------------- */
 void orc_predict_std(const double *acc, const double *acc2, int M, const uint8_t *mask,
-                     int64_t n_sites, float zmin, float zmax, float *out)
+                     int64_t n_sites, real_t zmin, real_t zmax, real_t *out)
 {
     for (int64_t n = 0; n < n_sites; ++n) {
-        if (mask[n]) { out[n] = 0.0f; continue; }
+        if (mask[n]) { out[n] = 0; continue; }
         double var = (acc2[n] - acc[n] * acc[n] / (double)M) / (double)(M - 1);
         if (var < 0.0) var = 0.0;
-        out[n] = (float)(sqrt(var) * ((double)zmax - (double)zmin) / TWO_PI);
+        out[n] = (real_t)(sqrt(var) * ((double)zmax - (double)zmin) / TWO_PI);
     }
 }
 
@@ -471,8 +483,8 @@ double orc_inv_norm_cdf(double p)
     return 0.5 * (lo + hi);
 }
 
-void orc_predict_quantile(const double *acc, const double *acc2, int M, double p, const float *z,
-                          const uint8_t *mask, int64_t n_sites, float zmin, float zmax, float *out)
+void orc_predict_quantile(const double *acc, const double *acc2, int M, double p, const real_t *z,
+                          const uint8_t *mask, int64_t n_sites, real_t zmin, real_t zmax, real_t *out)
 {
     const double xp = orc_inv_norm_cdf(p);
     const double scale = ((double)zmax - (double)zmin) / TWO_PI;
@@ -483,7 +495,7 @@ void orc_predict_quantile(const double *acc, const double *acc2, int M, double p
         double zq = (double)zmin + (acc[n] / (double)M) * scale + xp * sqrt(var) * scale;
         if (zq < (double)zmin) zq = (double)zmin;
         if (zq > (double)zmax) zq = (double)zmax;
-        out[n] = (float)zq;
+        out[n] = (real_t)zq;
     }
 }
 

@@ -15,16 +15,21 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mpr_oracle.c")
-_LIB = os.path.join(_HERE, "libmpr_oracle.so")
+# Storage type of data and state: float32 (the configurations; the paper's Table 3) in this module; the module
+# oracle.mpr_oracle64 executes this same file with _F64 set: -DORC_F64, float64 (the paper's Table 2; NEXT-3)
+_F64 = bool(globals().get("_F64", False))
+REAL = np.float64 if _F64 else np.float32
+_CREAL = C.c_double if _F64 else C.c_float
+_LIB = os.path.join(_HERE, "libmpr_oracle64.so" if _F64 else "libmpr_oracle.so")
 
-TWO_PI_F = float(np.float32(2.0 * np.pi))   # 6.2831854820251465
+TWO_PI_F = float(REAL(2.0 * np.pi))   # float32: 6.2831854820251465; float64: 6.283185307179586
 
 
 def build(force: bool = False) -> str:
     """gcc -O2, no FMA contraction, no fast-math; OpenMP over one colour's rows."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
-               "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+               "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"] + (["-DORC_F64"] if _F64 else [])
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -36,7 +41,7 @@ def lib():
     global _lib
     if _lib is None:
         L = C.CDLL(build())
-        f32p = np.ctypeslib.ndpointer(np.float32, flags="C_CONTIGUOUS")
+        f32p = np.ctypeslib.ndpointer(REAL, flags="C_CONTIGUOUS")     # the storage type
         f64p = np.ctypeslib.ndpointer(np.float64, flags="C_CONTIGUOUS")
         u8p = np.ctypeslib.ndpointer(np.uint8, flags="C_CONTIGUOUS")
         u32p = np.ctypeslib.ndpointer(np.uint32, flags="C_CONTIGUOUS")
@@ -44,12 +49,12 @@ def lib():
         L.orc_philox4x32_10.restype = None
         L.orc_u01.argtypes = [C.c_uint32]
         L.orc_u01.restype = C.c_double
-        L.orc_minmax.argtypes = [f32p, u8p, C.c_int64, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.orc_minmax.argtypes = [f32p, u8p, C.c_int64, C.POINTER(_CREAL), C.POINTER(_CREAL)]
         L.orc_minmax.restype = C.c_int64
-        L.orc_eq1.argtypes = [C.c_float, C.c_float, C.c_float]
-        L.orc_eq1.restype = C.c_float
+        L.orc_eq1.argtypes = [_CREAL, _CREAL, _CREAL]
+        L.orc_eq1.restype = _CREAL
         L.orc_transform.argtypes = [f32p, u8p, C.c_int, C.c_int, C.c_uint64, C.c_uint32,
-                                    C.c_float, C.c_float, f32p]
+                                    _CREAL, _CREAL, f32p]
         L.orc_transform.restype = None
         L.orc_local_energy.argtypes = [C.c_double] * 4
         L.orc_local_energy.restype = C.c_double
@@ -81,16 +86,18 @@ def lib():
                                     C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_int,
                                     C.POINTER(C.c_uint32), f64p, f64p]
         L.orc_simulate2.restype = None
-        L.orc_predict_std.argtypes = [f64p, f64p, C.c_int, u8p, C.c_int64, C.c_float, C.c_float, f32p]
+        L.orc_predict_std.argtypes = [f64p, f64p, C.c_int, u8p, C.c_int64, _CREAL, _CREAL, f32p]
         L.orc_predict_std.restype = None
         L.orc_inv_norm_cdf.argtypes = [C.c_double]
         L.orc_inv_norm_cdf.restype = C.c_double
-        L.orc_predict_quantile.argtypes = [f64p, f64p, C.c_int, C.c_double, f32p, u8p, C.c_int64, C.c_float, C.c_float, f32p]
+        L.orc_predict_quantile.argtypes = [f64p, f64p, C.c_int, C.c_double, f32p, u8p, C.c_int64, _CREAL, _CREAL, f32p]
         L.orc_predict_quantile.restype = None
-        L.orc_predict.argtypes = [f64p, C.c_int, f32p, u8p, C.c_int64, C.c_float, C.c_float, f32p]
+        L.orc_predict.argtypes = [f64p, C.c_int, f32p, u8p, C.c_int64, _CREAL, _CREAL, f32p]
         L.orc_predict.restype = None
         L.orc_num_threads.restype = C.c_int
         L.orc_set_num_threads.argtypes = [C.c_int]
+        L.orc_real_bytes.restype = C.c_int
+        assert L.orc_real_bytes() == np.dtype(REAL).itemsize
         _lib = L
     return _lib
 
@@ -111,24 +118,24 @@ def u01(x: int) -> float:
 
 
 def minmax(z: np.ndarray, mask: np.ndarray):
-    zf = np.ascontiguousarray(z, dtype=np.float32).ravel()
+    zf = np.ascontiguousarray(z, dtype=REAL).ravel()
     m = np.ascontiguousarray(mask, dtype=np.uint8).ravel()
-    lo, hi = C.c_float(), C.c_float()
+    lo, hi = _CREAL(), _CREAL()
     n = lib().orc_minmax(zf, m, zf.size, C.byref(lo), C.byref(hi))
-    return np.float32(lo.value), np.float32(hi.value), int(n)
+    return REAL(lo.value), REAL(hi.value), int(n)
 
 
-def eq1(z, zmin, zmax) -> np.float32:
-    return np.float32(lib().orc_eq1(float(z), float(zmin), float(zmax)))
+def eq1(z, zmin, zmax):
+    return REAL(lib().orc_eq1(float(z), float(zmin), float(zmax)))
 
 
 def transform(z: np.ndarray, mask: np.ndarray, seed: int, g: int = 0):
     """O1 + O2: returns (phi float32 [rows, cols], zmin, zmax)."""
     rows, cols = z.shape
-    zf = np.ascontiguousarray(z, dtype=np.float32)
+    zf = np.ascontiguousarray(z, dtype=REAL)
     m = np.ascontiguousarray(mask, dtype=np.uint8)
     zmin, zmax, _ = minmax(zf, m)
-    phi = np.empty((rows, cols), dtype=np.float32)
+    phi = np.empty((rows, cols), dtype=REAL)
     lib().orc_transform(zf, m, rows, cols, seed, g, float(zmin), float(zmax), phi)
     return phi, zmin, zmax
 
@@ -147,7 +154,7 @@ def sweep(phi: np.ndarray, mask: np.ndarray, q, T, a, seed, g, t, or_mode=0, dia
     """One UPDATE sweep IN PLACE on phi (float32 [rows, cols]); returns the
     accepted count, plus (margin, edge, R) double arrays when diag=True."""
     rows, cols = phi.shape
-    assert phi.dtype == np.float32 and phi.flags.c_contiguous
+    assert phi.dtype == REAL and phi.flags.c_contiguous
     m = np.ascontiguousarray(mask, dtype=np.uint8)
     if diag:
         mg = np.full((rows, cols), np.inf)
@@ -165,7 +172,7 @@ def n_bonds(rows, cols) -> int:
 
 def energy(phi: np.ndarray, q=0.5) -> float:
     rows, cols = phi.shape
-    return lib().orc_energy(np.ascontiguousarray(phi, dtype=np.float32), rows, cols, q)
+    return lib().orc_energy(np.ascontiguousarray(phi, dtype=REAL), rows, cols, q)
 
 
 def energy_per_bond(phi: np.ndarray, q=0.5) -> float:
@@ -263,7 +270,7 @@ def simulate_chains(phi, mask, T, a_eq, p: Params, chains: int, g=0, batch=1, t0
 def predict_std(acc, acc2, M, mask, zmin, zmax) -> np.ndarray:
     """Sample standard deviation of the M back-transformed realizations at the prediction sites (L212)."""
     m = np.ascontiguousarray(mask, dtype=np.uint8)
-    out = np.empty(m.shape, dtype=np.float32)
+    out = np.empty(m.shape, dtype=REAL)
     lib().orc_predict_std(np.ascontiguousarray(acc, dtype=np.float64).reshape(-1),
                           np.ascontiguousarray(acc2, dtype=np.float64).reshape(-1), M, m.reshape(-1), m.size,
                           float(zmin), float(zmax), out.reshape(-1))
@@ -276,7 +283,7 @@ def inv_norm_cdf(p: float) -> float:
 
 def predict_quantile(acc, acc2, M, p, z, mask, zmin, zmax) -> np.ndarray:
     """Gaussian p-quantile of the conditional distribution from mean and spread of the M realizations (R26)."""
-    zf = np.ascontiguousarray(z, dtype=np.float32)
+    zf = np.ascontiguousarray(z, dtype=REAL)
     m = np.ascontiguousarray(mask, dtype=np.uint8)
     out = np.empty_like(zf)
     lib().orc_predict_quantile(np.ascontiguousarray(acc, dtype=np.float64).reshape(-1),
@@ -286,7 +293,7 @@ def predict_quantile(acc, acc2, M, p, z, mask, zmin, zmax) -> np.ndarray:
 
 
 def predict(acc, M, z, mask, zmin, zmax) -> np.ndarray:
-    zf = np.ascontiguousarray(z, dtype=np.float32)
+    zf = np.ascontiguousarray(z, dtype=REAL)
     m = np.ascontiguousarray(mask, dtype=np.uint8)
     out = np.empty_like(zf)
     lib().orc_predict(np.ascontiguousarray(acc, dtype=np.float64).reshape(-1), M, zf.reshape(-1),
@@ -314,7 +321,7 @@ def sample_energy(phi: np.ndarray, mask: np.ndarray, q=0.5):
     """Step 4.1, Eq. 4: (e_s, N_SP) over the nearest-neighbour pairs of sample sites (reading R1)."""
     rows, cols = phi.shape
     n = C.c_int64()
-    e = lib().orc_sample_energy(np.ascontiguousarray(phi, dtype=np.float32),
+    e = lib().orc_sample_energy(np.ascontiguousarray(phi, dtype=REAL),
                                 np.ascontiguousarray(mask, dtype=np.uint8), rows, cols, float(q), C.byref(n))
     return float(e), int(n.value)
 
@@ -331,7 +338,7 @@ def energy_table(rows: int, cols: int, Ts, p: Params, n_meas: int):
     P = rows * cols
     out = []
     for k, T in enumerate(Ts):
-        phi = np.full((rows, cols), np.float32(np.pi), dtype=np.float32)
+        phi = np.full((rows, cols), REAL(np.pi), dtype=REAL)
         a, t = 1.0, 0
         for i in range(p.equil_cap):
             accepted = sweep(phi, mask, p.q, float(T), a, p.seed, k, t, p.or_mode)
