@@ -200,6 +200,32 @@ mpr_status mpr_energy_table(int rows, int cols, const mpr_params* h_params, cons
  * R24).  Host arithmetic on n_T numbers.  Errors: ARG. */
 mpr_status mpr_infer_temperature(const float* h_T, const double* h_e, int n_T, double e_s, double* h_T_hat);
 
+/* ---- double-precision path (Table 2 against Table 3) ----
+ * The same method with data, spin state, every site update and the realization sums in double: one grid per
+ * context, values and outputs are double, "2 pi" is the double nearest 2 pi, Eq. 1 keeps its pinned operation
+ * order (in double), the random streams are those of the fp32 path (same Philox counters, the same 24-bit
+ * uniforms, grid word 0).  Calls mirror the fp32 ones (same statuses, same ordering rules, mpr_params as is;
+ * T is one temperature).  mpr64_predict / mpr64_predict_std: d_out device double [rows][cols].  Angles are
+ * exchanged as device double [rows][cols].  Workspace: mpr64_query_workspace bytes (64.2 B per site), 256-byte aligned. */
+typedef struct mpr64_ctx mpr64_ctx; /* opaque */
+mpr_status mpr64_query_workspace(int rows, int cols, size_t* h_bytes);
+mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_values, const uint8_t* d_sample_mask,
+                        void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+mpr_status mpr64_set_params(mpr64_ctx* ctx, const mpr_params* h_params, double T);
+mpr_status mpr64_equilibrate(mpr64_ctx* ctx);                 /* Alg. 2 step 5; synchronises */
+mpr_status mpr64_simulate(mpr64_ctx* ctx);                    /* Alg. 2 step 6; asynchronous */
+mpr_status mpr64_predict(mpr64_ctx* ctx, double* d_out);      /* Alg. 2 step 7; asynchronous */
+mpr_status mpr64_predict_std(mpr64_ctx* ctx, double* d_out);  /* L212; needs >= 2 realizations; synchronises */
+mpr_status mpr64_destroy(mpr64_ctx* ctx);
+mpr_status mpr64_get_angles(mpr64_ctx* ctx, double* d_phi);
+mpr_status mpr64_set_angles(mpr64_ctx* ctx, const double* d_phi);     /* prediction sites only are overwritten */
+mpr_status mpr64_set_sweep_index(mpr64_ctx* ctx, uint32_t t);
+mpr_status mpr64_sweep(mpr64_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_accepted /* may be NULL */);
+mpr_status mpr64_energy(mpr64_ctx* ctx, double* h_e_per_bond);
+mpr_status mpr64_get_transform(mpr64_ctx* ctx, double* h_zmin, double* h_zmax);
+mpr_status mpr64_get_stats(mpr64_ctx* ctx, mpr_stats* h_out);          /* z_min / z_max rounded to float here */
+mpr_status mpr64_get_launch_count(mpr64_ctx* ctx, uint64_t* h_count);
+
 /* ---- diagnostic / test / checkpoint surface ---- */
 
 /* Current angles phi in [0, 2 pi], device float [batch][rows][cols]. Sample

@@ -14,7 +14,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libmpr_b200.so")
 SOURCES = ["mpr_api.cu"]
-HEADERS = ["mpr_device.cuh"]
+HEADERS = ["mpr_device.cuh", "mpr_f64.cuh", "mpr_f64_api.inl"]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

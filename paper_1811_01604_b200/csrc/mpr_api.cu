@@ -2,6 +2,7 @@
 // Everything on the path runs in the kernels of mpr_device.cuh; this file
 // validates arguments, lays out the caller's workspace and enqueues launches.
 #include "mpr_device.cuh"
+#include "mpr_f64.cuh"
 #include "../../include/mpr.h"
 
 #include <cmath>
@@ -829,3 +830,5 @@ mpr_status mpr_get_launch_count(mpr_ctx* ctx, uint64_t* h_count)
 }
 
 }  // extern "C"
+
+#include "mpr_f64_api.inl"

@@ -1,0 +1,379 @@
+// mpr_f64.cuh -- the double-precision path (Table 2 against Table 3):
+// data, spin state, every site update and the realization sums in double.  Included by mpr_api.cu after
+// mpr_device.cuh (Philox, the bitmask helpers and the error flags are shared with the fp32 path; no arithmetic is).
+//
+// State: v_i = (cos q phi_i, sin q phi_i) as double2, row-major [rows][cols], updated IN PLACE: the sites of one
+// colour depend only on the other colour, so a half-sweep is one kernel with one thread per
+// lattice site of that colour, as in the paper's own design (L261-267).  Why not the fp32 path's shared-memory tile
+// pass: in double the update is bound by the fp64 pipe (one division, exp and sincos per update, ~250 DP instructions
+// against ~445 MB of state traffic per 4096^2 sweep = 69 us at the measured HBM peak), so temporal blocking has no
+// bytes to win back; DESIGN.md section 13.  One grid per context.
+#pragma once
+#include "mpr_device.cuh"
+
+namespace mpr64 {
+
+using mpr::ERRF_DEGENERATE;
+using mpr::ERRF_NONFINITE;
+using mpr::ERRF_NO_FREE;
+using mpr::ERRF_NO_SAMPLES;
+using mpr::MAX_NFIT;
+using mpr::PHILOX_ROUNDS;
+using mpr::is_fixed;
+using mpr::philox4x32_10;
+
+constexpr double TWO_PI_D  = 6.28318530717958647692;   // double nearest 2 pi; state space [0, TWO_PI_D]
+constexpr int    E_BLOCKS  = 592;                      // energy partials: fixed, so that the sum order is deterministic
+constexpr int    E_THREADS = 256;
+constexpr int    MM_BLOCKS = 592;
+
+struct State64 {
+    uint32_t t, done, i, realizations;
+    uint32_t n_samples, n_free, err_flags, pad;
+    unsigned long long accepted;
+    double   a, k, A_last, e_last, T, zmin, zmax, e_query;
+    double   e_ring[MAX_NFIT];
+};
+
+struct Dev64 {
+    State64*  state;
+    uint32_t* done_flag;
+    double*   partials;       // [max(E_BLOCKS, 4 * MM_BLOCKS)]
+    double*   values;         // [N] verbatim copy of the input
+    double*   phi;            // [N] Eq. 1 at the sample sites; export buffer at the prediction sites
+    uint32_t* bits;           // [words] fixed-site bitmask
+    double2*  vec;            // [N] unit vectors
+    double*   acc;            // [N] sum over the realizations of phi
+    double*   acc2;           // [N] sum of phi^2 (spread, L212)
+    int       rows, cols;
+    uint32_t  N, words;
+    uint32_t  rk0[PHILOX_ROUNDS], rk1[PHILOX_ROUNDS];
+    double    q, inv_q, bc, bs, n_bonds;
+    uint32_t  n_f, n_fit, equil_cap;
+    double    A_targ, k_a;
+};
+
+// u = (2 (x >> 9) + 1) 2^-24 in (0,1): the same lattice as the fp32 path (R13), exact in double
+__device__ __forceinline__ double u01d(uint32_t x) { return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0); }
+
+// Eq. 1 in double, the oracle's pinned operation order, clamped to [0, TWO_PI_D]
+__device__ __forceinline__ double eq1d(double z, double zmin, double zmax)
+{
+    const double scale = __ddiv_rn(TWO_PI_D, __dsub_rn(zmax, zmin));
+    double p = __dmul_rn(__dsub_rn(z, zmin), scale);
+    p = p < 0.0 ? 0.0 : p;
+    p = p > TWO_PI_D ? TWO_PI_D : p;
+    return p;
+}
+
+__device__ __forceinline__ double angle_of_d(double2 v, double inv_q)
+{
+    double p = atan2(v.y, v.x) * inv_q;
+    p = p < 0.0 ? 0.0 : p;
+    p = p > TWO_PI_D ? TWO_PI_D : p;
+    return p;
+}
+
+// ---- a1: min / max over the SAMPLE values (L81), sample count, finiteness --------------------------------------
+__global__ void __launch_bounds__(256) k64_minmax(Dev64 d, const double* __restrict__ z, const uint8_t* __restrict__ m)
+{
+    __shared__ double s_lo[8], s_hi[8];
+    __shared__ uint32_t s_cnt[8], s_bad[8];
+    double lo = INFINITY, hi = -INFINITY;
+    uint32_t cnt = 0, bad = 0;
+    for (uint32_t n = blockIdx.x * blockDim.x + threadIdx.x; n < d.N; n += gridDim.x * blockDim.x)
+        if (m[n]) {
+            const double x = z[n];
+            bad |= !isfinite(x);
+            lo = fmin(lo, x); hi = fmax(hi, x);
+            ++cnt;
+        }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        lo = fmin(lo, __shfl_xor_sync(0xFFFFFFFFu, lo, o));
+        hi = fmax(hi, __shfl_xor_sync(0xFFFFFFFFu, hi, o));
+        cnt += __shfl_xor_sync(0xFFFFFFFFu, cnt, o);
+        bad |= __shfl_xor_sync(0xFFFFFFFFu, bad, o);
+    }
+    const int w = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) { s_lo[w] = lo; s_hi[w] = hi; s_cnt[w] = cnt; s_bad[w] = bad; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < 8; ++k) { lo = fmin(lo, s_lo[k]); hi = fmax(hi, s_hi[k]); cnt += s_cnt[k]; bad |= s_bad[k]; }
+        d.partials[4 * blockIdx.x + 0] = lo; d.partials[4 * blockIdx.x + 1] = hi;
+        d.partials[4 * blockIdx.x + 2] = (double)cnt; d.partials[4 * blockIdx.x + 3] = (double)bad;
+    }
+}
+
+__global__ void k64_minmax_finish(Dev64 d, int n_blocks)
+{
+    State64& s = *d.state;
+    double lo = INFINITY, hi = -INFINITY, cnt = 0.0, bad = 0.0;
+    for (int b = 0; b < n_blocks; ++b) {
+        lo = fmin(lo, d.partials[4 * b]); hi = fmax(hi, d.partials[4 * b + 1]);
+        cnt += d.partials[4 * b + 2]; bad += d.partials[4 * b + 3];
+    }
+    uint32_t err = bad > 0.0 ? ERRF_NONFINITE : 0u;
+    s.n_samples = (uint32_t)cnt; s.n_free = d.N - (uint32_t)cnt;
+    if (cnt == 0.0) err |= ERRF_NO_SAMPLES;
+    else {
+        s.zmin = lo; s.zmax = hi;
+        if (!(err & ERRF_NONFINITE) && !(hi > lo)) err |= ERRF_DEGENERATE;
+    }
+    if ((uint32_t)cnt == d.N) err |= ERRF_NO_FREE;
+    s.err_flags = err;
+    s.t = 0; s.done = 0; s.i = 0; s.realizations = 0; s.accepted = 0ull;
+    s.a = 1.0; s.k = -1.0; s.A_last = 0.0; s.e_last = 0.0; s.T = 0.0; s.e_query = 0.0;
+    *d.done_flag = 0;
+}
+
+// ---- a2: Eq. 1 at the sample sites, fixed-site bitmask, verbatim value copy ------------------------------------
+__global__ void __launch_bounds__(256) k64_transform(Dev64 d, const double* __restrict__ values,
+                                                     const uint8_t* __restrict__ mask)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;      // < 32 * words
+    const State64& s = *d.state;
+    bool fixed = false;
+    if (n < d.N) {
+        const double z = values[n];
+        fixed = mask[n] != 0;
+        d.values[n] = z;
+        d.phi[n] = fixed ? eq1d(z, s.zmin, s.zmax) : 0.0;
+    }
+    const uint32_t b = __ballot_sync(0xFFFFFFFFu, fixed);
+    if ((threadIdx.x & 31) == 0 && (n >> 5) < d.words) d.bits[n >> 5] = b;
+}
+
+// Alg. 2 step 2.2 (L176): prediction sites ~ U(0, 2 pi) from the INIT stream; unit vectors of every site
+__global__ void __launch_bounds__(256) k64_init_state(Dev64 d)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N) return;
+    double p = d.phi[n];
+    if (!is_fixed(d.bits, n)) {
+        const uint4 x = philox4x32_10(n >> 2, 0u, 0u, 0u, d.rk0, d.rk1);
+        const uint32_t w = (n & 3u) == 0 ? x.x : (n & 3u) == 1 ? x.y : (n & 3u) == 2 ? x.z : x.w;
+        p = __dmul_rn(TWO_PI_D, u01d(w));
+        d.phi[n] = p;
+    }
+    double sn, cs;
+    sincos(__dmul_rn(d.q, p), &sn, &cs);
+    d.vec[n] = make_double2(cs, sn);
+}
+
+// ---- a3: UPDATE of one prediction site (Alg. 1) in vector form, in double ----------------------------
+// The same algebra as the fp32 path's update_site, written out again in double.
+template <bool QHALF, int ORMODE>
+__device__ __forceinline__ double2 update_site_d(double2 v, double2 n_up, double2 n_dn, double2 n_lf, double2 n_rt,
+                                                 uint32_t w0, uint32_t w1, double hd_scale, double neg_inv_T,
+                                                 double bc, double bs, bool& accepted)
+{
+    const double hx = (n_up.x + n_dn.x) + (n_lf.x + n_rt.x), hy = (n_up.y + n_dn.y) + (n_lf.y + n_rt.y);
+    double px = v.x, py = v.y;
+    if (ORMODE == 0) {
+        // line 1, over-relaxation: v' = 2 (h.v)/(h.h) h - v keeps h.v (L156, L265; R2); out of [0, 2 pi]: keep the spin
+        const double R2 = fma(hx, hx, hy * hy);
+        const double dot = fma(px, hx, py * hy);
+        const double k = (dot + dot) / R2;                       // 0 / 0 -> NaN -> kept below (R17)
+        const double fx = fma(k, hx, -px), fy = fma(k, hy, -py);
+        bool in = fy >= 0.0 && hy >= 0.0;
+        if (!QHALF) in = in && (fma(fx, bs, -fy * bc) >= 0.0);
+        px = in ? fx : px; py = in ? fy : py;
+    } else if (ORMODE == 1) {
+        // Eq. 6 as printed (L158), q = 1/2 only
+        const double C1 = (n_up.x * n_up.x - n_up.y * n_up.y) + (n_dn.x * n_dn.x - n_dn.y * n_dn.y)
+                        + (n_lf.x * n_lf.x - n_lf.y * n_lf.y) + (n_rt.x * n_rt.x - n_rt.y * n_rt.y);
+        const double S1 = 2.0 * (n_up.x * n_up.y + n_dn.x * n_dn.y + n_lf.x * n_lf.y + n_rt.x * n_rt.y);
+        const double R2 = fma(C1, C1, S1 * S1);
+        const double inv = R2 > 0.0 ? rsqrt(R2) : 0.0;
+        const double ex = R2 > 0.0 ? C1 * inv : 1.0, ey = S1 * inv;
+        double fx = fma(ex, px, ey * py), fy = fma(ey, px, -ex * py);
+        if (fy < 0.0) { fx = -fx; fy = -fy; }
+        px = fx; py = fy;
+    }
+    // lines 2-3: rotate by d = q delta = 2 hd, hd = (u - 1/2) q pi / a
+    const double hd = (u01d(w0) - 0.5) * hd_scale;
+    double sh, ch;
+    sincos(hd, &sh, &ch);
+    const double sh2 = sh + sh;
+    const double sd = sh2 * ch, omc = sh2 * sh;                  // sin d, 1 - cos d
+    double rx = fma(-sd, py, fma(-omc, px, px));
+    double ry = fma(sd, px, fma(-omc, py, py));
+    // line 4: dH = -h.(v'' - v') = (1 - cos d)(h.v') + sin d (h x v')
+    const double hdotp = fma(hx, px, hy * py);
+    const double hcrossp = fma(hx, py, -hy * px);
+    double dH = fma(omc, hdotp, sd * hcrossp);
+    if (QHALF) {
+        if (ry < 0.0) { rx = -rx; ry = -ry; dH = fma(2.0, hdotp, -dH); }     // phi -/+ 2 pi <=> v -> -v (R3)
+    } else {
+        const bool under = hd < 0.0 && ry < 0.0;
+        const bool over = hd > 0.0 && !(ry >= 0.0 && fma(rx, bs, -ry * bc) >= 0.0);
+        if (under || over) {
+            const double s2 = under ? bs : -bs;
+            const double wx = fma(rx, bc, -ry * s2), wy = fma(rx, s2, ry * bc);
+            rx = wx; ry = wy;
+            dH = hdotp - fma(hx, rx, hy * ry);
+        }
+    }
+    // lines 5-6: AP = min{1, exp(-dH/T)}; accept phi'' if AP > r else keep phi'
+    accepted = dH <= 0.0 || exp(dH * neg_inv_T) > u01d(w1);
+    return make_double2(accepted ? rx : px, accepted ? ry : py);
+}
+
+// One colour of one sweep (L261-265): one thread per lattice site of the colour, in place.  half = ceil(cols / 2).
+template <bool QHALF, int ORMODE>
+__global__ void __launch_bounds__(256) k64_halfsweep(Dev64 d, int colour, uint32_t t_off, int half, int count)
+{
+    const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)(idx / (uint32_t)half);
+    const int c = 2 * (int)(idx - (uint32_t)r * (uint32_t)half) + ((r + colour) & 1);
+    bool accepted = false;
+    if (r < d.rows && c < d.cols) {
+        const uint32_t n = (uint32_t)r * d.cols + c;
+        if (!is_fixed(d.bits, n)) {
+            const State64& s = *d.state;
+            const uint32_t t = s.t + t_off;
+            const double2 zero = make_double2(0.0, 0.0);                 // open boundary (L109)
+            const double2 up = r > 0 ? d.vec[n - d.cols] : zero, dn = r < d.rows - 1 ? d.vec[n + d.cols] : zero;
+            const double2 lf = c > 0 ? d.vec[n - 1] : zero, rt = c < d.cols - 1 ? d.vec[n + 1] : zero;
+            const uint4 x = philox4x32_10(n, t >> 1, 2u, 0u, d.rk0, d.rk1);
+            const uint32_t w0 = (t & 1u) ? x.z : x.x, w1 = (t & 1u) ? x.w : x.y;
+            const double hd_scale = d.q * (0.5 * TWO_PI_D) / s.a;
+            d.vec[n] = update_site_d<QHALF, ORMODE>(d.vec[n], up, dn, lf, rt, w0, w1, hd_scale, -1.0 / s.T, d.bc, d.bs, accepted);
+        }
+    }
+    if (count) {
+        const uint32_t n_acc = __popc(__ballot_sync(0xFFFFFFFFu, accepted));
+        if ((threadIdx.x & 31) == 0 && n_acc) atomicAdd(&d.state->accepted, (unsigned long long)n_acc);
+    }
+}
+
+// ---- a5: H = - sum over the colour-1 sites of v . h (every bond joins the two colours; Eq. 2) -------------
+__global__ void __launch_bounds__(E_THREADS) k64_energy(Dev64 d)
+{
+    __shared__ double warp_sum[E_THREADS / 32];
+    double sum = 0.0;
+    for (int r = blockIdx.x; r < d.rows; r += gridDim.x) {
+        double row = 0.0;
+        for (int c = ((r + 1) & 1) + 2 * (int)threadIdx.x; c < d.cols; c += 2 * E_THREADS) {
+            const uint32_t n = (uint32_t)r * d.cols + c;
+            const double2 v = d.vec[n];
+            double hx = 0.0, hy = 0.0;
+            if (r > 0) { hx += d.vec[n - d.cols].x; hy += d.vec[n - d.cols].y; }
+            if (r < d.rows - 1) { hx += d.vec[n + d.cols].x; hy += d.vec[n + d.cols].y; }
+            if (c > 0) { hx += d.vec[n - 1].x; hy += d.vec[n - 1].y; }
+            if (c < d.cols - 1) { hx += d.vec[n + 1].x; hy += d.vec[n + 1].y; }
+            row += fma(v.x, hx, v.y * hy);
+        }
+        sum += row;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+    if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < E_THREADS / 32; ++w) s += warp_sum[w];
+        d.partials[blockIdx.x] = -s;
+    }
+}
+
+__device__ __forceinline__ double sum_partials64(const Dev64& d, int n)      // one warp, fixed order
+{
+    double s = 0.0;
+    for (int b = threadIdx.x; b < n; b += 32) s += d.partials[b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+    return s;
+}
+__global__ void k64_energy_query(Dev64 d, int n_partials)
+{
+    const double H = sum_partials64(d, n_partials);
+    if (threadIdx.x == 0) d.state->e_query = H / d.n_bonds;
+}
+
+// ---- a6: Alg. 2 steps 5.2-5.5 (L195-206) after a counted sweep and its energy -----------------------------------
+__global__ void k64_controller(Dev64 d, int n_partials)
+{
+    State64& s = *d.state;
+    if (s.done) return;
+    const double H = sum_partials64(d, n_partials);
+    if (threadIdx.x != 0) return;
+    const uint32_t i = s.i;
+    const double A = (double)s.accepted / (double)s.n_free;
+    double a = s.a;
+    if (A < d.A_targ) a = 1.0 + (double)(i + 1u) / d.k_a;                 // 5.2
+    const double e = H / d.n_bonds;                                       // 5.3
+    s.e_ring[(i + 1u) % d.n_fit] = e;
+    double k = s.k;
+    if (i >= d.n_fit && i % d.n_f == 0) {                                 // 5.4: OLS slope of the last n_fit energies (R9)
+        const int n = (int)d.n_fit;
+        const double tbar = 0.5 * (double)(n - 1);
+        double ebar = 0.0;
+        for (int j = 0; j < n; ++j) ebar += s.e_ring[(i + 2u - d.n_fit + j) % d.n_fit];
+        ebar /= (double)n;
+        double num = 0.0, den = 0.0;
+        for (int j = 0; j < n; ++j) {
+            const double dt = (double)j - tbar;
+            num += dt * (s.e_ring[(i + 2u - d.n_fit + j) % d.n_fit] - ebar);
+            den += dt * dt;
+        }
+        k = num / den;
+    }
+    s.i = i + 1u; s.t += 1u; s.a = a; s.k = k; s.A_last = A; s.e_last = e; s.accepted = 0ull;     // 5.5
+    if (!(k < 0.0 && i + 1u < d.equil_cap)) { s.done = 1u; *d.done_flag = 1u; }
+}
+
+// ---- a7 / a8 ----------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k64_accumulate(Dev64 d)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N || is_fixed(d.bits, n)) return;
+    const double p = angle_of_d(d.vec[n], d.inv_q);
+    d.acc[n] += p; d.acc2[n] += p * p;
+}
+__global__ void __launch_bounds__(256) k64_predict(Dev64 d, double* __restrict__ out, int what)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N) return;
+    const State64& s = *d.state;
+    const double scale = (s.zmax - s.zmin) / TWO_PI_D, M = (double)s.realizations;
+    if (what == 0) {            // step 7: mean, back-transformed (L148, L212); sample sites = the input
+        out[n] = is_fixed(d.bits, n) ? d.values[n] : s.zmin + (d.acc[n] / M) * scale;
+    } else {                    // spread of the realizations: unbiased sample standard deviation
+        const double var = fmax((d.acc2[n] - d.acc[n] * d.acc[n] / M) / (M - 1.0), 0.0);
+        out[n] = is_fixed(d.bits, n) ? 0.0 : sqrt(var) * scale;
+    }
+}
+__global__ void __launch_bounds__(256) k64_export_angles(Dev64 d)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N || is_fixed(d.bits, n)) return;
+    d.phi[n] = angle_of_d(d.vec[n], d.inv_q);
+}
+__global__ void __launch_bounds__(256) k64_import_angles(Dev64 d, const double* __restrict__ phi_in)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= d.N || is_fixed(d.bits, n)) return;
+    double p = phi_in[n];
+    p = p < 0.0 ? 0.0 : p;
+    p = p > TWO_PI_D ? TWO_PI_D : p;
+    d.phi[n] = p;
+    double sn, cs;
+    sincos(__dmul_rn(d.q, p), &sn, &cs);
+    d.vec[n] = make_double2(cs, sn);
+}
+// scalar state edits: what = 0 begin a run at temperature x; 1 set a = x; 2 commit u sweeps (t += u) and v realizations;
+// 3 set t = u
+__global__ void k64_edit(Dev64 d, int what, double x, uint32_t u, uint32_t v)
+{
+    State64& s = *d.state;
+    if (what == 0) {
+        s.t = 0; s.done = 0; s.i = 0; s.realizations = 0; s.accepted = 0ull;
+        s.a = 1.0; s.k = -1.0; s.A_last = 0.0; s.e_last = 0.0; s.T = x; *d.done_flag = 0;
+    } else if (what == 1) { s.a = x; s.accepted = 0ull; }
+    else if (what == 2) { s.t += u; s.realizations += v; }
+    else if (what == 3) { s.t = u; }
+}
+
+}  // namespace mpr64

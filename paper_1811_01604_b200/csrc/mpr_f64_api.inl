@@ -1,0 +1,357 @@
+// mpr_f64_api.inl -- host controller and C ABI (include/mpr.h, "double-precision path") of the kernels in
+// mpr_f64.cuh.  Included at the end of mpr_api.cu (uses its CU / cuda_ok / align_up / cdiv helpers).
+
+namespace {
+
+struct Layout64 { size_t state, done, partials, values, phi, bits, vec, acc, acc2, total; };
+
+bool geometry64(int rows, int cols, uint32_t* N, uint32_t* words)
+{
+    if (rows < 2 || cols < 2 || rows > 65534 || cols > 65534) return false;
+    const uint64_t n = (uint64_t)rows * (uint64_t)cols;
+    if (n >= (1ull << 31)) return false;
+    *N = (uint32_t)n; *words = (uint32_t)((n + 31) / 32);
+    return true;
+}
+
+Layout64 make_layout64(uint32_t N, uint32_t words)
+{
+    Layout64 L;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    L.state    = take(sizeof(mpr64::State64));
+    L.done     = take(sizeof(uint32_t));
+    L.partials = take(sizeof(double) * 4 * mpr64::MM_BLOCKS);
+    L.values   = take(sizeof(double) * N);
+    L.phi      = take(sizeof(double) * N);
+    L.bits     = take(sizeof(uint32_t) * words);
+    L.vec      = take(sizeof(double2) * N);
+    L.acc      = take(sizeof(double) * N);
+    L.acc2     = take(sizeof(double) * N);
+    L.total = o;
+    return L;
+}
+
+}  // namespace
+
+struct mpr64_ctx {
+    mpr64::Dev64   d;
+    cudaStream_t   stream;
+    mpr_params     prm;
+    RunState       state;
+    int            device, energy_blocks, half;
+    uint64_t       launches;
+    uint32_t*      h_done;        // pinned
+    mpr64::State64 h_state;
+    bool           qhalf, dirty;
+};
+
+namespace {
+
+#define ENTER64(ctx) do { if (!cuda_ok(cudaSetDevice((ctx)->device), "cudaSetDevice")) return MPR_ERR_CUDA; } while (0)
+
+mpr_status fetch_state64(mpr64_ctx* ctx)
+{
+    CU(cudaMemcpyAsync(&ctx->h_state, ctx->d.state, sizeof(mpr64::State64), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MPR_OK;
+}
+
+typedef void (*half_kernel)(mpr64::Dev64, int, uint32_t, int, int);
+half_kernel pick_half_kernel(bool qhalf, int or_mode)
+{
+    using namespace mpr64;
+    if (qhalf) return or_mode == 0 ? k64_halfsweep<true, 0> : or_mode == 1 ? k64_halfsweep<true, 1> : k64_halfsweep<true, 2>;
+    return or_mode == 0 ? k64_halfsweep<false, 0> : k64_halfsweep<false, 2>;
+}
+
+// one sweep at sweep index state.t + t_off: colour 0 (the one holding the upper-left node), then colour 1 (L261-265)
+mpr_status launch_sweep64(mpr64_ctx* ctx, uint32_t t_off, int count)
+{
+    const half_kernel kern = pick_half_kernel(ctx->qhalf, (int)ctx->prm.or_mode);
+    const unsigned blocks = cdiv((size_t)ctx->d.rows * ctx->half, 256);
+    for (int colour = 0; colour < 2; ++colour) {
+        kern<<<blocks, 256, 0, ctx->stream>>>(ctx->d, colour, t_off, ctx->half, count);
+        CU_LAUNCH();
+    }
+    ctx->dirty = true;
+    return MPR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+mpr_status mpr64_query_workspace(int rows, int cols, size_t* bytes)
+{
+    uint32_t N, words;
+    if (!bytes || !geometry64(rows, cols, &N, &words)) return MPR_ERR_ARG;
+    *bytes = make_layout64(N, words).total;
+    return MPR_OK;
+}
+
+mpr_status mpr64_destroy(mpr64_ctx* ctx)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    if (ctx->h_done) cudaFreeHost(ctx->h_done);
+    delete ctx;
+    return MPR_OK;
+}
+
+mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_values, const uint8_t* d_sample_mask,
+                        void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    uint32_t N, words;
+    if (!out || !d_values || !d_sample_mask || !geometry64(rows, cols, &N, &words)) return MPR_ERR_ARG;
+    const Layout64 lay = make_layout64(N, words);
+    if (!d_workspace || workspace_bytes < lay.total || ((uintptr_t)d_workspace & 255u)) return MPR_ERR_WORKSPACE;
+    mpr64_ctx* ctx = new (std::nothrow) mpr64_ctx();
+    if (!ctx) return MPR_ERR_ARG;
+    memset(ctx, 0, sizeof *ctx);
+    ctx->stream = (cudaStream_t)cuda_stream;
+    {
+        cudaPointerAttributes attr;
+        if (!cuda_ok(cudaPointerGetAttributes(&attr, d_workspace), "cudaPointerGetAttributes") ||
+            attr.type != cudaMemoryTypeDevice) { delete ctx; return MPR_ERR_WORKSPACE; }
+        ctx->device = attr.device;
+        if (!cuda_ok(cudaSetDevice(ctx->device), "cudaSetDevice")) { delete ctx; return MPR_ERR_CUDA; }
+    }
+    ctx->state = CREATED;
+    char* base = (char*)d_workspace;
+    mpr64::Dev64& d = ctx->d;
+    d.state = (mpr64::State64*)(base + lay.state);
+    d.done_flag = (uint32_t*)(base + lay.done);
+    d.partials = (double*)(base + lay.partials);
+    d.values = (double*)(base + lay.values);
+    d.phi = (double*)(base + lay.phi);
+    d.bits = (uint32_t*)(base + lay.bits);
+    d.vec = (double2*)(base + lay.vec);
+    d.acc = (double*)(base + lay.acc);
+    d.acc2 = (double*)(base + lay.acc2);
+    d.rows = rows; d.cols = cols; d.N = N; d.words = words;
+    d.q = 0.5; d.inv_q = 2.0;
+    d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
+    ctx->half = (cols + 1) / 2;
+    ctx->energy_blocks = rows < mpr64::E_BLOCKS ? rows : mpr64::E_BLOCKS;
+    auto fail = [&](mpr_status s) { mpr64_destroy(ctx); return s; };
+    if (!cuda_ok(cudaMallocHost((void**)&ctx->h_done, sizeof(uint32_t)), "cudaMallocHost")) return fail(MPR_ERR_CUDA);
+    unsigned mm_blocks = cdiv(N, 256 * 8);
+    if (mm_blocks > (unsigned)mpr64::MM_BLOCKS) mm_blocks = mpr64::MM_BLOCKS;
+    mpr64::k64_minmax<<<mm_blocks, 256, 0, ctx->stream>>>(d, d_values, d_sample_mask);
+    mpr64::k64_minmax_finish<<<1, 1, 0, ctx->stream>>>(d, (int)mm_blocks);
+    mpr64::k64_transform<<<cdiv((size_t)words * 32, 256), 256, 0, ctx->stream>>>(d, d_values, d_sample_mask);
+    ctx->launches += 3;
+    if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
+    mpr_status st = fetch_state64(ctx);
+    if (st != MPR_OK) return fail(st);
+    const uint32_t e = ctx->h_state.err_flags;
+    if (e & mpr::ERRF_NO_SAMPLES) return fail(MPR_ERR_NO_SAMPLES);
+    if (e & mpr::ERRF_NONFINITE) return fail(MPR_ERR_NONFINITE);
+    if (e & mpr::ERRF_DEGENERATE) return fail(MPR_ERR_DEGENERATE_RANGE);
+    if (e & mpr::ERRF_NO_FREE) return fail(MPR_ERR_NO_FREE);
+    *out = ctx;
+    return MPR_OK;
+}
+
+mpr_status mpr64_set_params(mpr64_ctx* ctx, const mpr_params* p, double T)
+{
+    if (!ctx || !p || p->struct_size != sizeof(mpr_params)) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (!(p->q > 0.0f && p->q <= 0.5f) || p->M < 1 || p->sweeps_per_real < 1 || p->n_f < 1 ||
+        p->n_fit < 2 || p->n_fit > (uint32_t)mpr::MAX_NFIT || !(p->k_a > 0.0f) || !std::isfinite(p->A_targ) ||
+        p->or_mode > 2 || p->a_eq_mode > 1 || !(T > 0.0) || !std::isfinite(T))
+        return MPR_ERR_ARG;
+    if (p->or_mode == 1 && p->q != 0.5f) return MPR_ERR_UNSUPPORTED;
+    ctx->prm = *p;
+    ctx->qhalf = p->q == 0.5f;
+    mpr64::Dev64& d = ctx->d;
+    for (int r = 0; r < mpr::PHILOX_ROUNDS; ++r) {
+        d.rk0[r] = (uint32_t)p->seed + (uint32_t)r * 0x9E3779B9u;
+        d.rk1[r] = (uint32_t)(p->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
+    d.q = (double)p->q; d.inv_q = 1.0 / (double)p->q;
+    d.bc = cos(d.q * mpr64::TWO_PI_D); d.bs = sin(d.q * mpr64::TWO_PI_D);
+    d.n_f = p->n_f; d.n_fit = p->n_fit; d.equil_cap = p->equil_cap;
+    d.A_targ = (double)p->A_targ; d.k_a = (double)p->k_a;
+    mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(d, 0, T, 0u, 0u);
+    CU_LAUNCH();
+    CU(cudaMemsetAsync(d.acc, 0, sizeof(double) * d.N, ctx->stream));
+    CU(cudaMemsetAsync(d.acc2, 0, sizeof(double) * d.N, ctx->stream));
+    mpr64::k64_init_state<<<cdiv(d.N, 256), 256, 0, ctx->stream>>>(d);
+    CU_LAUNCH();
+    ctx->state = READY;
+    ctx->dirty = false;
+    return MPR_OK;
+}
+
+mpr_status mpr64_equilibrate(mpr64_ctx* ctx)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const mpr64::Dev64& d = ctx->d;
+    const uint32_t cap = ctx->prm.equil_cap;
+    uint32_t issued = 0, chunk = ctx->prm.n_fit + 1;       // the first slope check happens at i = n_fit (step 5.4)
+    while (issued < cap) {
+        if (chunk > cap - issued) chunk = cap - issued;
+        for (uint32_t j = 0; j < chunk; ++j) {
+            mpr_status s = launch_sweep64(ctx, 0, 1);       // 5.1, accepted proposals counted
+            if (s != MPR_OK) return s;
+            mpr64::k64_energy<<<ctx->energy_blocks, mpr64::E_THREADS, 0, ctx->stream>>>(d);      // 5.3
+            CU_LAUNCH();
+            mpr64::k64_controller<<<1, 32, 0, ctx->stream>>>(d, ctx->energy_blocks);             // 5.2, 5.4, 5.5
+            CU_LAUNCH();
+        }
+        issued += chunk;
+        CU(cudaMemcpyAsync(ctx->h_done, d.done_flag, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        if (*ctx->h_done) break;
+        chunk = ctx->prm.n_f;
+    }
+    return MPR_OK;
+}
+
+mpr_status mpr64_simulate(mpr64_ctx* ctx)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    const mpr64::Dev64& d = ctx->d;
+    if (ctx->prm.a_eq_mode == 1) { mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(d, 1, 1.0, 0u, 0u); CU_LAUNCH(); }
+    uint32_t t_off = 0;
+    for (uint32_t j = 0; j < ctx->prm.M; ++j) {
+        for (uint32_t w = 0; w < ctx->prm.sweeps_per_real; ++w, ++t_off) {
+            mpr_status s = launch_sweep64(ctx, t_off, 0);
+            if (s != MPR_OK) return s;
+        }
+        mpr64::k64_accumulate<<<cdiv(d.N, 256), 256, 0, ctx->stream>>>(d);          // step 6.3
+        CU_LAUNCH();
+    }
+    mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(d, 2, 0.0, t_off, ctx->prm.M);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr64_predict(mpr64_ctx* ctx, double* d_out)
+{
+    if (!ctx || !d_out) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr64::k64_predict<<<cdiv(ctx->d.N, 256), 256, 0, ctx->stream>>>(ctx->d, d_out, 0);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr64_predict_std(mpr64_ctx* ctx, double* d_out)
+{
+    if (!ctx || !d_out) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr_status s = fetch_state64(ctx);
+    if (s != MPR_OK) return s;
+    if (ctx->h_state.realizations < 2u) return MPR_ERR_STATE;
+    mpr64::k64_predict<<<cdiv(ctx->d.N, 256), 256, 0, ctx->stream>>>(ctx->d, d_out, 1);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr64_get_angles(mpr64_ctx* ctx, double* d_phi)
+{
+    if (!ctx || !d_phi) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    if (ctx->dirty) {
+        mpr64::k64_export_angles<<<cdiv(ctx->d.N, 256), 256, 0, ctx->stream>>>(ctx->d);
+        CU_LAUNCH();
+        ctx->dirty = false;
+    }
+    CU(cudaMemcpyAsync(d_phi, ctx->d.phi, sizeof(double) * ctx->d.N, cudaMemcpyDeviceToDevice, ctx->stream));
+    return MPR_OK;
+}
+
+mpr_status mpr64_set_angles(mpr64_ctx* ctx, const double* d_phi)
+{
+    if (!ctx || !d_phi) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr64::k64_import_angles<<<cdiv(ctx->d.N, 256), 256, 0, ctx->stream>>>(ctx->d, d_phi);
+    CU_LAUNCH();
+    ctx->dirty = false;
+    return MPR_OK;
+}
+
+mpr_status mpr64_set_sweep_index(mpr64_ctx* ctx, uint32_t t)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(ctx->d, 3, 0.0, t, 0u);
+    CU_LAUNCH();
+    return MPR_OK;
+}
+
+mpr_status mpr64_sweep(mpr64_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_accepted)
+{
+    if (!ctx || !(a >= 1.0) || !std::isfinite(a)) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(ctx->d, 1, a, 0u, 0u);        // also zeroes the accepted counter
+    CU_LAUNCH();
+    for (uint32_t w = 0; w < n_sweeps; ++w) {
+        mpr_status s = launch_sweep64(ctx, w, h_accepted ? 1 : 0);
+        if (s != MPR_OK) return s;
+    }
+    mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(ctx->d, 2, 0.0, n_sweeps, 0u);
+    CU_LAUNCH();
+    if (h_accepted) {
+        mpr_status s = fetch_state64(ctx);
+        if (s != MPR_OK) return s;
+        *h_accepted = ctx->h_state.accepted;
+    }
+    return MPR_OK;
+}
+
+mpr_status mpr64_energy(mpr64_ctx* ctx, double* h_e)
+{
+    if (!ctx || !h_e) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    if (ctx->state != READY) return MPR_ERR_STATE;
+    mpr64::k64_energy<<<ctx->energy_blocks, mpr64::E_THREADS, 0, ctx->stream>>>(ctx->d);
+    CU_LAUNCH();
+    mpr64::k64_energy_query<<<1, 32, 0, ctx->stream>>>(ctx->d, ctx->energy_blocks);
+    CU_LAUNCH();
+    mpr_status s = fetch_state64(ctx);
+    if (s != MPR_OK) return s;
+    *h_e = ctx->h_state.e_query;
+    return MPR_OK;
+}
+
+mpr_status mpr64_get_transform(mpr64_ctx* ctx, double* h_zmin, double* h_zmax)
+{
+    if (!ctx || !h_zmin || !h_zmax) return MPR_ERR_ARG;
+    *h_zmin = ctx->h_state.zmin; *h_zmax = ctx->h_state.zmax;      // fixed since mpr64_create, which fetched them
+    return MPR_OK;
+}
+
+mpr_status mpr64_get_stats(mpr64_ctx* ctx, mpr_stats* o)
+{
+    if (!ctx || !o) return MPR_ERR_ARG;
+    ENTER64(ctx);
+    mpr_status s = fetch_state64(ctx);
+    if (s != MPR_OK) return s;
+    const mpr64::State64& g = ctx->h_state;
+    o->equil_sweeps = g.i; o->t = g.t; o->equilibrated = g.done; o->realizations = g.realizations;
+    o->n_free = g.n_free; o->n_samples = g.n_samples; o->n_bonds = (uint64_t)ctx->d.n_bonds;
+    o->a = g.a; o->k = g.k; o->A_last = g.A_last; o->e_last = g.e_last;
+    o->z_min = (float)g.zmin; o->z_max = (float)g.zmax;
+    return MPR_OK;
+}
+
+mpr_status mpr64_get_launch_count(mpr64_ctx* ctx, uint64_t* h_count)
+{
+    if (!ctx || !h_count) return MPR_ERR_ARG;
+    *h_count = ctx->launches;
+    return MPR_OK;
+}
+
+}  // extern "C"

@@ -34,6 +34,9 @@ EXPORTS = (
     "mpr_sample_energy", "mpr_create_unconditional", "mpr_measure_energy", "mpr_energy_table",
     "mpr_infer_temperature", "mpr_predict_std", "mpr_query_workspace_chains", "mpr_create_chains",
     "mpr_predict_quantile",
+    "mpr64_query_workspace", "mpr64_create", "mpr64_set_params", "mpr64_equilibrate", "mpr64_simulate", "mpr64_predict",
+    "mpr64_predict_std", "mpr64_destroy", "mpr64_get_angles", "mpr64_set_angles", "mpr64_set_sweep_index", "mpr64_sweep",
+    "mpr64_energy", "mpr64_get_transform", "mpr64_get_stats", "mpr64_get_launch_count",
 )
 
 
@@ -103,6 +106,19 @@ def lib():
                                        C.POINTER(C.c_double)]
         L.mpr_infer_temperature.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_double), i, C.c_double,
                                             C.POINTER(C.c_double)]
+        L.mpr64_query_workspace.argtypes = [i, i, C.POINTER(sz)]
+        L.mpr64_create.argtypes = [C.POINTER(vp), i, i, vp, vp, vp, sz, vp]
+        L.mpr64_set_params.argtypes = [vp, C.POINTER(mpr_params), C.c_double]
+        for name in ("mpr64_equilibrate", "mpr64_simulate", "mpr64_destroy"):
+            getattr(L, name).argtypes = [vp]
+        for name in ("mpr64_predict", "mpr64_predict_std", "mpr64_get_angles", "mpr64_set_angles"):
+            getattr(L, name).argtypes = [vp, vp]
+        L.mpr64_set_sweep_index.argtypes = [vp, u32]
+        L.mpr64_sweep.argtypes = [vp, u32, C.c_double, C.POINTER(u64)]
+        L.mpr64_energy.argtypes = [vp, C.POINTER(C.c_double)]
+        L.mpr64_get_transform.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.mpr64_get_stats.argtypes = [vp, C.POINTER(mpr_stats)]
+        L.mpr64_get_launch_count.argtypes = [vp, C.POINTER(u64)]
         for name in EXPORTS:
             getattr(L, name).restype = C.c_int
         L.mpr_default_params.restype = None
@@ -329,6 +345,118 @@ class Mpr:
     def launch_count(self) -> int:
         n = C.c_uint64()
         _check(lib().mpr_get_launch_count(self._ctx, C.byref(n)), "mpr_get_launch_count")
+        return int(n.value)
+
+
+class Mpr64:
+    """The double-precision path (mpr64_* calls): one grid of rows x cols.
+
+    values: float64 CUDA tensor [rows, cols]; sample_mask: uint8 CUDA tensor of the same shape, 1 = sample (fixed).
+    """
+
+    def __init__(self, values, sample_mask, stream=None):
+        import torch
+        if not values.is_cuda or not sample_mask.is_cuda:
+            raise ValueError("values and sample_mask must be CUDA tensors (there is no CPU path)")
+        if values.dtype != torch.float64 or sample_mask.dtype != torch.uint8 or values.shape != sample_mask.shape or values.dim() != 2:
+            raise ValueError("values float64 and sample_mask uint8 of the same [rows, cols] shape")
+        values, sample_mask = values.contiguous(), sample_mask.contiguous()
+        self.device = values.device
+        self.rows, self.cols = (int(x) for x in values.shape)
+        self._torch = torch
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        n = C.c_size_t()
+        _check(lib().mpr64_query_workspace(self.rows, self.cols, C.byref(n)), "mpr64_query_workspace")
+        self.workspace = torch.empty(int(n.value), dtype=torch.uint8, device=self.device)
+        self._ctx = C.c_void_p()
+        _check(lib().mpr64_create(C.byref(self._ctx), self.rows, self.cols, values.data_ptr(), sample_mask.data_ptr(),
+                                  self.workspace.data_ptr(), int(n.value), self._stream.cuda_stream), "mpr64_create")
+        self.params = None
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self._stream.synchronize()
+            lib().mpr64_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_params(self, T, params: mpr_params | None = None, **overrides):
+        p = params if params is not None else default_params(**overrides)
+        if params is not None:
+            for k, v in overrides.items():
+                setattr(p, k, v)
+        _check(lib().mpr64_set_params(self._ctx, C.byref(p), float(T)), "mpr64_set_params")
+        self.params = p
+        return self
+
+    def equilibrate(self):
+        _check(lib().mpr64_equilibrate(self._ctx), "mpr64_equilibrate")
+        return self
+
+    def simulate(self):
+        _check(lib().mpr64_simulate(self._ctx), "mpr64_simulate")
+        return self
+
+    def _out(self, out):
+        return out if out is not None else self._torch.empty((self.rows, self.cols), dtype=self._torch.float64, device=self.device)
+
+    def predict(self, out=None):
+        out = self._out(out)
+        _check(lib().mpr64_predict(self._ctx, out.data_ptr()), "mpr64_predict")
+        return out
+
+    def predict_std(self, out=None):
+        out = self._out(out)
+        _check(lib().mpr64_predict_std(self._ctx, out.data_ptr()), "mpr64_predict_std")
+        return out
+
+    def get_angles(self, out=None):
+        out = self._out(out)
+        _check(lib().mpr64_get_angles(self._ctx, out.data_ptr()), "mpr64_get_angles")
+        return out
+
+    def set_angles(self, phi):
+        phi = phi.to(device=self.device, dtype=self._torch.float64).reshape(self.rows, self.cols).contiguous()
+        _check(lib().mpr64_set_angles(self._ctx, phi.data_ptr()), "mpr64_set_angles")
+        self._stream.synchronize()          # phi may be a temporary
+        return self
+
+    def set_sweep_index(self, t: int):
+        _check(lib().mpr64_set_sweep_index(self._ctx, int(t)), "mpr64_set_sweep_index")
+        return self
+
+    def sweep(self, n_sweeps: int, a: float, count: bool = False):
+        if count:
+            acc = C.c_uint64()
+            _check(lib().mpr64_sweep(self._ctx, int(n_sweeps), float(a), C.byref(acc)), "mpr64_sweep")
+            return int(acc.value)
+        _check(lib().mpr64_sweep(self._ctx, int(n_sweeps), float(a), None), "mpr64_sweep")
+        return None
+
+    def energy(self) -> float:
+        e = C.c_double()
+        _check(lib().mpr64_energy(self._ctx, C.byref(e)), "mpr64_energy")
+        return float(e.value)
+
+    def get_transform(self):
+        lo, hi = C.c_double(), C.c_double()
+        _check(lib().mpr64_get_transform(self._ctx, C.byref(lo), C.byref(hi)), "mpr64_get_transform")
+        return float(lo.value), float(hi.value)
+
+    def get_stats(self) -> Stats:
+        s = mpr_stats()
+        _check(lib().mpr64_get_stats(self._ctx, C.byref(s)), "mpr64_get_stats")
+        return Stats(s.equil_sweeps, s.t, bool(s.equilibrated), s.realizations, s.n_free, s.n_samples,
+                     s.n_bonds, s.a, s.k, s.A_last, s.e_last, s.z_min, s.z_max)
+
+    def launch_count(self) -> int:
+        n = C.c_uint64()
+        _check(lib().mpr64_get_launch_count(self._ctx, C.byref(n)), "mpr64_get_launch_count")
         return int(n.value)
 
 

@@ -23,7 +23,7 @@ def lib():
 def _declared_symbols():
     text = open(os.path.join(ROOT, "include", "mpr.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(mpr_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(mpr(?:64)?_[a-z_]+)\s*\(", text)))
 
 
 def test_every_declared_symbol_is_exported(lib):
