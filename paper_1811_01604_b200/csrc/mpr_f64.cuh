@@ -4,7 +4,9 @@
 //
 // State: v_i = (cos q phi_i, sin q phi_i) as double2, row-major [rows][cols], updated IN PLACE: the sites of one
 // colour depend only on the other colour, so a half-sweep is one kernel with one thread per
-// lattice site of that colour, as in the paper's own design (L261-267).  Why not the fp32 path's shared-memory tile
+// PREDICTION site of that colour (the paper's own design, L261-267, gives every lattice site a thread and lets those
+// of the sample sites idle; here the prediction sites of each colour are listed once, in row-major order, so that
+// every lane of a warp has an update to do).  Why not the fp32 path's shared-memory tile
 // pass: in double the update is bound by the fp64 pipe (one division, exp and sincos per update, ~250 DP instructions
 // against ~445 MB of state traffic per 4096^2 sweep = 69 us at the measured HBM peak), so temporal blocking has no
 // bytes to win back; DESIGN.md section 13.  One grid per context.
@@ -30,6 +32,7 @@ constexpr int    MM_BLOCKS = 592;
 struct State64 {
     uint32_t t, done, i, realizations;
     uint32_t n_samples, n_free, err_flags, pad;
+    uint32_t n_colour[2];     // prediction sites per colour = lengths of the two site lists
     unsigned long long accepted;
     double   a, k, A_last, e_last, T, zmin, zmax, e_query;
     double   e_ring[MAX_NFIT];
@@ -42,6 +45,9 @@ struct Dev64 {
     double*   values;         // [N] verbatim copy of the input
     double*   phi;            // [N] Eq. 1 at the sample sites; export buffer at the prediction sites
     uint32_t* bits;           // [words] fixed-site bitmask
+    uint32_t* list;           // [n_colour[0]] then [n_colour[1]]: the prediction sites of colour 0, then of colour 1, ascending
+    uint32_t* list_counts;    // [2][list_blocks] prediction sites per colour of each block of 32 * LIST_THREADS sites
+    uint32_t  list_blocks;
     double2*  vec;            // [N] unit vectors
     double*   acc;            // [N] sum over the realizations of phi
     double*   acc2;           // [N] sum of phi^2 (spread, L212)
@@ -144,6 +150,74 @@ __global__ void __launch_bounds__(256) k64_transform(Dev64 d, const double* __re
     if ((threadIdx.x & 31) == 0 && (n >> 5) < d.words) d.bits[n >> 5] = b;
 }
 
+// The checkerboard split (L261) as two lists of prediction sites.  A thread takes one word of the bitmask (32 sites);
+// k64_list_count leaves the per-block counts, k64_list_scan turns them into offsets, k64_list_fill writes the sites.
+constexpr int LIST_THREADS = 256;
+__device__ __forceinline__ void word_free_masks(const Dev64& d, uint32_t w, uint32_t& f0, uint32_t& f1)
+{
+    f0 = f1 = 0u;
+    if (w >= d.words) return;
+    const uint32_t fixed = d.bits[w];
+    for (uint32_t b = 0; b < 32u; ++b) {
+        const uint32_t n = 32u * w + b;
+        if (n >= d.N || ((fixed >> b) & 1u)) continue;
+        const uint32_t r = n / (uint32_t)d.cols;
+        (((r + (n - r * (uint32_t)d.cols)) & 1u) ? f1 : f0) |= 1u << b;
+    }
+}
+// exclusive scan of (x0, x1) over the block's threads; totals returned through t0, t1
+__device__ __forceinline__ void block_scan2(uint32_t& x0, uint32_t& x1, uint32_t& t0, uint32_t& t1)
+{
+    __shared__ uint32_t w0[LIST_THREADS / 32], w1[LIST_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t i0 = x0, i1 = x1;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, i0, o), b = __shfl_up_sync(0xFFFFFFFFu, i1, o);
+        if (lane >= o) { i0 += a; i1 += b; }
+    }
+    if (lane == 31) { w0[warp] = i0; w1[warp] = i1; }
+    __syncthreads();
+    uint32_t b0 = 0, b1 = 0, s0 = 0, s1 = 0;
+    for (int k = 0; k < LIST_THREADS / 32; ++k) {
+        if (k < warp) { b0 += w0[k]; b1 += w1[k]; }
+        s0 += w0[k]; s1 += w1[k];
+    }
+    x0 = b0 + i0 - x0; x1 = b1 + i1 - x1; t0 = s0; t1 = s1;
+}
+__global__ void __launch_bounds__(LIST_THREADS) k64_list_count(Dev64 d)
+{
+    uint32_t f0, f1, t0, t1;
+    word_free_masks(d, blockIdx.x * LIST_THREADS + threadIdx.x, f0, f1);
+    uint32_t c0 = __popc(f0), c1 = __popc(f1);
+    block_scan2(c0, c1, t0, t1);
+    if (threadIdx.x == 0) { d.list_counts[blockIdx.x] = t0; d.list_counts[d.list_blocks + blockIdx.x] = t1; }
+}
+__global__ void k64_list_scan(Dev64 d)          // one thread: list_blocks <= 2^31 / 8192 additions
+{
+    uint32_t run = 0;
+    for (int c = 0; c < 2; ++c) {
+        const uint32_t start = run;
+        for (uint32_t b = 0; b < d.list_blocks; ++b) {
+            const uint32_t n = d.list_counts[c * d.list_blocks + b];
+            d.list_counts[c * d.list_blocks + b] = run;
+            run += n;
+        }
+        d.state->n_colour[c] = run - start;
+    }
+}
+__global__ void __launch_bounds__(LIST_THREADS) k64_list_fill(Dev64 d)
+{
+    uint32_t f0, f1, t0, t1;
+    const uint32_t w = blockIdx.x * LIST_THREADS + threadIdx.x;
+    word_free_masks(d, w, f0, f1);
+    uint32_t o0 = __popc(f0), o1 = __popc(f1);
+    block_scan2(o0, o1, t0, t1);
+    o0 += d.list_counts[blockIdx.x]; o1 += d.list_counts[d.list_blocks + blockIdx.x];
+    for (; f0; f0 &= f0 - 1u) d.list[o0++] = 32u * w + (uint32_t)(__ffs(f0) - 1);
+    for (; f1; f1 &= f1 - 1u) d.list[o1++] = 32u * w + (uint32_t)(__ffs(f1) - 1);
+}
+
 // Alg. 2 step 2.2 (L176): prediction sites ~ U(0, 2 pi) from the INIT stream; unit vectors of every site
 __global__ void __launch_bounds__(256) k64_init_state(Dev64 d)
 {
@@ -220,17 +294,17 @@ __device__ __forceinline__ double2 update_site_d(double2 v, double2 n_up, double
     return make_double2(accepted ? rx : px, accepted ? ry : py);
 }
 
-// One colour of one sweep (L261-265): one thread per lattice site of the colour, in place.  half = ceil(cols / 2).
+// One colour of one sweep (L261-265): one thread per prediction site of the colour (sites[0 .. n_sites)), in place.
 template <bool QHALF, int ORMODE>
-__global__ void __launch_bounds__(256) k64_halfsweep(Dev64 d, int colour, uint32_t t_off, int half, int count)
+__global__ void __launch_bounds__(256) k64_halfsweep(Dev64 d, const uint32_t* __restrict__ sites, uint32_t n_sites,
+                                                     uint32_t t_off, int count)
 {
     const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
-    const int r = (int)(idx / (uint32_t)half);
-    const int c = 2 * (int)(idx - (uint32_t)r * (uint32_t)half) + ((r + colour) & 1);
     bool accepted = false;
-    if (r < d.rows && c < d.cols) {
-        const uint32_t n = (uint32_t)r * d.cols + c;
-        if (!is_fixed(d.bits, n)) {
+    if (idx < n_sites) {
+        const uint32_t n = sites[idx];
+        const int r = (int)(n / (uint32_t)d.cols), c = (int)(n - (uint32_t)r * (uint32_t)d.cols);
+        {
             const State64& s = *d.state;
             const uint32_t t = s.t + t_off;
             const double2 zero = make_double2(0.0, 0.0);                 // open boundary (L109)

@@ -3,7 +3,7 @@
 
 namespace {
 
-struct Layout64 { size_t state, done, partials, values, phi, bits, vec, acc, acc2, total; };
+struct Layout64 { size_t state, done, partials, values, phi, bits, list, list_counts, vec, acc, acc2, total; };
 
 bool geometry64(int rows, int cols, uint32_t* N, uint32_t* words)
 {
@@ -25,6 +25,8 @@ Layout64 make_layout64(uint32_t N, uint32_t words)
     L.values   = take(sizeof(double) * N);
     L.phi      = take(sizeof(double) * N);
     L.bits     = take(sizeof(uint32_t) * words);
+    L.list     = take(sizeof(uint32_t) * N);
+    L.list_counts = take(sizeof(uint32_t) * 2 * cdiv(words, mpr64::LIST_THREADS));
     L.vec      = take(sizeof(double2) * N);
     L.acc      = take(sizeof(double) * N);
     L.acc2     = take(sizeof(double) * N);
@@ -39,7 +41,8 @@ struct mpr64_ctx {
     cudaStream_t   stream;
     mpr_params     prm;
     RunState       state;
-    int            device, energy_blocks, half;
+    int            device, energy_blocks;
+    uint32_t       n_colour[2];   // prediction sites per colour (lengths of the site lists)
     uint64_t       launches;
     uint32_t*      h_done;        // pinned
     mpr64::State64 h_state;
@@ -57,7 +60,7 @@ mpr_status fetch_state64(mpr64_ctx* ctx)
     return MPR_OK;
 }
 
-typedef void (*half_kernel)(mpr64::Dev64, int, uint32_t, int, int);
+typedef void (*half_kernel)(mpr64::Dev64, const uint32_t*, uint32_t, uint32_t, int);
 half_kernel pick_half_kernel(bool qhalf, int or_mode)
 {
     using namespace mpr64;
@@ -69,10 +72,13 @@ half_kernel pick_half_kernel(bool qhalf, int or_mode)
 mpr_status launch_sweep64(mpr64_ctx* ctx, uint32_t t_off, int count)
 {
     const half_kernel kern = pick_half_kernel(ctx->qhalf, (int)ctx->prm.or_mode);
-    const unsigned blocks = cdiv((size_t)ctx->d.rows * ctx->half, 256);
+    const uint32_t* sites = ctx->d.list;
     for (int colour = 0; colour < 2; ++colour) {
-        kern<<<blocks, 256, 0, ctx->stream>>>(ctx->d, colour, t_off, ctx->half, count);
-        CU_LAUNCH();
+        if (ctx->n_colour[colour]) {
+            kern<<<cdiv(ctx->n_colour[colour], 256), 256, 0, ctx->stream>>>(ctx->d, sites, ctx->n_colour[colour], t_off, count);
+            CU_LAUNCH();
+        }
+        sites += ctx->n_colour[colour];
     }
     ctx->dirty = true;
     return MPR_OK;
@@ -125,13 +131,15 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
     d.values = (double*)(base + lay.values);
     d.phi = (double*)(base + lay.phi);
     d.bits = (uint32_t*)(base + lay.bits);
+    d.list = (uint32_t*)(base + lay.list);
+    d.list_counts = (uint32_t*)(base + lay.list_counts);
+    d.list_blocks = cdiv(words, mpr64::LIST_THREADS);
     d.vec = (double2*)(base + lay.vec);
     d.acc = (double*)(base + lay.acc);
     d.acc2 = (double*)(base + lay.acc2);
     d.rows = rows; d.cols = cols; d.N = N; d.words = words;
     d.q = 0.5; d.inv_q = 2.0;
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
-    ctx->half = (cols + 1) / 2;
     ctx->energy_blocks = rows < mpr64::E_BLOCKS ? rows : mpr64::E_BLOCKS;
     auto fail = [&](mpr_status s) { mpr64_destroy(ctx); return s; };
     if (!cuda_ok(cudaMallocHost((void**)&ctx->h_done, sizeof(uint32_t)), "cudaMallocHost")) return fail(MPR_ERR_CUDA);
@@ -140,7 +148,10 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
     mpr64::k64_minmax<<<mm_blocks, 256, 0, ctx->stream>>>(d, d_values, d_sample_mask);
     mpr64::k64_minmax_finish<<<1, 1, 0, ctx->stream>>>(d, (int)mm_blocks);
     mpr64::k64_transform<<<cdiv((size_t)words * 32, 256), 256, 0, ctx->stream>>>(d, d_values, d_sample_mask);
-    ctx->launches += 3;
+    mpr64::k64_list_count<<<d.list_blocks, mpr64::LIST_THREADS, 0, ctx->stream>>>(d);
+    mpr64::k64_list_scan<<<1, 1, 0, ctx->stream>>>(d);
+    mpr64::k64_list_fill<<<d.list_blocks, mpr64::LIST_THREADS, 0, ctx->stream>>>(d);
+    ctx->launches += 6;
     if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
     mpr_status st = fetch_state64(ctx);
     if (st != MPR_OK) return fail(st);
@@ -149,6 +160,7 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
     if (e & mpr::ERRF_NONFINITE) return fail(MPR_ERR_NONFINITE);
     if (e & mpr::ERRF_DEGENERATE) return fail(MPR_ERR_DEGENERATE_RANGE);
     if (e & mpr::ERRF_NO_FREE) return fail(MPR_ERR_NO_FREE);
+    ctx->n_colour[0] = ctx->h_state.n_colour[0]; ctx->n_colour[1] = ctx->h_state.n_colour[1];
     *out = ctx;
     return MPR_OK;
 }
