@@ -46,6 +46,8 @@ def parse_args():
                     help="chains per grid in step 6 (DESIGN.md reading R25); 1 = the paper's single chain")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-inference", action="store_true", help="skip the Alg. 2 step 4 timing (extra key, not in the step)")
+    ap.add_argument("--no-f64", action="store_true",
+                    help="skip the double-precision run of the same workload (extra key 'double_precision', not in the step)")
     return ap.parse_args()
 
 
@@ -321,6 +323,37 @@ def run_b200(args, w):
                      "T_hat": mpr.infer_temperature(ladder, table, e_s[0]), "T_closed_form_R15": T_cf,
                      "ms_sample_energy": ev[0].elapsed_time(ev[1]), "ms_energy_table": ev[1].elapsed_time(ev[2]),
                      "table": f"5 unconditional {w.rows}x{w.cols} chains, 500 burn-in + 100 measured sweeps each"}
+    # The paper's DP / SP study (Table 2 against Table 3) on this workload: the whole path once in double
+    # (mpr64_* calls, grid 0) beside one fp32 pass, with the validation measures of both against the withheld truth
+    f64 = None
+    if not args.no_f64 and world == 1:
+        from paper_1811_01604_b200 import synth as _synth
+        z64 = torch.from_numpy(w.truth[0].astype(np.float64)).to(dev)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        ev[0].record(stream)
+        c64 = mpr.Mpr64(z64, d_mask[0])
+        c64.set_params(T[0], **prm).equilibrate().simulate()
+        pred64 = c64.predict()
+        ev[1].record(stream)
+        st64 = c64.get_stats()
+        c64.sweep(4, st64.a)
+        ev[2].record(stream)
+        c64.sweep(32, st64.a)
+        ev[3].record(stream)
+        ev[3].synchronize()
+        c32 = mpr.Mpr(d_values[:1], d_mask[:1])
+        c32.set_params(T[:1], **prm).equilibrate().simulate()
+        v32 = _synth.validation_measures(w.truth[0], c32.predict().cpu().numpy()[0], w.mask[0])
+        v64 = _synth.validation_measures(w.truth[0].astype(np.float64), pred64.cpu().numpy(), w.mask[0])
+        sweeps64 = st64.equil_sweeps + st64.realizations * w.sweeps_per_real
+        f64 = {"ms_per_grid": ev[0].elapsed_time(ev[1]), "equil_sweeps": st64.equil_sweeps,
+               "gupdates_per_s": st64.n_free * sweeps64 / ev[0].elapsed_time(ev[1]) / 1e6,
+               "us_per_sweep": ev[2].elapsed_time(ev[3]) / 32 * 1e3, "us_per_sweep_f32": sweep_s * 1e6,
+               "dp_over_sp_sweep_time": ev[2].elapsed_time(ev[3]) / 32 / 1e3 / sweep_s,
+               "mae_f64": v64["mae"], "mae_f32": v32["mae"], "rmse_f64": v64["rmse"], "rmse_f32": v32["rmse"],
+               "paper_context": "paper (L305-321): DP 5.1 x slower than SP on a GTX 980, validation measures equal to 3 decimals"}
+        c64.close(); c32.close()
+        del z64, pred64
     N_sites = w.rows * w.cols * w.batch
     P_sites = sum(s.n_free for s in st)
     equil_sweeps = [s.equil_sweeps for s in st]
@@ -372,6 +405,8 @@ def run_b200(args, w):
         }
         if inference is not None:
             out["temperature_inference"] = inference
+        if f64 is not None:
+            out["double_precision"] = f64
         if not args.no_cpu_baseline and world == 1:
             n_sweeps = oracle_sweeps_for(w)
             rate, dt, cores = oracle_sample(w, n_sweeps)

@@ -6,10 +6,11 @@
 // colour depend only on the other colour, so a half-sweep is one kernel with one thread per
 // PREDICTION site of that colour (the paper's own design, L261-267, gives every lattice site a thread and lets those
 // of the sample sites idle; here the prediction sites of each colour are listed once, in row-major order, so that
-// every lane of a warp has an update to do).  Why not the fp32 path's shared-memory tile
-// pass: in double the update is bound by the fp64 pipe (one division, exp and sincos per update, ~250 DP instructions
-// against ~445 MB of state traffic per 4096^2 sweep = 69 us at the measured HBM peak), so temporal blocking has no
-// bytes to win back; DESIGN.md section 13.  One grid per context.
+// every lane of a warp has an update to do).  Measured on cfg4 (profiles/r01h): 70 us per half-sweep, 346 MB of DRAM
+// traffic = 4.9 TB/s = 0.76 of the measured HBM peak, fp64 pipe 22 %: this kernel is bound by bytes (a 32-byte sector
+// of the row-major double2 state holds one site of each colour, so every half-sweep streams the whole state).  The
+// fp32 path's shared-memory tile pass (K sweeps per load) is what would lift it; not built for double yet
+// (DESIGN.md section 12).  One grid per context.
 #pragma once
 #include "mpr_device.cuh"
 
