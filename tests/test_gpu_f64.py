@@ -213,3 +213,22 @@ def test_error_statuses(torch_cuda, mpr):
         ctx.predict_std()
     assert e.value.name == "MPR_ERR_STATE"
     ctx.close()
+
+
+def test_t2_full_size_cfg4_and_cfg3_one_sweep(torch_cuda, mpr, orc64):
+    """BASELINE configs[3] (4096 x 4096, 33 % removed) and configs[2] (1024 x 1024 with 64 x 64 holes) at full size, in
+    the launch configuration bench.py's double_precision key times.  Generator-made near-equilibrium states (the truth
+    field's own angles plus thermal-size noise at the prediction sites), as in the fp32 test of the same sizes."""
+    torch = torch_cuda
+    for name, a in (("cfg4", 40.0), ("cfg3", 6.0)):
+        w = synth.make_workload(name)
+        z, m, T = w.truth[0].astype(np.float64), w.mask[0], float(w.T[0])
+        zmin, zmax, _ = orc64.minmax(z, m)
+        rng = np.random.default_rng(8)
+        phi = ((z - zmin) / (zmax - zmin) * TWO_PI + math.sqrt(T) * rng.standard_normal(z.shape)).clip(0.0, TWO_PI)
+        ref0, _, _ = orc64.transform(z, m, w.seed)
+        phi[m == 1] = ref0[m == 1]
+        ctx = mpr.Mpr64(_dev(torch, z), _dev(torch, m))
+        ctx.set_params(T, seed=w.seed)
+        _one_sweep(orc64, ctx, phi, m, 0.5, T, a, w.seed, 123, 0)
+        ctx.close()
