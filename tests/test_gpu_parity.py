@@ -655,3 +655,43 @@ def test_chains_full_run_cfg1_and_one_chain_is_the_plain_context(torch_cuda, mpr
         c.set_params(T, seed=5, equil_cap=200, sweeps_per_real=3, M=5).equilibrate().simulate()
         outs.append(c.predict().cpu().numpy()); c.close()
     assert np.array_equal(outs[0], outs[1])
+
+
+# ---------------------------------------------------------------------------
+# the paper's own workload and numbers (Table 3) on the CUDA path
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("col,p_removed", [(0, 0.33), (1, 0.66)])
+def test_paper_table3_validation_measures_on_the_gpu(torch_cuda, mpr, col, p_removed):
+    """The CUDA path on the paper's workload at the paper's size -- Z ~ N(50, 10), exponential covariance kappa = 0.2
+    (exact, circulant embedding), L = 1024, 33 % / 66 % removed, M = 100, one sweep per realization, the defaults of
+    reading R7 -- against the validation measures the paper prints (tests/golden/paper_table3_validation.txt).  No oracle
+    is involved: this pins the product to the paper directly.  Means over 4 fields; +-2.5 % covers the field-to-field
+    spread (the same tolerance as the oracle's pin in test_oracle_paper_workload.py).  Also run with Eq. 6 as printed
+    (or_mode = 1): on this low-contrast data both reflections give the same measures."""
+    import os
+    torch = torch_cuda
+    gold = {}
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_table3_validation.txt")) as f:
+        for line in f:
+            if not line.startswith("#") and line.strip():
+                name, p33, p66 = line.split()
+                gold[name] = (float(p33), float(p66))
+    L = 1024
+    res = {0: [], 1: []}
+    for k in range(4):
+        truth = synth.grf(L, L, 5.0, "exponential", 1009 + k, mean=50.0, sigma=10.0)
+        mask = synth.bernoulli_mask(L, L, p_removed, 2009 + 10 * k + col)
+        T = synth.choose_T(truth, mask)
+        ctx = mpr.Mpr(_dev(torch, truth), _dev(torch, mask))
+        for or_mode in (0, 1):
+            ctx.set_params(T, seed=3009 + k, M=100, sweeps_per_real=1, equil_cap=500, or_mode=or_mode).equilibrate().simulate()
+            assert ctx.get_stats()[0].equil_sweeps < 500
+            vm = synth.validation_measures(truth, ctx.predict().cpu().numpy()[0], mask)
+            res[or_mode].append((vm["mae"], vm["rmse"], vm["are_pct"], vm["aare_pct"]))
+        ctx.close()
+    m0, m1 = np.mean(res[0], axis=0), np.mean(res[1], axis=0)
+    assert m0[0] == pytest.approx(gold["MAAE"][col], rel=0.025), m0
+    assert m0[1] == pytest.approx(gold["MRASE"][col], rel=0.025), m0
+    assert m0[3] == pytest.approx(gold["MAARE"][col], rel=0.03), m0
+    assert m0[2] == pytest.approx(gold["MARE"][col], abs=0.35), m0
+    assert m1[0] == pytest.approx(m0[0], rel=0.01) and m1[1] == pytest.approx(m0[1], rel=0.01), (m0, m1)
