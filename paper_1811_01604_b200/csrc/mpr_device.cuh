@@ -924,14 +924,60 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         float* m2 = d.m2 + (size_t)g * d.N;
         const uint32_t k = st.realizations + real_no;
         const float inv_km1 = k > 1u ? 1.0f / (float)(k - 1u) : 0.0f, inv_k = 1.0f / (float)k;
-        for (int c = 0; c < 2; ++c) {
-            const uint32_t base = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
-            for (uint32_t e = tid; e < s_cle[c][0]; e += NT) {
-                const uint32_t off = E[base + e];
-                const int idx = nbase + (int)off + (int)((off * fc_inv) >> 24) * ncorr;
-                const float phi = angle_of(S[off], d.inv_q), before = acc[idx], after = before + phi;
-                acc[idx] = after;
-                if (k > 1u) m2[idx] += (phi - before * inv_km1) * (phi - after * inv_k);
+        // The core is walked row by row in groups of four sites (not along the entry lists, whose order is made for
+        // the shared-memory banks): a lane moves 16 bytes of acc and of m2, a warp whole lines; two groups per thread
+        // are in flight.  Needs cols, the tile's first column and its width to be multiples of four.
+        const uint32_t* bits = d.bits + (size_t)gd * d.words;
+        auto add_site = [&](float2 v, bool fixed, float& a_, float& m_) {
+            if (fixed) return;
+            const float phi = angle_of(v, d.inv_q), before = a_, after = before + phi;
+            a_ = after;
+            if (k > 1u) m_ += (phi - before * inv_km1) * (phi - after * inv_k);
+        };
+        if (((d.cols | tg.c0 | tg.TCc) & 3) == 0) {
+            const int q4 = tg.TCc >> 2, n4 = tg.TRc * q4;
+            for (int i0 = tid; i0 < n4; i0 += 2 * NT) {
+                int idx[2], off[2];
+                uint32_t fx[2];
+                float4 a4[2], m4[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int i = i0 + u * NT;
+                    fx[u] = 0xFu;
+                    if (i < n4) {
+                        const int lr = i / q4, j = i - lr * q4;
+                        idx[u] = (tg.r0 + lr) * d.cols + tg.c0 + 4 * j;
+                        off[u] = (H + lr) * FC + H + 4 * j;
+                        fx[u] = (__ldg(bits + (idx[u] >> 5)) >> (idx[u] & 31)) & 0xFu;
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 2; ++u)
+                    if (fx[u] != 0xFu) {
+                        a4[u] = *reinterpret_cast<const float4*>(acc + idx[u]);
+                        if (k > 1u) m4[u] = *reinterpret_cast<const float4*>(m2 + idx[u]);
+                        else m4[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+#pragma unroll
+                for (int u = 0; u < 2; ++u)
+                    if (fx[u] != 0xFu) {
+                        const float2* v = S + off[u];
+                        add_site(v[0], fx[u] & 1u, a4[u].x, m4[u].x);
+                        add_site(v[1], fx[u] & 2u, a4[u].y, m4[u].y);
+                        add_site(v[2], fx[u] & 4u, a4[u].z, m4[u].z);
+                        add_site(v[3], fx[u] & 8u, a4[u].w, m4[u].w);
+                        *reinterpret_cast<float4*>(acc + idx[u]) = a4[u];
+                        if (k > 1u) *reinterpret_cast<float4*>(m2 + idx[u]) = m4[u];
+                    }
+            }
+        } else {
+            for (int c = 0; c < 2; ++c) {
+                const uint32_t base = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
+                for (uint32_t e = tid; e < s_cle[c][0]; e += NT) {
+                    const uint32_t off = E[base + e];
+                    const int idx = nbase + (int)off + (int)((off * fc_inv) >> 24) * ncorr;
+                    add_site(S[off], false, acc[idx], m2[idx]);
+                }
             }
         }
     }
