@@ -382,9 +382,15 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     k_tile_count<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
     k_tile_scan<<<batch, 32, 0, s>>>(d);
     const size_t fill_smem = (size_t)g.FR * g.FC * sizeof(uint16_t);
-    if (fill_smem > 40960 &&
-        !cuda_ok(cudaFuncSetAttribute((const void*)k_tile_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fill_smem), "k_tile_fill smem"))
-        return fail(MPR_ERR_CUDA);
+    {
+        static size_t fill_set[64] = {};              // raised only, as for the tile pass below
+        size_t& have = fill_set[ctx->device & 63];
+        if (fill_smem > 40960 && fill_smem > have) {
+            if (!cuda_ok(cudaFuncSetAttribute((const void*)k_tile_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fill_smem), "k_tile_fill smem"))
+                return fail(MPR_ERR_CUDA);
+            have = fill_smem;
+        }
+    }
     k_tile_fill<<<dim3(g.ntiles, batch), 256, fill_smem, s>>>(d);
     ctx->launches += 7;
     if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
@@ -416,14 +422,23 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
         const int k = atoi(e);
         if (k >= 1 && (g.ntiles == 1 || k <= g.H / 2)) ctx->k_max = (uint32_t)k;
     }
-    for (int qh = 0; qh < 2; ++qh)
-        for (int om = 0; om < 3; ++om)
-            for (int fu = 0; fu < 2; ++fu)
-                for (int sd = 0; sd < 2; ++sd) {
-                    if (!qh && om == 1) continue;
-                    if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, g.FC == STD_FC, sd), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                      (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
-                }
+    // The attribute belongs to the kernel, not to this context: it is only ever raised (per device and frame-pitch
+    // variant), so that a context created later with smaller tiles does not take the room of an earlier one away.
+    {
+        static size_t attr_set[64][2] = {};
+        size_t& have = attr_set[ctx->device & 63][g.FC == STD_FC ? 1 : 0];
+        if (ctx->smem_bytes > have) {
+            for (int qh = 0; qh < 2; ++qh)
+                for (int om = 0; om < 3; ++om)
+                    for (int fu = 0; fu < 2; ++fu)
+                        for (int sd = 0; sd < 2; ++sd) {
+                            if (!qh && om == 1) continue;
+                            if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, g.FC == STD_FC, sd), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                              (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
+                        }
+            have = ctx->smem_bytes;
+        }
+    }
     *out = ctx;
     return MPR_OK;
 }

@@ -695,3 +695,37 @@ def test_paper_table3_validation_measures_on_the_gpu(torch_cuda, mpr, col, p_rem
     assert m0[3] == pytest.approx(gold["MAARE"][col], rel=0.03), m0
     assert m0[2] == pytest.approx(gold["MARE"][col], abs=0.35), m0
     assert m1[0] == pytest.approx(m0[0], rel=0.01) and m1[1] == pytest.approx(m0[1], rel=0.01), (m0, m1)
+
+
+def test_two_contexts_on_two_streams_are_independent(torch_cuda, mpr):
+    """include/mpr.h: 'distinct contexts are independent'.  Two contexts (one of them with chains) driven alternately
+    on two CUDA streams give bitwise the results each gives alone."""
+    torch = torch_cuda
+    za, ma = _field(200, 136, 10.0, 0.5, 901)
+    zb, mb = _field(96, 320, 6.0, 0.3, 902)
+
+    def run(z, m, stream, chains, seed):
+        with torch.cuda.stream(stream):
+            c = mpr.Mpr(_dev(torch, z), _dev(torch, m), stream=stream, chains=chains)
+            c.set_params(0.02, seed=seed, equil_cap=60, M=6, sweeps_per_real=4)
+        return c
+
+    s0 = torch.cuda.current_stream()
+    alone = []
+    for z, m, ch, seed in ((za, ma, 1, 11), (zb, mb, 3, 12)):
+        c = run(z, m, s0, ch, seed)
+        c.equilibrate().simulate()
+        alone.append((c.predict().cpu().numpy(), c.predict_std().cpu().numpy()))
+        c.close()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    ca, cb = run(za, ma, s1, 1, 11), run(zb, mb, s2, 3, 12)
+    ca.equilibrate(); cb.equilibrate()
+    cb.simulate(); ca.simulate()                      # both streams busy at once
+    with torch.cuda.stream(s1):
+        ra = (ca.predict(), ca.predict_std())
+    with torch.cuda.stream(s2):
+        rb = (cb.predict(), cb.predict_std())
+    s1.synchronize(); s2.synchronize()
+    for got, ref in ((ra, alone[0]), (rb, alone[1])):
+        assert np.array_equal(got[0].cpu().numpy(), ref[0]) and np.array_equal(got[1].cpu().numpy(), ref[1])
+    ca.close(); cb.close()
