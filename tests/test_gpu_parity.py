@@ -426,13 +426,15 @@ def test_t3_full_run_cfg3_and_cfg4_at_full_size_short_chains(torch_cuda, mpr, or
         assert abs(sw_g - sw_o) <= 10, (name, sw_g, sw_o)
 
 
-def test_accumulate_and_predict_against_oracle_back_transform(torch_cuda, mpr, orc):
+@pytest.mark.parametrize("rows,cols", [(40, 56), (37, 53), (70, 150), (130, 200), (200, 326)])
+def test_accumulate_and_predict_against_oracle_back_transform(torch_cuda, mpr, orc, rows, cols):
     """Step 6-7 alone, deterministic: import an oracle state, accumulate it
     M times with sweeps that cannot move (over-relaxation off, T so low and a
     so large that... no: use the API as is) -- here: M = 1, s = 1 and compare
     the prediction with the oracle's back-transform of the same one sweep."""
     torch = torch_cuda
-    z, m = _field(40, 56, 5.0, 0.5, 31)
+    # shapes: one tile and several, widths that are and are not multiples of four (the two accumulate walks)
+    z, m = _field(rows, cols, 5.0, 0.5, 31)
     z = (50.0 + 10.0 * z).astype(np.float32)
     seed, T = 8, 0.05
     phi, zmin, zmax = orc.transform(z, m, seed)
@@ -446,7 +448,7 @@ def test_accumulate_and_predict_against_oracle_back_transform(torch_cuda, mpr, o
     ok = (m == 1) | (margin > 1e-3)
     scale = (float(zmax) - float(zmin)) / TWO_PI_F
     assert np.abs(pred - ref)[ok].max() <= 2 * TOL_RAD * scale
-    assert (~ok).sum() <= 2
+    assert (~ok).sum() <= max(2, 1e-3 * m.size)
     assert ctx.get_stats()[0].realizations == 1 and ctx.get_stats()[0].t == 1
     ctx.close()
 
@@ -507,12 +509,13 @@ def test_same_seed_same_result_bitwise(torch_cuda, mpr):
 # ---------------------------------------------------------------------------
 # spread of the realizations
 # ---------------------------------------------------------------------------
-def test_predict_std_against_oracle_chain(torch_cuda, mpr, orc):
+@pytest.mark.parametrize("L", [192, 150])          # widths that are and are not multiples of four (the two accumulate walks)
+def test_predict_std_against_oracle_chain(torch_cuda, mpr, orc, L):
     """The same short chain on both sides from an identical oracle-made state (M = 4 realizations of 2 sweeps):
     the sample standard deviation per prediction site agrees except where a near-threshold decision fell the
     other way in one of the 8 sweeps."""
     torch = torch_cuda
-    w = synth.make_workload("cfg2", L=192)
+    w = synth.make_workload("cfg2", L=L)
     z, m, T = w.truth[0], w.mask[0], float(w.T[0])
     p = orc.Params(seed=w.seed, equil_cap=80, M=4, sweeps_per_real=2)
     phi, zmin, zmax = orc.transform(z, m, p.seed)
