@@ -732,3 +732,42 @@ def test_two_contexts_on_two_streams_are_independent(torch_cuda, mpr):
     for got, ref in ((ra, alone[0]), (rb, alone[1])):
         assert np.array_equal(got[0].cpu().numpy(), ref[0]) and np.array_equal(got[1].cpu().numpy(), ref[1])
     ca.close(); cb.close()
+
+
+def test_chains_in_a_batch_after_equilibration(torch_cuda, mpr, orc):
+    """Two grids with different temperatures (they stop equilibrating after different numbers of sweeps, i.e. in different
+    vector buffers) and 3 chains each: the whole path against the oracle's (equilibrate, then simulate_chains with
+    the batch's Philox grid words); MAE / RMSE means over seeds within 1.5 %, realization counts and sweep indices exact."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    z0, m0 = w.truth[0], w.mask[0]
+    z1, m1 = _field(64, 64, 5.0, 0.5, 77)
+    zs, ms = np.stack([z0, z1]), np.stack([m0, m1])
+    Ts = [float(w.T[0]), float(synth.choose_T(z1, m1))]
+    chains, M, s = 3, 9, 20
+    ctx = mpr.Mpr(_dev(torch, zs), _dev(torch, ms), chains=chains)
+    rows = []
+    odd_even = set()
+    for seed in range(9000, 9012):
+        ctx.set_params(Ts, seed=seed, equil_cap=400, sweeps_per_real=s, M=M).equilibrate().simulate()
+        pred = ctx.predict().cpu().numpy()
+        st = ctx.get_stats()
+        for g in range(2):
+            p = orc.Params(seed=seed, equil_cap=400, sweeps_per_real=s, M=M)
+            phi, zmin, zmax = orc.transform(zs[g], ms[g], seed, g)
+            eq = orc.equilibrate(phi, ms[g], Ts[g], p, g=g)
+            acc, _, M_tot, t_end, _ = orc.simulate_chains(phi, ms[g], Ts[g], eq["a"], p, chains, g=g, batch=2, t0=eq["t"])
+            assert st[g].realizations == M_tot
+            assert abs(st[g].equil_sweeps - eq["sweeps"]) <= 10
+            assert st[g].t == st[g].equil_sweeps + (M_tot // chains) * s
+            vg = synth.validation_measures(zs[g], pred[g], ms[g])
+            vo = synth.validation_measures(zs[g], orc.predict(acc, M_tot, zs[g], ms[g], zmin, zmax), ms[g])
+            rows.append((g, vg["mae"], vo["mae"], vg["rmse"], vo["rmse"]))
+            assert np.array_equal(pred[g][ms[g] == 1], zs[g][ms[g] == 1])
+        odd_even.add((st[0].equil_sweeps & 1, st[1].equil_sweeps & 1))
+    ctx.close()
+    r = np.array(rows)
+    for g in range(2):
+        mg = r[r[:, 0] == g].mean(axis=0)
+        assert mg[1] == pytest.approx(mg[2], rel=0.015) and mg[3] == pytest.approx(mg[4], rel=0.015), (g, mg)
+    assert any(a != b for a, b in odd_even)          # some run did end with the two grids in different buffers
