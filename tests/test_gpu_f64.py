@@ -105,7 +105,7 @@ def test_t2_one_sweep_from_equilibrated_oracle_state(torch_cuda, mpr, orc64, nam
     ctx.close()
 
 
-@pytest.mark.parametrize("rows,cols", [(2, 2), (2, 7), (7, 2), (3, 3), (37, 53), (64, 129)])
+@pytest.mark.parametrize("rows,cols", [(2, 2), (2, 7), (7, 2), (3, 3), (37, 53), (64, 129), (2, 20001), (20000, 3)])
 def test_t2_ragged_and_tiny_grids_hot_start(torch_cuda, mpr, orc64, rows, cols):
     torch = torch_cuda
     z, m = _field(rows, cols, 3.0, 0.5, 300 + rows * cols)

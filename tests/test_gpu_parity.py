@@ -165,7 +165,7 @@ def test_t2_one_sweep_from_equilibrated_oracle_state(torch_cuda, mpr, orc, name,
     ctx.close()
 
 
-@pytest.mark.parametrize("rows,cols", [(2, 2), (2, 7), (7, 2), (3, 3), (37, 53), (64, 129), (255, 64)])
+@pytest.mark.parametrize("rows,cols", [(2, 2), (2, 7), (7, 2), (3, 3), (37, 53), (64, 129), (255, 64), (2, 20001), (20000, 3), (65, 65534)])
 def test_t2_ragged_and_tiny_grids_hot_start(torch_cuda, mpr, orc, rows, cols):
     """Random (hot) states, a = 1: wraps, rejected reflections, edges and corners."""
     torch = torch_cuda
