@@ -771,3 +771,43 @@ def test_chains_in_a_batch_after_equilibration(torch_cuda, mpr, orc):
         mg = r[r[:, 0] == g].mean(axis=0)
         assert mg[1] == pytest.approx(mg[2], rel=0.015) and mg[3] == pytest.approx(mg[4], rel=0.015), (g, mg)
     assert any(a != b for a, b in odd_even)          # some run did end with the two grids in different buffers
+
+
+def test_t2_one_sweep_on_a_grid_whose_buffers_pass_4_GiB(torch_cuda, mpr, orc):
+    """20480 x 26624 = 545 M sites: one vector buffer is 4.36 GB, so element and byte offsets pass 2^32 (tile frames,
+    row stores, lists).  An analytic smooth field plus noise (an FFT field of this size would take minutes), 33 % removed,
+    a near-equilibrium state; one sweep against the oracle over the whole grid.  Sites beyond 1e-5 rad are counted
+    as flips without the margin diagnostics (three more 4 GB arrays): at most 1e-5 of the prediction sites."""
+    torch = torch_cuda
+    if torch.cuda.get_device_properties(0).total_memory < 40 * 2 ** 30:
+        pytest.skip("needs 25 GB of device memory")
+    rows, cols = 20480, 26624
+    rng = np.random.default_rng(5)
+    r = np.arange(rows, dtype=np.float32)[:, None]; c = np.arange(cols, dtype=np.float32)[None, :]
+    z = (np.sin(r / 97.0) + np.cos(c / 131.0)).astype(np.float32)
+    z += 0.05 * rng.standard_normal(z.shape, dtype=np.float32)
+    m = (rng.random(z.shape, dtype=np.float32) >= 0.33).astype(np.uint8)
+    T, a, seed, t = 2e-3, 12.0, 4242, 7
+    zmin, zmax, _ = orc.minmax(z, m)
+    phi = ((z - zmin) * (TWO_PI_F / (float(zmax) - float(zmin)))).astype(np.float32)
+    phi += math.sqrt(T) * rng.standard_normal(z.shape, dtype=np.float32)
+    np.clip(phi, 0.0, TWO_PI_F, out=phi)
+    ref0, _, _ = orc.transform(z, m, seed)
+    phi[m == 1] = ref0[m == 1]
+    del ref0
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed)
+    ctx.set_angles(torch.from_numpy(phi)[None].cuda())
+    ctx.set_sweep_index(t)
+    acc_g = ctx.sweep(1, a, count=True)[0]
+    got = ctx.get_angles().cpu().numpy()[0]
+    e_g = ctx.energy()[0]
+    ctx.close()
+    acc_o = orc.sweep(phi, m, 0.5, T, a, seed, 0, t)
+    free = m == 0
+    d = np.abs(got - phi)
+    assert d[~free].max() == 0.0
+    bad = int((d[free] > TOL_RAD).sum())
+    assert bad <= 1e-5 * free.sum(), bad
+    assert abs(int(acc_g) - int(acc_o)) <= bad
+    assert e_g == pytest.approx(orc.energy_per_bond(phi), abs=2e-6)
