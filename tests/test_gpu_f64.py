@@ -232,3 +232,29 @@ def test_t2_full_size_cfg4_and_cfg3_one_sweep(torch_cuda, mpr, orc64):
         ctx.set_params(T, seed=w.seed)
         _one_sweep(orc64, ctx, phi, m, 0.5, T, a, w.seed, 123, 0)
         ctx.close()
+
+
+def test_t2_one_sweep_on_a_grid_whose_state_passes_4_GiB(torch_cuda, mpr, orc64):
+    """16384 x 20480 = 335 M sites: the double2 state is 5.4 GB, so byte offsets pass 2^32.  An analytic smooth field
+    plus noise, 33 % removed, a near-equilibrium state; one sweep against the oracle's double build over the whole grid."""
+    torch = torch_cuda
+    if torch.cuda.get_device_properties(0).total_memory < 40 * 2 ** 30:
+        pytest.skip("needs 25 GB of device memory")
+    rows, cols = 16384, 20480
+    rng = np.random.default_rng(6)
+    r = np.arange(rows, dtype=np.float64)[:, None]; c = np.arange(cols, dtype=np.float64)[None, :]
+    z = np.sin(r / 97.0) + np.cos(c / 131.0)
+    z += 0.05 * rng.standard_normal(z.shape)
+    m = (rng.random(z.shape, dtype=np.float32) >= 0.33).astype(np.uint8)
+    T, a, seed = 2e-3, 12.0, 4243
+    zmin, zmax, _ = orc64.minmax(z, m)
+    phi = (z - zmin) * (TWO_PI / (zmax - zmin))
+    phi += math.sqrt(T) * rng.standard_normal(z.shape)
+    np.clip(phi, 0.0, TWO_PI, out=phi)
+    ref0, _, _ = orc64.transform(z, m, seed)
+    phi[m == 1] = ref0[m == 1]
+    del ref0
+    ctx = mpr.Mpr64(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed)
+    _one_sweep(orc64, ctx, phi, m, 0.5, T, a, seed, 8, 0)
+    ctx.close()
