@@ -811,3 +811,52 @@ def test_t2_one_sweep_on_a_grid_whose_buffers_pass_4_GiB(torch_cuda, mpr, orc):
     assert bad <= 1e-5 * free.sum(), bad
     assert abs(int(acc_g) - int(acc_o)) <= bad
     assert e_g == pytest.approx(orc.energy_per_bond(phi), abs=2e-6)
+
+
+def test_t2_only_one_colour_has_prediction_sites(torch_cuda, mpr, orc):
+    """Degenerate checkerboards: every prediction site on colour 0 (all of its neighbours are samples), then on colour 1;
+    the other colour's list is empty.  Both precisions."""
+    torch = torch_cuda
+    from oracle import mpr_oracle64 as orc64
+    rows, cols = 70, 90
+    z, _ = _field(rows, cols, 6.0, 0.5, 55)
+    rr, cc = np.indices((rows, cols))
+    for colour in (0, 1):
+        m = (((rr + cc) & 1) != colour).astype(np.uint8)          # colour `colour` free, the other fixed
+        m[0, 0] = 1 if colour == 0 else m[0, 0]
+        ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+        ctx.set_params(0.05, seed=13)
+        phi, _, _ = orc.transform(z, m, 13)
+        res = _compare_one_sweep(orc, ctx, phi[None], m[None], 0.5, [0.05], 1.5, 13, 3, 0)
+        assert res[0][2] <= TOL_RAD
+        ctx.close()
+        z64 = z.astype(np.float64)
+        c64 = mpr.Mpr64(_dev(torch, z64), _dev(torch, m))
+        c64.set_params(0.05, seed=13)
+        p64, _, _ = orc64.transform(z64, m, 13)
+        c64.set_sweep_index(3)
+        n_acc = c64.sweep(1, 1.5, count=True)
+        assert n_acc == orc64.sweep(p64, m, 0.5, 0.05, 1.5, 13, 0, 3)
+        assert np.abs(c64.get_angles().cpu().numpy() - p64).max() < 1e-11
+        c64.close()
+
+
+@pytest.mark.parametrize("cap,n_fit,n_f", [(1, 20, 5), (5, 20, 5), (21, 20, 5), (23, 20, 5), (40, 2, 1), (300, 256, 7)])
+def test_equilibration_caps_and_windows_follow_the_oracle(torch_cuda, mpr, orc, cap, n_fit, n_f):
+    """Alg. 2 step 5 at the edges of its parameters: caps below, at and just above the first slope check, the smallest
+    and the largest fit window.  Sweep counts equal to the oracle's up to what a near-threshold flip can shift (one
+    check interval), a and the sweep index consistent."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=31, equil_cap=cap, n_fit=n_fit, n_f=n_f).equilibrate()
+    st = ctx.get_stats()[0]
+    p = orc.Params(seed=31, equil_cap=cap, n_fit=n_fit, n_f=n_f)
+    phi, _, _ = orc.transform(z, m, 31)
+    eq = orc.equilibrate(phi, m, T, p)
+    assert st.equil_sweeps <= cap and st.t == st.equil_sweeps and st.equilibrated
+    assert abs(st.equil_sweeps - eq["sweeps"]) <= n_f
+    if st.equil_sweeps == eq["sweeps"]:
+        assert st.a == pytest.approx(eq["a"], rel=1e-12)
+    ctx.close()
