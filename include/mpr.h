@@ -12,8 +12,8 @@
  * Conventions (all entry points)
  *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.
  *   - The caller owns every buffer it passes (inputs, workspace, outputs).
- *     The library owns only the small host-side mpr_ctx (plus a few bytes of
- *     pinned host memory used to poll device flags).  All device state lives
+ *     The library owns only the small host-side mpr_ctx (with host copies of
+ *     the per-grid scalars and flags it polls).  All device state lives
  *     inside the caller's workspace.
  *   - Every call returns an mpr_status; nothing throws, aborts or sets errno.
  *     Output parameters are left untouched when the status is not MPR_OK.

@@ -122,7 +122,7 @@ struct mpr_ctx {
     uint32_t     k_max;           // sweeps per tile pass
     size_t       smem_bytes;      // dynamic shared memory of k_tilepass
     uint64_t     launches;
-    uint32_t*    h_pinned;        // [batch] pinned host, done flags
+    uint32_t*    h_done;          // [batch] host copy of the done flags (pageable: a pinned allocation costs ~1 ms per context)
     GridState*   h_states;        // [batch] pageable host copy
     bool         qhalf;
     bool         dirty;           // vectors changed since d.phi was last written at the free sites
@@ -364,7 +364,8 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     mpr_status st = MPR_OK;
     auto fail = [&](mpr_status s) { mpr_destroy(ctx); return s; };
     if (!ctx->h_states) return fail(MPR_ERR_ARG);
-    if (!cuda_ok(cudaMallocHost((void**)&ctx->h_pinned, sizeof(uint32_t) * batch), "cudaMallocHost")) return fail(MPR_ERR_CUDA);
+    ctx->h_done = new (std::nothrow) uint32_t[batch];
+    if (!ctx->h_done) return fail(MPR_ERR_ARG);
 
     cudaStream_t s = ctx->stream;
     // the pad column of an odd-width grid stays zero
@@ -470,7 +471,7 @@ mpr_status mpr_create_unconditional(mpr_ctx** out, int batch, int rows, int cols
 mpr_status mpr_destroy(mpr_ctx* ctx)
 {
     if (!ctx) return MPR_ERR_ARG;
-    if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    delete[] ctx->h_done;
     delete[] ctx->h_states;
     delete ctx;
     return MPR_OK;
@@ -537,10 +538,10 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
             CU_LAUNCH();
         }
         issued += chunk;
-        CU(cudaMemcpyAsync(ctx->h_pinned, d.done_flags, sizeof(uint32_t) * d.batch, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->h_done, d.done_flags, sizeof(uint32_t) * d.batch, cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         bool all = true;
-        for (int b = 0; b < d.batch; ++b) all = all && ctx->h_pinned[b];
+        for (int b = 0; b < d.batch; ++b) all = all && ctx->h_done[b];
         if (all) break;
         chunk = ctx->prm.n_f;
     }

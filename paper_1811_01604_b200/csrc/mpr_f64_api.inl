@@ -44,7 +44,7 @@ struct mpr64_ctx {
     int            device, energy_blocks;
     uint32_t       n_colour[2];   // prediction sites per colour (lengths of the site lists)
     uint64_t       launches;
-    uint32_t*      h_done;        // pinned
+    uint32_t       h_done;        // host copy of the done flag
     mpr64::State64 h_state;
     bool           qhalf, dirty;
 };
@@ -99,7 +99,6 @@ mpr_status mpr64_query_workspace(int rows, int cols, size_t* bytes)
 mpr_status mpr64_destroy(mpr64_ctx* ctx)
 {
     if (!ctx) return MPR_ERR_ARG;
-    if (ctx->h_done) cudaFreeHost(ctx->h_done);
     delete ctx;
     return MPR_OK;
 }
@@ -142,7 +141,6 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
     ctx->energy_blocks = rows < mpr64::E_BLOCKS ? rows : mpr64::E_BLOCKS;
     auto fail = [&](mpr_status s) { mpr64_destroy(ctx); return s; };
-    if (!cuda_ok(cudaMallocHost((void**)&ctx->h_done, sizeof(uint32_t)), "cudaMallocHost")) return fail(MPR_ERR_CUDA);
     unsigned mm_blocks = cdiv(N, 256 * 8);
     if (mm_blocks > (unsigned)mpr64::MM_BLOCKS) mm_blocks = mpr64::MM_BLOCKS;
     mpr64::k64_minmax<<<mm_blocks, 256, 0, ctx->stream>>>(d, d_values, d_sample_mask);
@@ -215,9 +213,9 @@ mpr_status mpr64_equilibrate(mpr64_ctx* ctx)
             CU_LAUNCH();
         }
         issued += chunk;
-        CU(cudaMemcpyAsync(ctx->h_done, d.done_flag, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync(&ctx->h_done, d.done_flag, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
-        if (*ctx->h_done) break;
+        if (ctx->h_done) break;
         chunk = ctx->prm.n_f;
     }
     return MPR_OK;
