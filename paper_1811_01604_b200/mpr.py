@@ -484,11 +484,29 @@ def infer_temperature(Ts, es, e_s: float) -> float:
     return float(out.value)
 
 
-def interpolate(values, sample_mask, T, chains: int = 1, **params):
-    """The whole path for a batch of grids: create, set_params, equilibrate,
-    simulate, predict.  Returns (prediction tensor, list of Stats)."""
+def infer_T(ctx: "Mpr", n_meas: int = 100, ladder=(0.25, 0.5, 1.0, 2.0, 4.0), **params):
+    """Alg. 2 step 4 for every grid of a context, by the library's own calls: e_s (mpr_sample_energy), a ladder of
+    temperatures around the point where the low-temperature equipartition line e = -1 + (N - 1) T / (2 N_GP) meets e_s
+    (that line only centres the ladder), e(T, L) of the ladder from unconditional chains (mpr_energy_table) and the
+    inversion (mpr_infer_temperature).  Returns the list of T-hat."""
+    e_s, _ = ctx.sample_energy()
+    n_gp = ctx.rows * (ctx.cols - 1) + ctx.cols * (ctx.rows - 1)
+    out = []
+    for e in e_s:
+        centre = max(2.0 * n_gp * (1.0 + e) / (ctx.rows * ctx.cols - 1), 1e-12)
+        Ts = [centre * f for f in ladder]
+        table = energy_table(ctx.rows, ctx.cols, Ts, n_meas, ctx.device, **params)
+        out.append(infer_temperature(Ts, table, e))
+    return out
+
+
+def interpolate(values, sample_mask, T=None, chains: int = 1, **params):
+    """The whole path for a batch of grids: create, (T = None: infer the temperatures, Alg. 2 step 4,) set_params,
+    equilibrate, simulate, predict.  Returns (prediction tensor, list of Stats)."""
     m = Mpr(values, sample_mask, chains=chains)
     try:
+        if T is None:
+            T = infer_T(m, **{k: v for k, v in params.items() if k in ("seed", "q", "equil_cap", "or_mode")})
         m.set_params(T, **params).equilibrate().simulate()
         out = m.predict()
         stats = m.get_stats()

@@ -109,3 +109,27 @@ def test_energy_table_and_inferred_temperature(torch_cuda, mpr, orc):
     T_ref = orc.infer_T(e_s, Ts, e_ref)
     assert T_gpu == pytest.approx(T_ref, rel=0.03)
     assert T_gpu == pytest.approx(synth.choose_T(z, m), rel=0.05)
+
+
+def test_interpolate_with_inferred_temperature(torch_cuda, mpr, orc):
+    """The parameter-free path the paper intends (L11, L63 'automatic'): T = None makes the binding run Alg. 2 step 4 with the
+    library's own calls before the sweeps.  On a cfg1-shaped grid the inferred T-hat is within 5 % of the closed form
+    (reading R15) and the prediction's RMSE within 3 % of the run with the closed-form T."""
+    import numpy as np
+    from paper_1811_01604_b200 import synth
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    z, m, T_cf = w.truth[0], w.mask[0], float(w.T[0])
+    dz, dm = torch.from_numpy(z).cuda(), torch.from_numpy(m).cuda()
+    ctx = mpr.Mpr(dz, dm)
+    T_hat = mpr.infer_T(ctx, seed=5, equil_cap=500)[0]
+    ctx.close()
+    assert T_hat == pytest.approx(T_cf, rel=0.05)
+    scores = []
+    for T in (None, T_cf):
+        rm = []
+        for seed in range(40, 48):
+            pred, _ = mpr.interpolate(dz, dm, T, seed=seed, equil_cap=500, M=10, sweeps_per_real=100)
+            rm.append(synth.validation_measures(z, pred.cpu().numpy()[0], m)["rmse"])
+        scores.append(np.mean(rm))
+    assert scores[0] == pytest.approx(scores[1], rel=0.03)
