@@ -238,8 +238,9 @@ def test_t2_one_sweep_on_a_grid_whose_state_passes_4_GiB(torch_cuda, mpr, orc64)
     """16384 x 20480 = 335 M sites: the double2 state is 5.4 GB, so byte offsets pass 2^32.  An analytic smooth field
     plus noise, 33 % removed, a near-equilibrium state; one sweep against the oracle's double build over the whole grid."""
     torch = torch_cuda
-    if torch.cuda.get_device_properties(0).total_memory < 40 * 2 ** 30:
-        pytest.skip("needs 25 GB of device memory")
+    import psutil
+    if torch.cuda.get_device_properties(0).total_memory < 40 * 2 ** 30 or psutil.virtual_memory().available < 32 * 2 ** 30:
+        pytest.skip("needs 25 GB of device memory and 20 GB of host memory")
     rows, cols = 16384, 20480
     rng = np.random.default_rng(6)
     r = np.arange(rows, dtype=np.float64)[:, None]; c = np.arange(cols, dtype=np.float64)[None, :]

@@ -779,8 +779,9 @@ def test_t2_one_sweep_on_a_grid_whose_buffers_pass_4_GiB(torch_cuda, mpr, orc):
     a near-equilibrium state; one sweep against the oracle over the whole grid.  Sites beyond 1e-5 rad are counted
     as flips without the margin diagnostics (three more 4 GB arrays): at most 1e-5 of the prediction sites."""
     torch = torch_cuda
-    if torch.cuda.get_device_properties(0).total_memory < 40 * 2 ** 30:
-        pytest.skip("needs 25 GB of device memory")
+    import psutil
+    if torch.cuda.get_device_properties(0).total_memory < 40 * 2 ** 30 or psutil.virtual_memory().available < 32 * 2 ** 30:
+        pytest.skip("needs 25 GB of device memory and 20 GB of host memory")
     rows, cols = 20480, 26624
     rng = np.random.default_rng(5)
     r = np.arange(rows, dtype=np.float32)[:, None]; c = np.arange(cols, dtype=np.float32)[None, :]
