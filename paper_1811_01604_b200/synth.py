@@ -204,8 +204,8 @@ def _single(name, c, L, ell, kind, p, M, noise=0.0, holes=0, s=100, cap=1000):
 def make_workload(name: str, batch: int | None = None, L: int | None = None) -> Workload:
     """BASELINE.json `configs` 1..5 (cfg1..cfg5) and the paper's own workload
     (N(50,10), exponential covariance kappa=0.2, one sweep
-    per realization) as `paper33` / `paper66`.  `L`/`batch` override the size
-    for tests."""
+    per realization) as `paper33` / `paper66` (`paperNN`: NN % of the nodes removed).  `L`/`batch` override the
+    size for tests."""
     if name == "cfg1":
         return _single(name, 1, L or 64, 8.0, "gaussian", 0.33, M=10)
     if name == "cfg2":
@@ -230,8 +230,8 @@ def make_workload(name: str, batch: int | None = None, L: int | None = None) -> 
         return Workload(name, truth, mask, T, 3005, M=100,
                         meta={"L": side, "ell": [float(x) for x in ells],
                               "cov": "gaussian", "p_removed": 0.66})
-    if name in ("paper33", "paper66"):
-        p = 0.33 if name == "paper33" else 0.66
+    if name.startswith("paper") and name[5:].isdigit() and 1 <= int(name[5:]) <= 99:
+        p = int(name[5:]) / 100.0            # paper33 / paper66 are the paper's two cases; any other percentage for sweeps
         side = L or 1024
         truth = grf(side, side, 5.0, "exponential", 1009, mean=50.0, sigma=10.0)
         mask = bernoulli_mask(side, side, p, 2009 + int(p * 100))
