@@ -278,6 +278,7 @@ def run_b200(args, w):
             updates += sum(s.n_free * (s.equil_sweeps + s.realizations * w.sweeps_per_real) for s in st)
             launches += ctx.launch_count()
             ctx.close()
+            del ctx         # its workspace goes back to torch's cache now: the next step must not need a second block
         return total_ms / 1e3, updates, launches
 
     for _ in range(max(args.warmup, 1)):
