@@ -330,6 +330,10 @@ def run_b200(args, w):
     if not args.no_f64 and world == 1:
         from paper_1811_01604_b200 import synth as _synth
         z64 = torch.from_numpy(w.truth[0].astype(np.float64)).to(dev)
+        warm = mpr.Mpr64(z64, d_mask[0])              # untimed: the workspace's first allocation, lazy kernel loading
+        warm.set_params(T[0], **prm).sweep(2, 1.0)
+        warm.close()
+        del warm
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
         ev[0].record(stream)
         c64 = mpr.Mpr64(z64, d_mask[0])
