@@ -2,13 +2,12 @@
 // data, spin state, every site update and the realization sums in double.  Included by mpr_api.cu after
 // mpr_device.cuh (Philox, the bitmask helpers and the error flags are shared with the fp32 path; no arithmetic is).
 //
-// State: v_i = (cos q phi_i, sin q phi_i) as double2, row-major [rows][cols], updated IN PLACE: the sites of one
-// colour depend only on the other colour, so a half-sweep is one kernel with one thread per
-// PREDICTION site of that colour (the paper's own design, L261-267, gives every lattice site a thread and lets those
-// of the sample sites idle; here the prediction sites of each colour are listed once, in row-major order, so that
-// every lane of a warp has an update to do).  Measured on cfg4 (profiles/r01h): 70 us per half-sweep, 346 MB of DRAM
-// traffic = 4.9 TB/s = 0.76 of the measured HBM peak, fp64 pipe 22 %: this kernel is bound by bytes (a 32-byte sector
-// of the row-major double2 state holds one site of each colour, so every half-sweep streams the whole state).  The
+// State: v_i = (cos q phi_i, sin q phi_i) as double2, one plane per checkerboard colour (vpos), updated IN PLACE: the
+// sites of one colour depend only on the other colour, so a half-sweep is one kernel with one
+// thread per PREDICTION site of that colour (the paper's own design, L261-267, gives every lattice site a thread and
+// lets those of the sample sites idle; here the prediction sites of each colour are listed once, in row-major order,
+// so that every lane of a warp has an update to do).  Measured on cfg4 (profiles/r01h): 62 us per half-sweep, 327 MB
+// of DRAM traffic = 5.3 TB/s = 0.82 of the measured HBM peak, fp64 pipe 26 %: this kernel is bound by bytes.  The
 // fp32 path's shared-memory tile pass (K sweeps per load) is what would lift it; not built for double yet
 // (DESIGN.md section 12).  One grid per context.
 #pragma once
@@ -49,7 +48,9 @@ struct Dev64 {
     uint32_t* list;           // [n_colour[0]] then [n_colour[1]]: the prediction sites of colour 0, then of colour 1, ascending
     uint32_t* list_counts;    // [2][list_blocks] prediction sites per colour of each block of 32 * LIST_THREADS sites
     uint32_t  list_blocks;
-    double2*  vec;            // [N] unit vectors
+    double2*  vec;            // [2][rows][half] unit vectors, one plane per checkerboard colour (vpos)
+    int       half;           // ceil(cols / 2): sites of one colour in a row (at most)
+    uint32_t  plane;          // rows * half
     double*   acc;            // [N] sum over the realizations of phi
     double*   acc2;           // [N] sum of phi^2 (spread, L212)
     int       rows, cols;
@@ -59,6 +60,26 @@ struct Dev64 {
     uint32_t  n_f, n_fit, equil_cap;
     double    A_targ, k_a;
 };
+
+// Where the vector of site (r, c) lives: the two colours in separate planes, so that a half-sweep reads the OTHER
+// colour's plane as a stream and touches its own only at the prediction sites (in one row-major array a 32-byte sector
+// holds one site of each colour and every half-sweep streamed both: 346 MB and 70 us per half-sweep of cfg4 against
+// 327 MB and 62 us now; DRAM moves 64 bytes at a time, i.e. four sites of a colour, of which one in three is free).
+// Neighbours of (r, c) sit in the other plane at o = vpos_other(r, c): up o - half, down o + half,
+// left o - 1 + (c & 1), right o + (c & 1).
+__device__ __forceinline__ size_t vpos(const Dev64& d, int r, int c)
+{
+    return (size_t)((r + c) & 1) * d.plane + (size_t)r * d.half + (size_t)(c >> 1);
+}
+__device__ __forceinline__ size_t vpos_other(const Dev64& d, int r, int c)
+{
+    return (size_t)(((r + c) & 1) ^ 1) * d.plane + (size_t)r * d.half + (size_t)(c >> 1);
+}
+__device__ __forceinline__ size_t vpos_n(const Dev64& d, uint32_t n)
+{
+    const int r = (int)(n / (uint32_t)d.cols);
+    return vpos(d, r, (int)(n - (uint32_t)r * (uint32_t)d.cols));
+}
 
 // u = (2 (x >> 9) + 1) 2^-24 in (0,1): the same lattice as the fp32 path (R13), exact in double
 __device__ __forceinline__ double u01d(uint32_t x) { return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0); }
@@ -233,7 +254,7 @@ __global__ void __launch_bounds__(256) k64_init_state(Dev64 d)
     }
     double sn, cs;
     sincos(__dmul_rn(d.q, p), &sn, &cs);
-    d.vec[n] = make_double2(cs, sn);
+    d.vec[vpos_n(d, n)] = make_double2(cs, sn);
 }
 
 // ---- a3: UPDATE of one prediction site (Alg. 1) in vector form, in double ----------------------------
@@ -309,12 +330,13 @@ __global__ void __launch_bounds__(256) k64_halfsweep(Dev64 d, const uint32_t* __
             const State64& s = *d.state;
             const uint32_t t = s.t + t_off;
             const double2 zero = make_double2(0.0, 0.0);                 // open boundary (L109)
-            const double2 up = r > 0 ? d.vec[n - d.cols] : zero, dn = r < d.rows - 1 ? d.vec[n + d.cols] : zero;
-            const double2 lf = c > 0 ? d.vec[n - 1] : zero, rt = c < d.cols - 1 ? d.vec[n + 1] : zero;
+            const size_t self = vpos(d, r, c), o = vpos_other(d, r, c);
+            const double2 up = r > 0 ? d.vec[o - d.half] : zero, dn = r < d.rows - 1 ? d.vec[o + d.half] : zero;
+            const double2 lf = c > 0 ? d.vec[o - 1 + (c & 1)] : zero, rt = c < d.cols - 1 ? d.vec[o + (c & 1)] : zero;
             const uint4 x = philox4x32_10(n, t >> 1, 2u, 0u, d.rk0, d.rk1);
             const uint32_t w0 = (t & 1u) ? x.z : x.x, w1 = (t & 1u) ? x.w : x.y;
             const double hd_scale = d.q * (0.5 * TWO_PI_D) / s.a;
-            d.vec[n] = update_site_d<QHALF, ORMODE>(d.vec[n], up, dn, lf, rt, w0, w1, hd_scale, -1.0 / s.T, d.bc, d.bs, accepted);
+            d.vec[self] = update_site_d<QHALF, ORMODE>(d.vec[self], up, dn, lf, rt, w0, w1, hd_scale, -1.0 / s.T, d.bc, d.bs, accepted);
         }
     }
     if (count) {
@@ -331,13 +353,13 @@ __global__ void __launch_bounds__(E_THREADS) k64_energy(Dev64 d)
     for (int r = blockIdx.x; r < d.rows; r += gridDim.x) {
         double row = 0.0;
         for (int c = ((r + 1) & 1) + 2 * (int)threadIdx.x; c < d.cols; c += 2 * E_THREADS) {
-            const uint32_t n = (uint32_t)r * d.cols + c;
-            const double2 v = d.vec[n];
+            const double2 v = d.vec[vpos(d, r, c)];
+            const size_t o = vpos_other(d, r, c);
             double hx = 0.0, hy = 0.0;
-            if (r > 0) { hx += d.vec[n - d.cols].x; hy += d.vec[n - d.cols].y; }
-            if (r < d.rows - 1) { hx += d.vec[n + d.cols].x; hy += d.vec[n + d.cols].y; }
-            if (c > 0) { hx += d.vec[n - 1].x; hy += d.vec[n - 1].y; }
-            if (c < d.cols - 1) { hx += d.vec[n + 1].x; hy += d.vec[n + 1].y; }
+            if (r > 0) { hx += d.vec[o - d.half].x; hy += d.vec[o - d.half].y; }
+            if (r < d.rows - 1) { hx += d.vec[o + d.half].x; hy += d.vec[o + d.half].y; }
+            if (c > 0) { hx += d.vec[o - 1 + (c & 1)].x; hy += d.vec[o - 1 + (c & 1)].y; }
+            if (c < d.cols - 1) { hx += d.vec[o + (c & 1)].x; hy += d.vec[o + (c & 1)].y; }
             row += fma(v.x, hx, v.y * hy);
         }
         sum += row;
@@ -404,7 +426,7 @@ __global__ void __launch_bounds__(256) k64_accumulate(Dev64 d)
 {
     const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= d.N || is_fixed(d.bits, n)) return;
-    const double p = angle_of_d(d.vec[n], d.inv_q);
+    const double p = angle_of_d(d.vec[vpos_n(d, n)], d.inv_q);
     d.acc[n] += p; d.acc2[n] += p * p;
 }
 __global__ void __launch_bounds__(256) k64_predict(Dev64 d, double* __restrict__ out, int what)
@@ -424,7 +446,7 @@ __global__ void __launch_bounds__(256) k64_export_angles(Dev64 d)
 {
     const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= d.N || is_fixed(d.bits, n)) return;
-    d.phi[n] = angle_of_d(d.vec[n], d.inv_q);
+    d.phi[n] = angle_of_d(d.vec[vpos_n(d, n)], d.inv_q);
 }
 __global__ void __launch_bounds__(256) k64_import_angles(Dev64 d, const double* __restrict__ phi_in)
 {
@@ -436,7 +458,7 @@ __global__ void __launch_bounds__(256) k64_import_angles(Dev64 d, const double* 
     d.phi[n] = p;
     double sn, cs;
     sincos(__dmul_rn(d.q, p), &sn, &cs);
-    d.vec[n] = make_double2(cs, sn);
+    d.vec[vpos_n(d, n)] = make_double2(cs, sn);
 }
 // scalar state edits: what = 0 begin a run at temperature x; 1 set a = x; 2 commit u sweeps (t += u) and v realizations;
 // 3 set t = u

@@ -14,7 +14,7 @@ bool geometry64(int rows, int cols, uint32_t* N, uint32_t* words)
     return true;
 }
 
-Layout64 make_layout64(uint32_t N, uint32_t words)
+Layout64 make_layout64(int rows, int cols, uint32_t N, uint32_t words)
 {
     Layout64 L;
     size_t o = 0;
@@ -27,7 +27,7 @@ Layout64 make_layout64(uint32_t N, uint32_t words)
     L.bits     = take(sizeof(uint32_t) * words);
     L.list     = take(sizeof(uint32_t) * N);
     L.list_counts = take(sizeof(uint32_t) * 2 * cdiv(words, mpr64::LIST_THREADS));
-    L.vec      = take(sizeof(double2) * N);
+    L.vec      = take(sizeof(double2) * 2 * (size_t)rows * (size_t)((cols + 1) / 2));
     L.acc      = take(sizeof(double) * N);
     L.acc2     = take(sizeof(double) * N);
     L.total = o;
@@ -92,7 +92,7 @@ mpr_status mpr64_query_workspace(int rows, int cols, size_t* bytes)
 {
     uint32_t N, words;
     if (!bytes || !geometry64(rows, cols, &N, &words)) return MPR_ERR_ARG;
-    *bytes = make_layout64(N, words).total;
+    *bytes = make_layout64(rows, cols, N, words).total;
     return MPR_OK;
 }
 
@@ -108,7 +108,7 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
 {
     uint32_t N, words;
     if (!out || !d_values || !d_sample_mask || !geometry64(rows, cols, &N, &words)) return MPR_ERR_ARG;
-    const Layout64 lay = make_layout64(N, words);
+    const Layout64 lay = make_layout64(rows, cols, N, words);
     if (!d_workspace || workspace_bytes < lay.total || ((uintptr_t)d_workspace & 255u)) return MPR_ERR_WORKSPACE;
     mpr64_ctx* ctx = new (std::nothrow) mpr64_ctx();
     if (!ctx) return MPR_ERR_ARG;
@@ -137,6 +137,7 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
     d.acc = (double*)(base + lay.acc);
     d.acc2 = (double*)(base + lay.acc2);
     d.rows = rows; d.cols = cols; d.N = N; d.words = words;
+    d.half = (cols + 1) / 2; d.plane = (uint32_t)rows * (uint32_t)d.half;
     d.q = 0.5; d.inv_q = 2.0;
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
     ctx->energy_blocks = rows < mpr64::E_BLOCKS ? rows : mpr64::E_BLOCKS;
