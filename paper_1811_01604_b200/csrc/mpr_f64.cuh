@@ -339,9 +339,14 @@ __global__ void __launch_bounds__(256) k64_halfsweep(Dev64 d, const uint32_t* __
             d.vec[self] = update_site_d<QHALF, ORMODE>(d.vec[self], up, dn, lf, rt, w0, w1, hd_scale, -1.0 / s.T, d.bc, d.bs, accepted);
         }
     }
-    if (count) {
+    if (count) {        // one global atomic per block (one per warp on the same address doubled the kernel's time)
+        __shared__ uint32_t s_acc;
+        if (threadIdx.x == 0) s_acc = 0;
+        __syncthreads();
         const uint32_t n_acc = __popc(__ballot_sync(0xFFFFFFFFu, accepted));
-        if ((threadIdx.x & 31) == 0 && n_acc) atomicAdd(&d.state->accepted, (unsigned long long)n_acc);
+        if ((threadIdx.x & 31) == 0 && n_acc) atomicAdd(&s_acc, n_acc);
+        __syncthreads();
+        if (threadIdx.x == 0 && s_acc) atomicAdd(&d.state->accepted, (unsigned long long)s_acc);
     }
 }
 
