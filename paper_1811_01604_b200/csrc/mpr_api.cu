@@ -163,6 +163,17 @@ pass_kernel pick_fused_kernel_fc(bool qhalf, int or_mode)
     if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true, FCT, false> : or_mode == 1 ? k_tilepass<true, 1, true, FCT, false> : k_tilepass<true, 2, true, FCT, false>;
     return or_mode == 0 ? k_tilepass<false, 0, true, FCT, false> : k_tilepass<false, 2, true, FCT, false>;
 }
+// Alg. 2 step 5 inside the pass (grids that are one tile)
+template <int FCT>
+pass_kernel pick_equil_kernel_fc(bool qhalf, int or_mode)
+{
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true, FCT, false, true> : or_mode == 1 ? k_tilepass<true, 1, true, FCT, false, true> : k_tilepass<true, 2, true, FCT, false, true>;
+    return or_mode == 0 ? k_tilepass<false, 0, true, FCT, false, true> : k_tilepass<false, 2, true, FCT, false, true>;
+}
+pass_kernel pick_equil_kernel(bool qhalf, int or_mode, bool std_fc)
+{
+    return std_fc ? pick_equil_kernel_fc<STD_FC>(qhalf, or_mode) : pick_equil_kernel_fc<0>(qhalf, or_mode);
+}
 pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused, bool std_fc, bool small_d)
 {
     if (fused) return std_fc ? pick_fused_kernel_fc<STD_FC>(qhalf, or_mode) : pick_fused_kernel_fc<0>(qhalf, or_mode);
@@ -179,11 +190,12 @@ void note_a(mpr_ctx* ctx, double a_min)
 // K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile.
 // flip = 0 / 1: read buffer ctx->cur ^ flip (known to the host); PER_GRID: each grid reads its own GridState::cur
 enum : uint32_t { PER_GRID = 2u };
-mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags, uint32_t real_no = 0)
+mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags, uint32_t real_no = 0, bool equil = false)
 {
     ctx->dirty = true;
     const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
-    const pass_kernel kern = pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC, ctx->small_d);
+    const pass_kernel kern = equil ? pick_equil_kernel(ctx->qhalf, (int)ctx->prm.or_mode, ctx->d.FC == STD_FC)
+                                   : pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC, ctx->small_d);
     if (!ctx->pf_dist) {
         int per_sm = 0, sms = 0;
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)kern, TILE_THREADS, ctx->smem_bytes));
@@ -413,7 +425,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     const size_t frame_bytes = (size_t)g.FR * g.FC * sizeof(float2);
     int smem_max = 0;
     if (!cuda_ok(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device), "smem attr")) return fail(MPR_ERR_CUDA);
-    const size_t budget = (size_t)smem_max - 2048;               // static shared memory of the kernel
+    const size_t budget = (size_t)smem_max - 4096;               // static shared memory of the kernel (2.7 KB with the state copy of k_tilepass<EQUIL>)
     d.use_spare = g.ntiles == 1 || g.H >= 4;                       // pointless when every pass is a single sweep
     if (frame_bytes + 10ull * max_entries > budget) d.use_spare = 0;
     ctx->smem_bytes = frame_bytes + (d.use_spare ? 10ull : 2ull) * max_entries;
@@ -435,6 +447,9 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
                         for (int sd = 0; sd < 2; ++sd) {
                             if (!qh && om == 1) continue;
                             if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, g.FC == STD_FC, sd), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                              (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
+                            if (fu && !sd &&
+                                !cuda_ok(cudaFuncSetAttribute((const void*)pick_equil_kernel(qh, om, g.FC == STD_FC), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                               (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
                         }
             have = ctx->smem_bytes;
@@ -527,6 +542,18 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
     uint32_t issued = 0;
     // the first slope check happens at i = n_fit, then every n_f sweeps (Alg. 2 step 5.4)
     uint32_t chunk = ctx->prm.n_fit + 1;
+    // grids that are one tile: steps 5.1-5.5 of up to k_max sweeps in ONE launch per grid batch (k_tilepass<EQUIL>)
+    while (d.ntiles == 1 && issued < cap) {
+        const uint32_t K = cap - issued < ctx->k_max ? cap - issued : ctx->k_max;
+        mpr_status s = launch_pass(ctx, K, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE, 0, true);
+        if (s != MPR_OK) return s;
+        issued += K;
+        CU(cudaMemcpyAsync(ctx->h_done, d.done_flags, sizeof(uint32_t) * d.batch, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        bool all = true;
+        for (int b = 0; b < d.batch; ++b) all = all && ctx->h_done[b];
+        if (all) break;
+    }
     while (issued < cap) {
         if (chunk > cap - issued) chunk = cap - issued;
         for (uint32_t j = 0; j < chunk; ++j) {

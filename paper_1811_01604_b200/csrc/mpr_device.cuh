@@ -665,6 +665,50 @@ __device__ __forceinline__ void update_pair(float2& vA, float2 upA, float2 dnA, 
     }
 }
 
+// ---------------------------------------------------------------------------
+// a6  equilibration controller: Alg. 2 steps 5.2-5.5 for
+// one grid, by ONE thread, after the sweep (5.1) whose accepted proposals sit in
+// GridState::accepted and whose energy is H.  Commits the sweep: t += 1 and the
+// vector buffers swap roles.  Called by k_controller (one block per grid after a
+// K = 1 tile pass) and, for a grid that is a single tile, from inside the tile pass.
+// ---------------------------------------------------------------------------
+// s: the grid's state, in global memory or a copy of it (the tile pass keeps one in shared memory while it loops)
+__device__ __forceinline__ void controller_step(const Dev& d, GridState& s, double H)
+{
+    const uint32_t i = s.i;
+    const double P = (double)s.n_free[0] + (double)s.n_free[1];
+    // 5.2 acceptance control: a(i+1) = 1 + (i+1)/k_a while A < A_targ
+    const double A = (double)s.accepted / P;
+    double a = s.a;
+    if (A < d.A_targ) a = 1.0 + (double)(i + 1u) / d.k_a;
+    // 5.3 e(i+1) = H / N_GP
+    const double e = H / d.n_bonds;
+    s.e_ring[(i + 1u) % d.n_fit] = e;
+    // 5.4 slope of the last n_fit energies e(i+2-n_fit) .. e(i+1): degree-1 Savitzky-Golay = OLS (R9)
+    double k = s.k;
+    if (i >= d.n_fit && i % d.n_f == 0) {
+        const int n = (int)d.n_fit;
+        const double tbar = 0.5 * (double)(n - 1);
+        double ebar = 0.0;
+        for (int j = 0; j < n; ++j) ebar += s.e_ring[(i + 2u - d.n_fit + j) % d.n_fit];
+        ebar /= (double)n;
+        double num = 0.0, den = 0.0;
+        for (int j = 0; j < n; ++j) {
+            const double dt = (double)j - tbar;
+            num += dt * (s.e_ring[(i + 2u - d.n_fit + j) % d.n_fit] - ebar);
+            den += dt * dt;
+        }
+        k = num / den;
+    }
+    // 5.5
+    s.i = i + 1u; s.t += 1u; s.cur ^= 1u; s.a = a; s.k = k; s.A_last = A; s.e_last = e; s.accepted = 0ull;
+    s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F) / a);
+    // unconditional chains burn in for exactly equil_cap sweeps: from their ordered start the energy rises, so the
+    // slope criterion would stop them at its first check (reading R23)
+    const bool go_on = d.burn_in_only ? i + 1u < d.equil_cap : (k < 0.0 && i + 1u < d.equil_cap);
+    if (!go_on) s.done = 1u;
+}
+
 // ---- TMA / mbarrier PTX (sm_100a) -------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
@@ -737,6 +781,27 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 //   PASS_COUNT       a5: accepted proposals of the core sites                          [FUSED only]
 //   PASS_ACCUMULATE  a7: acc += phi at the core's prediction sites (and the squared deviations for L212)
 // ---------------------------------------------------------------------------
+// a5 inside a tile pass: this warp's share of sum over the core's colour-1 sites (fixed ones too) of v . h, rows dealt
+// over the warps, float per row, double over the rows, then the warp's shuffle tree: a fixed order
+__device__ __forceinline__ double core_energy_warp(const float2* S, const TileGeom& tg, int H, int FC, int warp, int lane, int NW)
+{
+    double sum = 0.0;
+    for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
+        const int r = tg.r0 - H + lr;
+        float row = 0.0f;
+        // first colour-1 column of this row at or after the core's first column
+        for (int lc = H + ((r + tg.c0 + 1) & 1) + 2 * lane; lc < H + tg.TCc; lc += 64) {
+            const int off = lr * FC + lc;
+            const float2 v = S[off], up = S[off - FC], dn = S[off + FC], lf = S[off - 1], rt = S[off + 1];
+            row += fmaf(v.x, (up.x + dn.x) + (lf.x + rt.x), v.y * ((up.y + dn.y) + (lf.y + rt.y)));
+        }
+        sum += (double)row;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+    return sum;
+}
+
 // what one half-sweep of a tile pass needs to know (tabulated per CTA, see k_tilepass)
 struct __align__(16) HalfSweep { uint32_t n, cbase, c1, flags; };   // entries to walk, list offset, Philox counter word 1, HS_*
 enum : uint32_t { HS_ODD = 1u, HS_FRESH = 2u, HS_STASH = 4u, HS_RENORM = 8u };
@@ -747,7 +812,11 @@ constexpr int HS_CHUNK = 16;
 enum { DRAW_STORED = 0, DRAW_EVEN_STORE = 1, DRAW_ANY = 2 };
 template <int M> struct DrawTag { static constexpr int value = M; };
 
-template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD>
+// EQUIL (a grid that is ONE tile, with FUSED): Alg. 2 step 5 runs inside the pass -- after every sweep the energy and
+// the accepted count are reduced in the CTA, thread 0 takes steps 5.2-5.5 (controller_step) and the CTA goes on with the
+// new proposal width or stops; K is then the most sweeps this launch may do.  Bit for bit the sweeps of the K = 1
+// passes with k_controller between them (every sweep renormalises, as a K = 1 pass does), without 2 launches per sweep.
+template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD, bool EQUIL = false>
 __global__ void __launch_bounds__(TILE_THREADS, TILE_THREADS >= 384 ? 2 : 3)
 k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
            uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist, uint32_t real_no)
@@ -814,7 +883,17 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             bulk_prefetch(d.entries + (size_t)gd * d.entry_stride + (size_t)(tile + pf_dist) * d.tile_entries,
                           d.max_entries * (uint32_t)sizeof(uint16_t));
     }
-    const float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f, nlT = st.neg_log2e_over_T;
+    float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f;
+    const float nlT = st.neg_log2e_over_T;
+    __shared__ float s_ctrl[2];            // EQUIL: the controller's verdict for the CTA: new hd_scale, stop flag
+    bool finished = false;
+    GridState* s_state = nullptr;          // EQUIL: the grid's state while the CTA loops (written back at the end)
+    if constexpr (EQUIL) {
+        __shared__ GridState s_state_copy;
+        s_state = &s_state_copy;
+        for (uint32_t w = tid; w < sizeof(GridState) / 4; w += NT)
+            reinterpret_cast<uint32_t*>(s_state)[w] = reinterpret_cast<const uint32_t*>(&d.states[g])[w];
+    }
     const uint32_t t0 = st.t + t_off;
     const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H), ncorr = d.cols - FC;
     const bool count = FUSED && (flags & PASS_COUNT);
@@ -827,14 +906,14 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1).  What a half-sweep needs to
     // know is tabulated by one warp for 16 half-sweeps at a time (HalfSweep), so that the other warps do not redo it.
 #pragma unroll 1
-    for (uint32_t j0 = 0; j0 < 2u * K; j0 += HS_CHUNK) {
+    for (uint32_t j0 = 0; j0 < 2u * K && !(EQUIL && finished); j0 += HS_CHUNK) {
         if (tid < HS_CHUNK && j0 + tid < 2u * K) {
             const uint32_t j = j0 + tid, s = j >> 1, c = j & 1u, t = t0 + s;
             const bool odd = t & 1u;
             const bool fresh = !odd || s == 0 || !use_spare;            // draw a new Philox block for (site, t >> 1)
             const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
             // |v| = 1 against rounding drift: in the sweep whose result leaves the tile, and every 8th sweep of a long pass
-            const bool renorm = s + 1 == K || (s & 7u) == 7u;
+            const bool renorm = EQUIL || s + 1 == K || (s & 7u) == 7u;
             const uint32_t R = 2u * K - 1u - j;                          // rings still needed: 0 .. R
             HalfSweep h;
             h.n = s_cle[c][R < (uint32_t)MAX_H ? R : (uint32_t)MAX_H - 1u];
@@ -846,7 +925,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         __syncthreads();
         const uint32_t j_end = min(2u * K - j0, (uint32_t)HS_CHUNK);
 #pragma unroll 1
-      for (uint32_t jj = 0; jj < j_end; ++jj) {
+      for (uint32_t jj = 0; jj < j_end && !(EQUIL && finished); ++jj) {
         const HalfSweep h = s_hs[jj];
         const bool odd = h.flags & HS_ODD, fresh = h.flags & HS_FRESH, stash = h.flags & HS_STASH, renorm = h.flags & HS_RENORM;
         const uint32_t n = h.n, tc1 = h.c1;
@@ -904,6 +983,28 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         else if (!odd && stash) half_sweep(DrawTag<DRAW_EVEN_STORE>{});
         else half_sweep(DrawTag<DRAW_ANY>{});
         __syncthreads();
+        if constexpr (EQUIL) {
+            if (h.flags >> 8) {                 // a whole sweep is done (colour 1 was its second half): steps 5.2-5.5
+                n_accepted = __reduce_add_sync(0xFFFFFFFFu, n_accepted);
+                if (lane == 0 && n_accepted) atomicAdd(&s_accepted, n_accepted);
+                n_accepted = 0;
+                const double e_warp = core_energy_warp(S, tg, H, FC, warp, lane, NW);
+                if (lane == 0) s_red[warp] = e_warp;
+                __syncthreads();
+                if (tid == 0) {
+                    double sum = 0.0;
+                    for (int w = 0; w < NW; ++w) sum += s_red[w];
+                    s_state->accepted = (unsigned long long)s_accepted;
+                    s_accepted = 0;
+                    controller_step(d, *s_state, -sum);
+                    s_ctrl[0] = s_state->hd_scale;
+                    s_ctrl[1] = s_state->done ? 1.0f : 0.0f;
+                }
+                __syncthreads();
+                hs = s_ctrl[0]; hc1 = hs * 5.9604644775390625e-08f;
+                finished = s_ctrl[1] != 0.0f;
+            }
+        }
       }
     }
     fence_proxy_async_smem();
@@ -981,27 +1082,14 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             }
         }
     }
-    if (FUSED) {
+    if (FUSED && !EQUIL) {
         if (count) {
             n_accepted = __reduce_add_sync(0xFFFFFFFFu, n_accepted);
             if (lane == 0 && n_accepted) atomicAdd(&s_accepted, n_accepted);
         }
         if (flags & PASS_ENERGY) {
             // a5: H_tile = - sum over the core's colour-1 sites (fixed ones too) of v . h; fixed summation order
-            double sum = 0.0;
-            for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
-                const int r = tg.r0 - H + lr;
-                float row = 0.0f;
-                // first colour-1 column of this row at or after the core's first column
-                for (int lc = H + ((r + tg.c0 + 1) & 1) + 2 * lane; lc < H + tg.TCc; lc += 64) {
-                    const int off = lr * FC + lc;
-                    const float2 v = S[off], up = S[off - FC], dn = S[off + FC], lf = S[off - 1], rt = S[off + 1];
-                    row += fmaf(v.x, (up.x + dn.x) + (lf.x + rt.x), v.y * ((up.y + dn.y) + (lf.y + rt.y)));
-                }
-                sum += (double)row;
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+            const double sum = core_energy_warp(S, tg, H, FC, warp, lane, NW);
             if (lane == 0) s_red[warp] = sum;
         }
         __syncthreads();
@@ -1013,6 +1101,13 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
                 d.e_partials[(size_t)g * d.n_partials + tile] = -s;
             }
         }
+    }
+    if constexpr (EQUIL) {
+        // the state goes back: cur = where the row copies above put the vectors, whatever the sweep count
+        if (tid == 0) { s_state->cur = src_buf ^ 1u; if (s_state->done) d.done_flags[g] = 1u; }
+        __syncthreads();
+        for (uint32_t w = tid; w < sizeof(GridState) / 4; w += NT)
+            reinterpret_cast<uint32_t*>(&d.states[g])[w] = reinterpret_cast<const uint32_t*>(s_state)[w];
     }
     bulk_commit_wait_read();      // shared memory must stay until the row copies have read it
 }
@@ -1158,38 +1253,8 @@ __global__ void k_controller(Dev d)
     if (s.done) return;
     const double H = sum_energy_partials(d, g, d.ntiles);
     if (threadIdx.x != 0) return;
-    const uint32_t i = s.i;
-    const double P = (double)s.n_free[0] + (double)s.n_free[1];
-    // 5.2 acceptance control: a(i+1) = 1 + (i+1)/k_a while A < A_targ
-    const double A = (double)s.accepted / P;
-    double a = s.a;
-    if (A < d.A_targ) a = 1.0 + (double)(i + 1u) / d.k_a;
-    // 5.3 e(i+1) = H / N_GP
-    const double e = H / d.n_bonds;
-    s.e_ring[(i + 1u) % d.n_fit] = e;
-    // 5.4 slope of the last n_fit energies e(i+2-n_fit) .. e(i+1): degree-1 Savitzky-Golay = OLS (R9)
-    double k = s.k;
-    if (i >= d.n_fit && i % d.n_f == 0) {
-        const int n = (int)d.n_fit;
-        const double tbar = 0.5 * (double)(n - 1);
-        double ebar = 0.0;
-        for (int j = 0; j < n; ++j) ebar += s.e_ring[(i + 2u - d.n_fit + j) % d.n_fit];
-        ebar /= (double)n;
-        double num = 0.0, den = 0.0;
-        for (int j = 0; j < n; ++j) {
-            const double dt = (double)j - tbar;
-            num += dt * (s.e_ring[(i + 2u - d.n_fit + j) % d.n_fit] - ebar);
-            den += dt * dt;
-        }
-        k = num / den;
-    }
-    // 5.5
-    s.i = i + 1u; s.t += 1u; s.cur ^= 1u; s.a = a; s.k = k; s.A_last = A; s.e_last = e; s.accepted = 0ull;
-    s.hd_scale = (float)((double)d.q * (0.5 * (double)TWO_PI_F) / a);
-    // unconditional chains burn in for exactly equil_cap sweeps: from their ordered start the energy rises, so the
-    // slope criterion would stop them at its first check (reading R23)
-    const bool go_on = d.burn_in_only ? i + 1u < d.equil_cap : (k < 0.0 && i + 1u < d.equil_cap);
-    if (!go_on) { s.done = 1u; d.done_flags[g] = 1u; }
+    controller_step(d, s, H);
+    if (s.done) d.done_flags[g] = 1u;
 }
 
 // scalar state edits ---------------------------------------------------------
