@@ -861,3 +861,26 @@ def test_equilibration_caps_and_windows_follow_the_oracle(torch_cuda, mpr, orc, 
     if st.equil_sweeps == eq["sweeps"]:
         assert st.a == pytest.approx(eq["a"], rel=1e-12)
     ctx.close()
+
+
+def test_in_pass_equilibration_is_independent_of_the_sweeps_per_launch(torch_cuda, mpr):
+    """A grid that is one tile equilibrates inside the tile pass; with the experiment hook MPR_KMAX = 7 the same
+    equilibration takes several launches that start at even and odd sweep indices: same state bit for bit."""
+    import os
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+    out = []
+    for kmax in (None, "7"):
+        if kmax:
+            os.environ["MPR_KMAX"] = kmax
+        try:
+            ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+        finally:
+            os.environ.pop("MPR_KMAX", None)
+        ctx.set_params(T, seed=99, equil_cap=1000).equilibrate()
+        st = ctx.get_stats()[0]
+        out.append((ctx.get_angles().cpu().numpy(), st.equil_sweeps, st.a, st.e_last, st.t, ctx.launch_count()))
+        ctx.close()
+    assert np.array_equal(out[0][0], out[1][0]) and out[0][1:5] == out[1][1:5]
+    assert out[1][5] > out[0][5]
