@@ -46,6 +46,9 @@ def parse_args():
                     help="chains per grid in step 6 (DESIGN.md reading R25); 1 = the paper's single chain")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-inference", action="store_true", help="skip the Alg. 2 step 4 timing (extra key, not in the step)")
+    ap.add_argument("--sfu-peak", action="store_true",
+                    help="run the pipe-rate micro-benchmarks (MUFU / FFMA / FFMA2 / IMAD.WIDE / LOP3 / IMAD) with the SM clock "
+                         "held during each, print one JSON line and exit (BASELINE.md section 4)")
     ap.add_argument("--no-f64", action="store_true",
                     help="skip the double-precision run of the same workload (extra key 'double_precision', not in the step)")
     return ap.parse_args()
@@ -135,6 +138,43 @@ ISSUE_PEAK_PER_S = 148 * 4 * 32 * 1.965e9
 ALGORITHMIC_INSTR_PER_UPDATE = 68.0
 # DRAM bytes of one 4-sweep tile-pass launch on cfg4 from the committed ncu capture (profiles/r01g_tilepass_v7.md)
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4": 244.9e6}
+
+
+# ---------------------------------------------------------------------------
+# measured pipe rates (the roofline's special-function denominator)
+# ---------------------------------------------------------------------------
+MICROBENCH_OPS = {"mufu_ex2": 0, "mufu_rcp": 1, "ffma": 2, "ffma2": 3, "imad_wide": 4, "lop3": 5, "imad": 6}
+
+
+def run_sfu_peak():
+    """csrc/mpr_microbench.cu through its C ABI: thread-level results per second of back-to-back independent
+    instruction chains on every SM, with the SM clock sampled (NVML) while each runs."""
+    import ctypes as C
+    import torch
+    from paper_1811_01604_b200 import build as mpr_build
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --sfu-peak needs a CUDA device")
+    torch.cuda.init()
+    torch.zeros(1, device="cuda")                       # the primary context the library's runtime shares
+    lib = C.CDLL(mpr_build.build_microbench())
+    lib.mprbench_rate.argtypes = [C.c_int, C.c_uint32, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    out = {"kernel": "csrc/mpr_microbench.cu k_chain<op>: 8 independent chains per thread, 2 x 1024 threads per SM",
+           "rates": {}}
+    for name, op in MICROBENCH_OPS.items():
+        rate, sms = C.c_double(), C.c_int()
+        with ClockSampler(0) as clk:
+            rc = lib.mprbench_rate(op, 400_000, C.byref(rate), C.byref(sms))     # ~0.1-0.3 s per operation
+        if rc != 0:
+            raise RuntimeError(f"mprbench_rate({name}) failed with {rc}")
+        c = clk.summary()
+        mhz = c["sm_mhz"] or 0.0
+        per_clk_sm = rate.value / (sms.value * mhz * 1e6) if mhz else None
+        out["rates"][name] = {"per_s": rate.value, "sm_mhz_held": mhz, "reasons": c["reasons"], "sm_count": sms.value,
+                              "results_per_clk_per_sm": per_clk_sm,
+                              "warp_instr_per_clk_per_subpartition": per_clk_sm / 128.0 if per_clk_sm else None}
+    out["sfu_peak_per_s"] = min(out["rates"]["mufu_ex2"]["per_s"], out["rates"]["mufu_rcp"]["per_s"])
+    out["sfu_peak_used_by_bench"] = SFU_PEAK_PER_S
+    print(json.dumps(out))
 
 
 # ---------------------------------------------------------------------------
@@ -434,6 +474,10 @@ def run_b200(args, w):
 
 def main():
     args = parse_args()
+    if args.sfu_peak:
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_sfu_peak()
+        return
     from paper_1811_01604_b200 import synth
     rank = int(os.environ.get("RANK", "0"))
     if args.impl == "reference" and rank != 0:

@@ -128,8 +128,8 @@ mpr_status mpr_simulate(mpr_ctx* ctx);
 
 /* Alg. 2 step 7 + back-transform (L148, L210-212): d_out device float
  * [batch][rows][cols]; prediction sites = z_min + mean(phi) (z_max - z_min)/(2 pi)
- * over the realizations accumulated so far (>= 1), sample sites = the input
- * value bit for bit.  Asynchronous. */
+ * over the realizations accumulated so far (>= 1, else MPR_ERR_STATE), sample
+ * sites = the input value bit for bit.  Asynchronous. */
 mpr_status mpr_predict(mpr_ctx* ctx, float* d_out);
 
 /* "Statistics of M realizations" (Alg. 2 step 7, L212; L148: the realizations sample the conditional
@@ -200,6 +200,26 @@ mpr_status mpr_energy_table(int rows, int cols, const mpr_params* h_params, cons
  * R24).  Host arithmetic on n_T numbers.  Errors: ARG. */
 mpr_status mpr_infer_temperature(const float* h_T, const double* h_e, int n_T, double e_s, double* h_T_hat);
 
+/* The ladder step 4.2 uses when the caller has none: n_T temperatures h_T[k] = T_c * h_factors[k] around
+ * T_c = 2 N_GP (1 + e_s) / (N - 1), the temperature at which the low-temperature equipartition energy
+ * e(T) = -1 + (N - 1) T / (2 N_GP) of a rows x cols grid (N - 1 harmonic modes, N_GP bonds, J = 1; DESIGN.md
+ * reading R15) equals e_s.  That line only CENTRES the ladder; e(T_k, L) itself comes from the chains of
+ * mpr_energy_table.  h_factors host float [n_T], ascending, > 0; NULL = {1/4, 1/2, 1, 2, 4} (then n_T must be 5).
+ * h_T host float [n_T].  Host arithmetic.  Errors: ARG. */
+mpr_status mpr_default_ladder(int rows, int cols, double e_s, const float* h_factors, int n_T, float* h_T);
+
+/* Alg. 2 step 4 as ONE call (L97-111, L186-190), for every grid of `ctx` (which needs only mpr_create):
+ * e_s by Eq. 4 with q of h_params (mpr_sample_energy), the ladder of mpr_default_ladder around it, e(T_k, L)
+ * of Eq. 5 from unconditional chains (mpr_energy_table: h_params->equil_cap burn-in sweeps, n_meas measured
+ * ones, h_params->seed), and T-hat = argmin |e_s - e(T, L)| over the ladder's interpolant (mpr_infer_temperature).
+ * d_workspace: device, at least mpr_query_workspace(n_T, rows, cols) bytes, 256-byte aligned; it is scratch for the
+ * unconditional chains (one grid's ladder at a time) and distinct from the context's own workspace.
+ * h_T_hat host double [batch]; h_e_s host double [batch] or NULL.  The result goes to mpr_set_params as T.
+ * Synchronises.  Errors: ARG, NO_SAMPLES (a grid without a pair of neighbouring samples), WORKSPACE, CUDA. */
+mpr_status mpr_infer_temperature_auto(mpr_ctx* ctx, const mpr_params* h_params, const float* h_factors, int n_T,
+                                      uint32_t n_meas, void* d_workspace, size_t workspace_bytes,
+                                      double* h_T_hat, double* h_e_s);
+
 /* ---- double-precision path (Table 2 against Table 3) ----
  * The same method with data, spin state, every site update and the realization sums in double: one grid per
  * context, values and outputs are double, "2 pi" is the double nearest 2 pi, Eq. 1 keeps its pinned operation
@@ -253,6 +273,14 @@ mpr_status mpr_get_mask_bits(mpr_ctx* ctx, uint32_t* d_bits);
 mpr_status mpr_get_stats(mpr_ctx* ctx, mpr_stats* h_out);
 /* Number of kernels this context has launched so far (bench bookkeeping). */
 mpr_status mpr_get_launch_count(mpr_ctx* ctx, uint64_t* h_count);
+/* Temporal blocking of the sweep kernel: one launch advances every tile by up to
+ * `k` whole sweeps of Alg. 1 on a shared-memory copy of the tile and its halo.  The result does not depend
+ * on k (halo sites are recomputed bit for bit: the random numbers are keyed by site and sweep); this call
+ * exists so that tests can drive every depth.  k = 0 restores the default (halo / 2; 1024 for a grid that is
+ * one tile); k above the default is MPR_ERR_ARG.  Host-side only. */
+mpr_status mpr_set_pass_depth(mpr_ctx* ctx, uint32_t k);
+/* The tiling mpr_create chose: core tile rows x cols, halo width, and the current pass depth. */
+mpr_status mpr_get_tiling(mpr_ctx* ctx, int* h_tile_rows, int* h_tile_cols, int* h_halo, uint32_t* h_pass_depth);
 
 const char* mpr_status_string(mpr_status s);
 /* Text of the last CUDA error seen by this library in the calling process. */

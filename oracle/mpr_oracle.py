@@ -366,6 +366,28 @@ def infer_T(e_s: float, Ts, es) -> float:
     return Ts[k]
 
 
+def default_ladder(rows: int, cols: int, e_s: float, factors=(0.25, 0.5, 1.0, 2.0, 4.0)):
+    """The ladder of step 4.2 when the caller has none: temperatures T_c f_k around the T_c at which the low-temperature
+    equipartition energy per bond equals e_s (reading R15): N - 1 harmonic modes carry T / 2 each (k_B = 1), shared by
+    N_GP bonds above the ground state e = -1, so 1 + e_s = (N - 1) T_c / (2 N_GP).  Float32 like the temperatures the
+    CUDA path takes."""
+    N = rows * cols
+    T_c = max(2.0 * n_bonds(rows, cols) * (1.0 + e_s) / (N - 1), 1e-12)
+    return [float(np.float32(T_c * float(np.float32(f)))) for f in factors]
+
+
+def infer_T_auto(phi, mask, p: Params, n_meas: int, factors=(0.25, 0.5, 1.0, 2.0, 4.0)):
+    """Alg. 2 step 4 for one grid (L97-111, L186-190): 4.1 e_s (Eq. 4), 4.2 the ladder's e(T_k, L) from unconditional
+    chains (Eq. 5) and T-hat = argmin |e_s - e(T, L)| (L111).  Returns (T_hat, e_s, ladder, table)."""
+    rows, cols = phi.shape
+    e_s, n_sp = sample_energy(phi, mask, p.q)
+    if n_sp == 0:
+        raise ValueError("no pair of neighbouring samples: e_s is undefined")
+    Ts = default_ladder(rows, cols, e_s, factors)
+    table = energy_table(rows, cols, Ts, p, n_meas)
+    return infer_T(e_s, Ts, table), e_s, Ts, table
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())
 

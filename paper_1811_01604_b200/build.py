@@ -15,6 +15,9 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libmpr_b200.so")
 SOURCES = ["mpr_api.cu"]
 HEADERS = ["mpr_device.cuh", "mpr_f64.cuh", "mpr_f64_api.inl"]
+# pipe-rate micro-benchmarks behind `bench.py --sfu-peak` (the roofline's measured denominators); not part of the MPR library
+MICROBENCH_LIB = os.path.join(_HERE, "libmpr_microbench.so")
+MICROBENCH_SOURCES = ["mpr_microbench.cu"]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -37,7 +40,15 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def build_microbench(force: bool = False) -> str:
+    srcs = [os.path.join(CSRC, f) for f in MICROBENCH_SOURCES]
+    if force or not os.path.exists(MICROBENCH_LIB) or any(os.path.getmtime(f) > os.path.getmtime(MICROBENCH_LIB) for f in srcs):
+        subprocess.run([_nvcc(), *NVCC_FLAGS, "-o", MICROBENCH_LIB] + srcs, check=True)
+    return MICROBENCH_LIB
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
+    build_microbench(force)
     if force or _stale():
         cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
         if verbose:

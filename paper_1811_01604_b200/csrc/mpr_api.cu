@@ -10,7 +10,9 @@
 #include <cstdlib>
 #include <cstring>
 #include <cudaTypedefs.h>
+#include <mutex>
 #include <new>
+#include <vector>
 
 using namespace mpr;
 
@@ -46,7 +48,8 @@ constexpr long RESIDENT_TILE_PASSES = 148L * 3L;
 // Tile shape.  A grid that fits one frame is a single tile with a
 // two-site zero border (any number of sweeps per pass); otherwise TR x TC cores with a halo of H
 // (H/2 sweeps per pass).  TC, H and FC are even so that every core row starts on a 16-byte boundary
-// of shared memory (bulk row copies).  MPR_TILE="TR,TC,H" overrides the default for experiments.
+// of shared memory (bulk row copies).  (Built with -DMPR_EXPERIMENT_HOOKS, which the shipped library is not,
+// MPR_TILE="TR,TC,H" overrides the default.)
 void choose_tiles(int batch, int rows, int cols, Geometry* g)
 {
     int TR = 64, TC = 64, H = 8;
@@ -56,11 +59,13 @@ void choose_tiles(int batch, int rows, int cols, Geometry* g)
     if ((long)batch * ntx64 * ((rows + 63) / 64) < RESIDENT_TILE_PASSES)
         for (int tr = 16; tr < 64; tr += 8)
             if ((long)batch * ntx64 * ((rows + tr - 1) / tr) <= RESIDENT_TILE_PASSES) { TR = tr; break; }
+#ifdef MPR_EXPERIMENT_HOOKS
     if (const char* e = getenv("MPR_TILE")) {
         int a, b, c;
         if (sscanf(e, "%d,%d,%d", &a, &b, &c) == 3 && a >= 8 && b >= 8 && (b & 1) == 0 && c >= 2 && c <= MAX_H &&
             (c & 1) == 0 && (a + 2 * c) * (b + 2 * c + 2) <= 65535 && a + 2 * c <= 255 && b + 2 * c <= 252) { TR = a; TC = b; H = c; }
     }
+#endif
     if ((long)rows * cols <= 128L * 128L && rows <= 250 && cols <= 250) { TR = rows; TC = cols; H = 2; }
     g->TR = TR; g->TC = TC; g->H = H; g->FR = TR + 2 * H;
     g->FC = ((TC + 2 * H + 1) & ~3) + 2;        // >= TC + 2H and = 2 (mod 4): a column's rows spread over the banks
@@ -127,7 +132,7 @@ struct mpr_ctx {
     bool         qhalf;
     bool         dirty;           // vectors changed since d.phi was last written at the free sites
     int          device;          // device the workspace lives on
-    bool         no_pdl;          // MPR_NO_PDL=1: launch the tile passes without programmatic stream serialization (experiments)
+    bool         no_pdl;          // launch the tile passes without programmatic stream serialization (-DMPR_EXPERIMENT_HOOKS builds only)
     bool         unconditional;   // no data: every node free, ordered start (Alg. 2 step 4.2)
     double       a_min;           // smallest proposal-width parameter a over the grids, as far as the host knows it (0 = unknown)
     bool         small_d;         // every grid's proposal half-rotation q pi / (2 a) is below SMALL_HD (host knowledge of a)
@@ -135,6 +140,7 @@ struct mpr_ctx {
     uint32_t     pf_dist;         // tile passes resident on the device at once (L2 prefetch distance), 0 = not yet known
     int          active;          // states the tile passes cover: the grids (chain 0), or every chain inside mpr_simulate
     bool         forked;          // chains >= 1 hold a copy of their grid's state (until chain 0 alone moves again)
+    uint64_t     n_realizations;  // realizations accumulated per grid (all of its chains) since mpr_set_params
 };
 
 namespace {
@@ -201,7 +207,9 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)kern, TILE_THREADS, ctx->smem_bytes));
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
         ctx->pf_dist = (uint32_t)(per_sm > 0 ? per_sm * sms : sms);
-        if (const char* e = getenv("MPR_PF_DIST")) ctx->pf_dist = (uint32_t)atoi(e) ? (uint32_t)atoi(e) : ctx->pf_dist;   // experiments
+#ifdef MPR_EXPERIMENT_HOOKS
+        if (const char* e = getenv("MPR_PF_DIST")) ctx->pf_dist = (uint32_t)atoi(e) ? (uint32_t)atoi(e) : ctx->pf_dist;
+#endif
     }
     const uint32_t src_sel = flip == PER_GRID ? PER_GRID : (ctx->cur ^ flip);
     // programmatic stream serialization: this pass's CTAs may start (and load their tile lists) while the last
@@ -345,7 +353,9 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     }
     ctx->state = CREATED;
     ctx->unconditional = unconditional;
+#ifdef MPR_EXPERIMENT_HOOKS
     ctx->no_pdl = getenv("MPR_NO_PDL") != nullptr;
+#endif
     ctx->prm.q = 0.5f; ctx->d.q = 0.5f; ctx->d.inv_q = 2.0f;      // until mpr_set_params says otherwise (L89)
     char* base = (char*)d_workspace;
     Dev& d = ctx->d;
@@ -396,6 +406,8 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     k_tile_scan<<<batch, 32, 0, s>>>(d);
     const size_t fill_smem = (size_t)g.FR * g.FC * sizeof(uint16_t);
     {
+        static std::mutex fill_lock;                  // contexts may be created from several host threads
+        std::lock_guard<std::mutex> hold(fill_lock);
         static size_t fill_set[64] = {};              // raised only, as for the tile pass below
         size_t& have = fill_set[ctx->device & 63];
         if (fill_smem > 40960 && fill_smem > have) {
@@ -430,14 +442,12 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     if (frame_bytes + 10ull * max_entries > budget) d.use_spare = 0;
     ctx->smem_bytes = frame_bytes + (d.use_spare ? 10ull : 2ull) * max_entries;
     if (ctx->smem_bytes > budget) return fail(MPR_ERR_WORKSPACE);
-    ctx->k_max = g.ntiles == 1 ? 1024u : (uint32_t)(g.H / 2);
-    if (const char* e = getenv("MPR_KMAX")) {
-        const int k = atoi(e);
-        if (k >= 1 && (g.ntiles == 1 || k <= g.H / 2)) ctx->k_max = (uint32_t)k;
-    }
+    ctx->k_max = g.ntiles == 1 ? 1024u : (uint32_t)(g.H / 2);        // mpr_set_pass_depth lowers it (diagnostic)
     // The attribute belongs to the kernel, not to this context: it is only ever raised (per device and frame-pitch
     // variant), so that a context created later with smaller tiles does not take the room of an earlier one away.
     {
+        static std::mutex attr_lock;                  // contexts may be created from several host threads
+        std::lock_guard<std::mutex> hold(attr_lock);
         static size_t attr_set[64][2] = {};
         size_t& have = attr_set[ctx->device & 63][g.FC == STD_FC ? 1 : 0];
         if (ctx->smem_bytes > have) {
@@ -527,6 +537,7 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     ctx->dirty = false;
     ctx->cur = 0;
     ctx->forked = false;
+    ctx->n_realizations = 0;
     note_a(ctx, 1.0);
     return MPR_OK;
 }
@@ -540,37 +551,47 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
     ctx->forked = false;           // chain 0 of every grid moves alone (Alg. 2 step 5 is one chain per grid)
     const uint32_t cap = ctx->prm.equil_cap;
     uint32_t issued = 0;
-    // the first slope check happens at i = n_fit, then every n_f sweeps (Alg. 2 step 5.4)
-    uint32_t chunk = ctx->prm.n_fit + 1;
-    // grids that are one tile: steps 5.1-5.5 of up to k_max sweeps in ONE launch per grid batch (k_tilepass<EQUIL>)
-    while (d.ntiles == 1 && issued < cap) {
-        const uint32_t K = cap - issued < ctx->k_max ? cap - issued : ctx->k_max;
-        mpr_status s = launch_pass(ctx, K, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE, 0, true);
-        if (s != MPR_OK) return s;
-        issued += K;
+    auto all_done = [&](bool* all) -> mpr_status {
         CU(cudaMemcpyAsync(ctx->h_done, d.done_flags, sizeof(uint32_t) * d.batch, cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
-        bool all = true;
-        for (int b = 0; b < d.batch; ++b) all = all && ctx->h_done[b];
-        if (all) break;
-    }
-    while (issued < cap) {
-        if (chunk > cap - issued) chunk = cap - issued;
-        for (uint32_t j = 0; j < chunk; ++j) {
-            // 5.1 one sweep with the energy (5.3) and the accepted count fused; the controller does
-            // 5.2, 5.4, 5.5 and commits the sweep (t, buffer swap) for the grids still running
-            mpr_status s = launch_pass(ctx, 1, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
+        *all = true;
+        for (int b = 0; b < d.batch; ++b) *all = *all && ctx->h_done[b];
+        return MPR_OK;
+    };
+    if (d.ntiles == 1) {
+        // grids that are one tile: steps 5.1-5.5 of up to k_max sweeps in ONE launch per grid batch (k_tilepass<EQUIL>)
+        while (issued < cap) {
+            const uint32_t K = cap - issued < ctx->k_max ? cap - issued : ctx->k_max;
+            mpr_status s = launch_pass(ctx, K, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE, 0, true);
             if (s != MPR_OK) return s;
-            k_controller<<<d.batch, REDUCE_THREADS, 0, ctx->stream>>>(d);
-            CU_LAUNCH();
+            issued += K;
+            bool all = false;
+            s = all_done(&all);
+            if (s != MPR_OK) return s;
+            if (all) break;
         }
-        issued += chunk;
-        CU(cudaMemcpyAsync(ctx->h_done, d.done_flags, sizeof(uint32_t) * d.batch, cudaMemcpyDeviceToHost, ctx->stream));
-        CU(cudaStreamSynchronize(ctx->stream));
-        bool all = true;
-        for (int b = 0; b < d.batch; ++b) all = all && ctx->h_done[b];
-        if (all) break;
-        chunk = ctx->prm.n_f;
+    } else {
+        // The controller checks the slope after the sweep with index i when i >= n_fit and i % n_f == 0 (step 5.4), so
+        // a grid can only stop after i + 1 sweeps with i such an index: the host polls the flags exactly there.
+        const uint32_t n_f = ctx->prm.n_f;
+        uint32_t chunk = (ctx->prm.n_fit + n_f - 1) / n_f * n_f + 1;
+        while (issued < cap) {
+            if (chunk > cap - issued) chunk = cap - issued;
+            for (uint32_t j = 0; j < chunk; ++j) {
+                // 5.1 one sweep with the energy (5.3) and the accepted count fused; the controller does
+                // 5.2, 5.4, 5.5 and commits the sweep (t, buffer swap) for the grids still running
+                mpr_status s = launch_pass(ctx, 1, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
+                if (s != MPR_OK) return s;
+                k_controller<<<d.batch, REDUCE_THREADS, 0, ctx->stream>>>(d);
+                CU_LAUNCH();
+            }
+            issued += chunk;
+            bool all = false;
+            mpr_status s = all_done(&all);
+            if (s != MPR_OK) return s;
+            if (all) break;
+            chunk = n_f;
+        }
     }
     // the grids stopped after different numbers of sweeps: bring every state into the same vector buffer
     mpr_status fs = fetch_states(ctx);
@@ -624,6 +645,7 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
     k_commit<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, d.chains > 1 ? d.nv : d.batch, t_off, flip, n_real);
     CU_LAUNCH();
     ctx->cur ^= flip;
+    ctx->n_realizations += (uint64_t)n_real * (uint64_t)d.chains;
     return MPR_OK;
 }
 
@@ -631,7 +653,7 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out)
 {
     if (!ctx || !d_out) return MPR_ERR_ARG;
     ENTER(ctx);
-    if (ctx->state != READY) return MPR_ERR_STATE;
+    if (ctx->state != READY || ctx->n_realizations == 0) return MPR_ERR_STATE;     // the mean of no realization is 0 / 0
     const Dev& d = ctx->d;
     k_predict<<<site_grid(ctx), 256, 0, ctx->stream>>>(d, d_out);
     CU_LAUNCH();
@@ -748,6 +770,54 @@ mpr_status mpr_infer_temperature(const float* h_T, const double* h_e, int n_T, d
     for (int k = 1; k < n_T; ++k)
         if (std::fabs(h_e[k] - e_s) < std::fabs(h_e[best] - e_s)) best = k;
     *h_T_hat = (double)h_T[best];
+    return MPR_OK;
+}
+
+mpr_status mpr_default_ladder(int rows, int cols, double e_s, const float* h_factors, int n_T, float* h_T)
+{
+    if (rows < 2 || cols < 2 || !h_T || n_T < 1 || !std::isfinite(e_s)) return MPR_ERR_ARG;
+    static const float standard[5] = {0.25f, 0.5f, 1.0f, 2.0f, 4.0f};
+    if (!h_factors) { if (n_T != 5) return MPR_ERR_ARG; h_factors = standard; }
+    for (int k = 0; k < n_T; ++k)
+        if (!(h_factors[k] > 0.0f) || !std::isfinite(h_factors[k]) || (k && !(h_factors[k] > h_factors[k - 1]))) return MPR_ERR_ARG;
+    // low-temperature equipartition, e(T) = -1 + (N - 1) T / (2 N_GP): N - 1 harmonic modes of T / 2 each over
+    // N_GP bonds (J = 1; reading R15).  Its crossing with e_s only centres the ladder.
+    const double n_gp = (double)rows * (cols - 1) + (double)cols * (rows - 1);
+    double centre = 2.0 * n_gp * (1.0 + e_s) / ((double)rows * (double)cols - 1.0);
+    if (!(centre > 1e-12)) centre = 1e-12;
+    for (int k = 0; k < n_T; ++k) h_T[k] = (float)(centre * (double)h_factors[k]);
+    return MPR_OK;
+}
+
+mpr_status mpr_infer_temperature_auto(mpr_ctx* ctx, const mpr_params* h_params, const float* h_factors, int n_T,
+                                      uint32_t n_meas, void* d_workspace, size_t workspace_bytes,
+                                      double* h_T_hat, double* h_e_s)
+{
+    if (!ctx || !h_params || !h_T_hat || n_T < 1 || n_T > 4096 || n_meas == 0) return MPR_ERR_ARG;
+    const int batch = ctx->d.batch, rows = ctx->d.rows, cols = ctx->d.cols;
+    std::vector<double> e_s, table, T_hat;
+    std::vector<uint64_t> pairs;
+    std::vector<float> ladder;
+    try {
+        e_s.resize((size_t)batch); table.resize((size_t)n_T); T_hat.resize((size_t)batch);
+        pairs.resize((size_t)batch); ladder.resize((size_t)n_T);
+    } catch (...) { return MPR_ERR_ARG; }
+    // step 4.1 with the q of h_params: Eq. 4 depends on q only through cos q(phi_i - phi_j)
+    const float q_keep = ctx->d.q;
+    if (!(h_params->q > 0.0f && h_params->q <= 0.5f)) return MPR_ERR_ARG;
+    ctx->d.q = h_params->q;
+    mpr_status s = mpr_sample_energy(ctx, e_s.data(), pairs.data());
+    ctx->d.q = q_keep;
+    if (s != MPR_OK) return s;
+    for (int g = 0; g < batch; ++g) {
+        if (pairs[(size_t)g] == 0) return MPR_ERR_NO_SAMPLES;       // no pair of neighbouring samples: e_s is undefined
+        s = mpr_default_ladder(rows, cols, e_s[(size_t)g], h_factors, n_T, ladder.data());
+        if (s == MPR_OK) s = mpr_energy_table(rows, cols, h_params, ladder.data(), n_T, n_meas, d_workspace, workspace_bytes,
+                                              (void*)ctx->stream, table.data());
+        if (s == MPR_OK) s = mpr_infer_temperature(ladder.data(), table.data(), n_T, e_s[(size_t)g], &T_hat[(size_t)g]);
+        if (s != MPR_OK) return s;
+    }
+    for (int g = 0; g < batch; ++g) { h_T_hat[g] = T_hat[(size_t)g]; if (h_e_s) h_e_s[g] = e_s[(size_t)g]; }
     return MPR_OK;
 }
 
@@ -869,6 +939,22 @@ mpr_status mpr_get_launch_count(mpr_ctx* ctx, uint64_t* h_count)
 {
     if (!ctx || !h_count) return MPR_ERR_ARG;
     *h_count = ctx->launches;
+    return MPR_OK;
+}
+
+mpr_status mpr_set_pass_depth(mpr_ctx* ctx, uint32_t k)
+{
+    if (!ctx) return MPR_ERR_ARG;
+    const uint32_t most = ctx->d.ntiles == 1 ? 1024u : (uint32_t)(ctx->d.H / 2);
+    if (k > most) return MPR_ERR_ARG;
+    ctx->k_max = k ? k : most;
+    return MPR_OK;
+}
+
+mpr_status mpr_get_tiling(mpr_ctx* ctx, int* h_tile_rows, int* h_tile_cols, int* h_halo, uint32_t* h_pass_depth)
+{
+    if (!ctx || !h_tile_rows || !h_tile_cols || !h_halo || !h_pass_depth) return MPR_ERR_ARG;
+    *h_tile_rows = ctx->d.TR; *h_tile_cols = ctx->d.TC; *h_halo = ctx->d.H; *h_pass_depth = ctx->k_max;
     return MPR_OK;
 }
 

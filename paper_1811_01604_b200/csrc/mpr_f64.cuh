@@ -319,8 +319,9 @@ __device__ __forceinline__ double2 update_site_d(double2 v, double2 n_up, double
 // One colour of one sweep (L261-265): one thread per prediction site of the colour (sites[0 .. n_sites)), in place.
 template <bool QHALF, int ORMODE>
 __global__ void __launch_bounds__(256) k64_halfsweep(Dev64 d, const uint32_t* __restrict__ sites, uint32_t n_sites,
-                                                     uint32_t t_off, int count)
+                                                     uint32_t t_off, int count, int check_done)
 {
+    if (check_done && d.state->done) return;        // the equilibration has stopped (Alg. 2 step 5 loop condition false)
     const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
     bool accepted = false;
     if (idx < n_sites) {

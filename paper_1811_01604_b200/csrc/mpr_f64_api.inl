@@ -47,6 +47,7 @@ struct mpr64_ctx {
     uint32_t       h_done;        // host copy of the done flag
     mpr64::State64 h_state;
     bool           qhalf, dirty;
+    uint64_t       n_realizations;   // realizations accumulated since mpr64_set_params
 };
 
 namespace {
@@ -60,7 +61,7 @@ mpr_status fetch_state64(mpr64_ctx* ctx)
     return MPR_OK;
 }
 
-typedef void (*half_kernel)(mpr64::Dev64, const uint32_t*, uint32_t, uint32_t, int);
+typedef void (*half_kernel)(mpr64::Dev64, const uint32_t*, uint32_t, uint32_t, int, int);
 half_kernel pick_half_kernel(bool qhalf, int or_mode)
 {
     using namespace mpr64;
@@ -69,13 +70,14 @@ half_kernel pick_half_kernel(bool qhalf, int or_mode)
 }
 
 // one sweep at sweep index state.t + t_off: colour 0 (the one holding the upper-left node), then colour 1 (L261-265)
-mpr_status launch_sweep64(mpr64_ctx* ctx, uint32_t t_off, int count)
+// check_done: the sweep does nothing once the equilibration has stopped (State64::done)
+mpr_status launch_sweep64(mpr64_ctx* ctx, uint32_t t_off, int count, int check_done = 0)
 {
     const half_kernel kern = pick_half_kernel(ctx->qhalf, (int)ctx->prm.or_mode);
     const uint32_t* sites = ctx->d.list;
     for (int colour = 0; colour < 2; ++colour) {
         if (ctx->n_colour[colour]) {
-            kern<<<cdiv(ctx->n_colour[colour], 256), 256, 0, ctx->stream>>>(ctx->d, sites, ctx->n_colour[colour], t_off, count);
+            kern<<<cdiv(ctx->n_colour[colour], 256), 256, 0, ctx->stream>>>(ctx->d, sites, ctx->n_colour[colour], t_off, count, check_done);
             CU_LAUNCH();
         }
         sites += ctx->n_colour[colour];
@@ -192,6 +194,7 @@ mpr_status mpr64_set_params(mpr64_ctx* ctx, const mpr_params* p, double T)
     CU_LAUNCH();
     ctx->state = READY;
     ctx->dirty = false;
+    ctx->n_realizations = 0;
     return MPR_OK;
 }
 
@@ -202,11 +205,15 @@ mpr_status mpr64_equilibrate(mpr64_ctx* ctx)
     if (ctx->state != READY) return MPR_ERR_STATE;
     const mpr64::Dev64& d = ctx->d;
     const uint32_t cap = ctx->prm.equil_cap;
-    uint32_t issued = 0, chunk = ctx->prm.n_fit + 1;       // the first slope check happens at i = n_fit (step 5.4)
+    // The controller checks the slope after the sweep with index i when i >= n_fit and i % n_f == 0 (step 5.4), so the
+    // run can only stop after i + 1 sweeps with i such an index: the host polls the flag exactly there (and a sweep
+    // enqueued after the stop does nothing: check_done).
+    const uint32_t n_f = ctx->prm.n_f;
+    uint32_t issued = 0, chunk = (ctx->prm.n_fit + n_f - 1) / n_f * n_f + 1;
     while (issued < cap) {
         if (chunk > cap - issued) chunk = cap - issued;
         for (uint32_t j = 0; j < chunk; ++j) {
-            mpr_status s = launch_sweep64(ctx, 0, 1);       // 5.1, accepted proposals counted
+            mpr_status s = launch_sweep64(ctx, 0, 1, 1);    // 5.1, accepted proposals counted
             if (s != MPR_OK) return s;
             mpr64::k64_energy<<<ctx->energy_blocks, mpr64::E_THREADS, 0, ctx->stream>>>(d);      // 5.3
             CU_LAUNCH();
@@ -217,7 +224,7 @@ mpr_status mpr64_equilibrate(mpr64_ctx* ctx)
         CU(cudaMemcpyAsync(&ctx->h_done, d.done_flag, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         if (ctx->h_done) break;
-        chunk = ctx->prm.n_f;
+        chunk = n_f;
     }
     return MPR_OK;
 }
@@ -240,6 +247,7 @@ mpr_status mpr64_simulate(mpr64_ctx* ctx)
     }
     mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(d, 2, 0.0, t_off, ctx->prm.M);
     CU_LAUNCH();
+    ctx->n_realizations += ctx->prm.M;
     return MPR_OK;
 }
 
@@ -247,7 +255,7 @@ mpr_status mpr64_predict(mpr64_ctx* ctx, double* d_out)
 {
     if (!ctx || !d_out) return MPR_ERR_ARG;
     ENTER64(ctx);
-    if (ctx->state != READY) return MPR_ERR_STATE;
+    if (ctx->state != READY || ctx->n_realizations == 0) return MPR_ERR_STATE;     // the mean of no realization is 0 / 0
     mpr64::k64_predict<<<cdiv(ctx->d.N, 256), 256, 0, ctx->stream>>>(ctx->d, d_out, 0);
     CU_LAUNCH();
     return MPR_OK;

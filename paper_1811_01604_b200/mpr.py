@@ -33,7 +33,8 @@ EXPORTS = (
     "mpr_get_stats", "mpr_get_launch_count", "mpr_status_string", "mpr_last_cuda_error",
     "mpr_sample_energy", "mpr_create_unconditional", "mpr_measure_energy", "mpr_energy_table",
     "mpr_infer_temperature", "mpr_predict_std", "mpr_query_workspace_chains", "mpr_create_chains",
-    "mpr_predict_quantile",
+    "mpr_predict_quantile", "mpr_set_pass_depth", "mpr_get_tiling",
+    "mpr_default_ladder", "mpr_infer_temperature_auto",
     "mpr64_query_workspace", "mpr64_create", "mpr64_set_params", "mpr64_equilibrate", "mpr64_simulate", "mpr64_predict",
     "mpr64_predict_std", "mpr64_destroy", "mpr64_get_angles", "mpr64_set_angles", "mpr64_set_sweep_index", "mpr64_sweep",
     "mpr64_energy", "mpr64_get_transform", "mpr64_get_stats", "mpr64_get_launch_count",
@@ -97,6 +98,8 @@ def lib():
         L.mpr_get_mask_bits.argtypes = [vp, vp]
         L.mpr_get_stats.argtypes = [vp, C.POINTER(mpr_stats)]
         L.mpr_get_launch_count.argtypes = [vp, C.POINTER(u64)]
+        L.mpr_set_pass_depth.argtypes = [vp, u32]
+        L.mpr_get_tiling.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i), C.POINTER(u32)]
         L.mpr_predict_std.argtypes = [vp, vp]
         L.mpr_predict_quantile.argtypes = [vp, C.c_double, vp]
         L.mpr_sample_energy.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(u64)]
@@ -106,6 +109,9 @@ def lib():
                                        C.POINTER(C.c_double)]
         L.mpr_infer_temperature.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_double), i, C.c_double,
                                             C.POINTER(C.c_double)]
+        L.mpr_default_ladder.argtypes = [i, i, C.c_double, C.POINTER(C.c_float), i, C.POINTER(C.c_float)]
+        L.mpr_infer_temperature_auto.argtypes = [vp, C.POINTER(mpr_params), C.POINTER(C.c_float), i, u32, vp, sz,
+                                                 C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.mpr64_query_workspace.argtypes = [i, i, C.POINTER(sz)]
         L.mpr64_create.argtypes = [C.POINTER(vp), i, i, vp, vp, vp, sz, vp]
         L.mpr64_set_params.argtypes = [vp, C.POINTER(mpr_params), C.c_double]
@@ -347,6 +353,16 @@ class Mpr:
         _check(lib().mpr_get_launch_count(self._ctx, C.byref(n)), "mpr_get_launch_count")
         return int(n.value)
 
+    def set_pass_depth(self, k: int):
+        _check(lib().mpr_set_pass_depth(self._ctx, int(k)), "mpr_set_pass_depth")
+        return self
+
+    def get_tiling(self):
+        """(tile rows, tile cols, halo, sweeps per pass)"""
+        tr, tc, h, k = C.c_int(), C.c_int(), C.c_int(), C.c_uint32()
+        _check(lib().mpr_get_tiling(self._ctx, C.byref(tr), C.byref(tc), C.byref(h), C.byref(k)), "mpr_get_tiling")
+        return int(tr.value), int(tc.value), int(h.value), int(k.value)
+
 
 class Mpr64:
     """The double-precision path (mpr64_* calls): one grid of rows x cols.
@@ -484,20 +500,31 @@ def infer_temperature(Ts, es, e_s: float) -> float:
     return float(out.value)
 
 
-def infer_T(ctx: "Mpr", n_meas: int = 100, ladder=(0.25, 0.5, 1.0, 2.0, 4.0), **params):
-    """Alg. 2 step 4 for every grid of a context, by the library's own calls: e_s (mpr_sample_energy), a ladder of
-    temperatures around the point where the low-temperature equipartition line e = -1 + (N - 1) T / (2 N_GP) meets e_s
-    (that line only centres the ladder), e(T, L) of the ladder from unconditional chains (mpr_energy_table) and the
-    inversion (mpr_infer_temperature).  Returns the list of T-hat."""
-    e_s, _ = ctx.sample_energy()
-    n_gp = ctx.rows * (ctx.cols - 1) + ctx.cols * (ctx.rows - 1)
-    out = []
-    for e in e_s:
-        centre = max(2.0 * n_gp * (1.0 + e) / (ctx.rows * ctx.cols - 1), 1e-12)
-        Ts = [centre * f for f in ladder]
-        table = energy_table(ctx.rows, ctx.cols, Ts, n_meas, ctx.device, **params)
-        out.append(infer_temperature(Ts, table, e))
-    return out
+def default_ladder(rows: int, cols: int, e_s: float, factors=None):
+    """mpr_default_ladder: the temperatures step 4.2 uses when the caller has no ladder."""
+    n = 5 if factors is None else len(factors)
+    f = None if factors is None else (C.c_float * n)(*[float(x) for x in factors])
+    out = (C.c_float * n)()
+    _check(lib().mpr_default_ladder(int(rows), int(cols), float(e_s), f, n, out), "mpr_default_ladder")
+    return [float(x) for x in out]
+
+
+def infer_T(ctx: "Mpr", n_meas: int = 100, ladder=None, return_e_s: bool = False, **params):
+    """mpr_infer_temperature_auto: Alg. 2 step 4 for every grid of a context, in the library (e_s, ladder around the
+    equipartition estimate, e(T, L) of the ladder from unconditional chains, inversion).  `ladder` = the factors of
+    the ladder (None: the library's).  Returns the list of T-hat (and the list of e_s)."""
+    import torch
+    p = default_params(**params)
+    n_T = 5 if ladder is None else len(ladder)
+    f = None if ladder is None else (C.c_float * n_T)(*[float(x) for x in ladder])
+    nbytes = mpr_query_workspace(n_T, ctx.rows, ctx.cols)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=ctx.device)
+    T_hat, e_s = (C.c_double * ctx.batch)(), (C.c_double * ctx.batch)()
+    _check(lib().mpr_infer_temperature_auto(ctx._ctx, C.byref(p), f, n_T, int(n_meas), ws.data_ptr(), nbytes, T_hat, e_s),
+           "mpr_infer_temperature_auto")
+    if return_e_s:
+        return [float(x) for x in T_hat], [float(x) for x in e_s]
+    return [float(x) for x in T_hat]
 
 
 def interpolate(values, sample_mask, T=None, chains: int = 1, **params):

@@ -2,7 +2,9 @@
 
 This module is the ONE piece shared by the CPU oracle's tests and the CUDA
 path's tests/bench: it produces inputs (truth field, sample mask, temperature)
-and scores outputs (MAE/RMSE).  It holds none of the sweep's arithmetic and it
+and scores outputs (MAE/RMSE).  It holds none of the sweep's arithmetic (`choose_T`, which
+manufactures the input temperature, restates Eq. 1, Eq. 4 and the closed form of reading R15 in
+float64; tests/test_oracle_inference_pins.py checks it against the oracle's e_s and ladder centre) and it
 imports neither `oracle/` nor the CUDA binding.
 
 What the paper measures on: synthetic Gaussian random fields on L x L grids,

@@ -163,6 +163,31 @@ def test_equilibration_controller_and_full_run_follow_the_oracle(torch_cuda, mpr
     ctx.close()
 
 
+@pytest.mark.parametrize("cap,n_fit,n_f", [(21, 20, 5), (40, 20, 7), (300, 256, 7), (300, 20, 7), (23, 20, 5)])
+def test_equilibration_windows_not_aligned_with_the_check_interval(torch_cuda, mpr, orc64, cap, n_fit, n_f):
+    """Alg. 2 step 5 with n_fit not a multiple of n_f (L201: the slope is checked at i >= n_fit, i % n_f == 0): the run
+    stops right after the check that finds k >= 0 -- no sweep is enqueued past it (the host polls on the controller's
+    schedule and a sweep after the stop does nothing) -- so t = equil_sweeps, and in double the chain is the oracle's:
+    same stopping sweep, same a, same state."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg1")
+    z, m, T = w.truth[0].astype(np.float64), w.mask[0], float(w.T[0])
+    ctx = mpr.Mpr64(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=31, equil_cap=cap, n_fit=n_fit, n_f=n_f).equilibrate()
+    st = ctx.get_stats()
+    p = orc64.Params(seed=31, equil_cap=cap, n_fit=n_fit, n_f=n_f)
+    phi, _, _ = orc64.transform(z, m, 31)
+    eq = orc64.equilibrate(phi, m, T, p)
+    assert st.equilibrated and st.t == st.equil_sweeps == eq["sweeps"]
+    assert st.a == pytest.approx(eq["a"], rel=1e-12)
+    assert np.abs(ctx.get_angles().cpu().numpy() - phi).max() < 1e-9
+    # the next sweep draws from sweep index t on both sides
+    n_acc = ctx.sweep(1, st.a, count=True)
+    assert n_acc == orc64.sweep(phi, m, 0.5, T, eq["a"], 31, 0, eq["t"])
+    assert np.abs(ctx.get_angles().cpu().numpy() - phi).max() < 1e-9
+    ctx.close()
+
+
 def test_double_and_float_paths_give_the_same_validation_measures(torch_cuda, mpr):
     """The paper's Table 2 against Table 3 (L305-321): MAE and RMSE of the double- and single-precision runs agree to
     well under the seed-to-seed noise (cfg2 shape, M = 100, s = 10; means over 4 seeds, within 1 %)."""

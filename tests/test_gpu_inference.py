@@ -111,6 +111,37 @@ def test_energy_table_and_inferred_temperature(torch_cuda, mpr, orc):
     assert T_gpu == pytest.approx(synth.choose_T(z, m), rel=0.05)
 
 
+def test_infer_temperature_auto_against_the_oracle(torch_cuda, mpr, orc):
+    """mpr_infer_temperature_auto (Alg. 2 step 4 in ONE library call) for a batch of two grids against the oracle's
+    infer_T_auto grid by grid: e_s to 1e-12, the ladder bit for bit, T-hat within the chains' noise (3 %)."""
+    torch = torch_cuda
+    L = 96
+    zs, ms = zip(*[_field(L, L, ell, p_rm, seed) for ell, p_rm, seed in ((6.0, 0.33, 71), (14.0, 0.6, 72))])
+    ctx = mpr.Mpr(_dev(torch, np.stack(zs)), _dev(torch, np.stack(ms)))
+    T_hat, e_s = mpr.infer_T(ctx, n_meas=150, return_e_s=True, seed=31, equil_cap=300)
+    # a second call is reproducible bit for bit; other factors give another ladder but nearly the same answer
+    assert mpr.infer_T(ctx, n_meas=150, seed=31, equil_cap=300) == T_hat
+    T_wide = mpr.infer_T(ctx, n_meas=150, ladder=(0.5, 0.8, 1.25, 2.0), seed=31, equil_cap=300)
+    ctx.close()
+    p = orc.Params(seed=31, equil_cap=300)
+    for g in range(2):
+        phi, _, _ = orc.transform(zs[g], ms[g], 0)
+        T_ref, e_ref, Ts, _ = orc.infer_T_auto(phi, ms[g], p, 150)
+        assert e_s[g] == pytest.approx(e_ref, abs=1e-12)
+        assert mpr.default_ladder(L, L, e_s[g]) == Ts
+        assert T_hat[g] == pytest.approx(T_ref, rel=0.03)
+        assert T_wide[g] == pytest.approx(T_hat[g], rel=0.03)
+        assert T_hat[g] == pytest.approx(synth.choose_T(zs[g], ms[g]), rel=0.05)
+    # a grid whose samples never touch has no e_s
+    m = np.zeros((8, 8), dtype=np.uint8); m[::2, ::2] = 1
+    z = np.random.default_rng(0).standard_normal((8, 8)).astype(np.float32)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    with pytest.raises(mpr.MprError) as e:
+        mpr.infer_T(ctx)
+    assert e.value.name == "MPR_ERR_NO_SAMPLES"
+    ctx.close()
+
+
 def test_interpolate_with_inferred_temperature(torch_cuda, mpr, orc):
     """The parameter-free path the paper intends (L11, L63 'automatic'): T = None makes the binding run Alg. 2 step 4 with the
     library's own calls before the sweeps.  On a cfg1-shaped grid the inferred T-hat is within 5 % of the closed form

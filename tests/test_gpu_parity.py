@@ -133,13 +133,19 @@ def _compare_one_sweep(orc, ctx, phi0, mask, q, T, a, seed, t, or_mode, g_list=(
         assert np.array_equal(got[g][~free].view(np.uint32), ref[~free].view(np.uint32))
         bad = free & (d > tol)
         n_bad, P = int(bad.sum()), int(free.sum())
-        # every disagreement must be a near-threshold decision in the oracle's own margins, or a
-        # site whose neighbour of the colour updated before it in this sweep is such a site
+        # Every disagreement must be a decision the oracle's OWN margins call near-threshold (Metropolis |AP - r| < 1e-3,
+        # or an interval-end test within 1e-4 rad), or a colour-1 site next to such a colour-0 site that disagrees: colour 0
+        # is updated first (L265), so only its flips can reach a neighbour within the sweep.  Two bad sites do not vouch
+        # for each other.
         if n_bad:
+            flipped = bad & ((margin < 1e-3) | (edge < 1e-4))
+            rr, cc = np.indices(bad.shape)
+            c0 = flipped & (((rr + cc) & 1) == 0)
             nb = np.zeros_like(bad)
-            nb[1:, :] |= bad[:-1, :]; nb[:-1, :] |= bad[1:, :]; nb[:, 1:] |= bad[:, :-1]; nb[:, :-1] |= bad[:, 1:]
-            near = (margin[bad] < 1e-3) | (edge[bad] < 1e-4) | nb[bad]
-            assert near.all(), (n_bad, margin[bad][~near][:5], edge[bad][~near][:5], d[bad][~near][:5])
+            nb[1:, :] |= c0[:-1, :]; nb[:-1, :] |= c0[1:, :]; nb[:, 1:] |= c0[:, :-1]; nb[:, :-1] |= c0[:, 1:]
+            nb &= ((rr + cc) & 1) == 1
+            ok = flipped | nb
+            assert ok[bad].all(), (n_bad, margin[bad & ~ok][:5], edge[bad & ~ok][:5], d[bad & ~ok][:5])
         assert n_bad <= max(1, math.ceil(FLIP_FRACTION * P)), (n_bad, P)
         assert abs(acc_gpu[g] - acc_ref) <= n_bad
         assert abs(e_gpu0[g] - e_ref0) < 2e-6 and abs(e_gpu1[g] - e_ref1) < 2e-6 + 8.0 * n_bad / max(1, orc.n_bonds(*ref.shape))
@@ -332,6 +338,158 @@ def test_t2_after_batch_equilibration_grids_share_one_buffer(torch_cuda, mpr, or
 
 
 # ---------------------------------------------------------------------------
+# T2 over a whole K-sweep tile pass: the kernel instantiations mpr_simulate and bench.py run
+# ---------------------------------------------------------------------------
+def _diamond(seed_mask, radius):
+    """Sites within Manhattan distance `radius` of a set site."""
+    out = seed_mask.copy()
+    for _ in range(radius):
+        grown = out.copy()
+        grown[1:, :] |= out[:-1, :]; grown[:-1, :] |= out[1:, :]; grown[:, 1:] |= out[:, :-1]; grown[:, :-1] |= out[:, 1:]
+        out = grown
+    return out
+
+
+def _compare_n_sweeps(orc, ctx, phi0, mask, q, T, a, seed, t, n, or_mode=0, g_list=(0,), tol=TOL_RAD, margin_thr=1e-3):
+    """n sweeps in ONE mpr_sweep call without the accepted count (h_accepted = NULL): the NON-fused tile pass at the
+    context's pass depth K -- halo rings 2K-1 .. 0, the ring-prefix walk of the entry lists, the stashed second
+    Philox pair, renormalisation in the last sweep of a pass only, and for a >= q pi / 0.2 the short sin / cos
+    polynomials -- against n oracle sweeps (Alg. 1) from the same state.
+
+    A decision that falls the other way on the two sides (Metropolis accept, interval-end test) changes the site and,
+    sweep by sweep, its surroundings: after the sweep a disagreement has reached at most Manhattan distance 1, after r
+    more sweeps 1 + 2 r.  So a site may differ by more than `tol` only inside that light cone of a site that the
+    oracle's OWN margins of some sweep call near-threshold (|AP - r| < margin_thr = 1e-3 or an interval-end test within
+    1e-4 rad); the disagreeing sites must form at most n * 1e-4 * P separate clusters (north_star's flip budget per
+    sweep), each no larger than a cone.  About 1e-3 of the sites are near-threshold in a sweep, so the cones of n = 4
+    sweeps cover about 20 % of the grid (a fault that is not a decision flip and touches ten sites fails with
+    probability 1 - 1e-7); for n >= 7 they would cover everything, and such calls pass a smaller margin_thr.
+    Returns per grid (bad sites, clusters, P, largest error outside the cones)."""
+    import torch
+    from scipy import ndimage
+    ctx.set_angles(torch.from_numpy(phi0).cuda())
+    ctx.set_sweep_index(t)
+    assert ctx.sweep(n, a) is None
+    got = ctx.get_angles().cpu().numpy()
+    assert ctx.get_stats()[0].t == t + n
+    out = []
+    for g in g_list:
+        ref = phi0[g].copy()
+        free = mask[g] == 0
+        cone = np.zeros_like(free)
+        for s in range(n):
+            _, margin, edge, _ = orc.sweep(ref, mask[g], q, T[g], a, seed, g, t + s, or_mode, diag=True)
+            near = free & ((margin < margin_thr) | (edge < 1e-4))
+            cone |= _diamond(near, 1 + 2 * (n - 1 - s))
+        assert np.array_equal(got[g][~free].view(np.uint32), ref[~free].view(np.uint32))
+        d = np.abs(got[g].astype(np.float64) - ref.astype(np.float64))
+        bad = free & (d > tol)
+        n_bad, P = int(bad.sum()), int(free.sum())
+        assert not (bad & ~cone).any(), (n_bad, int((bad & ~cone).sum()), np.argwhere(bad & ~cone)[:5], d[bad & ~cone][:5])
+        n_clusters = 0
+        if n_bad:
+            # sites of one divergence are within distance 2 of each other (same-colour neighbours): 5 x 5 diamond linkage
+            link = ndimage.generate_binary_structure(2, 1)
+            labels, n_clusters = ndimage.label(ndimage.binary_dilation(bad, link), structure=np.ones((3, 3), bool))
+            sizes = ndimage.sum(bad, labels, index=np.arange(1, n_clusters + 1))
+            r = 2 * n - 1
+            assert sizes.max() <= 2 * r * r + 2 * r + 1, sizes.max()
+        assert n_clusters <= max(1, math.ceil(n * FLIP_FRACTION * P)), (n_clusters, n_bad, P)
+        out.append((n_bad, n_clusters, P, float(d[free & ~cone].max()) if (free & ~cone).any() else 0.0))
+    return out
+
+
+@pytest.mark.parametrize("t0", [40, 41])
+@pytest.mark.parametrize("a", [3.0, 12.0])
+def test_t2_k_sweep_passes_on_a_multi_tile_grid(torch_cuda, mpr, orc, t0, a):
+    """A ragged multi-tile grid (64-row tiles: 5 x 7 of them, the last row and column of tiles partial) from an
+    oracle-equilibrated state: n = 4 (one full pass), 5 (4 + 1), 6 (4 + 2) and 8 (two full passes) sweeps per call at
+    pass depth 4, and depths 2, 3 and 1, starting at an even and at an odd sweep index (the stored-pair and the
+    draw-anew start of a pass), with the long (a = 3) and the short (a = 12 >= q pi / 0.2) sin / cos polynomials."""
+    torch = torch_cuda
+    rows, cols = 300, 420
+    z, m = _field(rows, cols, 9.0, 0.45, 4100)
+    T = synth.choose_T(z, m)
+    seed = 515
+    phi, _, _ = orc.transform(z, m, seed)
+    orc.equilibrate(phi, m, T, orc.Params(seed=seed, equil_cap=40, n_fit=200))      # exactly 40 sweeps
+    ctx = mpr.Mpr(_dev(torch, np.stack([z, z])), _dev(torch, np.stack([m, m])))     # two grids: 70 tiles of 64 rows
+    assert ctx.get_tiling()[:3] == (64, 64, 8)
+    ctx.set_params([T, T], seed=seed)
+    state = np.stack([phi, phi])
+    worst = 0.0
+    for depth, n in ((4, 4), (4, 5), (4, 6), (4, 8), (2, 4), (2, 5), (3, 3), (3, 6), (1, 2)):
+        ctx.set_pass_depth(depth)
+        assert ctx.get_tiling()[3] == depth
+        l0 = ctx.launch_count()
+        res = _compare_n_sweeps(orc, ctx, state, np.stack([m, m]), 0.5, [T, T], a, seed, t0, n, g_list=(0, 1),
+                                margin_thr=1e-3 if n < 7 else 1e-4)
+        assert ctx.launch_count() - l0 == 5 + -(-n // depth)         # import, set t, set a, the passes, commit, export
+        worst = max(worst, max(r[3] for r in res))
+    ctx.set_pass_depth(0)
+    assert ctx.get_tiling()[3] == 4
+    with pytest.raises(mpr.MprError) as e:
+        ctx.set_pass_depth(5)
+    assert e.value.name == "MPR_ERR_ARG"
+    assert worst <= TOL_RAD
+    ctx.close()
+
+
+@pytest.mark.parametrize("q,or_mode", [(0.5, 2), (0.5, 1), (0.3, 0)])
+def test_t2_k_sweep_passes_other_q_and_over_relaxation_modes(torch_cuda, mpr, orc, q, or_mode):
+    """The other instantiation families of the non-fused pass (general q, Eq. 6 as printed, no over-relaxation), 4 and 6
+    sweeps per call on a multi-tile grid, both polynomial lengths."""
+    torch = torch_cuda
+    z, m = _field(200, 330, 7.0, 0.5, 4200)
+    seed, T = 88, 0.02
+    phi, _, _ = orc.transform(z, m, seed)
+    st = orc.equilibrate(phi, m, T, orc.Params(q=q, seed=seed, equil_cap=30, n_fit=200, or_mode=or_mode))
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed, q=q, or_mode=or_mode)
+    tol = 1e-3 if or_mode == 1 else TOL_RAD          # see test_t2_other_q_and_over_relaxation_modes
+    for a, n, t0 in ((2.0, 4, 30), (20.0, 6, 31)):
+        _compare_n_sweeps(orc, ctx, phi[None].copy(), m[None], q, [T], a, seed, t0, n, or_mode=or_mode, tol=tol)
+    ctx.close()
+
+
+def test_t2_k_sweep_pass_full_size_cfg4_shape(torch_cuda, mpr, orc):
+    """BASELINE configs[3] at full size in the launch configuration bench.py times: 4096 x 4096, 33 % removed,
+    `mpr_sweep(4, a)` without the count = ONE launch of k_tilepass<q = 1/2, exact reflection, not fused, pitch 82,
+    short polynomials> at K = 4, from an even and from an odd sweep index; against four oracle sweeps."""
+    torch = torch_cuda
+    L = 4096
+    z = synth.grf(L, L, 64.0, "gaussian", 1004)
+    m = synth.bernoulli_mask(L, L, 0.33, 2004)
+    T = synth.choose_T(z, m)
+    phi = _generator_state(orc, z, m, T, 3004, 8)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=3004)
+    assert ctx.get_tiling() == (64, 64, 8, 4)
+    for t0 in (122, 123):
+        l0 = ctx.launch_count()
+        res = _compare_n_sweeps(orc, ctx, phi[None], m[None], 0.5, [T], 40.0, 3004, t0, 4)
+        assert ctx.launch_count() - l0 == 6            # import, set t, set a, ONE tile pass, commit, export
+        assert res[0][3] <= TOL_RAD
+    ctx.close()
+
+
+def test_t2_k_sweep_pass_full_size_cfg5_grid(torch_cuda, mpr, orc):
+    """One 2048 x 2048 grid of BASELINE configs[4] (66 % removed, its own correlation length), 4 and 8 sweeps per call."""
+    torch = torch_cuda
+    L, seed = 2048, 3005
+    z = synth.grf(L, L, 47.0, "gaussian", 1105)
+    m = synth.bernoulli_mask(L, L, 0.66, 2105)
+    T = synth.choose_T(z, m)
+    phi = _generator_state(orc, z, m, T, seed, 11)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed)
+    for t0, n in ((200, 4), (201, 8)):
+        res = _compare_n_sweeps(orc, ctx, phi[None], m[None], 0.5, [T], 12.0, seed, t0, n, margin_thr=1e-3 if n < 7 else 1e-4)
+        assert res[0][3] <= TOL_RAD
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------
 # equilibration controller (Alg. 2 step 5) and T3
 # ---------------------------------------------------------------------------
 def test_equilibration_controller_follows_the_oracle(torch_cuda, mpr, orc):
@@ -359,9 +517,9 @@ def test_equilibration_controller_follows_the_oracle(torch_cuda, mpr, orc):
     g = ctx.get_stats()[0]
     assert g.equilibrated and g.t == g.equil_sweeps and g.k >= 0.0
     assert g.equil_sweeps >= p.n_fit and (g.equil_sweeps - 1) % p.n_f == 0     # stops right after a check
-    assert 0.5 * st["sweeps"] <= g.equil_sweeps <= 2.0 * st["sweeps"]
-    assert g.a == pytest.approx(st["a"], rel=0.3)
-    assert g.e_last == pytest.approx(st["e_hist"][-1], abs=3e-4)
+    assert abs(g.equil_sweeps - st["sweeps"]) <= 2 * p.n_f, (g.equil_sweeps, st["sweeps"])
+    assert g.a == pytest.approx(st["a"], rel=0.15)
+    assert g.e_last == pytest.approx(st["e_hist"][-1], abs=2e-4)
     # the fused per-tile reduction and mpr_energy add the same fp32 bond terms in different orders
     assert ctx.energy()[0] == pytest.approx(g.e_last, abs=1e-8)
     ctx.close()
@@ -842,7 +1000,7 @@ def test_t2_only_one_colour_has_prediction_sites(torch_cuda, mpr, orc):
         c64.close()
 
 
-@pytest.mark.parametrize("cap,n_fit,n_f", [(1, 20, 5), (5, 20, 5), (21, 20, 5), (23, 20, 5), (40, 2, 1), (300, 256, 7)])
+@pytest.mark.parametrize("cap,n_fit,n_f", [(1, 20, 5), (5, 20, 5), (21, 20, 5), (23, 20, 5), (40, 2, 1), (300, 256, 7), (40, 20, 7), (300, 20, 7)])
 def test_equilibration_caps_and_windows_follow_the_oracle(torch_cuda, mpr, orc, cap, n_fit, n_f):
     """Alg. 2 step 5 at the edges of its parameters: caps below, at and just above the first slope check, the smallest
     and the largest fit window.  Sweep counts equal to the oracle's up to what a near-threshold flip can shift (one
@@ -864,23 +1022,43 @@ def test_equilibration_caps_and_windows_follow_the_oracle(torch_cuda, mpr, orc, 
 
 
 def test_in_pass_equilibration_is_independent_of_the_sweeps_per_launch(torch_cuda, mpr):
-    """A grid that is one tile equilibrates inside the tile pass; with the experiment hook MPR_KMAX = 7 the same
+    """A grid that is one tile equilibrates inside the tile pass; at pass depth 7 (mpr_set_pass_depth) the same
     equilibration takes several launches that start at even and odd sweep indices: same state bit for bit."""
-    import os
     torch = torch_cuda
     w = synth.make_workload("cfg1")
     z, m, T = w.truth[0], w.mask[0], float(w.T[0])
     out = []
-    for kmax in (None, "7"):
-        if kmax:
-            os.environ["MPR_KMAX"] = kmax
-        try:
-            ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
-        finally:
-            os.environ.pop("MPR_KMAX", None)
+    for depth in (0, 7):
+        ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+        ctx.set_pass_depth(depth)
         ctx.set_params(T, seed=99, equil_cap=1000).equilibrate()
         st = ctx.get_stats()[0]
         out.append((ctx.get_angles().cpu().numpy(), st.equil_sweeps, st.a, st.e_last, st.t, ctx.launch_count()))
         ctx.close()
     assert np.array_equal(out[0][0], out[1][0]) and out[0][1:5] == out[1][1:5]
     assert out[1][5] > out[0][5]
+
+
+def test_predict_needs_a_realization(torch_cuda, mpr):
+    """include/mpr.h: mpr_predict is the mean over >= 1 realizations; before mpr_simulate it is MPR_ERR_STATE (not NaN)."""
+    torch = torch_cuda
+    z, m = _field(40, 40, 4.0, 0.5, 3)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(0.05, seed=1, M=2, equil_cap=5).equilibrate()
+    with pytest.raises(mpr.MprError) as e:
+        ctx.predict()
+    assert e.value.name == "MPR_ERR_STATE"
+    ctx.simulate()
+    assert np.isfinite(ctx.predict().cpu().numpy()).all()
+    ctx.set_params(0.05, seed=1, M=2, equil_cap=5)          # a restart forgets the realizations
+    with pytest.raises(mpr.MprError):
+        ctx.predict()
+    ctx.close()
+    c64 = mpr.Mpr64(_dev(torch, z.astype(np.float64)), _dev(torch, m))
+    c64.set_params(0.05, seed=1, M=2, equil_cap=5)
+    with pytest.raises(mpr.MprError) as e:
+        c64.predict()
+    assert e.value.name == "MPR_ERR_STATE"
+    c64.simulate()
+    assert np.isfinite(c64.predict().cpu().numpy()).all()
+    c64.close()

@@ -108,3 +108,16 @@ def test_infer_temperature_is_host_arithmetic_and_matches_the_oracle(lib, orc):
     with pytest.raises(mpr.MprError) as e:
         mpr.infer_temperature([2, 1], [-0.9, -0.8], -0.85)          # ladder not ascending
     assert e.value.name == "MPR_ERR_ARG"
+
+
+def test_default_ladder_is_host_arithmetic_and_matches_the_oracle(lib, orc):
+    """mpr_default_ladder (the ladder of Alg. 2 step 4.2 when the caller has none) needs no device; the oracle builds the
+    same float32 temperatures."""
+    for rows, cols, e_s in ((64, 64, -0.9946), (2048, 2048, -0.99995), (37, 53, -0.9), (4096, 4096, -1.0)):
+        assert mpr.default_ladder(rows, cols, e_s) == orc.default_ladder(rows, cols, e_s)
+        f = (0.1, 0.9, 1.0, 7.5)
+        assert mpr.default_ladder(rows, cols, e_s, f) == orc.default_ladder(rows, cols, e_s, f)
+    for bad in ((1.0, 0.5), (0.0, 1.0), (-1.0, 2.0)):
+        with pytest.raises(mpr.MprError) as e:
+            mpr.default_ladder(8, 8, -0.99, bad)
+        assert e.value.name == "MPR_ERR_ARG"

@@ -114,3 +114,48 @@ def test_infer_T_on_ladders(orc):
     assert orc.infer_T(-0.965, Ts, es) == pytest.approx(0.03, rel=1e-12)
     # a noisy, non-monotone ladder: the first bracketing segment
     assert orc.infer_T(-0.975, [1, 2, 3, 4], [-0.99, -0.97, -0.98, -0.96]) == pytest.approx(1.75)
+
+
+def test_default_ladder_is_centred_where_the_chain_energy_meets_e_s(orc):
+    """Step 4.2 without a ladder of the caller's: the oracle centres its ladder on the temperature at which the
+    low-temperature equipartition energy equals e_s (reading R15).  Pinned by the chains themselves, not by the formula:
+    an unconditional 32 x 32 chain run AT the centre has (1 + e) within 1 % of (1 + e_s), at the ladder's ends it has
+    not (factors 1/4 and 4 give a quarter and four times the excess energy), and the default ladder is ascending
+    with the standard factors."""
+    L, e_s = 32, -0.9975
+    centre = orc.default_ladder(L, L, e_s, (1.0,))[0]
+    p = orc.Params(seed=11, equil_cap=300)
+    ladder = orc.default_ladder(L, L, e_s)
+    assert len(ladder) == 5 and all(b > a for a, b in zip(ladder, ladder[1:]))
+    assert [t / centre for t in ladder] == pytest.approx([0.25, 0.5, 1.0, 2.0, 4.0], rel=1e-6)
+    e = orc.energy_table(L, L, [ladder[0], centre, ladder[-1]], p, 400)
+    assert (1 + e[1]) == pytest.approx(1 + e_s, rel=0.01)
+    assert (1 + e[0]) == pytest.approx(0.25 * (1 + e_s), rel=0.02)
+    assert (1 + e[2]) == pytest.approx(4.0 * (1 + e_s), rel=0.03)
+    # the whole of step 4 on a full sample set drawn from such a chain returns the chain's temperature
+    phi = np.full((L, L), np.float32(PI), dtype=np.float32)
+    mask0 = np.zeros((L, L), dtype=np.uint8)
+    a, T_true = 1.0, 0.02
+    for t in range(400):
+        acc = orc.sweep(phi, mask0, 0.5, T_true, a, 5, 0, t)
+        if acc / (L * L) < 0.3:
+            a = 1.0 + (t + 1) / 3.0
+    T_hat, e_chain, Ts, table = orc.infer_T_auto(phi, np.ones((L, L), dtype=np.uint8), orc.Params(seed=12, equil_cap=300), 300)
+    assert e_chain == pytest.approx(orc.energy_per_bond(phi), abs=1e-12)
+    assert T_hat == pytest.approx(T_true, rel=0.1)          # one state's energy fluctuates by ~3 % at this size
+
+
+def test_harness_temperature_is_the_sample_energy_through_the_closed_form(orc):
+    """synth.choose_T (the input generator's temperature, reading R15) is e_s of Eq. 4 pushed through the equipartition
+    line: checked against the oracle's e_s and ladder centre on three kinds of input, so that the generator cannot
+    drift from the method (it is an input recipe, but it does restate Eq. 1 and Eq. 4)."""
+    from paper_1811_01604_b200 import synth
+    for rows, cols, ell, p_rm, seed in ((64, 64, 8.0, 0.33, 1), (40, 90, 3.0, 0.66, 2), (128, 128, 30.0, 0.5, 3)):
+        z = synth.grf(rows, cols, ell, "gaussian", seed)
+        m = synth.bernoulli_mask(rows, cols, p_rm, seed + 10)
+        phi, _, _ = orc.transform(z, m, 0)
+        e_s, n_sp = orc.sample_energy(phi, m)
+        assert n_sp > 0
+        T_orc = orc.default_ladder(rows, cols, e_s, (1.0,))[0]
+        # Eq. 1 in float32 (oracle) against float64 (generator): (1 + e_s) ~ 1e-3 .. 1e-5 carries ~1e-4 relative
+        assert synth.choose_T(z, m) == pytest.approx(T_orc, rel=2e-3)

@@ -292,6 +292,33 @@ def _boltzmann_bin_probs(nbrs, T, q, edges):
                      for i in range(len(edges) - 1)])
 
 
+@pytest.mark.parametrize("a", [1.0, 4.0, 37.5])
+def test_proposal_is_u_scaled_by_two_pi_over_a(orc, a):
+    """Alg. 1 line 3: phi'' = phi' + alpha (u - 0.5) with alpha = 2 pi / a (L156), u the FIRST of the
+    site's two uniforms (the second, r, decides acceptance, line 6).  A symmetric proposal of any width has the same
+    stationary law, so the chi-square pins cannot see a wrong width; this one does.  One free site, over-relaxation
+    off (phi' = phi), T so high that every proposal is accepted (AP = exp(-dH/T) > 1 - 2^-24 >= r): the step of every
+    sweep must be exactly 2 pi (u - 0.5) / a with u rebuilt here from the Philox words (pinned against cuRAND above),
+    up to the one rounding of the state to float32."""
+    seed, site, T = 777, 4, 1e12
+    phi = np.full((3, 3), 3.0, dtype=np.float32)
+    mask = np.ones((3, 3), dtype=np.uint8); mask[1, 1] = 0
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    steps = []
+    for t in range(400):
+        before = float(phi[1, 1])
+        assert orc.sweep(phi, mask, 0.5, T, a, seed, 0, t, 2) == 1            # accepted
+        x = orc.philox4x32_10([site, t >> 1, 2, 0], key)
+        u = orc.u01(int(x[2 * (t & 1)]))
+        want = before + TWO_PI_F * (u - 0.5) / a             # "2 pi" is the float nearest 2 pi everywhere (reading R4)
+        want = want + TWO_PI_F if want < 0.0 else want - TWO_PI_F if want >= TWO_PI_F else want
+        assert float(phi[1, 1]) == pytest.approx(want, abs=2.5e-7), (t, u)      # half an ulp of a float in [4, 8)
+        steps.append(2.0 * PI * (u - 0.5) / a)
+    steps = np.abs(np.array(steps))
+    assert steps.max() <= PI / a and steps.max() >= 0.97 * PI / a              # the window is [-pi/a, pi/a], and it is used
+    assert np.mean(steps) == pytest.approx(0.5 * PI / a, rel=0.1)
+
+
 @pytest.mark.parametrize("nbrs,or_mode", [
     ((1.0, 2.5, 4.0, 5.5), 0),
     ((1.0, 2.5, 4.0, 5.5), 2),
