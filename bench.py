@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=None, help="override the batch of cfg5 (debugging only)")
     ap.add_argument("--chains", type=int, default=1,
                     help="chains per grid in step 6 (DESIGN.md reading R25); 1 = the paper's single chain")
+    ap.add_argument("--grid-group", type=int, default=0,
+                    help="mpr_set_grid_group: grids per group in step 6 of a batch (SURVEY.md H6); 0 = all grids in every launch")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-inference", action="store_true", help="skip the Alg. 2 step 4 timing (extra key, not in the step)")
     ap.add_argument("--sfu-peak", action="store_true",
@@ -143,7 +145,8 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4": 244.9e6}
 # ---------------------------------------------------------------------------
 # measured pipe rates (the roofline's special-function denominator)
 # ---------------------------------------------------------------------------
-MICROBENCH_OPS = {"mufu_ex2": 0, "mufu_rcp": 1, "ffma": 2, "ffma2": 3, "imad_wide": 4, "lop3": 5, "imad": 6}
+MICROBENCH_OPS = {"mufu_ex2": 0, "mufu_rcp": 1, "ffma": 2, "ffma2": 3, "imad_wide_plus_lop": 4, "lop3": 5, "imad": 6,
+                  "imad_wide": 7, "imad_hi": 8, "philox4x32_10_calls": 9, "lds64": 10}
 
 
 def run_sfu_peak():
@@ -180,47 +183,71 @@ def run_sfu_peak():
 # ---------------------------------------------------------------------------
 # reference arm: the CPU oracle, as it stands, on the host cores
 # ---------------------------------------------------------------------------
-def oracle_sample(w, n_sweeps: int):
-    """Times n_sweeps oracle UPDATE sweeps on grid 0 of the workload from the
-    oracle's own initial state at a = 1 (bounded sample of the same workload).
-    Returns (updates per second, seconds, threads)."""
-    from oracle import mpr_oracle as orc
-    z, m, T = w.truth[0], w.mask[0], float(w.T[0])
-    phi, _, _ = orc.transform(z, m, w.seed)
-    P = int((m == 0).sum())
-    orc.sweep(phi, m, w.q, T, 1.0, w.seed, 0, 0)               # warm the caches / thread pool
-    t0 = time.perf_counter()
-    for t in range(1, n_sweeps + 1):
-        orc.sweep(phi, m, w.q, T, 1.0 + t / 3.0, w.seed, 0, t)
-    dt = time.perf_counter() - t0
-    return P * n_sweeps / dt, dt, orc.num_threads()
+class OracleSample:
+    """The sample of BASELINE.md section 5 / SURVEY.md 8(d): grid 0 of the workload is equilibrated by the oracle
+    itself (Alg. 2 step 5, as it stands, all host cores), then `n_sweeps` UPDATE sweeps at the a reached are timed
+    on that equilibrated state.  ms per grid is EXTRAPOLATED from the sweep rate: (equilibration sweeps + M x s)
+    sweeps of grid 0 at the timed rate (the full-length oracle run would take minutes to hours)."""
+
+    def __init__(self, w):
+        from oracle import mpr_oracle as orc
+        self.orc, self.w = orc, w
+        z, m, T = w.truth[0], w.mask[0], float(w.T[0])
+        self.m, self.T = m, T
+        self.P = int((m == 0).sum())
+        self.phi, _, _ = orc.transform(z, m, w.seed)
+        t0 = time.perf_counter()
+        self.eq = orc.equilibrate(self.phi, m, T, orc.Params(q=w.q, seed=w.seed, equil_cap=w.equil_cap))
+        self.equil_seconds = time.perf_counter() - t0
+        self.t = self.eq["t"]
+
+    def sweeps(self, n_sweeps: int):
+        """Times n_sweeps sweeps continuing the chain; returns (updates per second, seconds, threads)."""
+        orc, w = self.orc, self.w
+        t0 = time.perf_counter()
+        for _ in range(n_sweeps):
+            orc.sweep(self.phi, self.m, w.q, self.T, self.eq["a"], w.seed, 0, self.t)
+            self.t += 1
+        dt = time.perf_counter() - t0
+        return self.P * n_sweeps / dt, dt, orc.num_threads()
+
+    def describe(self, n_sweeps: int) -> str:
+        w = self.w
+        return (f"{n_sweeps} UPDATE sweeps of grid 0 of {w.name} ({w.rows}x{w.cols}) on the state the oracle equilibrated "
+                f"({self.eq['sweeps']} sweeps of Alg. 2 step 5, a = {self.eq['a']:.2f}, {self.equil_seconds:.1f} s, untimed)")
+
+    def extrapolated_ms_per_grid(self, rate: float) -> float:
+        w = self.w
+        return 1e3 * self.P * (self.eq["sweeps"] + w.M * w.sweeps_per_real) / rate
 
 
-def oracle_sweeps_for(w) -> int:
-    """About 10-30 s of CPU work at the ~5e7-1e8 updates/s the OpenMP oracle reaches on a host."""
-    P = int((w.mask[0] == 0).sum())
-    return int(max(3, min(20000, 1.2e9 / max(P, 1))))
+def oracle_sweeps_for(smp: "OracleSample", seconds: float = 6.0) -> int:
+    """Sweeps that make about `seconds` of CPU work, from the rate of three calibration sweeps on the same state."""
+    rate, _, _ = smp.sweeps(3)
+    return int(max(3, min(20000, seconds * rate / max(smp.P, 1))))
 
 
 def run_reference(args, w):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_sweeps = oracle_sweeps_for(w)
+    smp = OracleSample(w)
+    n_sweeps = oracle_sweeps_for(smp)
     for _ in range(args.warmup):
-        oracle_sample(w, max(1, n_sweeps // 10))
+        smp.sweeps(max(1, n_sweeps // 10))
     rates, secs, cores = [], 0.0, 1
     for _ in range(args.steps):
-        r, dt, cores = oracle_sample(w, n_sweeps)
+        r, dt, cores = smp.sweeps(n_sweeps)
         rates.append(r); secs += dt
     value = float(np.mean(rates)) / 1e9
-    sample = f"{n_sweeps} UPDATE sweeps of grid 0 of {w.name} ({w.rows}x{w.cols}) per step from the initial state"
+    sample = smp.describe(n_sweeps) + " per step"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "rows": w.rows, "cols": w.cols, "batch": w.batch},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "ms_per_grid_extrapolated": smp.extrapolated_ms_per_grid(value * 1e9)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -285,6 +312,7 @@ def run_b200(args, w):
 
     def one_pass(values, mask):
         ctx = mpr.Mpr(values, mask, chains=args.chains)
+        ctx.set_grid_group(args.grid_group)
         ctx.set_params(T, **prm).equilibrate().simulate()
         ctx.predict(d_out)
         return ctx
@@ -422,7 +450,8 @@ def run_b200(args, w):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "rows": w.rows, "cols": w.cols, "batch": w.batch,
                        "n_free_per_rank": int(P_sites), "equil_cap": w.equil_cap, "M": w.M,
-                       "sweeps_per_real": w.sweeps_per_real, "chains": args.chains, "equil_sweeps": equil_sweeps,
+                       "sweeps_per_real": w.sweeps_per_real, "chains": args.chains, "grid_group": args.grid_group,
+                       "equil_sweeps": equil_sweeps,
                        "parallelism": f"replicas x{world}", "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)",
                        "step": "mpr_create+set_params+equilibrate+simulate+predict"},
             "ms_per_grid": 1e3 * secs / args.steps / w.batch,
@@ -453,18 +482,21 @@ def run_b200(args, w):
         if f64 is not None:
             out["double_precision"] = f64
         if not args.no_cpu_baseline and world == 1:
-            n_sweeps = oracle_sweeps_for(w)
-            rate, dt, cores = oracle_sample(w, n_sweeps)
+            smp = OracleSample(w)
+            n_sweeps = oracle_sweeps_for(smp, 10.0)
+            rate, dt, cores = smp.sweeps(n_sweeps)
             out["cpu_baseline"] = {
                 "value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
-                "sample": f"{n_sweeps} UPDATE sweeps of grid 0 of {w.name} ({w.rows}x{w.cols}) from the initial state"}
-            # the same oracle on ONE thread (a shorter sample), the arm the paper's speedups are quoted against
-            from oracle import mpr_oracle as orc
-            orc.set_num_threads(1)
-            rate1, dt1, _ = oracle_sample(w, max(2, n_sweeps // 16))
-            orc.set_num_threads(cores)
+                "sample": smp.describe(n_sweeps),
+                "ms_per_grid_extrapolated": smp.extrapolated_ms_per_grid(rate),
+                "extrapolation": "prediction sites of grid 0 x (oracle's equilibration sweeps + M x s) / the timed rate"}
+            # the same oracle on ONE thread (a shorter sample of the same chain), the arm the paper's speedups are quoted against
+            smp.orc.set_num_threads(1)
+            rate1, dt1, _ = smp.sweeps(max(2, n_sweeps // 16))
+            smp.orc.set_num_threads(cores)
             out["cpu_baseline"].update({
                 "value_1_thread": rate1 / 1e9, "seconds_1_thread": dt1,
+                "ms_per_grid_extrapolated_1_thread": smp.extrapolated_ms_per_grid(rate1),
                 "paper_context": "paper (BASELINE.md): 166x-306x end to end at 1024^2 and 'almost 500 times' at 2048^2, "
                                  "GTX 980 against one i5-4440 core, single precision; another machine, context only"})
         print(json.dumps(out))

@@ -279,6 +279,12 @@ mpr_status mpr_get_launch_count(mpr_ctx* ctx, uint64_t* h_count);
  * exists so that tests can drive every depth.  k = 0 restores the default (halo / 2; 1024 for a grid that is
  * one tile); k above the default is MPR_ERR_ARG.  Host-side only. */
 mpr_status mpr_set_pass_depth(mpr_ctx* ctx, uint32_t k);
+/* Schedule of mpr_simulate for a batch: `grids` > 0 runs the M x sweeps_per_real sweeps of step 6
+ * for `grids` grids at a time, group after group, instead of every grid in every launch, so that a group's state can
+ * stay in the L2 cache between consecutive passes (one 2048 x 2048 grid is 2 x 32 MiB of vectors).  The result does not
+ * depend on the schedule (grids are independent).  0 = all grids in every launch (default).  Ignored with chains > 1.
+ * Host-side only. */
+mpr_status mpr_set_grid_group(mpr_ctx* ctx, int grids);
 /* The tiling mpr_create chose: core tile rows x cols, halo width, and the current pass depth. */
 mpr_status mpr_get_tiling(mpr_ctx* ctx, int* h_tile_rows, int* h_tile_cols, int* h_halo, uint32_t* h_pass_depth);
 

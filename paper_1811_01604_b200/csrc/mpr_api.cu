@@ -38,7 +38,7 @@ struct Geometry {
     uint32_t N, words, pitch;
     size_t VG;
     int TR, TC, H, FR, FC, ntx, nty, ntiles;
-    uint32_t n_partials;
+    uint32_t n_partials, acc_stride;
     size_t entry_stride;
 };
 
@@ -71,6 +71,7 @@ void choose_tiles(int batch, int rows, int cols, Geometry* g)
     g->FC = ((TC + 2 * H + 1) & ~3) + 2;        // >= TC + 2H and = 2 (mod 4): a column's rows spread over the banks
     g->ntx = (cols + TC - 1) / TC; g->nty = (rows + TR - 1) / TR; g->ntiles = g->ntx * g->nty;
     g->n_partials = (uint32_t)(g->ntiles > ENERGY_BLOCKS ? g->ntiles : ENERGY_BLOCKS);
+    g->acc_stride = (((uint32_t)TR * (uint32_t)TC + 15u) & ~15u) + 16u;   // two 16-aligned runs of core entries per tile
     g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 31) & ~(size_t)15);   // two 16-aligned lists per tile
 }
 
@@ -104,8 +105,8 @@ Layout make_layout(int batch, int chains, const Geometry& g)
     L.phi       = take(B * g.N * sizeof(float));
     L.bits      = take(B * g.words * sizeof(uint32_t));
     L.vec       = take(2 * V * g.VG * sizeof(float2));
-    L.acc       = take(V * g.N * sizeof(float));
-    L.m2        = take(V * g.N * sizeof(float));
+    L.acc       = take(V * (size_t)g.ntiles * g.acc_stride * sizeof(float));
+    L.m2        = take(V * (size_t)g.ntiles * g.acc_stride * sizeof(float));
     L.tile_meta = take(B * g.ntiles * sizeof(TileMeta));
     L.entries   = take((B * g.entry_stride + 16) * sizeof(uint16_t));
     L.total = o;
@@ -117,7 +118,7 @@ enum RunState { CREATED = 0, READY = 1 };
 }  // namespace
 
 struct mpr_ctx {
-    alignas(64) CUtensorMap map[2];   // frame boxes of the two vector buffers (TMA descriptors)
+    alignas(64) CUtensorMap map[2][MAX_H / 2 + 1];   // frame boxes of the two vector buffers (TMA descriptors), [buffer][row halo / 2]
     Dev          d;
     Layout       lay;
     cudaStream_t stream;
@@ -137,8 +138,10 @@ struct mpr_ctx {
     double       a_min;           // smallest proposal-width parameter a over the grids, as far as the host knows it (0 = unknown)
     bool         small_d;         // every grid's proposal half-rotation q pi / (2 a) is below SMALL_HD (host knowledge of a)
     uint32_t     cur;             // vector buffer holding the current state, the same for every grid outside mpr_equilibrate
-    uint32_t     pf_dist;         // tile passes resident on the device at once (L2 prefetch distance), 0 = not yet known
-    int          active;          // states the tile passes cover: the grids (chain 0), or every chain inside mpr_simulate
+    uint32_t     pf_dist[2];      // tile passes resident on the device at once (L2 prefetch distance), 0 = not yet known; [1]: single-sweep passes
+    int          active;          // states the tile passes cover: the grids (chain 0), or every chain inside mpr_simulate,
+    int          first;           //   or one group of grids (mpr_set_grid_group): states first .. first + active - 1
+    int          group;           // grids per group in mpr_simulate (0 = all at once)
     bool         forked;          // chains >= 1 hold a copy of their grid's state (until chain 0 alone moves again)
     uint64_t     n_realizations;  // realizations accumulated per grid (all of its chains) since mpr_set_params
 };
@@ -152,22 +155,23 @@ mpr_status fetch_states(mpr_ctx* ctx)
     return MPR_OK;
 }
 
-typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t);
+typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t);
 
 // fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps);
 // std_fc = the frame pitch is the compile-time STD_FC (standard tile shape)
 // small_d = every proposal half-rotation is below SMALL_HD (short sin / cos polynomials); only without the fused tails
-template <int FCT, bool SMALLD>
+// MINB = CTAs per SM the kernel is built for (4: single-sweep passes of the standard tile shape)
+template <int FCT, bool SMALLD, int MINB>
 pass_kernel pick_pass_kernel_fc(bool qhalf, int or_mode)
 {
-    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, false, FCT, SMALLD> : or_mode == 1 ? k_tilepass<true, 1, false, FCT, SMALLD> : k_tilepass<true, 2, false, FCT, SMALLD>;
-    return or_mode == 0 ? k_tilepass<false, 0, false, FCT, SMALLD> : k_tilepass<false, 2, false, FCT, SMALLD>;
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, false, FCT, SMALLD, false, MINB> : or_mode == 1 ? k_tilepass<true, 1, false, FCT, SMALLD, false, MINB> : k_tilepass<true, 2, false, FCT, SMALLD, false, MINB>;
+    return or_mode == 0 ? k_tilepass<false, 0, false, FCT, SMALLD, false, MINB> : k_tilepass<false, 2, false, FCT, SMALLD, false, MINB>;
 }
-template <int FCT>
+template <int FCT, int MINB>
 pass_kernel pick_fused_kernel_fc(bool qhalf, int or_mode)
 {
-    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true, FCT, false> : or_mode == 1 ? k_tilepass<true, 1, true, FCT, false> : k_tilepass<true, 2, true, FCT, false>;
-    return or_mode == 0 ? k_tilepass<false, 0, true, FCT, false> : k_tilepass<false, 2, true, FCT, false>;
+    if (qhalf) return or_mode == 0 ? k_tilepass<true, 0, true, FCT, false, false, MINB> : or_mode == 1 ? k_tilepass<true, 1, true, FCT, false, false, MINB> : k_tilepass<true, 2, true, FCT, false, false, MINB>;
+    return or_mode == 0 ? k_tilepass<false, 0, true, FCT, false, false, MINB> : k_tilepass<false, 2, true, FCT, false, false, MINB>;
 }
 // Alg. 2 step 5 inside the pass (grids that are one tile)
 template <int FCT>
@@ -180,11 +184,16 @@ pass_kernel pick_equil_kernel(bool qhalf, int or_mode, bool std_fc)
 {
     return std_fc ? pick_equil_kernel_fc<STD_FC>(qhalf, or_mode) : pick_equil_kernel_fc<0>(qhalf, or_mode);
 }
-pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused, bool std_fc, bool small_d)
+// four = a single-sweep pass of the standard tile shape: the instantiation budgeted for four CTAs per SM
+pass_kernel pick_pass_kernel(bool qhalf, int or_mode, bool fused, bool std_fc, bool small_d, bool four = false)
 {
-    if (fused) return std_fc ? pick_fused_kernel_fc<STD_FC>(qhalf, or_mode) : pick_fused_kernel_fc<0>(qhalf, or_mode);
-    if (small_d) return std_fc ? pick_pass_kernel_fc<STD_FC, true>(qhalf, or_mode) : pick_pass_kernel_fc<0, true>(qhalf, or_mode);
-    return std_fc ? pick_pass_kernel_fc<STD_FC, false>(qhalf, or_mode) : pick_pass_kernel_fc<0, false>(qhalf, or_mode);
+    if (four && std_fc) {
+        if (fused) return pick_fused_kernel_fc<STD_FC, 4>(qhalf, or_mode);
+        return small_d ? pick_pass_kernel_fc<STD_FC, true, 4>(qhalf, or_mode) : pick_pass_kernel_fc<STD_FC, false, 4>(qhalf, or_mode);
+    }
+    if (fused) return std_fc ? pick_fused_kernel_fc<STD_FC, 3>(qhalf, or_mode) : pick_fused_kernel_fc<0, 3>(qhalf, or_mode);
+    if (small_d) return std_fc ? pick_pass_kernel_fc<STD_FC, true, 3>(qhalf, or_mode) : pick_pass_kernel_fc<0, true, 3>(qhalf, or_mode);
+    return std_fc ? pick_pass_kernel_fc<STD_FC, false, 3>(qhalf, or_mode) : pick_pass_kernel_fc<0, false, 3>(qhalf, or_mode);
 }
 
 void note_a(mpr_ctx* ctx, double a_min)
@@ -200,29 +209,39 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
 {
     ctx->dirty = true;
     const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
+    // A pass of K sweeps loads 2K halo rows (a grid that is one tile has its zero border instead of a halo) and, when
+    // it is a single sweep, needs no room for stored random words: less shared memory, less to load
+    const uint32_t row_halo = ctx->d.ntiles == 1 ? (uint32_t)ctx->d.H : (2u * K < (uint32_t)ctx->d.H ? 2u * K : (uint32_t)ctx->d.H);
+    Dev d = ctx->d;
+    const bool single = K == 1 && !equil && d.ntiles > 1;
+    if (single) d.use_spare = 0;
+    const size_t smem = (size_t)(d.TR + 2 * (int)row_halo) * d.FC * sizeof(float2) + (d.use_spare ? 10u : 2u) * (size_t)d.max_entries;
     const pass_kernel kern = equil ? pick_equil_kernel(ctx->qhalf, (int)ctx->prm.or_mode, ctx->d.FC == STD_FC)
-                                   : pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC, ctx->small_d);
-    if (!ctx->pf_dist) {
+                                   : pick_pass_kernel(ctx->qhalf, (int)ctx->prm.or_mode, fused, ctx->d.FC == STD_FC, ctx->small_d, single);
+    uint32_t& pf_dist = ctx->pf_dist[single ? 1 : 0];
+    if (!pf_dist) {
         int per_sm = 0, sms = 0;
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)kern, TILE_THREADS, ctx->smem_bytes));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)kern, TILE_THREADS, smem));
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
-        ctx->pf_dist = (uint32_t)(per_sm > 0 ? per_sm * sms : sms);
+        pf_dist = (uint32_t)(per_sm > 0 ? per_sm * sms : sms);
 #ifdef MPR_EXPERIMENT_HOOKS
-        if (const char* e = getenv("MPR_PF_DIST")) ctx->pf_dist = (uint32_t)atoi(e) ? (uint32_t)atoi(e) : ctx->pf_dist;
+        if (const char* e = getenv("MPR_PF_DIST")) pf_dist = (uint32_t)atoi(e) ? (uint32_t)atoi(e) : pf_dist;
 #endif
     }
     const uint32_t src_sel = flip == PER_GRID ? PER_GRID : (ctx->cur ^ flip);
     // programmatic stream serialization: this pass's CTAs may start (and load their tile lists) while the last
     // CTAs of the previous kernel still run; k_tilepass waits for that kernel before it reads any result of it
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(ctx->d.ntiles, ctx->active); cfg.blockDim = dim3(TILE_THREADS);
-    cfg.dynamicSmemBytes = ctx->smem_bytes; cfg.stream = ctx->stream;
+    cfg.gridDim = dim3(ctx->d.ntiles, ctx->active); cfg.blockDim = dim3(TILE_THREADS);      // states first .. first + active - 1
+    cfg.dynamicSmemBytes = smem; cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = ctx->no_pdl ? 0 : 1;
     ++ctx->launches;
-    if (!cuda_ok(cudaLaunchKernelEx(&cfg, kern, ctx->map[0], ctx->map[1], ctx->d, K, t_off, src_sel, flags, ctx->pf_dist, real_no),
+    const CUtensorMap* maps0 = &ctx->map[0][row_halo / 2], *maps1 = &ctx->map[1][row_halo / 2];
+    if (!cuda_ok(cudaLaunchKernelEx(&cfg, kern, *maps0, *maps1, d, K, t_off, src_sel, flags, pf_dist, real_no, row_halo,
+                                    (uint32_t)ctx->first),
                  "tile pass launch")) return MPR_ERR_CUDA;
     return MPR_OK;
 }
@@ -242,7 +261,7 @@ mpr_status launch_sweeps(mpr_ctx* ctx, uint32_t n, uint32_t* t_off, uint32_t* fl
 
 // TMA descriptor of one vector buffer: [batch][rows][cols] eight-byte elements with row pitch d.pitch,
 // box = one tile frame; elements outside the grid are delivered as zeros (open boundary)
-mpr_status make_frame_map(mpr_ctx* ctx, int which)
+mpr_status make_frame_map(mpr_ctx* ctx, int which, int row_halo)
 {
     static PFN_cuTensorMapEncodeTiled encode = nullptr;
     if (!encode) {
@@ -258,9 +277,9 @@ mpr_status make_frame_map(mpr_ctx* ctx, int which)
     const Dev& d = ctx->d;
     const cuuint64_t dims[3] = {(cuuint64_t)d.cols, (cuuint64_t)d.rows, (cuuint64_t)d.nv};
     const cuuint64_t strides[2] = {(cuuint64_t)d.pitch * sizeof(float2), (cuuint64_t)d.VG * sizeof(float2)};
-    const cuuint32_t box[3] = {(cuuint32_t)d.FC, (cuuint32_t)d.FR, 1u};
+    const cuuint32_t box[3] = {(cuuint32_t)d.FC, (cuuint32_t)(d.TR + 2 * row_halo), 1u};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
-    const CUresult r = encode(&ctx->map[which], CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, (void*)(d.vec + (size_t)which * d.VB),
+    const CUresult r = encode(&ctx->map[which][row_halo / 2], CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, (void*)(d.vec + (size_t)which * d.VB),
                               dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -372,7 +391,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     d.entries = (uint16_t*)(base + lay.entries);
     d.chains = chains; d.nv = batch * chains;
     d.VG = g.VG; d.VB = (size_t)d.nv * g.VG;
-    d.entry_stride = g.entry_stride; d.n_partials = g.n_partials;
+    d.entry_stride = g.entry_stride; d.n_partials = g.n_partials; d.acc_stride = g.acc_stride;
     d.tile_entries = (uint32_t)(g.entry_stride / (size_t)g.ntiles);
     d.fc_inv = (uint32_t)(((1u << 24) + (uint32_t)g.FC - 1u) / (uint32_t)g.FC);
     d.TR = g.TR; d.TC = g.TC; d.H = g.H; d.FR = g.FR; d.FC = g.FC; d.ntx = g.ntx; d.nty = g.nty; d.ntiles = g.ntiles;
@@ -392,7 +411,8 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     cudaStream_t s = ctx->stream;
     // the pad column of an odd-width grid stays zero
     if (!cuda_ok(cudaMemsetAsync(d.vec, 0, 2 * d.VB * sizeof(float2), s), "memset vec")) return fail(MPR_ERR_CUDA);
-    for (int w = 0; w < 2; ++w) { st = make_frame_map(ctx, w); if (st != MPR_OK) return fail(st); }
+    for (int w = 0; w < 2; ++w)
+        for (int hr = 2; hr <= g.H; hr += 2) { st = make_frame_map(ctx, w, hr); if (st != MPR_OK) return fail(st); }
     k_state_reset<<<cdiv(d.nv, 128), 128, 0, s>>>(d);
     unsigned mm_blocks = cdiv(g.N, 256 * 8);
     if (mm_blocks > 1184) mm_blocks = 1184;
@@ -457,6 +477,9 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
                         for (int sd = 0; sd < 2; ++sd) {
                             if (!qh && om == 1) continue;
                             if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, g.FC == STD_FC, sd), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                              (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
+                            if (g.FC == STD_FC &&
+                                !cuda_ok(cudaFuncSetAttribute((const void*)pick_pass_kernel(qh, om, fu, true, sd, true), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                               (int)ctx->smem_bytes), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
                             if (fu && !sd &&
                                 !cuda_ok(cudaFuncSetAttribute((const void*)pick_equil_kernel(qh, om, g.FC == STD_FC), cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -528,8 +551,8 @@ mpr_status mpr_set_params(mpr_ctx* ctx, const mpr_params* p, const float* h_T)
     CU(cudaMemcpyAsync(d.e_partials, h_T, sizeof(float) * d.batch, cudaMemcpyHostToDevice, ctx->stream));
     k_begin_run<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, (const float*)d.e_partials);
     CU_LAUNCH();
-    CU(cudaMemsetAsync(d.acc, 0, (size_t)d.nv * d.N * sizeof(float), ctx->stream));
-    CU(cudaMemsetAsync(d.m2, 0, (size_t)d.nv * d.N * sizeof(float), ctx->stream));
+    CU(cudaMemsetAsync(d.acc, 0, (size_t)d.nv * d.ntiles * d.acc_stride * sizeof(float), ctx->stream));
+    CU(cudaMemsetAsync(d.m2, 0, (size_t)d.nv * d.ntiles * d.acc_stride * sizeof(float), ctx->stream));
     k_init_state<<<dim3(cdiv(d.N, 256), d.batch), 256, 0, ctx->stream>>>(d, ctx->unconditional ? 1 : 0);
     CU_LAUNCH();
     CU(cudaStreamSynchronize(ctx->stream));      // h_T may be pageable and reused by the caller
@@ -635,14 +658,22 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
         n_real = (ctx->prm.M + (uint32_t)d.chains - 1u) / (uint32_t)d.chains;
         ctx->active = d.nv;
     }
+    // One group of grids after the other (mpr_set_grid_group; one chain per grid only): a group's vectors stay in L2
+    // from pass to pass when they fit.  Every group does the same passes, so t_off and flip end alike.
+    const int group = (ctx->group > 0 && d.chains == 1 && ctx->group < d.batch) ? ctx->group : ctx->active;
+    const int n_states = ctx->active;
     uint32_t t_off = 0, flip = 0;
     mpr_status s = MPR_OK;
-    for (uint32_t j = 0; j < n_real && s == MPR_OK; ++j)
-        // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
-        s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE, j + 1u);   // realization number: realizations so far + j + 1
-    ctx->active = d.batch;
+    for (int g0 = 0; g0 < n_states && s == MPR_OK; g0 += group) {
+        ctx->first = g0; ctx->active = n_states - g0 < group ? n_states - g0 : group;
+        t_off = 0; flip = 0;
+        for (uint32_t j = 0; j < n_real && s == MPR_OK; ++j)
+            // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
+            s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE, j + 1u);   // realization number: realizations so far + j + 1
+    }
+    ctx->first = 0; ctx->active = d.batch;
     if (s != MPR_OK) return s;
-    k_commit<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, d.chains > 1 ? d.nv : d.batch, t_off, flip, n_real);
+    k_commit<<<cdiv(d.nv, 128), 128, 0, ctx->stream>>>(d, 0, d.chains > 1 ? d.nv : d.batch, t_off, flip, n_real);
     CU_LAUNCH();
     ctx->cur ^= flip;
     ctx->n_realizations += (uint64_t)n_real * (uint64_t)d.chains;
@@ -655,7 +686,7 @@ mpr_status mpr_predict(mpr_ctx* ctx, float* d_out)
     ENTER(ctx);
     if (ctx->state != READY || ctx->n_realizations == 0) return MPR_ERR_STATE;     // the mean of no realization is 0 / 0
     const Dev& d = ctx->d;
-    k_predict<<<site_grid(ctx), 256, 0, ctx->stream>>>(d, d_out);
+    k_predict<0><<<dim3(d.ntiles, d.batch), 256, 0, ctx->stream>>>(d, 0.0, d_out);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -672,7 +703,7 @@ mpr_status mpr_predict_std(mpr_ctx* ctx, float* d_out)
         for (int c = 0; c < ctx->d.chains; ++c) n += ctx->h_states[b + c * ctx->d.batch].realizations;
         if (n < 2u) return MPR_ERR_STATE;
     }
-    k_predict_std<<<site_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, d_out);
+    k_predict<1><<<dim3(ctx->d.ntiles, ctx->d.batch), 256, 0, ctx->stream>>>(ctx->d, 0.0, d_out);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -695,7 +726,7 @@ mpr_status mpr_predict_quantile(mpr_ctx* ctx, double p, float* d_out)
         const double mid = 0.5 * (lo + hi);
         (0.5 * std::erfc(-mid / std::sqrt(2.0)) < p ? lo : hi) = mid;
     }
-    k_predict_quantile<<<site_grid(ctx), 256, 0, ctx->stream>>>(ctx->d, 0.5 * (lo + hi), d_out);
+    k_predict<2><<<dim3(ctx->d.ntiles, ctx->d.batch), 256, 0, ctx->stream>>>(ctx->d, 0.5 * (lo + hi), d_out);
     CU_LAUNCH();
     return MPR_OK;
 }
@@ -872,7 +903,7 @@ mpr_status mpr_sweep(mpr_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_acce
     uint32_t t_off = 0, flip = 0;
     mpr_status rs = launch_sweeps(ctx, n_sweeps, &t_off, &flip, h_accepted ? PASS_COUNT : 0u, 0);
     if (rs != MPR_OK) return rs;
-    k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, d.batch, t_off, flip, 0);
+    k_commit<<<cdiv(d.batch, 128), 128, 0, ctx->stream>>>(d, 0, d.batch, t_off, flip, 0);
     CU_LAUNCH();
     ctx->cur ^= flip;
     if (h_accepted) {
@@ -948,6 +979,13 @@ mpr_status mpr_set_pass_depth(mpr_ctx* ctx, uint32_t k)
     const uint32_t most = ctx->d.ntiles == 1 ? 1024u : (uint32_t)(ctx->d.H / 2);
     if (k > most) return MPR_ERR_ARG;
     ctx->k_max = k ? k : most;
+    return MPR_OK;
+}
+
+mpr_status mpr_set_grid_group(mpr_ctx* ctx, int grids)
+{
+    if (!ctx || grids < 0) return MPR_ERR_ARG;
+    ctx->group = grids;
     return MPR_OK;
 }
 

@@ -73,8 +73,9 @@ struct Dev {
     float*     phi;            // [batch][N] angle view: Eq. 1 at sample sites (never rewritten), export buffer at free sites
     uint32_t*  bits;           // [batch][words] fixed-site bitmask
     float2*    vec;            // [2 buffers][nv][rows][pitch] row-major unit vectors (pitch = cols rounded up to even)
-    float*     acc;            // [nv][N] sum over realizations of phi at the prediction sites
-    float*     m2;             // [nv][N] sum of squared deviations from the running mean (Welford), for the spread (L212)
+    float*     acc;            // [nv][ntiles][acc_stride] sum over realizations of phi at the prediction sites, per tile in the
+                               // order of the tile's CORE entries: colour 0's at 0.., colour 1's from colour1_base(count of colour 0)
+    float*     m2;             // same shape: sum of squared deviations from the running mean (Welford), for the spread (L212)
     TileMeta*  tile_meta;      // [batch][ntiles]
     uint16_t*  entries;        // [batch][entry_stride] tile frames' free sites: offset in the frame (row * FC + col)
     int        batch, rows, cols;   // batch = grids with data of their own
@@ -87,6 +88,7 @@ struct Dev {
     uint32_t   tile_entries;   // room of one tile's lists (worst case: every frame site free), multiple of 16; tile i's
                                // lists start at i * tile_entries, so that loading them needs nothing read first
     uint32_t   n_partials;
+    uint32_t   acc_stride;     // floats of one tile's accumulators: TR * TC rounded up to 16, + 16
     // tiling
     int        TR, TC, H, FR, FC, ntx, nty, ntiles;
     uint32_t   max_entries;    // shared-memory capacity for entries (multiple of 8)
@@ -816,10 +818,13 @@ template <int M> struct DrawTag { static constexpr int value = M; };
 // the accepted count are reduced in the CTA, thread 0 takes steps 5.2-5.5 (controller_step) and the CTA goes on with the
 // new proposal width or stops; K is then the most sweeps this launch may do.  Bit for bit the sweeps of the K = 1
 // passes with k_controller between them (every sweep renormalises, as a K = 1 pass does), without 2 launches per sweep.
-template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD, bool EQUIL = false>
-__global__ void __launch_bounds__(TILE_THREADS, TILE_THREADS >= 384 ? 2 : 3)
+// MINB: CTAs per SM the registers are budgeted for: 3 for the K-sweep passes (their shared memory allows no more), 4 for
+// single-sweep passes (row halo 2, no stored random words: 49 KB), whose length is mostly a CTA's own latency
+template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD, bool EQUIL = false, int MINB = 3>
+__global__ void __launch_bounds__(TILE_THREADS, MINB)
 k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
-           uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist, uint32_t real_no)
+           uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist, uint32_t real_no, uint32_t row_halo,
+           uint32_t g_first)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar[2];       // [0] frame, [1] entry list
@@ -830,7 +835,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 
     constexpr int NT = TILE_THREADS, NW = TILE_THREADS / 32;
     static_assert(TILE_THREADS >= 96 + 2 * MAX_H && TILE_THREADS >= HS_CHUNK, "the prologue gives warps 0-3 their own jobs");
-    const int tile = blockIdx.x, g = blockIdx.y;            // g: state (grid and chain), gd: the grid whose data it shares
+    const int tile = blockIdx.x, g = (int)(blockIdx.y + g_first);   // g: state (grid and chain), gd: the grid whose data it shares
     const int gd = g < d.batch ? g : g % d.batch;
     const GridState& st = d.states[g];
     // Programmatic dependent launch: the next kernel of the stream may start its CTAs while the last of this
@@ -841,8 +846,14 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     // frame pitch: a compile-time constant for the standard tile shape (neighbour offsets become immediates)
     const int H = d.H, FC = FCT ? FCT : d.FC;
     const uint32_t fc_inv = FCT ? (uint32_t)(((1u << 24) + (uint32_t)(FCT ? FCT : 1) - 1u) / (uint32_t)(FCT ? FCT : 1)) : d.fc_inv;
-    float2*   S  = reinterpret_cast<float2*>(smem_raw);
-    uint2*    SP = reinterpret_cast<uint2*>(S + d.FR * FC);
+    // A pass of K sweeps needs 2K rings of halo.  The frame that is loaded keeps the full pitch FC (entry offsets are
+    // row * FC + col of the full frame) but only row_halo = min(H, 2K) halo rows above and below the core: the maps'
+    // box has TR + 2 row_halo rows.  S points where row 0 of the FULL frame would be, so that the offsets stay valid;
+    // rows above S_load are never touched (an entry of ring <= 2K - 1 has its upper neighbour in ring <= 2K).
+    const int HR = (int)row_halo, FRK = d.TR + 2 * HR;
+    float2*   S_load = reinterpret_cast<float2*>(smem_raw);
+    float2*   S  = S_load - (H - HR) * FC;
+    uint2*    SP = reinterpret_cast<uint2*>(S_load + FRK * FC);
     uint16_t* E  = reinterpret_cast<uint16_t*>(SP + (d.use_spare ? d.max_entries : 0u));
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -872,16 +883,22 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     const uint32_t src_buf = src_sel < 2u ? src_sel : st.cur;
     float2* dst = vec_grid(d, g, src_buf ^ 1u);
     if (tid == 0) {
-        mbar_expect_tx(&s_bar[0], (uint32_t)(d.FR * FC * sizeof(float2)));
-        tma_load_frame(S, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - H, g, &s_bar[0]);
+        mbar_expect_tx(&s_bar[0], (uint32_t)(FRK * FC * sizeof(float2)));
+        tma_load_frame(S_load, src_buf ? &map1 : &map0, tg.c0 - H, tg.r0 - HR, g, &s_bar[0]);
     }
     // warp 2 pulls what the tile that will run in this CTA slot next needs towards L2: its frame and its entry list
     if (tid == 64 && pf_dist && tile + (int)pf_dist < d.ntiles) {
         const TileGeom tn = tile_geom(d, tile + (int)pf_dist);
-        tma_prefetch_frame(src_buf ? &map1 : &map0, tn.c0 - H, tn.r0 - H, g);
+        tma_prefetch_frame(src_buf ? &map1 : &map0, tn.c0 - H, tn.r0 - HR, g);
         if (d.max_entries)
             bulk_prefetch(d.entries + (size_t)gd * d.entry_stride + (size_t)(tile + pf_dist) * d.tile_entries,
                           d.max_entries * (uint32_t)sizeof(uint16_t));
+    }
+    if (tid == 65 && (flags & PASS_ACCUMULATE)) {       // the tile's accumulators towards L2 while the sweeps run
+        const size_t at = ((size_t)g * d.ntiles + tile) * d.acc_stride;
+        const uint32_t bytes = ((uint32_t)(tg.TRc * tg.TCc) * 4u + 15u) & ~15u;      // never more than the tile can hold
+        bulk_prefetch(d.acc + at, bytes);
+        bulk_prefetch(d.m2 + at, bytes);
     }
     float hs = st.hd_scale, hc1 = hs * 5.9604644775390625e-08f;
     const float nlT = st.neg_log2e_over_T;
@@ -1020,65 +1037,33 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     if (flags & PASS_ACCUMULATE) {
         // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites; and for the spread of the
         // realizations (L212) the sum of squared deviations, updated from the running mean so that nothing cancels:
-        // m2 += (phi - mean_{k-1}) (phi - mean_k), k = number of this realization
-        float* acc = d.acc + (size_t)g * d.N;
-        float* m2 = d.m2 + (size_t)g * d.N;
+        // m2 += (phi - mean_{k-1}) (phi - mean_k), k = number of this realization.
+        // The accumulators are kept per tile in the order of the tile's core entries, so that a pass touches only
+        // prediction sites' words, consecutive lanes consecutive words (and the tile's range was sent for at the start).
+        float* acc = d.acc + ((size_t)g * d.ntiles + tile) * d.acc_stride;
+        float* m2 = d.m2 + ((size_t)g * d.ntiles + tile) * d.acc_stride;
         const uint32_t k = st.realizations + real_no;
         const float inv_km1 = k > 1u ? 1.0f / (float)(k - 1u) : 0.0f, inv_k = 1.0f / (float)k;
-        // The core is walked row by row in groups of four sites (not along the entry lists, whose order is made for
-        // the shared-memory banks): a lane moves 16 bytes of acc and of m2, a warp whole lines; two groups per thread
-        // are in flight.  Needs cols, the tile's first column and its width to be multiples of four.
-        const uint32_t* bits = d.bits + (size_t)gd * d.words;
-        auto add_site = [&](float2 v, bool fixed, float& a_, float& m_) {
-            if (fixed) return;
-            const float phi = angle_of(v, d.inv_q), before = a_, after = before + phi;
-            a_ = after;
-            if (k > 1u) m_ += (phi - before * inv_km1) * (phi - after * inv_k);
-        };
-        if (((d.cols | tg.c0 | tg.TCc) & 3) == 0) {
-            const int q4 = tg.TCc >> 2, n4 = tg.TRc * q4;
-            for (int i0 = tid; i0 < n4; i0 += 2 * NT) {
-                int idx[2], off[2];
-                uint32_t fx[2];
-                float4 a4[2], m4[2];
+        const uint32_t n0 = s_cle[0][0], a1 = colour1_base(n0), n_acc = a1 + s_cle[1][0], e1 = colour1_base(s_cle[0][MAX_H - 1]);
+        // position i of the tile's accumulators: colour 0's core entry i (i < n0), colour 1's core entry i - a1 (i >= a1)
+#pragma unroll 1
+        for (uint32_t i0 = tid; i0 < n_acc; i0 += 4u * NT) {
+            float a_[4], m_[4];
+            bool on[4];
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int i = i0 + u * NT;
-                    fx[u] = 0xFu;
-                    if (i < n4) {
-                        const int lr = i / q4, j = i - lr * q4;
-                        idx[u] = (tg.r0 + lr) * d.cols + tg.c0 + 4 * j;
-                        off[u] = (H + lr) * FC + H + 4 * j;
-                        fx[u] = (__ldg(bits + (idx[u] >> 5)) >> (idx[u] & 31)) & 0xFu;
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 2; ++u)
-                    if (fx[u] != 0xFu) {
-                        a4[u] = *reinterpret_cast<const float4*>(acc + idx[u]);
-                        if (k > 1u) m4[u] = *reinterpret_cast<const float4*>(m2 + idx[u]);
-                        else m4[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    }
-#pragma unroll
-                for (int u = 0; u < 2; ++u)
-                    if (fx[u] != 0xFu) {
-                        const float2* v = S + off[u];
-                        add_site(v[0], fx[u] & 1u, a4[u].x, m4[u].x);
-                        add_site(v[1], fx[u] & 2u, a4[u].y, m4[u].y);
-                        add_site(v[2], fx[u] & 4u, a4[u].z, m4[u].z);
-                        add_site(v[3], fx[u] & 8u, a4[u].w, m4[u].w);
-                        *reinterpret_cast<float4*>(acc + idx[u]) = a4[u];
-                        if (k > 1u) *reinterpret_cast<float4*>(m2 + idx[u]) = m4[u];
-                    }
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = i0 + (uint32_t)u * NT;
+                on[u] = i < n_acc && (i < n0 || i >= a1);
+                if (on[u]) { a_[u] = acc[i]; m_[u] = k > 1u ? m2[i] : 0.0f; }
             }
-        } else {
-            for (int c = 0; c < 2; ++c) {
-                const uint32_t base = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
-                for (uint32_t e = tid; e < s_cle[c][0]; e += NT) {
-                    const uint32_t off = E[base + e];
-                    const int idx = nbase + (int)off + (int)((off * fc_inv) >> 24) * ncorr;
-                    add_site(S[off], false, acc[idx], m2[idx]);
-                }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (!on[u]) continue;
+                const uint32_t i = i0 + (uint32_t)u * NT;
+                const uint32_t off = E[i < n0 ? i : e1 + (i - a1)];
+                const float phi = angle_of(S[off], d.inv_q), before = a_[u], after = before + phi;
+                acc[i] = after;
+                if (k > 1u) m2[i] = m_[u] + (phi - before * inv_km1) * (phi - after * inv_k);
             }
         }
     }
@@ -1269,10 +1254,10 @@ __global__ void k_set_a(Dev d, int mode, double a_value, int zero_accepted)
     if (zero_accepted) s.accepted = 0ull;
 }
 // commit passes that ran with (t_off, flip) arguments: t += n_sweeps, swap buffers if the pass count was odd
-__global__ void k_commit(Dev d, int n_states, uint32_t n_sweeps, uint32_t flip, uint32_t n_realizations)
+__global__ void k_commit(Dev d, int first, int n_states, uint32_t n_sweeps, uint32_t flip, uint32_t n_realizations)
 {
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= n_states) return;
+    const int g = first + blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= first + n_states) return;
     GridState& s = d.states[g];
     s.t += n_sweeps; s.cur ^= flip; s.realizations += n_realizations;
 }
@@ -1323,86 +1308,63 @@ __global__ void k_begin_run(Dev d, const float* __restrict__ T)
 }
 
 // ---------------------------------------------------------------------------
-// a8  prediction (Alg. 2 step 7, L148, L212): mean angle over the realizations,
-// back-transformed by the inverse of Eq. 1 at the prediction sites; sample
-// sites return the input value bit for bit.
+// a8  prediction (Alg. 2 step 7, L148, L212) and the statistics of the realizations.  One block per tile: the
+// tile's accumulators are in the order of its core entries (k_tilepass, PASS_ACCUMULATE), the entry gives the site.
+// WHAT 0: mean angle over the realizations, back-transformed by the inverse of Eq. 1; sample sites return the input
+//         value bit for bit.
+// WHAT 1: spread (L212): sample standard deviation of the back-transformed values, 0 at sample sites.
+// WHAT 2: Gaussian p-quantile from the pooled mean and spread (reading R26): z_p = mean_z + x_p s_z with
+//         x_p = Phi^-1(p) computed on the host, clamped to the data range; sample sites = input.
+// The realizations of every chain of the grid are pooled (one chain: the paper's step 7): sum of squared deviations
+// from the pooled mean = sum over the chains of [their own m2 + n_c (mean_c - mean)^2].
 // ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_predict(Dev d, float* __restrict__ out)
+template <int WHAT>
+__global__ void __launch_bounds__(256) k_predict(Dev d, double x_p, float* __restrict__ out)
 {
-    const int g = blockIdx.y;
-    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= d.N) return;
-    const size_t o = (size_t)g * d.N + n;
-    if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = d.values[o]; return; }
+    const int tile = blockIdx.x, g = blockIdx.y;
+    const TileGeom tg = tile_geom(d, tile);
     const GridState& s = d.states[g];
-    // the realizations of every chain of the grid are pooled (one chain: the paper's step 7)
-    double sum = 0.0, count = 0.0;
-    for (int c = 0; c < d.chains; ++c) {
-        const int v = g + c * d.batch;
-        sum += (double)d.acc[(size_t)v * d.N + n]; count += (double)d.states[v].realizations;
+    const uint32_t* bits = d.bits + (size_t)g * d.words;
+    // sample sites of the core
+    for (int i = threadIdx.x; i < tg.TRc * tg.TCc; i += blockDim.x) {
+        const int lr = i / tg.TCc, lc = i - lr * tg.TCc;
+        const uint32_t n = (uint32_t)(tg.r0 + lr) * d.cols + (uint32_t)(tg.c0 + lc);
+        if (is_fixed(bits, n)) out[(size_t)g * d.N + n] = WHAT == 1 ? 0.0f : d.values[(size_t)g * d.N + n];
     }
-    const double mean_phi = sum / count;
-    const double z = (double)s.zmin + mean_phi * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F;
-    out[o] = (float)z;
-}
-
-// spread of the realizations (L212): sample standard deviation of the back-transformed values, 0 at sample sites
-__global__ void __launch_bounds__(256) k_predict_std(Dev d, float* __restrict__ out)
-{
-    const int g = blockIdx.y;
-    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= d.N) return;
-    const size_t o = (size_t)g * d.N + n;
-    if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = 0.0f; return; }
-    const GridState& s = d.states[g];
-    // pooled over the chains: sum of squared deviations from the pooled mean =
-    // sum over the chains of [their own m2 + n_c (mean_c - mean)^2]
-    double sum = 0.0, count = 0.0;
-    for (int c = 0; c < d.chains; ++c) {
-        const int v = g + c * d.batch;
-        sum += (double)d.acc[(size_t)v * d.N + n]; count += (double)d.states[v].realizations;
-    }
-    const double mean = sum / count;
-    double ssd = 0.0;
-    for (int c = 0; c < d.chains; ++c) {
-        const int v = g + c * d.batch;
-        const double nc = (double)d.states[v].realizations;
-        if (nc == 0.0) continue;
-        const double dev = (double)d.acc[(size_t)v * d.N + n] / nc - mean;
-        ssd += fmax((double)d.m2[(size_t)v * d.N + n], 0.0) + nc * dev * dev;
-    }
-    const double var = count > 1.0 ? ssd / (count - 1.0) : 0.0;
-    out[o] = (float)(sqrt(var) * ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F);
-}
-
-// Gaussian p-quantile of the conditional distribution from the pooled mean and spread (reading R26):
-// z_p = mean_z + x_p s_z with x_p = Phi^-1(p) computed on the host, clamped to the data range; sample sites = input
-__global__ void __launch_bounds__(256) k_predict_quantile(Dev d, double x_p, float* __restrict__ out)
-{
-    const int g = blockIdx.y;
-    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= d.N) return;
-    const size_t o = (size_t)g * d.N + n;
-    if (is_fixed(d.bits + (size_t)g * d.words, n)) { out[o] = d.values[o]; return; }
-    const GridState& s = d.states[g];
-    double sum = 0.0, count = 0.0;
-    for (int c = 0; c < d.chains; ++c) {
-        const int v = g + c * d.batch;
-        sum += (double)d.acc[(size_t)v * d.N + n]; count += (double)d.states[v].realizations;
-    }
-    const double mean = sum / count;
-    double ssd = 0.0;
-    for (int c = 0; c < d.chains; ++c) {
-        const int v = g + c * d.batch;
-        const double nc = (double)d.states[v].realizations;
-        if (nc == 0.0) continue;
-        const double dev = (double)d.acc[(size_t)v * d.N + n] / nc - mean;
-        ssd += fmax((double)d.m2[(size_t)v * d.N + n], 0.0) + nc * dev * dev;
-    }
-    const double sd = count > 1.0 ? sqrt(ssd / (count - 1.0)) : 0.0;
+    // prediction sites: the core entries of both colours
+    const TileMeta& meta = d.tile_meta[(size_t)g * d.ntiles + tile];
+    const uint16_t* E = d.entries + (size_t)g * d.entry_stride + (size_t)tile * d.tile_entries;
+    const uint32_t n0 = meta.cle[0][0], a1 = colour1_base(n0), n_acc = a1 + meta.cle[1][0], e1 = colour1_base(meta.cle[0][MAX_H - 1]);
     const double scale = ((double)s.zmax - (double)s.zmin) / (double)TWO_PI_F;
-    const double z = (double)s.zmin + mean * scale + x_p * sd * scale;
-    out[o] = (float)fmin(fmax(z, (double)s.zmin), (double)s.zmax);
+    for (uint32_t i = threadIdx.x; i < n_acc; i += blockDim.x) {
+        if (i >= n0 && i < a1) continue;
+        const uint32_t off = E[i < n0 ? i : e1 + (i - a1)];
+        const uint32_t lr = off / (uint32_t)d.FC, lc = off - lr * (uint32_t)d.FC;
+        const uint32_t n = (uint32_t)(tg.r0 - d.H + (int)lr) * d.cols + (uint32_t)(tg.c0 - d.H + (int)lc);
+        double sum = 0.0, count = 0.0;
+        for (int c = 0; c < d.chains; ++c) {
+            const int v = g + c * d.batch;
+            sum += (double)d.acc[((size_t)v * d.ntiles + tile) * d.acc_stride + i]; count += (double)d.states[v].realizations;
+        }
+        const double mean = sum / count;
+        double z;
+        if (WHAT == 0) z = (double)s.zmin + mean * scale;
+        else {
+            double ssd = 0.0;
+            for (int c = 0; c < d.chains; ++c) {
+                const int v = g + c * d.batch;
+                const double nc = (double)d.states[v].realizations;
+                if (nc == 0.0) continue;
+                const size_t at = ((size_t)v * d.ntiles + tile) * d.acc_stride + i;
+                const double dev = (double)d.acc[at] / nc - mean;
+                ssd += fmax((double)d.m2[at], 0.0) + nc * dev * dev;
+            }
+            const double sd = count > 1.0 ? sqrt(ssd / (count - 1.0)) : 0.0;
+            if (WHAT == 1) z = sd * scale;
+            else z = fmin(fmax((double)s.zmin + mean * scale + x_p * sd * scale, (double)s.zmin), (double)s.zmax);
+        }
+        out[(size_t)g * d.N + n] = (float)z;
+    }
 }
 
 // angle import / export at the prediction sites ------------------------------

@@ -34,7 +34,7 @@ EXPORTS = (
     "mpr_sample_energy", "mpr_create_unconditional", "mpr_measure_energy", "mpr_energy_table",
     "mpr_infer_temperature", "mpr_predict_std", "mpr_query_workspace_chains", "mpr_create_chains",
     "mpr_predict_quantile", "mpr_set_pass_depth", "mpr_get_tiling",
-    "mpr_default_ladder", "mpr_infer_temperature_auto",
+    "mpr_default_ladder", "mpr_infer_temperature_auto", "mpr_set_grid_group",
     "mpr64_query_workspace", "mpr64_create", "mpr64_set_params", "mpr64_equilibrate", "mpr64_simulate", "mpr64_predict",
     "mpr64_predict_std", "mpr64_destroy", "mpr64_get_angles", "mpr64_set_angles", "mpr64_set_sweep_index", "mpr64_sweep",
     "mpr64_energy", "mpr64_get_transform", "mpr64_get_stats", "mpr64_get_launch_count",
@@ -99,6 +99,7 @@ def lib():
         L.mpr_get_stats.argtypes = [vp, C.POINTER(mpr_stats)]
         L.mpr_get_launch_count.argtypes = [vp, C.POINTER(u64)]
         L.mpr_set_pass_depth.argtypes = [vp, u32]
+        L.mpr_set_grid_group.argtypes = [vp, i]
         L.mpr_get_tiling.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i), C.POINTER(u32)]
         L.mpr_predict_std.argtypes = [vp, vp]
         L.mpr_predict_quantile.argtypes = [vp, C.c_double, vp]
@@ -355,6 +356,10 @@ class Mpr:
 
     def set_pass_depth(self, k: int):
         _check(lib().mpr_set_pass_depth(self._ctx, int(k)), "mpr_set_pass_depth")
+        return self
+
+    def set_grid_group(self, grids: int):
+        _check(lib().mpr_set_grid_group(self._ctx, int(grids)), "mpr_set_grid_group")
         return self
 
     def get_tiling(self):

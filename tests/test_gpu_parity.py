@@ -413,17 +413,18 @@ def test_t2_k_sweep_passes_on_a_multi_tile_grid(torch_cuda, mpr, orc, t0, a):
     seed = 515
     phi, _, _ = orc.transform(z, m, seed)
     orc.equilibrate(phi, m, T, orc.Params(seed=seed, equil_cap=40, n_fit=200))      # exactly 40 sweeps
-    ctx = mpr.Mpr(_dev(torch, np.stack([z, z])), _dev(torch, np.stack([m, m])))     # two grids: 70 tiles of 64 rows
+    B = 13                  # 13 x 35 = 455 tiles >= 148 x 3: the batch fills the device, so the tiles are 64 x 64 (halo 8)
+    ctx = mpr.Mpr(_dev(torch, np.stack([z] * B)), _dev(torch, np.stack([m] * B)))
     assert ctx.get_tiling()[:3] == (64, 64, 8)
-    ctx.set_params([T, T], seed=seed)
-    state = np.stack([phi, phi])
+    ctx.set_params([T] * B, seed=seed)
+    state, masks = np.stack([phi] * B), np.stack([m] * B)
     worst = 0.0
     for depth, n in ((4, 4), (4, 5), (4, 6), (4, 8), (2, 4), (2, 5), (3, 3), (3, 6), (1, 2)):
         ctx.set_pass_depth(depth)
         assert ctx.get_tiling()[3] == depth
         l0 = ctx.launch_count()
-        res = _compare_n_sweeps(orc, ctx, state, np.stack([m, m]), 0.5, [T, T], a, seed, t0, n, g_list=(0, 1),
-                                margin_thr=1e-3 if n < 7 else 1e-4)
+        res = _compare_n_sweeps(orc, ctx, state, masks, 0.5, [T] * B, a, seed, t0, n, g_list=(0, B - 1),
+                                margin_thr=1e-3 if n < 7 else 1e-4)          # the first and the last Philox grid word
         assert ctx.launch_count() - l0 == 5 + -(-n // depth)         # import, set t, set a, the passes, commit, export
         worst = max(worst, max(r[3] for r in res))
     ctx.set_pass_depth(0)
@@ -1062,3 +1063,65 @@ def test_predict_needs_a_realization(torch_cuda, mpr):
     c64.simulate()
     assert np.isfinite(c64.predict().cpu().numpy()).all()
     c64.close()
+
+
+# ---------------------------------------------------------------------------
+# BASELINE configs[4]: the batch of 32 grids of 2048 x 2048 in one context
+# ---------------------------------------------------------------------------
+def test_cfg5_full_batch_t1_t2_t3(torch_cuda, mpr, orc):
+    """The whole of BASELINE configs[4] in one context, as bench.py --workload cfg5 runs it: 32 grids of 2048 x 2048, 66 %
+    removed, each with its own correlation length, temperature and Philox grid word.
+    T1 on the last grid (largest grid word, largest offsets into the vector buffers, lists and accumulators): z_min / z_max,
+        Eq. 1 angles and the initial draw bit for bit.
+    T2 on the last grid from a generator-made state: one counted sweep (the fused single-sweep pass) and four sweeps in one
+        call (the K = 4 pass bench.py times) against the oracle.
+    T3 with one sweep per realization (M = 100; the full-length oracle run is infeasible) on the first and the
+        last grid and those with the smallest and the largest correlation length: energy, MAE, RMSE within 1 %, stopping sweep
+        within two check intervals; run once with every grid in every launch and once with mpr_set_grid_group(2), which
+        must give the same bits."""
+    torch = torch_cuda
+    w = synth.make_workload("cfg5")
+    B, L = w.batch, w.rows
+    assert (B, L) == (32, 2048)
+    ells = w.meta["ell"]
+    picks = sorted({0, B - 1, int(np.argmin(ells)), int(np.argmax(ells))})
+    Ts = [float(x) for x in w.T]
+    ctx = mpr.Mpr(_dev(torch, w.truth), _dev(torch, w.mask))
+    assert ctx.get_tiling() == (64, 64, 8, 4)
+    ctx.set_params(Ts, seed=w.seed)
+    # T1
+    g = B - 1
+    lo, hi = ctx.get_transform()
+    init = ctx.get_angles().cpu().numpy()
+    ref, zmin, zmax = orc.transform(w.truth[g], w.mask[g], w.seed, g)
+    assert np.float32(lo[g]) == zmin and np.float32(hi[g]) == zmax
+    assert np.array_equal(init[g].view(np.uint32), ref.view(np.uint32))
+    # T2 (the other grids keep their initial draw)
+    state = init.copy()
+    state[g] = _generator_state(orc, w.truth[g], w.mask[g], Ts[g], w.seed, 31, g)
+    res = _compare_one_sweep(orc, ctx, state, w.mask, 0.5, Ts, 15.0, w.seed, 200, 0, g_list=(g,))
+    assert res[0][2] <= TOL_RAD
+    res = _compare_n_sweeps(orc, ctx, state, w.mask, 0.5, Ts, 15.0, w.seed, 201, 4, g_list=(g,))
+    assert res[0][3] <= TOL_RAD
+    del state, init
+    # T3
+    kw = dict(seed=w.seed, equil_cap=w.equil_cap, sweeps_per_real=1, M=100)
+    ctx.set_params(Ts, **kw).equilibrate().simulate()
+    pred = ctx.predict().cpu().numpy()
+    e_gpu = ctx.energy()
+    st = ctx.get_stats()
+    assert all(s.equilibrated and s.realizations == 100 and s.t == s.equil_sweeps + 100 for s in st)
+    for g in picks:
+        r = orc.run(w.truth[g], w.mask[g], Ts[g], orc.Params(**kw), g=g)
+        vg = synth.validation_measures(w.truth[g], pred[g], w.mask[g])
+        vo = synth.validation_measures(w.truth[g], r["pred"], w.mask[g])
+        assert np.array_equal(pred[g][w.mask[g] == 1], w.truth[g][w.mask[g] == 1])
+        assert vg["mae"] == pytest.approx(vo["mae"], rel=0.01), (g, ells[g])
+        assert vg["rmse"] == pytest.approx(vo["rmse"], rel=0.01), (g, ells[g])
+        assert (1.0 + e_gpu[g]) == pytest.approx(1.0 + r["stats"]["e_final"], rel=0.01), (g, ells[g])
+        assert abs(st[g].equil_sweeps - r["stats"]["sweeps"]) <= 10, (g, st[g].equil_sweeps, r["stats"]["sweeps"])
+    # the grid-wise schedule of step 6 gives the same bits
+    ctx.set_grid_group(2)
+    ctx.set_params(Ts, **kw).equilibrate().simulate()
+    assert np.array_equal(ctx.predict().cpu().numpy().view(np.uint32), pred.view(np.uint32))
+    ctx.close()

@@ -121,3 +121,14 @@ def test_default_ladder_is_host_arithmetic_and_matches_the_oracle(lib, orc):
         with pytest.raises(mpr.MprError) as e:
             mpr.default_ladder(8, 8, -0.99, bad)
         assert e.value.name == "MPR_ERR_ARG"
+
+
+def test_batch_limits_of_the_boundary(lib):
+    """include/mpr.h: batch * chains <= 65535 states, rows * cols < 2^31 per grid, rows, cols <= 65534 (host checks)."""
+    assert mpr.mpr_query_workspace_chains(65535, 1, 8, 8) > 0
+    assert mpr.mpr_query_workspace_chains(255, 257, 8, 8) > 0
+    for bad in ((65536, 1, 8, 8), (256, 256, 8, 8), (1, 1, 46341, 46341), (1, 1, 65535, 8), (1, 1, 8, 65535)):
+        with pytest.raises(mpr.MprError) as e:
+            mpr.mpr_query_workspace_chains(*bad)
+        assert e.value.name == "MPR_ERR_ARG"
+    assert mpr.mpr_query_workspace(1, 46340, 46340) > 35 * 46340 ** 2          # just below 2^31 sites: 75 GB
