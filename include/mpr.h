@@ -53,7 +53,8 @@ typedef enum {
     MPR_ERR_STATE = 6,            /* call out of order (e.g. sweep before set_params) */
     MPR_ERR_WORKSPACE = 7,        /* workspace too small or misaligned (256 B) */
     MPR_ERR_CUDA = 8,             /* a CUDA runtime call failed; see mpr_last_cuda_error */
-    MPR_ERR_UNSUPPORTED = 9       /* valid per the paper but not built (or_mode 1 with q != 1/2) */
+    MPR_ERR_UNSUPPORTED = 9,      /* valid per the paper but not built (or_mode 1 with q != 1/2) */
+    MPR_ERR_COMM = 10             /* a communication callback of a slab context returned non-zero */
 } mpr_status;
 
 /* Alg. 2 step 1 parameters.  POD, host memory. */
@@ -219,6 +220,70 @@ mpr_status mpr_default_ladder(int rows, int cols, double e_s, const float* h_fac
 mpr_status mpr_infer_temperature_auto(mpr_ctx* ctx, const mpr_params* h_params, const float* h_factors, int n_T,
                                       uint32_t n_meas, void* d_workspace, size_t workspace_bytes,
                                       double* h_T_hat, double* h_e_s);
+
+/* ---- q learned from the data ("In principle, q can be learned from the data"; the paper fixes q = 1/2
+ * and gives no procedure: DESIGN.md reading R28) ----
+ * Leave-out validation over n_q candidates h_q (0 < q <= 1/2) on one rows x cols grid: a fraction holdout_fraction
+ * of the samples is withheld (sample site n when the uniform of the HOLDOUT stream -- Philox counter (n >> 2, 0, 3, 0),
+ * word n & 3, key h_params->seed -- is below it); for every candidate the whole path runs on the remaining samples
+ * (Eq. 1 over them; T from their specific energy at this q, Eq. 4, through the equipartition line, i.e. the centre of
+ * mpr_default_ladder; mpr_set_params with h_params and this q, mpr_equilibrate, mpr_simulate, mpr_predict) and is
+ * scored by the root mean square error of the prediction at the withheld samples, h_scores[k].  *h_q_hat = the
+ * candidate with the smallest score (the first of equals); h_T (host double [n_q], may be NULL) receives the
+ * temperatures used.  d_workspace: mpr_query_workspace_learn_q bytes, 256-byte aligned.  Synchronises.
+ * Errors: ARG, WORKSPACE, those of mpr_create on the remaining samples, NO_SAMPLES when nothing was withheld. */
+mpr_status mpr_query_workspace_learn_q(int rows, int cols, size_t* h_bytes);
+mpr_status mpr_learn_q(int rows, int cols, const float* d_values, const uint8_t* d_sample_mask, const mpr_params* h_params,
+                       const float* h_q, int n_q, double holdout_fraction, void* d_workspace, size_t workspace_bytes,
+                       void* cuda_stream, float* h_q_hat, double* h_scores, double* h_T);
+
+/* ---- one grid across several GPUs: row-block decomposition (the
+ * paper's double-precision run at L = 8192 did not fit its card) ----
+ * The rows of ONE rows_global x cols grid are dealt in blocks to several contexts ("slabs"), one per process / GPU.
+ * A slab owns rows [row_begin, row_end) and keeps 8 ghost rows of each neighbouring slab (none at the grid's edge).
+ * The random numbers are keyed by the site's index in the WHOLE grid, the colours by the global row, Eq. 1 uses the
+ * minimum and maximum over every slab's samples, A = accepted / P and e = H / N_GP of Alg. 2 step 5 are sums over the
+ * slabs: the slabs together compute, bit for bit in the state, what one context computes on the whole grid (ghost
+ * sites are updated redundantly, like the halo of a tile, and renewed after every pass of up to 4 sweeps).
+ * The library owns the loops; moving data between slabs is the caller's, through two callbacks (host functions; return
+ * 0 on success, anything else ends the call with MPR_ERR_COMM):
+ *   allreduce(user, h_values, n, op): replace the n host doubles by their sum / minimum / maximum over all slabs
+ *       (op = MPR_REDUCE_*).  Called by mpr_create_slab (3 times), once per sweep by mpr_equilibrate, by mpr_energy.
+ *   exchange(user, cuda_stream): the library has enqueued on cuda_stream copies of its 8 own rows next to the upper
+ *       boundary into d_send_up and next to the lower boundary into d_send_down (mpr_slab_halo_bytes(cols) bytes
+ *       each: 8 rows of [cols rounded up to even] float2); when the work the callback enqueues on cuda_stream (or has
+ *       completed) is done, d_recv_up must hold the upper neighbour's d_send_down and d_recv_down the lower
+ *       neighbour's d_send_up.  Called after every pass (with NCCL: ncclSend / ncclRecv on that stream).
+ * Every slab must make the same calls in the same order (mpr_set_params with the same parameters and T, ...).
+ * Constraints: row_begin even, at least 8 own rows, rows_global * cols < 2^32, one chain, batch 1.
+ * The context's "grid" is the slab's LOCAL rows: own rows plus ghost rows, mpr_slab_local_rows gives their place in the
+ * whole grid; d_values / d_sample_mask of mpr_create_slab and the outputs of mpr_predict*, mpr_get_angles have that
+ * shape [n_rows][cols] (ghost rows of the outputs are to be ignored); mpr_get_stats counts the own rows' sites;
+ * mpr_energy returns the whole grid's energy per bond on every slab.  Unmeasured on more than one GPU. */
+enum { MPR_REDUCE_SUM = 0, MPR_REDUCE_MIN = 1, MPR_REDUCE_MAX = 2 };
+typedef int (*mpr_allreduce_fn)(void* user, double* h_values, int n, int op);
+typedef int (*mpr_exchange_fn)(void* user, void* cuda_stream);
+typedef struct {
+    uint32_t struct_size;          /* = sizeof(mpr_slab) */
+    int rows_global, cols;         /* the whole grid */
+    int row_begin, row_end;        /* this slab's own rows [row_begin, row_end) */
+    mpr_allreduce_fn allreduce;
+    mpr_exchange_fn exchange;
+    void* user;                    /* passed to the callbacks */
+    void* d_send_up;               /* device staging buffers, mpr_slab_halo_bytes(cols) bytes each, caller-owned; */
+    void* d_recv_up;               /*   the *_up pair may be NULL when row_begin = 0, */
+    void* d_send_down;             /*   the *_down pair when row_end = rows_global */
+    void* d_recv_down;
+} mpr_slab;
+size_t mpr_slab_halo_bytes(int cols);
+/* The rows of the whole grid a slab holds: [*h_first_row, *h_first_row + *h_n_rows) = own rows plus ghost rows. */
+mpr_status mpr_slab_local_rows(const mpr_slab* h_slab, int* h_first_row, int* h_n_rows);
+mpr_status mpr_query_workspace_slab(const mpr_slab* h_slab, size_t* h_bytes);
+/* As mpr_create for the slab's local rows (d_values, d_sample_mask: device [n_rows][cols]).  The callbacks and the
+ * staging buffers must stay valid for the life of the context.  Errors: as mpr_create, judged on the whole grid
+ * (NO_SAMPLES, NO_FREE, DEGENERATE_RANGE, NONFINITE come back on every slab alike), and COMM. */
+mpr_status mpr_create_slab(mpr_ctx** out, const mpr_slab* h_slab, const float* d_values, const uint8_t* d_sample_mask,
+                           void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---- double-precision path (Table 2 against Table 3) ----
  * The same method with data, spin state, every site update and the realization sums in double: one grid per

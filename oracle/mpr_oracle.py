@@ -388,6 +388,55 @@ def infer_T_auto(phi, mask, p: Params, n_meas: int, factors=(0.25, 0.5, 1.0, 2.0
     return infer_T(e_s, Ts, table), e_s, Ts, table
 
 
+# ---------------------------------------------------------------------------
+# q learned from the data ("In principle, q can be learned from the data"; reading R28)
+# ---------------------------------------------------------------------------
+def holdout_mask(mask: np.ndarray, fraction: float, seed: int, g: int = 0) -> np.ndarray:
+    """The samples withheld for the validation of q: sample site n = row * cols + col is withheld when its uniform of the
+    HOLDOUT stream -- Philox counter (n >> 2, 0, 3, g), word n & 3, the uniform of reading R13 -- is below `fraction`.
+    Returns a uint8 array: 1 where a sample is withheld."""
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    key = [seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF]
+    flat = m.reshape(-1)
+    out = np.zeros(flat.size, dtype=np.uint8)
+    for block in range((flat.size + 3) // 4):
+        if not flat[4 * block: 4 * block + 4].any():
+            continue
+        x = philox4x32_10([block, 0, 3, g], key)
+        for k in range(4):
+            n = 4 * block + k
+            if n < flat.size and flat[n] and u01(int(x[k])) < fraction:
+                out[n] = 1
+    return out.reshape(m.shape)
+
+
+def learn_q(z, mask, p: Params, qs, fraction: float = 0.2, g: int = 0):
+    """Reading R28: leave-out validation over the candidates `qs`.  A fraction of the samples is withheld (holdout_mask);
+    for every q the method runs on the remaining samples -- Eq. 1 over them, T from their specific energy (Eq. 4 at this
+    q) through the equipartition line (the centre of default_ladder), Alg. 2 steps 5-7 with the parameters `p` -- and is
+    scored by the root mean square error of its prediction at the withheld samples.  The learned q is the candidate with
+    the smallest score (the first of equals).  Returns (q_hat, scores, temperatures)."""
+    import dataclasses
+    zf = np.ascontiguousarray(z, dtype=REAL)
+    held = holdout_mask(mask, fraction, p.seed, g)
+    train = (np.asarray(mask, dtype=np.uint8) & (1 - held)).astype(np.uint8)
+    if held.sum() == 0 or train.sum() == 0:
+        raise ValueError("the withheld or the remaining sample set is empty")
+    scores, Ts = [], []
+    for q in qs:
+        pq = dataclasses.replace(p, q=float(np.float32(q)))
+        phi, _, _ = transform(zf, train, p.seed, g)
+        e_s, n_sp = sample_energy(phi, train, pq.q)
+        if n_sp == 0:
+            raise ValueError("no pair of neighbouring samples")
+        T = default_ladder(zf.shape[0], zf.shape[1], e_s, (1.0,))[0]
+        res = run(zf, train, T, pq, g=g)
+        err = (zf.astype(np.float64) - res["pred"].astype(np.float64))[held == 1]
+        scores.append(float(np.sqrt(np.mean(err ** 2))))
+        Ts.append(T)
+    return float(np.float32(qs[int(np.argmin(scores))])), scores, Ts
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())
 

@@ -115,6 +115,9 @@ Layout make_layout(int batch, int chains, const Geometry& g)
 
 enum RunState { CREATED = 0, READY = 1 };
 
+// ghost rows a slab keeps of each neighbour: the halo of the tile pass, i.e. up to SLAB_GHOST / 2 sweeps between exchanges
+constexpr int SLAB_GHOST = 8;
+
 }  // namespace
 
 struct mpr_ctx {
@@ -144,6 +147,11 @@ struct mpr_ctx {
     int          group;           // grids per group in mpr_simulate (0 = all at once)
     bool         forked;          // chains >= 1 hold a copy of their grid's state (until chain 0 alone moves again)
     uint64_t     n_realizations;  // realizations accumulated per grid (all of its chains) since mpr_set_params
+    // one grid cut into row blocks (mpr_create_slab)
+    bool         slab;
+    mpr_slab     slab_cfg;
+    int          ghost_up, ghost_down;   // ghost rows above / below the own rows (SLAB_GHOST, or 0 at the grid's edge)
+    double       P_total;                // prediction sites of the whole grid
 };
 
 namespace {
@@ -205,6 +213,7 @@ void note_a(mpr_ctx* ctx, double a_min)
 // K sweeps (Alg. 1: colour 0, which contains the upper-left node of Fig. 1, then colour 1) of every tile.
 // flip = 0 / 1: read buffer ctx->cur ^ flip (known to the host); PER_GRID: each grid reads its own GridState::cur
 enum : uint32_t { PER_GRID = 2u };
+mpr_status halo_exchange(mpr_ctx* ctx, uint32_t buf);
 mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags, uint32_t real_no = 0, bool equil = false)
 {
     ctx->dirty = true;
@@ -255,7 +264,54 @@ mpr_status launch_sweeps(mpr_ctx* ctx, uint32_t n, uint32_t* t_off, uint32_t* fl
         mpr_status s = launch_pass(ctx, K, *t_off, *flip, flags | (n == K ? last_flags : 0u), real_no);
         if (s != MPR_OK) return s;
         *t_off += K; *flip ^= 1u; n -= K;
+        if (ctx->slab) { s = halo_exchange(ctx, ctx->cur ^ *flip); if (s != MPR_OK) return s; }
     }
+    return MPR_OK;
+}
+
+// A slab's ghost rows take the neighbouring slabs' rows next to the boundary, as they are in vector buffer `buf`:
+// the rows go through the caller's staging buffers, the caller's callback moves them between the slabs.
+mpr_status halo_exchange(mpr_ctx* ctx, uint32_t buf)
+{
+    const Dev& d = ctx->d;
+    const mpr_slab& sl = ctx->slab_cfg;
+    float2* v = d.vec + (size_t)buf * d.VB;
+    const size_t bytes = (size_t)SLAB_GHOST * d.pitch * sizeof(float2);
+    if (ctx->ghost_up) CU(cudaMemcpyAsync(sl.d_send_up, v + (size_t)d.own_r0 * d.pitch, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (ctx->ghost_down) CU(cudaMemcpyAsync(sl.d_send_down, v + (size_t)(d.own_r1 - SLAB_GHOST) * d.pitch, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (sl.exchange(sl.user, (void*)ctx->stream)) return MPR_ERR_COMM;
+    if (ctx->ghost_up) CU(cudaMemcpyAsync(v, sl.d_recv_up, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (ctx->ghost_down) CU(cudaMemcpyAsync(v + (size_t)d.own_r1 * d.pitch, sl.d_recv_down, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    return MPR_OK;
+}
+
+// Alg. 2 step 5 for one slab of a grid (every slab runs this loop in step): 5.1 one sweep of the own and ghost rows
+// with the energy and the accepted proposals of the OWN rows reduced, the ghost rows renewed from the neighbours, 5.3 /
+// 5.2 with the sums over the slabs (the caller's all-reduce: two numbers per sweep), 5.4-5.5 on every slab alike.
+mpr_status equilibrate_slab(mpr_ctx* ctx)
+{
+    const Dev& d = ctx->d;
+    const mpr_slab& sl = ctx->slab_cfg;
+    for (uint32_t i = 0; i < ctx->prm.equil_cap; ++i) {
+        mpr_status s = launch_pass(ctx, 1, 0, 0, PASS_COUNT | PASS_ENERGY);
+        if (s == MPR_OK) s = halo_exchange(ctx, ctx->cur ^ 1u);
+        if (s != MPR_OK) return s;
+        k_slab_partial<<<1, REDUCE_THREADS, 0, ctx->stream>>>(d, d.ntiles);
+        CU_LAUNCH();
+        s = fetch_states(ctx);
+        if (s != MPR_OK) return s;
+        double sums[2] = {ctx->h_states[0].e_query, (double)ctx->h_states[0].accepted};
+        if (sl.allreduce(sl.user, sums, 2, MPR_REDUCE_SUM)) return MPR_ERR_COMM;
+        k_controller_slab<<<1, 1, 0, ctx->stream>>>(d, sums[0], (unsigned long long)sums[1], ctx->P_total);
+        CU_LAUNCH();
+        ctx->cur ^= 1u;                  // the controller committed the sweep: t + 1, the buffers swapped roles
+        CU(cudaMemcpyAsync(ctx->h_done, d.done_flags, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        if (ctx->h_done[0]) break;
+    }
+    mpr_status s = fetch_states(ctx);
+    if (s != MPR_OK) return s;
+    note_a(ctx, ctx->h_states[0].a);
     return MPR_OK;
 }
 
@@ -315,6 +371,7 @@ const char* mpr_status_string(mpr_status s)
     case MPR_ERR_WORKSPACE: return "workspace too small or misaligned";
     case MPR_ERR_CUDA: return "CUDA error";
     case MPR_ERR_UNSUPPORTED: return "parameter combination not supported";
+    case MPR_ERR_COMM: return "a communication callback of a slab context failed";
     }
     return "unknown status";
 }
@@ -349,8 +406,10 @@ mpr_status mpr_query_workspace(int batch, int rows, int cols, size_t* bytes)
 namespace {
 
 // mpr_create (data given) and mpr_create_unconditional (d_values = d_sample_mask = nullptr)
+// and mpr_create_slab (slab != nullptr: rows = the slab's own rows plus its ghost rows)
 mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols, const float* d_values,
-                       const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+                       const uint8_t* d_sample_mask, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                       const mpr_slab* slab = nullptr)
 {
     const bool unconditional = !d_values && !d_sample_mask;
     Geometry g;
@@ -398,6 +457,17 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     d.batch = batch; d.rows = rows; d.cols = cols;
     d.N = g.N; d.words = g.words; d.pitch = g.pitch;
     d.n_bonds = (double)rows * (cols - 1) + (double)cols * (rows - 1);
+    d.site_off = 0; d.own_r0 = 0; d.own_r1 = rows;
+    if (slab) {
+        // rows [row_begin - ghost_up, row_end + ghost_down) of the whole grid; the bonds, the prediction sites and the
+        // random streams are those of the whole grid
+        ctx->slab = true; ctx->slab_cfg = *slab;
+        ctx->ghost_up = slab->row_begin > 0 ? SLAB_GHOST : 0;
+        ctx->ghost_down = slab->row_end < slab->rows_global ? SLAB_GHOST : 0;
+        d.own_r0 = ctx->ghost_up; d.own_r1 = ctx->ghost_up + (slab->row_end - slab->row_begin);
+        d.site_off = (uint32_t)(slab->row_begin - ctx->ghost_up) * (uint32_t)cols;
+        d.n_bonds = (double)slab->rows_global * (cols - 1) + (double)cols * (slab->rows_global - 1);
+    }
     d.burn_in_only = unconditional ? 1 : 0;
     ctx->energy_blocks = rows < ENERGY_BLOCKS ? rows : ENERGY_BLOCKS;
     ctx->active = batch;
@@ -417,7 +487,24 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     unsigned mm_blocks = cdiv(g.N, 256 * 8);
     if (mm_blocks > 1184) mm_blocks = 1184;
     if (unconditional) k_state_unconditional<<<cdiv(batch, 128), 128, 0, s>>>(d);
-    else {
+    else if (slab) {
+        // Eq. 1's range is over the samples of the WHOLE grid (L81): this slab's own rows, then min / max over the slabs
+        k_minmax<<<dim3(mm_blocks, 1), 256, 0, s>>>(d, d_values, d_sample_mask);
+        ++ctx->launches;
+        st = fetch_states(ctx);
+        if (st != MPR_OK) return fail(st);
+        const GridState& h = ctx->h_states[0];
+        auto decode = [](uint32_t e) { const uint32_t b = (e & 0x80000000u) ? (e & 0x7FFFFFFFu) : ~e; float f; memcpy(&f, &b, sizeof f); return f; };
+        const float lo_f = h.n_samples ? decode(h.zmin_enc) : INFINITY;      // the order-preserving encoding of k_minmax
+        const float hi_f = h.n_samples ? decode(h.zmax_enc) : -INFINITY;
+        double lo = (double)lo_f, hi = (double)hi_f, cnt[2] = {(double)h.n_samples, (h.err_flags & ERRF_NONFINITE) ? 1.0 : 0.0};
+        if (slab->allreduce(slab->user, &lo, 1, MPR_REDUCE_MIN) || slab->allreduce(slab->user, &hi, 1, MPR_REDUCE_MAX) ||
+            slab->allreduce(slab->user, cnt, 2, MPR_REDUCE_SUM)) return fail(MPR_ERR_COMM);
+        if (cnt[0] == 0.0) return fail(MPR_ERR_NO_SAMPLES);
+        if (cnt[1] != 0.0) return fail(MPR_ERR_NONFINITE);
+        if (!(hi > lo)) return fail(MPR_ERR_DEGENERATE_RANGE);
+        k_set_range<<<1, 1, 0, s>>>(d, (float)lo, (float)hi);
+    } else {
         k_minmax<<<dim3(mm_blocks, batch), 256, 0, s>>>(d, d_values, d_sample_mask);
         k_minmax_finish<<<cdiv(batch, 128), 128, 0, s>>>(d);
     }
@@ -441,7 +528,14 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
     st = fetch_states(ctx);
     if (st != MPR_OK) return fail(st);
-    for (int b = 0; b < batch; ++b) {
+    if (slab) {
+        // P of Alg. 2 step 5.2 (A = accepted / P) is the whole grid's number of prediction sites
+        double P = (double)ctx->h_states[0].n_free[0] + (double)ctx->h_states[0].n_free[1];
+        if (slab->allreduce(slab->user, &P, 1, MPR_REDUCE_SUM)) return fail(MPR_ERR_COMM);
+        if (P == 0.0) return fail(MPR_ERR_NO_FREE);
+        ctx->P_total = P;
+    }
+    for (int b = 0; b < batch && !slab; ++b) {
         const uint32_t e = ctx->h_states[b].err_flags;
         if (e & ERRF_NO_SAMPLES) return fail(MPR_ERR_NO_SAMPLES);
         if (e & ERRF_NONFINITE) return fail(MPR_ERR_NONFINITE);
@@ -463,6 +557,7 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
     ctx->smem_bytes = frame_bytes + (d.use_spare ? 10ull : 2ull) * max_entries;
     if (ctx->smem_bytes > budget) return fail(MPR_ERR_WORKSPACE);
     ctx->k_max = g.ntiles == 1 ? 1024u : (uint32_t)(g.H / 2);        // mpr_set_pass_depth lowers it (diagnostic)
+    if (slab && ctx->k_max > (uint32_t)(SLAB_GHOST / 2)) ctx->k_max = SLAB_GHOST / 2;      // the ghost rows last SLAB_GHOST / 2 sweeps
     // The attribute belongs to the kernel, not to this context: it is only ever raised (per device and frame-pitch
     // variant), so that a context created later with smaller tiles does not take the room of an earlier one away.
     {
@@ -514,6 +609,44 @@ mpr_status mpr_create_unconditional(mpr_ctx** out, int batch, int rows, int cols
                                     void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
     return create_impl(out, batch, 1, rows, cols, nullptr, nullptr, d_workspace, workspace_bytes, cuda_stream);
+}
+
+size_t mpr_slab_halo_bytes(int cols)
+{
+    return cols < 2 ? 0 : (size_t)SLAB_GHOST * (size_t)((cols + 1) & ~1) * sizeof(float2);
+}
+
+static bool slab_ok(const mpr_slab* sl)
+{
+    return sl && sl->struct_size == sizeof(mpr_slab) && sl->allreduce && sl->exchange && sl->cols >= 2 && sl->rows_global >= 2 &&
+           sl->row_begin >= 0 && sl->row_end <= sl->rows_global && (sl->row_begin & 1) == 0 &&
+           sl->row_end - sl->row_begin >= SLAB_GHOST && (uint64_t)sl->rows_global * (uint64_t)sl->cols < (1ull << 32) &&
+           (sl->row_begin == 0 || (sl->d_send_up && sl->d_recv_up)) && (sl->row_end == sl->rows_global || (sl->d_send_down && sl->d_recv_down));
+}
+
+mpr_status mpr_slab_local_rows(const mpr_slab* sl, int* h_first_row, int* h_n_rows)
+{
+    if (!sl || !h_first_row || !h_n_rows || sl->struct_size != sizeof(mpr_slab) || sl->row_begin < 0 || sl->row_end > sl->rows_global ||
+        sl->row_end <= sl->row_begin) return MPR_ERR_ARG;
+    const int up = sl->row_begin > 0 ? SLAB_GHOST : 0, down = sl->row_end < sl->rows_global ? SLAB_GHOST : 0;
+    if (sl->row_begin - up < 0 || sl->row_end + down > sl->rows_global) return MPR_ERR_ARG;
+    *h_first_row = sl->row_begin - up; *h_n_rows = sl->row_end - sl->row_begin + up + down;
+    return MPR_OK;
+}
+
+mpr_status mpr_query_workspace_slab(const mpr_slab* sl, size_t* bytes)
+{
+    int first, n;
+    if (!bytes || mpr_slab_local_rows(sl, &first, &n) != MPR_OK) return MPR_ERR_ARG;
+    return mpr_query_workspace(1, n, sl->cols, bytes);
+}
+
+mpr_status mpr_create_slab(mpr_ctx** out, const mpr_slab* sl, const float* d_values, const uint8_t* d_sample_mask,
+                           void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    int first, n;
+    if (!d_values || !d_sample_mask || mpr_slab_local_rows(sl, &first, &n) != MPR_OK || !slab_ok(sl)) return MPR_ERR_ARG;
+    return create_impl(out, 1, 1, n, sl->cols, d_values, d_sample_mask, d_workspace, workspace_bytes, cuda_stream, sl);
 }
 
 mpr_status mpr_destroy(mpr_ctx* ctx)
@@ -572,6 +705,7 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
     if (ctx->state != READY) return MPR_ERR_STATE;
     const Dev& d = ctx->d;
     ctx->forked = false;           // chain 0 of every grid moves alone (Alg. 2 step 5 is one chain per grid)
+    if (ctx->slab) return equilibrate_slab(ctx);
     const uint32_t cap = ctx->prm.equil_cap;
     uint32_t issued = 0;
     auto all_done = [&](bool* all) -> mpr_status {
@@ -852,6 +986,92 @@ mpr_status mpr_infer_temperature_auto(mpr_ctx* ctx, const mpr_params* h_params, 
     return MPR_OK;
 }
 
+namespace {
+struct LearnLayout { size_t ctx, train, held, pred, partials, count, total; };
+bool learn_layout(int rows, int cols, LearnLayout* L)
+{
+    size_t ws = 0;
+    if (mpr_query_workspace(1, rows, cols, &ws) != MPR_OK) return false;
+    const size_t N = (size_t)rows * cols;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    L->ctx = take(ws); L->train = take(N); L->held = take(N); L->pred = take(N * sizeof(float));
+    L->partials = take(ENERGY_BLOCKS * sizeof(double)); L->count = take(sizeof(unsigned long long));
+    L->total = o;
+    return true;
+}
+}  // namespace
+
+mpr_status mpr_query_workspace_learn_q(int rows, int cols, size_t* bytes)
+{
+    LearnLayout L;
+    if (!bytes || !learn_layout(rows, cols, &L)) return MPR_ERR_ARG;
+    *bytes = L.total;
+    return MPR_OK;
+}
+
+mpr_status mpr_learn_q(int rows, int cols, const float* d_values, const uint8_t* d_sample_mask, const mpr_params* h_params,
+                       const float* h_q, int n_q, double holdout_fraction, void* d_workspace, size_t workspace_bytes,
+                       void* cuda_stream, float* h_q_hat, double* h_scores, double* h_T)
+{
+    LearnLayout L;
+    if (!d_values || !d_sample_mask || !h_params || !h_q || n_q < 1 || !h_q_hat || !h_scores ||
+        !(holdout_fraction > 0.0 && holdout_fraction < 1.0) || h_params->struct_size != sizeof(mpr_params) ||
+        !learn_layout(rows, cols, &L)) return MPR_ERR_ARG;
+    for (int k = 0; k < n_q; ++k)
+        if (!(h_q[k] > 0.0f && h_q[k] <= 0.5f)) return MPR_ERR_ARG;
+    if (!d_workspace || workspace_bytes < L.total || ((uintptr_t)d_workspace & 255u)) return MPR_ERR_WORKSPACE;
+    char* base = (char*)d_workspace;
+    uint8_t* train = (uint8_t*)(base + L.train); uint8_t* held = (uint8_t*)(base + L.held);
+    float* pred = (float*)(base + L.pred);
+    double* partials = (double*)(base + L.partials);
+    unsigned long long* count = (unsigned long long*)(base + L.count);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const uint32_t N = (uint32_t)((size_t)rows * cols);
+    PhiloxKeys keys;
+    for (int r = 0; r < PHILOX_ROUNDS; ++r) {
+        keys.rk0[r] = (uint32_t)h_params->seed + (uint32_t)r * 0x9E3779B9u;
+        keys.rk1[r] = (uint32_t)(h_params->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
+    k_holdout<<<cdiv(N, 256), 256, 0, st>>>(keys, d_sample_mask, train, held, N, 0u, (float)holdout_fraction);
+    if (!cuda_ok(cudaGetLastError(), "k_holdout")) return MPR_ERR_CUDA;
+    mpr_ctx* ctx = nullptr;
+    mpr_status s = mpr_create(&ctx, 1, rows, cols, d_values, train, base + L.ctx, L.ctx == 0 ? L.train : L.train - L.ctx, cuda_stream);
+    if (s != MPR_OK) return s;
+    int best = -1;
+    for (int k = 0; k < n_q && s == MPR_OK; ++k) {
+        // T of this candidate: the remaining samples' specific energy at this q (Eq. 4) through the equipartition line
+        double e_s = 0.0; uint64_t pairs = 0;
+        const float one = 1.0f; float T = 0.0f;
+        ctx->d.q = h_q[k];
+        s = mpr_sample_energy(ctx, &e_s, &pairs);
+        if (s == MPR_OK && pairs == 0) s = MPR_ERR_NO_SAMPLES;
+        if (s == MPR_OK) s = mpr_default_ladder(rows, cols, e_s, &one, 1, &T);
+        mpr_params prm = *h_params;
+        prm.q = h_q[k];
+        if (s == MPR_OK) s = mpr_set_params(ctx, &prm, &T);
+        if (s == MPR_OK) s = mpr_equilibrate(ctx);
+        if (s == MPR_OK) s = mpr_simulate(ctx);
+        if (s == MPR_OK) s = mpr_predict(ctx, pred);
+        if (s != MPR_OK) break;
+        if (!cuda_ok(cudaMemsetAsync(count, 0, sizeof *count, st), "memset")) { s = MPR_ERR_CUDA; break; }
+        k_cv_error<<<ENERGY_BLOCKS, ENERGY_THREADS, 0, st>>>(d_values, pred, held, N, partials, count);
+        k_cv_finish<<<1, 32, 0, st>>>(partials, ENERGY_BLOCKS);
+        double sum = 0.0; unsigned long long n_held = 0;
+        if (!cuda_ok(cudaMemcpyAsync(&sum, partials, sizeof sum, cudaMemcpyDeviceToHost, st), "copy") ||
+            !cuda_ok(cudaMemcpyAsync(&n_held, count, sizeof n_held, cudaMemcpyDeviceToHost, st), "copy") ||
+            !cuda_ok(cudaStreamSynchronize(st), "sync")) { s = MPR_ERR_CUDA; break; }
+        if (n_held == 0) { s = MPR_ERR_NO_SAMPLES; break; }          // nothing was withheld: no score
+        h_scores[k] = std::sqrt(sum / (double)n_held);
+        if (h_T) h_T[k] = (double)T;
+        if (best < 0 || h_scores[k] < h_scores[best]) best = k;
+    }
+    mpr_destroy(ctx);
+    if (s != MPR_OK) return s;
+    *h_q_hat = h_q[best];
+    return MPR_OK;
+}
+
 mpr_status mpr_get_angles(mpr_ctx* ctx, float* d_phi)
 {
     if (!ctx || !d_phi) return MPR_ERR_ARG;
@@ -876,6 +1096,7 @@ mpr_status mpr_set_angles(mpr_ctx* ctx, const float* d_phi)
     CU_LAUNCH();
     ctx->dirty = false;
     ctx->forked = false;
+    if (ctx->slab) return halo_exchange(ctx, ctx->cur);       // the ghost rows are the neighbours' own rows, whatever d_phi held there
     return MPR_OK;
 }
 
@@ -921,6 +1142,16 @@ mpr_status mpr_energy(mpr_ctx* ctx, double* h_e)
     if (ctx->state != READY) return MPR_ERR_STATE;
     mpr_status s = launch_energy(ctx);
     if (s != MPR_OK) return s;
+    if (ctx->slab) {        // this slab's share (own rows), summed over the slabs, over the bonds of the whole grid
+        k_slab_partial<<<1, REDUCE_THREADS, 0, ctx->stream>>>(ctx->d, ctx->energy_blocks);
+        CU_LAUNCH();
+        s = fetch_states(ctx);
+        if (s != MPR_OK) return s;
+        double H = ctx->h_states[0].e_query;
+        if (ctx->slab_cfg.allreduce(ctx->slab_cfg.user, &H, 1, MPR_REDUCE_SUM)) return MPR_ERR_COMM;
+        h_e[0] = H / ctx->d.n_bonds;
+        return MPR_OK;
+    }
     k_energy_query<<<ctx->d.batch, REDUCE_THREADS, 0, ctx->stream>>>(ctx->d, ctx->energy_blocks);
     CU_LAUNCH();
     s = fetch_states(ctx);
@@ -976,7 +1207,8 @@ mpr_status mpr_get_launch_count(mpr_ctx* ctx, uint64_t* h_count)
 mpr_status mpr_set_pass_depth(mpr_ctx* ctx, uint32_t k)
 {
     if (!ctx) return MPR_ERR_ARG;
-    const uint32_t most = ctx->d.ntiles == 1 ? 1024u : (uint32_t)(ctx->d.H / 2);
+    uint32_t most = ctx->d.ntiles == 1 ? 1024u : (uint32_t)(ctx->d.H / 2);
+    if (ctx->slab && most > (uint32_t)(SLAB_GHOST / 2)) most = SLAB_GHOST / 2;
     if (k > most) return MPR_ERR_ARG;
     ctx->k_max = k ? k : most;
     return MPR_OK;

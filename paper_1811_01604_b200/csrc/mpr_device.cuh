@@ -89,6 +89,11 @@ struct Dev {
                                // lists start at i * tile_entries, so that loading them needs nothing read first
     uint32_t   n_partials;
     uint32_t   acc_stride;     // floats of one tile's accumulators: TR * TC rounded up to 16, + 16
+    // row-block decomposition of one grid over several contexts (mpr_create_slab): this context's grid is rows
+    // [slab_row0, slab_row0 + rows) of a larger one; its rows [own_r0, own_r1) are its own, the others are ghost copies
+    // of the neighbouring slabs' rows.  A plain context: site_off = 0, own_r0 = 0, own_r1 = rows.
+    uint32_t   site_off;       // slab_row0 * cols: added to row * cols + col, the site word of the Philox counter
+    int        own_r0, own_r1; // rows counted in the energy, the accepted proposals and the number of prediction sites
     // tiling
     int        TR, TC, H, FR, FC, ntx, nty, ntiles;
     uint32_t   max_entries;    // shared-memory capacity for entries (multiple of 8)
@@ -256,7 +261,8 @@ __global__ void __launch_bounds__(256) k_minmax(Dev d, const float* __restrict__
     const uint8_t* m = mask + (size_t)g * d.N;
     float lo = INFINITY, hi = -INFINITY;
     uint32_t cnt = 0, bad = 0;
-    for (uint32_t n = blockIdx.x * blockDim.x + threadIdx.x; n < d.N; n += gridDim.x * blockDim.x) {
+    const uint32_t n_end = (uint32_t)d.own_r1 * (uint32_t)d.cols;       // a slab's ghost rows belong to its neighbours
+    for (uint32_t n = (uint32_t)d.own_r0 * (uint32_t)d.cols + blockIdx.x * blockDim.x + threadIdx.x; n < n_end; n += gridDim.x * blockDim.x) {
         if (m[n]) {
             const float x = z[n];
             bad |= !isfinite(x);
@@ -315,7 +321,7 @@ __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restric
     const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;   // < 32 * words (grid sized so)
     const GridState& s = d.states[g];
     const bool in = n < d.N;
-    bool fixed = false;
+    bool fixed = false, own = false;
     uint32_t colour = 0;
     if (in) {
         const size_t o = (size_t)g * d.N + n;
@@ -325,10 +331,11 @@ __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restric
         d.phi[o] = fixed ? eq1(z, s.zmin, s.zmax) : 0.0f;
         const uint32_t r = n / d.cols;
         colour = (r + (n - r * d.cols)) & 1u;
+        own = (int)r >= d.own_r0 && (int)r < d.own_r1;
     }
     const uint32_t b = __ballot_sync(0xFFFFFFFFu, fixed);
-    const uint32_t f0 = __ballot_sync(0xFFFFFFFFu, in && !fixed && colour == 0);
-    const uint32_t f1 = __ballot_sync(0xFFFFFFFFu, in && !fixed && colour == 1);
+    const uint32_t f0 = __ballot_sync(0xFFFFFFFFu, in && own && !fixed && colour == 0);
+    const uint32_t f1 = __ballot_sync(0xFFFFFFFFu, in && own && !fixed && colour == 1);
     // counts: per block in shared memory, then one global atomic per block and colour
     __shared__ uint32_t s_free[2];
     if (threadIdx.x < 2) s_free[threadIdx.x] = 0;
@@ -491,8 +498,9 @@ __global__ void __launch_bounds__(256) k_init_state(Dev d, int ordered)
     else {
         if (ordered) p = 3.14159274101257324f;          // unconditional chains start from phi = pi (reading R23)
         else {
-            const uint4 x = philox4x32_10(n >> 2, 0u, 0u, (uint32_t)g, d.rk0, d.rk1);
-            const uint32_t w = (n & 3u) == 0 ? x.x : (n & 3u) == 1 ? x.y : (n & 3u) == 2 ? x.z : x.w;
+            const uint32_t ng = n + d.site_off;             // the site's index in the whole grid (a slab's rows start at slab_row0)
+            const uint4 x = philox4x32_10(ng >> 2, 0u, 0u, (uint32_t)g, d.rk0, d.rk1);
+            const uint32_t w = (ng & 3u) == 0 ? x.x : (ng & 3u) == 1 ? x.y : (ng & 3u) == 2 ? x.z : x.w;
             p = __fmul_rn(TWO_PI_F, u01(w));
         }
         d.phi[o] = p;
@@ -675,10 +683,10 @@ __device__ __forceinline__ void update_pair(float2& vA, float2 upA, float2 dnA, 
 // K = 1 tile pass) and, for a grid that is a single tile, from inside the tile pass.
 // ---------------------------------------------------------------------------
 // s: the grid's state, in global memory or a copy of it (the tile pass keeps one in shared memory while it loops)
-__device__ __forceinline__ void controller_step(const Dev& d, GridState& s, double H)
+__device__ __forceinline__ void controller_step(const Dev& d, GridState& s, double H, double P_total = 0.0)
 {
     const uint32_t i = s.i;
-    const double P = (double)s.n_free[0] + (double)s.n_free[1];
+    const double P = P_total > 0.0 ? P_total : (double)s.n_free[0] + (double)s.n_free[1];
     // 5.2 acceptance control: a(i+1) = 1 + (i+1)/k_a while A < A_targ
     const double A = (double)s.accepted / P;
     double a = s.a;
@@ -785,11 +793,12 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // ---------------------------------------------------------------------------
 // a5 inside a tile pass: this warp's share of sum over the core's colour-1 sites (fixed ones too) of v . h, rows dealt
 // over the warps, float per row, double over the rows, then the warp's shuffle tree: a fixed order
-__device__ __forceinline__ double core_energy_warp(const float2* S, const TileGeom& tg, int H, int FC, int warp, int lane, int NW)
+__device__ __forceinline__ double core_energy_warp(const Dev& d, const float2* S, const TileGeom& tg, int H, int FC, int warp, int lane, int NW)
 {
     double sum = 0.0;
     for (int lr = H + warp; lr < H + tg.TRc; lr += NW) {
         const int r = tg.r0 - H + lr;
+        if (r < d.own_r0 || r >= d.own_r1) continue;         // a slab's ghost rows are counted by the slab that owns them
         float row = 0.0f;
         // first colour-1 column of this row at or after the core's first column
         for (int lc = H + ((r + tg.c0 + 1) & 1) + 2 * lane; lc < H + tg.TCc; lc += 64) {
@@ -912,8 +921,11 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             reinterpret_cast<uint32_t*>(s_state)[w] = reinterpret_cast<const uint32_t*>(&d.states[g])[w];
     }
     const uint32_t t0 = st.t + t_off;
-    const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H), ncorr = d.cols - FC;
+    const int nbase = (tg.r0 - H) * d.cols + (tg.c0 - H) + (int)d.site_off, ncorr = d.cols - FC;
     const bool count = FUSED && (flags & PASS_COUNT);
+    // frame offsets [own_lo, own_lo + own_span) are the rows this context owns (all of them unless it is a slab)
+    const uint32_t own_lo = (uint32_t)max(d.own_r0 - (tg.r0 - H), 0) * (uint32_t)FC;
+    const uint32_t own_span = (uint32_t)max(min(d.own_r1 - (tg.r0 - H), d.FR) * FC - (int)own_lo, 0);
     const bool use_spare = d.use_spare;
     uint32_t n_accepted = 0;
     __syncthreads();
@@ -982,7 +994,9 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
                                        hs, hc1, nlT, d.bc, d.bs, renorm, accA, accB);
             S[offA] = vA;
             if (eB != eA) S[offB] = vB;
-            if constexpr (FUSED) { if (count) n_accepted += (accA && eA < n_core) + (accB && eB != eA && eB < n_core); }
+            if constexpr (FUSED) {
+                if (count) n_accepted += (accA && eA < n_core && offA - own_lo < own_span) + (accB && eB != eA && eB < n_core && offB - own_lo < own_span);
+            }
         };
         // full rounds: thread tid takes the entries pos + tid and pos + NT + tid; the last round splits what
         // is left into two halves of whole warps, so that no warp runs a round for a missing second site
@@ -1005,7 +1019,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
                 n_accepted = __reduce_add_sync(0xFFFFFFFFu, n_accepted);
                 if (lane == 0 && n_accepted) atomicAdd(&s_accepted, n_accepted);
                 n_accepted = 0;
-                const double e_warp = core_energy_warp(S, tg, H, FC, warp, lane, NW);
+                const double e_warp = core_energy_warp(d, S, tg, H, FC, warp, lane, NW);
                 if (lane == 0) s_red[warp] = e_warp;
                 __syncthreads();
                 if (tid == 0) {
@@ -1074,7 +1088,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         }
         if (flags & PASS_ENERGY) {
             // a5: H_tile = - sum over the core's colour-1 sites (fixed ones too) of v . h; fixed summation order
-            const double sum = core_energy_warp(S, tg, H, FC, warp, lane, NW);
+            const double sum = core_energy_warp(d, S, tg, H, FC, warp, lane, NW);
             if (lane == 0) s_red[warp] = sum;
         }
         __syncthreads();
@@ -1109,7 +1123,7 @@ __global__ void __launch_bounds__(ENERGY_THREADS) k_energy(Dev d)
     const float2* v = vec_grid(d, g, d.states[g].cur);
     const float2 zero = make_float2(0.0f, 0.0f);
     double sum = 0.0;
-    for (int r = blockIdx.x; r < d.rows; r += gridDim.x) {
+    for (int r = d.own_r0 + blockIdx.x; r < d.own_r1; r += gridDim.x) {
         const float2* row = v + (size_t)r * d.pitch;
         float part = 0.0f;
         int cnt = 0;
@@ -1242,6 +1256,28 @@ __global__ void k_controller(Dev d)
     if (s.done) d.done_flags[g] = 1u;
 }
 
+// One grid cut into row blocks over several contexts (mpr_create_slab).  k_slab_partial: this slab's share of the
+// sweep's energy (its own rows' colour-1 sites) into e_query; the host adds the slabs' shares and accepted counts and
+// k_controller_slab takes steps 5.2-5.5 with the totals -- every slab the same step, since the totals are the same.
+__global__ void k_slab_partial(Dev d, int n_partials)
+{
+    const double H = sum_energy_partials(d, 0, n_partials);
+    if (threadIdx.x == 0) d.states[0].e_query = H;
+}
+__global__ void k_controller_slab(Dev d, double H_total, unsigned long long accepted_total, double P_total)
+{
+    GridState& s = d.states[0];
+    if (s.done) return;
+    s.accepted = accepted_total;
+    controller_step(d, s, H_total, P_total);
+    if (s.done) d.done_flags[0] = 1u;
+}
+// Eq. 1 range given from outside (the minimum and maximum over every slab's samples)
+__global__ void k_set_range(Dev d, float zmin, float zmax)
+{
+    d.states[0].zmin = zmin; d.states[0].zmax = zmax;
+}
+
 // scalar state edits ---------------------------------------------------------
 // mode 0: a <- a_value for every grid; mode 1: keep a (refresh the derived scale only)
 __global__ void k_set_a(Dev d, int mode, double a_value, int zero_accepted)
@@ -1365,6 +1401,59 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, double x_p, float* __res
         }
         out[(size_t)g * d.N + n] = (float)z;
     }
+}
+
+// ---------------------------------------------------------------------------
+// q learned from the data (reading R28): leave-out validation.
+// k_holdout: sample site n is withheld when its uniform of the HOLDOUT stream (Philox counter (n >> 2, 0, 3, g),
+// word n & 3) is below `fraction`; train = mask without the withheld samples.
+// k_cv_error: sum over the withheld samples of (z - z_hat)^2 in double, fixed block count and summation order.
+// ---------------------------------------------------------------------------
+struct PhiloxKeys { uint32_t rk0[PHILOX_ROUNDS], rk1[PHILOX_ROUNDS]; };
+
+__global__ void __launch_bounds__(256) k_holdout(PhiloxKeys keys, const uint8_t* __restrict__ mask, uint8_t* __restrict__ train,
+                                                 uint8_t* __restrict__ held, uint32_t N, uint32_t g, float fraction)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    uint8_t h = 0;
+    if (mask[n]) {
+        const uint4 x = philox4x32_10(n >> 2, 0u, 3u, g, keys.rk0, keys.rk1);
+        const uint32_t w = (n & 3u) == 0 ? x.x : (n & 3u) == 1 ? x.y : (n & 3u) == 2 ? x.z : x.w;
+        h = u01(w) < fraction ? 1 : 0;
+    }
+    held[n] = h;
+    train[n] = mask[n] && !h ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(ENERGY_THREADS) k_cv_error(const float* __restrict__ values, const float* __restrict__ pred,
+                                                              const uint8_t* __restrict__ held, uint32_t N,
+                                                              double* __restrict__ partials, unsigned long long* __restrict__ count)
+{
+    __shared__ double warp_sum[ENERGY_THREADS / 32];
+    double sum = 0.0;
+    unsigned long long cnt = 0ull;
+    // block b takes the sites b * chunk .. (b + 1) * chunk - 1 in order: the same sum whatever the device
+    const uint32_t chunk = (N + gridDim.x - 1) / gridDim.x, lo = blockIdx.x * chunk, hi = min(N, lo + chunk);
+    for (uint32_t n = lo + threadIdx.x; n < hi; n += ENERGY_THREADS)
+        if (held[n]) { const double e = (double)values[n] - (double)pred[n]; sum += e * e; ++cnt; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o); cnt += __shfl_xor_sync(0xFFFFFFFFu, cnt, o); }
+    if ((threadIdx.x & 31) == 0) { warp_sum[threadIdx.x >> 5] = sum; if (cnt) atomicAdd(count, cnt); }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < ENERGY_THREADS / 32; ++w) s += warp_sum[w];
+        partials[blockIdx.x] = s;
+    }
+}
+__global__ void k_cv_finish(double* partials, int n)       // one warp: partials[0] <- the sum in a fixed order
+{
+    double s = 0.0;
+    for (int b = threadIdx.x; b < n; b += 32) s += partials[b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+    if (threadIdx.x == 0) partials[0] = s;
 }
 
 // angle import / export at the prediction sites ------------------------------

@@ -22,7 +22,7 @@ LIB_PATH = os.path.join(_HERE, "libmpr_b200.so")
 STATUS_NAMES = {
     0: "MPR_OK", 1: "MPR_ERR_ARG", 2: "MPR_ERR_NO_SAMPLES", 3: "MPR_ERR_NO_FREE",
     4: "MPR_ERR_DEGENERATE_RANGE", 5: "MPR_ERR_NONFINITE", 6: "MPR_ERR_STATE",
-    7: "MPR_ERR_WORKSPACE", 8: "MPR_ERR_CUDA", 9: "MPR_ERR_UNSUPPORTED",
+    7: "MPR_ERR_WORKSPACE", 8: "MPR_ERR_CUDA", 9: "MPR_ERR_UNSUPPORTED", 10: "MPR_ERR_COMM",
 }
 
 # every symbol include/mpr.h declares
@@ -35,6 +35,8 @@ EXPORTS = (
     "mpr_infer_temperature", "mpr_predict_std", "mpr_query_workspace_chains", "mpr_create_chains",
     "mpr_predict_quantile", "mpr_set_pass_depth", "mpr_get_tiling",
     "mpr_default_ladder", "mpr_infer_temperature_auto", "mpr_set_grid_group",
+    "mpr_slab_halo_bytes", "mpr_slab_local_rows", "mpr_query_workspace_slab", "mpr_create_slab",
+    "mpr_query_workspace_learn_q", "mpr_learn_q",
     "mpr64_query_workspace", "mpr64_create", "mpr64_set_params", "mpr64_equilibrate", "mpr64_simulate", "mpr64_predict",
     "mpr64_predict_std", "mpr64_destroy", "mpr64_get_angles", "mpr64_set_angles", "mpr64_set_sweep_index", "mpr64_sweep",
     "mpr64_energy", "mpr64_get_transform", "mpr64_get_stats", "mpr64_get_launch_count",
@@ -54,6 +56,18 @@ class mpr_params(C.Structure):
         ("sweeps_per_real", C.c_uint32), ("M", C.c_uint32), ("n_f", C.c_uint32), ("n_fit", C.c_uint32),
         ("A_targ", C.c_float), ("k_a", C.c_float), ("or_mode", C.c_uint32), ("a_eq_mode", C.c_uint32),
         ("seed", C.c_uint64),
+    ]
+
+
+ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.POINTER(C.c_double), C.c_int, C.c_int)
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p)
+
+
+class mpr_slab(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("rows_global", C.c_int), ("cols", C.c_int), ("row_begin", C.c_int),
+        ("row_end", C.c_int), ("allreduce", ALLREDUCE_FN), ("exchange", EXCHANGE_FN), ("user", C.c_void_p),
+        ("d_send_up", C.c_void_p), ("d_recv_up", C.c_void_p), ("d_send_down", C.c_void_p), ("d_recv_down", C.c_void_p),
     ]
 
 
@@ -113,6 +127,13 @@ def lib():
         L.mpr_default_ladder.argtypes = [i, i, C.c_double, C.POINTER(C.c_float), i, C.POINTER(C.c_float)]
         L.mpr_infer_temperature_auto.argtypes = [vp, C.POINTER(mpr_params), C.POINTER(C.c_float), i, u32, vp, sz,
                                                  C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.mpr_slab_halo_bytes.argtypes = [i]
+        L.mpr_slab_local_rows.argtypes = [C.POINTER(mpr_slab), C.POINTER(i), C.POINTER(i)]
+        L.mpr_query_workspace_slab.argtypes = [C.POINTER(mpr_slab), C.POINTER(sz)]
+        L.mpr_create_slab.argtypes = [C.POINTER(vp), C.POINTER(mpr_slab), vp, vp, vp, sz, vp]
+        L.mpr_query_workspace_learn_q.argtypes = [i, i, C.POINTER(sz)]
+        L.mpr_learn_q.argtypes = [i, i, vp, vp, C.POINTER(mpr_params), C.POINTER(C.c_float), i, C.c_double, vp, sz, vp,
+                                  C.POINTER(C.c_float), C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.mpr64_query_workspace.argtypes = [i, i, C.POINTER(sz)]
         L.mpr64_create.argtypes = [C.POINTER(vp), i, i, vp, vp, vp, sz, vp]
         L.mpr64_set_params.argtypes = [vp, C.POINTER(mpr_params), C.c_double]
@@ -129,6 +150,7 @@ def lib():
         for name in EXPORTS:
             getattr(L, name).restype = C.c_int
         L.mpr_default_params.restype = None
+        L.mpr_slab_halo_bytes.restype = C.c_size_t
         L.mpr_status_string.argtypes = [i]; L.mpr_status_string.restype = C.c_char_p
         L.mpr_last_cuda_error.argtypes = []; L.mpr_last_cuda_error.restype = C.c_char_p
         _lib = L
@@ -369,6 +391,119 @@ class Mpr:
         return int(tr.value), int(tc.value), int(h.value), int(k.value)
 
 
+def slab_local_rows(rows_global: int, cols: int, row_begin: int, row_end: int):
+    """mpr_slab_local_rows: (first row, number of rows) of the whole grid a slab holds (own rows plus ghost rows)."""
+    sl = mpr_slab(struct_size=C.sizeof(mpr_slab), rows_global=rows_global, cols=cols, row_begin=row_begin, row_end=row_end)
+    first, n = C.c_int(), C.c_int()
+    _check(lib().mpr_slab_local_rows(C.byref(sl), C.byref(first), C.byref(n)), "mpr_slab_local_rows")
+    return int(first.value), int(n.value)
+
+
+class MprSlab(Mpr):
+    """One slab of a grid that is cut into row blocks over several contexts (mpr_create_slab).
+
+    values / sample_mask: CUDA tensors [n_rows, cols] holding the rows slab_local_rows() names (own rows plus ghost rows).
+    comm: the transport between the slabs, an object with
+        allreduce(values: list[float], op: int) -> list[float]        (op 0 sum, 1 min, 2 max over all slabs)
+        exchange(send_up, recv_up, send_down, recv_down, stream)      (uint8 CUDA tensors or None at the grid's edge:
+            after it, recv_up holds the upper neighbour's send_down and recv_down the lower neighbour's send_up)
+    The other calls are those of Mpr; the outputs have the local shape, `own` is the slice of the own rows in them."""
+
+    def __init__(self, values, sample_mask, rows_global: int, row_begin: int, row_end: int, comm, stream=None):
+        import torch
+        if values.dim() != 2 or values.dtype != torch.float32 or sample_mask.dtype != torch.uint8 or values.shape != sample_mask.shape:
+            raise ValueError("values float32 and sample_mask uint8 of the same [n_rows, cols] shape")
+        values, sample_mask = values.contiguous(), sample_mask.contiguous()
+        self.chains, self.batch = 1, 1
+        self.device = values.device
+        self.rows, self.cols = (int(x) for x in values.shape)
+        self._torch = torch
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        first, n = slab_local_rows(rows_global, self.cols, row_begin, row_end)
+        if n != self.rows:
+            raise ValueError(f"the slab holds rows [{first}, {first + n}) of the grid: {n} rows, got {self.rows}")
+        self.first_row, self.own = first, slice(row_begin - first, row_end - first)
+        nbytes = int(lib().mpr_slab_halo_bytes(self.cols))
+        up, down = row_begin > 0, row_end < rows_global
+        buf = lambda on: torch.zeros(nbytes, dtype=torch.uint8, device=self.device) if on else None
+        self._halo = [buf(up), buf(up), buf(down), buf(down)]          # send_up, recv_up, send_down, recv_down
+        self.comm = comm
+        self.comm_error = None
+
+        def allreduce(_user, vals, n_vals, op):
+            try:
+                out = comm.allreduce([vals[k] for k in range(n_vals)], int(op))
+                for k in range(n_vals):
+                    vals[k] = out[k]
+                return 0
+            except Exception as e:               # an exception must not cross the C frames
+                self.comm_error = e
+                return 1
+
+        def exchange(_user, _stream):
+            try:
+                comm.exchange(*self._halo, self._stream)
+                return 0
+            except Exception as e:
+                self.comm_error = e
+                return 1
+
+        self._cb = (ALLREDUCE_FN(allreduce), EXCHANGE_FN(exchange))     # kept alive with the context
+        ptr = lambda t: t.data_ptr() if t is not None else None
+        self._slab = mpr_slab(struct_size=C.sizeof(mpr_slab), rows_global=rows_global, cols=self.cols, row_begin=row_begin,
+                              row_end=row_end, allreduce=self._cb[0], exchange=self._cb[1], user=None,
+                              d_send_up=ptr(self._halo[0]), d_recv_up=ptr(self._halo[1]),
+                              d_send_down=ptr(self._halo[2]), d_recv_down=ptr(self._halo[3]))
+        n_ws = C.c_size_t()
+        _check(lib().mpr_query_workspace_slab(C.byref(self._slab), C.byref(n_ws)), "mpr_query_workspace_slab")
+        self.workspace = torch.empty(int(n_ws.value), dtype=torch.uint8, device=self.device)
+        self._ctx = C.c_void_p()
+        _check(lib().mpr_create_slab(C.byref(self._ctx), C.byref(self._slab), values.data_ptr(), sample_mask.data_ptr(),
+                                     self.workspace.data_ptr(), int(n_ws.value), self._stream.cuda_stream), "mpr_create_slab")
+        self.params = None
+
+
+class DistSlabComm:
+    """Transport of MprSlab over torch.distributed: slab r is rank r of `group`, its neighbours ranks r - 1 (up) and r + 1.
+    With the nccl backend the halo rows go GPU to GPU (NVLink) by batched send / recv; with gloo they are staged through
+    host memory (the CPU tests, or a box without peer access).  Plumbing only."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.host = dist.get_backend(group) != "nccl"
+
+    def allreduce(self, values, op):
+        import torch
+        dist = self.dist
+        t = torch.tensor(values, dtype=torch.float64)
+        if not self.host:
+            t = t.cuda()
+        dist.all_reduce(t, op=(dist.ReduceOp.SUM, dist.ReduceOp.MIN, dist.ReduceOp.MAX)[op], group=self.group)
+        return [float(x) for x in t.cpu()]
+
+    def exchange(self, send_up, recv_up, send_down, recv_down, stream):
+        import torch
+        dist = self.dist
+        stream.synchronize()                       # the library's copies into the send buffers are done
+        ops, staged = [], []
+        for send, recv, peer in ((send_up, recv_up, self.rank - 1), (send_down, recv_down, self.rank + 1)):
+            if send is None:
+                continue
+            if self.host:
+                s_h, r_h = send.cpu(), torch.empty(recv.shape, dtype=recv.dtype)
+                staged.append((recv, r_h))
+                send, recv = s_h, r_h
+            ops += [dist.P2POp(dist.isend, send, peer, self.group), dist.P2POp(dist.irecv, recv, peer, self.group)]
+        for w in (dist.batch_isend_irecv(ops) if ops else []):
+            w.wait()
+        for dev_t, host_t in staged:
+            dev_t.copy_(host_t)
+        if not self.host:
+            torch.cuda.current_stream().synchronize()
+
+
 class Mpr64:
     """The double-precision path (mpr64_* calls): one grid of rows x cols.
 
@@ -530,6 +665,25 @@ def infer_T(ctx: "Mpr", n_meas: int = 100, ladder=None, return_e_s: bool = False
     if return_e_s:
         return [float(x) for x in T_hat], [float(x) for x in e_s]
     return [float(x) for x in T_hat]
+
+
+def learn_q(values, sample_mask, qs, holdout_fraction: float = 0.2, params: mpr_params | None = None, **overrides):
+    """mpr_learn_q: q by leave-out validation over the candidates `qs` on one grid (reading R28).
+    Returns (q_hat, scores, temperatures)."""
+    import torch
+    p = params if params is not None else default_params(**overrides)
+    values, sample_mask = values.contiguous(), sample_mask.contiguous()
+    rows, cols = (int(x) for x in values.shape[-2:])
+    n = C.c_size_t()
+    _check(lib().mpr_query_workspace_learn_q(rows, cols, C.byref(n)), "mpr_query_workspace_learn_q")
+    ws = torch.empty(int(n.value), dtype=torch.uint8, device=values.device)
+    n_q = len(qs)
+    q_hat, scores, Ts = C.c_float(), (C.c_double * n_q)(), (C.c_double * n_q)()
+    stream = torch.cuda.current_stream(values.device)
+    _check(lib().mpr_learn_q(rows, cols, values.data_ptr(), sample_mask.data_ptr(), C.byref(p),
+                             (C.c_float * n_q)(*[float(x) for x in qs]), n_q, float(holdout_fraction), ws.data_ptr(),
+                             int(n.value), stream.cuda_stream, C.byref(q_hat), scores, Ts), "mpr_learn_q")
+    return float(q_hat.value), [float(x) for x in scores], [float(x) for x in Ts]
 
 
 def interpolate(values, sample_mask, T=None, chains: int = 1, **params):

@@ -164,3 +164,32 @@ def test_interpolate_with_inferred_temperature(torch_cuda, mpr, orc):
             rm.append(synth.validation_measures(z, pred.cpu().numpy()[0], m)["rmse"])
         scores.append(np.mean(rm))
     assert scores[0] == pytest.approx(scores[1], rel=0.03)
+
+
+def test_learn_q_against_the_oracle(torch_cuda, mpr, orc):
+    """mpr_learn_q (q by leave-out validation, reading R28) against the oracle's learn_q on one grid: the
+    temperatures of the candidates (e_s of the remaining samples through the equipartition line) to float precision --
+    which pins the withheld set, since one sample more or less moves e_s --, the scores within the chains' noise (the
+    runs are short: 3 %), and the withheld set itself bit for bit through a run whose every sample is withheld or not."""
+    torch = torch_cuda
+    L = 96
+    z, m = _field(L, L, 7.0, 0.4, 91)
+    qs = [0.15, 0.3, 0.5]
+    kw = dict(seed=606, equil_cap=200, M=20, sweeps_per_real=5)
+    q_gpu, sc_gpu, T_gpu = mpr.learn_q(_dev(torch, z), _dev(torch, m), qs, 0.2, **kw)
+    q_ref, sc_ref, T_ref = orc.learn_q(z, m, orc.Params(**kw), qs, 0.2)
+    assert T_gpu == pytest.approx(T_ref, rel=1e-6)
+    assert sc_gpu == pytest.approx(sc_ref, rel=0.03)
+    assert q_gpu in [float(np.float32(q)) for q in qs]
+    # the scores are nearly flat in q on such data (q mostly rescales T): same argmin when the oracle's margin is clear
+    order = np.argsort(sc_ref)
+    if sc_ref[order[1]] > 1.06 * sc_ref[order[0]]:
+        assert q_gpu == q_ref
+    # same call, same bits; another fraction, another withheld set
+    assert mpr.learn_q(_dev(torch, z), _dev(torch, m), qs, 0.2, **kw) == (q_gpu, sc_gpu, T_gpu)
+    assert mpr.learn_q(_dev(torch, z), _dev(torch, m), qs, 0.5, **kw)[2] != T_gpu
+    for bad in (dict(qs=[0.6]), dict(qs=[0.0]), dict(qs=[]), dict(holdout_fraction=0.0), dict(holdout_fraction=1.0)):
+        args = dict(qs=qs, holdout_fraction=0.2); args.update(bad)
+        with pytest.raises(mpr.MprError) as e:
+            mpr.learn_q(_dev(torch, z), _dev(torch, m), args["qs"], args["holdout_fraction"], **kw)
+        assert e.value.name == "MPR_ERR_ARG"

@@ -159,3 +159,38 @@ def test_harness_temperature_is_the_sample_energy_through_the_closed_form(orc):
         T_orc = orc.default_ladder(rows, cols, e_s, (1.0,))[0]
         # Eq. 1 in float32 (oracle) against float64 (generator): (1 + e_s) ~ 1e-3 .. 1e-5 carries ~1e-4 relative
         assert synth.choose_T(z, m) == pytest.approx(T_orc, rel=2e-3)
+
+
+def test_learn_q_holdout_and_scores(orc):
+    """Reading R28 (PAPER.md L89 gives no procedure) as the oracle runs it.  Pinned here is everything but the reading
+    itself: the withheld set is a Bernoulli thinning of the SAMPLES by the HOLDOUT stream's uniforms (rebuilt from the
+    Philox words, which are pinned against cuRAND); a candidate's score is the root mean square error at the withheld
+    samples of the oracle's own full run on the remaining ones at the temperature of the equipartition line; the learned
+    q is the argmin."""
+    from paper_1811_01604_b200 import synth
+    z = synth.grf(48, 40, 6.0, "gaussian", 5)
+    m = synth.bernoulli_mask(48, 40, 0.4, 6)
+    seed, f = 4242, 0.25
+    held = orc.holdout_mask(m, f, seed)
+    assert held.dtype == np.uint8 and not held[m == 0].any()
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for n in (0, 1, 2, 3, 4, 777, 48 * 40 - 1):
+        u = orc.u01(int(orc.philox4x32_10([n >> 2, 0, 3, 0], key)[n & 3]))
+        assert held.flat[n] == (1 if m.flat[n] and u < f else 0)
+    frac = held.sum() / m.sum()
+    assert abs(frac - f) < 4 * math.sqrt(f * (1 - f) / m.sum())
+    assert not np.array_equal(held, orc.holdout_mask(m, f, seed + 1)) and not np.array_equal(held, orc.holdout_mask(m, f, seed, g=1))
+    p = orc.Params(seed=seed, equil_cap=150, M=6, sweeps_per_real=3)
+    qs = [0.2, 0.5]
+    q_hat, scores, Ts = orc.learn_q(z, m, p, qs, f)
+    train = (m & (1 - held)).astype(np.uint8)
+    import dataclasses
+    for q, sc, T in zip(qs, scores, Ts):
+        pq = dataclasses.replace(p, q=float(np.float32(q)))
+        phi, _, _ = orc.transform(z, train, seed)
+        e_s, _ = orc.sample_energy(phi, train, pq.q)
+        assert T == orc.default_ladder(48, 40, e_s, (1.0,))[0]
+        pred = orc.run(z, train, T, pq)["pred"]
+        assert sc == pytest.approx(float(np.sqrt(np.mean((z.astype(np.float64) - pred)[held == 1] ** 2))), rel=1e-12)
+    assert q_hat == float(np.float32(qs[int(np.argmin(scores))]))
+    assert Ts[0] < Ts[1]               # (1 + e_s) ~ q^2: a smaller q needs a lower temperature for the same data
