@@ -48,7 +48,8 @@ struct Dev64 {
     uint32_t* list;           // [n_colour[0]] then [n_colour[1]]: the prediction sites of colour 0, then of colour 1, ascending
     uint32_t* list_counts;    // [2][list_blocks] prediction sites per colour of each block of 32 * LIST_THREADS sites
     uint32_t  list_blocks;
-    double2*  vec;            // [2][rows][half] unit vectors, one plane per checkerboard colour (vpos)
+    double2*  vec;            // [2][rows][half] unit vectors, one plane per checkerboard colour (vpos): the CURRENT buffer
+    double2*  vec_other;      // the other of the two vector buffers (the tile pass writes it; the host swaps the two)
     int       half;           // ceil(cols / 2): sites of one colour in a row (at most)
     uint32_t  plane;          // rows * half
     double*   acc;            // [N] sum over the realizations of phi
@@ -82,7 +83,11 @@ __device__ __forceinline__ size_t vpos_n(const Dev64& d, uint32_t n)
 }
 
 // u = (2 (x >> 9) + 1) 2^-24 in (0,1): the same lattice as the fp32 path (R13), exact in double
-__device__ __forceinline__ double u01d(uint32_t x) { return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0); }
+// built without an integer -> double conversion: f = 1.m in [1, 2) with m = x >> 9 in the top 23 mantissa bits, u = f - (1 - 2^-24)
+__device__ __forceinline__ double u01d(uint32_t x)
+{
+    return __hiloint2double((int)(0x3FF00000u | (x >> 12)), (int)(x >> 9 << 29)) - 0.99999994039535522461;
+}
 
 // Eq. 1 in double, the oracle's pinned operation order, clamped to [0, TWO_PI_D]
 __device__ __forceinline__ double eq1d(double z, double zmin, double zmax)
@@ -255,6 +260,57 @@ __global__ void __launch_bounds__(256) k64_init_state(Dev64 d)
     double sn, cs;
     sincos(__dmul_rn(d.q, p), &sn, &cs);
     d.vec[vpos_n(d, n)] = make_double2(cs, sn);
+    d.vec_other[vpos_n(d, n)] = make_double2(cs, sn);        // sample sites are never written again
+}
+
+// sin and cos of the half rotation |x| <= q pi / 2 <= pi / 4 by their Maclaurin series, to x^17 and x^16 (truncation
+// below 1e-19 and 2e-18 relative at pi / 4): no range reduction and no special cases, a third of the library sincos'
+// instructions
+// (the coefficients sit in the constant bank: a DFMA takes them as an operand, an immediate double costs two moves)
+__constant__ double C_SIN[8] = {2.8114572543455206e-15, -7.6471637318198164e-13, 1.6059043836821613e-10, -2.5052108385441720e-08,
+                                2.7557319223985893e-06, -1.9841269841269841e-04, 8.3333333333333332e-03, -1.6666666666666666e-01};
+__constant__ double C_COS[8] = {4.7794773323873853e-14, -1.1470745597729725e-11, 2.0876756987868100e-09, -2.7557319223985888e-07,
+                                2.4801587301587302e-05, -1.3888888888888889e-03, 4.1666666666666664e-02, -0.5};
+__constant__ double C_EXP[12] = {1.6059043836821613e-10, 2.0876756987868100e-09, 2.5052108385441720e-08, 2.7557319223985888e-07,
+                                 2.7557319223985893e-06, 2.4801587301587302e-05, 1.9841269841269841e-04, 1.3888888888888889e-03,
+                                 8.3333333333333332e-03, 4.1666666666666664e-02, 1.6666666666666666e-01, 0.5};
+__constant__ double C_LN2[3] = {1.4426950408889634, 6.93147180369123816490e-01, 1.90821492927058770002e-10};   // log2 e; ln 2 high (low 21 bits zero), low
+__device__ __forceinline__ void sincos_small_d(double x, double& s, double& c)
+{
+    const double x2 = x * x;
+    double ps = C_SIN[0], pc = C_COS[0];
+#pragma unroll
+    for (int k = 1; k < 8; ++k) { ps = fma(x2, ps, C_SIN[k]); pc = fma(x2, pc, C_COS[k]); }       // 1/17! ... -1/3!;  1/16! ... -1/2!
+    s = fma(x * x2, ps, x);
+    c = fma(x2, pc, 1.0);
+}
+
+// exp(x) for x <= 0 as the acceptance test needs it (AP = exp(-dH / T) is compared with r >= 2^-24): x = k ln 2 + r
+// with |r| <= ln 2 / 2, Maclaurin series of exp r to r^13 (truncation 4e-18), scaled by 2^k through the exponent
+// bits; below 2^-40 the result is returned as 0 (it loses against every r).  No special cases, half the library exp.
+__device__ __forceinline__ double exp_nonpos_d(double x)
+{
+    const double t = x * C_LN2[0];
+    const double kd = rint(fmax(t, -40.0));
+    double r = fma(-kd, C_LN2[1], x);
+    r = fma(-kd, C_LN2[2], r);
+    double p = C_EXP[0];                                           // 1/13!
+#pragma unroll
+    for (int k = 1; k < 12; ++k) p = fma(r, p, C_EXP[k]);         // 1/12! ... 1/2!
+    p = fma(r, p, 1.0);
+    p = fma(r, p, 1.0);
+    const long long bits = (long long)((int)kd + 1023) << 52;     // 2^k, k in [-40, 0]
+    return t < -40.0 ? 0.0 : p * __longlong_as_double(bits);
+}
+
+// 1 / x by the special-function unit's 20-bit estimate and two Newton steps (a division is 25 instructions and a call)
+__device__ __forceinline__ double rcp_d(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(fma(-x, r, 1.0), r, r);
+    r = fma(fma(-x, r, 1.0), r, r);
+    return r;
 }
 
 // ---- a3: UPDATE of one prediction site (Alg. 1) in vector form, in double ----------------------------
@@ -270,7 +326,7 @@ __device__ __forceinline__ double2 update_site_d(double2 v, double2 n_up, double
         // line 1, over-relaxation: v' = 2 (h.v)/(h.h) h - v keeps h.v (L156, L265; R2); out of [0, 2 pi]: keep the spin
         const double R2 = fma(hx, hx, hy * hy);
         const double dot = fma(px, hx, py * hy);
-        const double k = (dot + dot) / R2;                       // 0 / 0 -> NaN -> kept below (R17)
+        const double k = (dot + dot) * rcp_d(R2);                // 0 * inf -> NaN -> kept below (R17)
         const double fx = fma(k, hx, -px), fy = fma(k, hy, -py);
         bool in = fy >= 0.0 && hy >= 0.0;
         if (!QHALF) in = in && (fma(fx, bs, -fy * bc) >= 0.0);
@@ -290,7 +346,7 @@ __device__ __forceinline__ double2 update_site_d(double2 v, double2 n_up, double
     // lines 2-3: rotate by d = q delta = 2 hd, hd = (u - 1/2) q pi / a
     const double hd = (u01d(w0) - 0.5) * hd_scale;
     double sh, ch;
-    sincos(hd, &sh, &ch);
+    sincos_small_d(hd, sh, ch);
     const double sh2 = sh + sh;
     const double sd = sh2 * ch, omc = sh2 * sh;                  // sin d, 1 - cos d
     double rx = fma(-sd, py, fma(-omc, px, px));
@@ -312,7 +368,7 @@ __device__ __forceinline__ double2 update_site_d(double2 v, double2 n_up, double
         }
     }
     // lines 5-6: AP = min{1, exp(-dH/T)}; accept phi'' if AP > r else keep phi'
-    accepted = dH <= 0.0 || exp(dH * neg_inv_T) > u01d(w1);
+    accepted = dH <= 0.0 || exp_nonpos_d(dH * neg_inv_T) > u01d(w1);
     return make_double2(accepted ? rx : px, accepted ? ry : py);
 }
 
@@ -466,6 +522,91 @@ __global__ void __launch_bounds__(256) k64_import_angles(Dev64 d, const double* 
     sincos(__dmul_rn(d.q, p), &sn, &cs);
     d.vec[vpos_n(d, n)] = make_double2(cs, sn);
 }
+// ---- a3 / a4 in shared memory: K whole sweeps of one tile per launch (temporal blocking, DESIGN.md sections 6, 12) ----
+// The fp32 path's tile pass for double vectors.  A tile's frame (core + halo of H sites) is loaded by two TMA tensor loads,
+// one per colour plane, into a shared-memory copy with the planes' own layout (element (lr, lc) of colour p at
+// S[p][lr * FCH + (lc >> 1)]; out-of-grid elements arrive as zeros: the open boundary, L109); 2K half-sweeps walk the
+// prefixes of the tile's entry lists (built by the fp32 path's k_tile_count / k_tile_fill on this grid's bitmask: frame
+// offsets lr * FC + lc, core first, then ring by ring), halo sites being recomputed bit for bit because the random
+// numbers are keyed by (site, sweep); the core's rows leave by one bulk copy per row and plane into the OTHER vector
+// buffer.  Every sweep draws its own Philox block (40 integer instructions against ~250 of double arithmetic per update:
+// nothing to save by storing the second pair).  Accepted proposals are not counted here: counted sweeps and the
+// equilibration (which needs the energy after every sweep, L199) use k64_halfsweep.
+constexpr int T64_THREADS = 512;
+__device__ __forceinline__ void tma_load_plane(void* dst, const CUtensorMap* map, int c64, int r, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(mpr::smem_u32(dst)), "l"((uint64_t)map), "r"(c64), "r"(r), "r"(mpr::smem_u32(bar)) : "memory");
+}
+
+template <bool QHALF, int ORMODE>
+__global__ void __launch_bounds__(T64_THREADS, 2)
+k64_tilepass(const __grid_constant__ CUtensorMap map_p0, const __grid_constant__ CUtensorMap map_p1, const Dev64 d,
+             const mpr::Dev dt, double2* __restrict__ dst, uint32_t K, uint32_t t_off)
+{
+    extern __shared__ __align__(128) unsigned char smem64[];
+    __shared__ __align__(8) uint64_t s_bar[2];
+    __shared__ uint32_t s_cle[2][mpr::MAX_H];
+    const int tile = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NT = T64_THREADS, NW = T64_THREADS / 32;
+    const int H = dt.H, FC = dt.FC, FCH = FC / 2, FR = dt.FR;
+    double2* S0 = reinterpret_cast<double2*>(smem64);
+    double2* S1 = S0 + FR * FCH;
+    uint16_t* E = reinterpret_cast<uint16_t*>(S1 + FR * FCH);
+    const mpr::TileGeom tg = mpr::tile_geom(dt, tile);
+    const mpr::TileMeta& meta = dt.tile_meta[tile];
+    const uint32_t entry_bytes = dt.max_entries * (uint32_t)sizeof(uint16_t);
+    if (tid == 0) {
+        mpr::mbar_init(&s_bar[0], 1);
+        mpr::mbar_expect_tx(&s_bar[0], (uint32_t)(2 * FR * FCH * sizeof(double2)));
+        tma_load_plane(S0, &map_p0, tg.c0 - H, tg.r0 - H, &s_bar[0]);      // inner coordinate in 8-byte units: 2 * ((c0 - H) >> 1)
+        tma_load_plane(S1, &map_p1, tg.c0 - H, tg.r0 - H, &s_bar[0]);
+    } else if (tid == 32) {
+        mpr::mbar_init(&s_bar[1], 1);
+        mpr::mbar_expect_tx(&s_bar[1], entry_bytes);
+        if (entry_bytes) mpr::bulk_load(E, dt.entries + (size_t)tile * dt.tile_entries, entry_bytes, &s_bar[1]);
+    }
+    if (tid >= 64 && tid < 64 + 2 * mpr::MAX_H) (&s_cle[0][0])[tid - 64] = (&meta.cle[0][0])[tid - 64];
+    const State64& st = *d.state;
+    const uint32_t t0 = st.t + t_off;
+    const double hd_scale = d.q * (0.5 * TWO_PI_D) / st.a, neg_inv_T = -1.0 / st.T;
+    __syncthreads();
+    mpr::mbar_wait(&s_bar[1], 0);
+    mpr::mbar_wait(&s_bar[0], 0);
+    const uint32_t base1 = mpr::colour1_base(s_cle[0][mpr::MAX_H - 1]);
+#pragma unroll 1
+    for (uint32_t j = 0; j < 2u * K; ++j) {
+        const uint32_t c = j & 1u, t = t0 + (j >> 1), R = 2u * K - 1u - j;
+        const uint32_t n = s_cle[c][R < (uint32_t)mpr::MAX_H ? R : (uint32_t)mpr::MAX_H - 1u];
+        const uint16_t* Ec = E + (c ? base1 : 0u);
+        double2* own = c ? S1 : S0;
+        const double2* oth = c ? S0 : S1;
+#pragma unroll 1
+        for (uint32_t e = tid; e < n; e += NT) {
+            const int off = Ec[e];
+            const int lr = (int)(((uint32_t)off * dt.fc_inv) >> 24), lc = off - lr * FC;
+            const int o = lr * FCH + (lc >> 1);
+            const double2 up = oth[o - FCH], dn = oth[o + FCH], lf = oth[o - 1 + (lc & 1)], rt = oth[o + (lc & 1)];
+            const uint32_t site = (uint32_t)((tg.r0 - H + lr) * d.cols + (tg.c0 - H + lc));
+            const uint4 x = philox4x32_10(site, t >> 1, 2u, 0u, d.rk0, d.rk1);
+            const uint32_t w0 = (t & 1u) ? x.z : x.x, w1 = (t & 1u) ? x.w : x.y;
+            bool accepted;
+            own[o] = update_site_d<QHALF, ORMODE>(own[o], up, dn, lf, rt, w0, w1, hd_scale, neg_inv_T, d.bc, d.bs, accepted);
+        }
+        __syncthreads();
+    }
+    mpr::fence_proxy_async_smem();
+    __syncthreads();
+    // the core's rows, one bulk copy per row and plane (both planes take ceil(width / 2) elements: the odd one out is a pad)
+    const uint32_t row_bytes = (uint32_t)((tg.TCc + 1) / 2) * (uint32_t)sizeof(double2);
+    for (int i = warp + NW * lane; i < 2 * tg.TRc; i += NW * 32) {
+        const int p = i & 1, lr = i >> 1;
+        const double2* src = (p ? S1 : S0) + (H + lr) * FCH + (H >> 1);
+        mpr::bulk_store(dst + (size_t)p * d.plane + (size_t)(tg.r0 + lr) * d.half + (size_t)(tg.c0 >> 1), src, row_bytes);
+    }
+    mpr::bulk_commit_wait_read();
+}
+
 // scalar state edits: what = 0 begin a run at temperature x; 1 set a = x; 2 commit u sweeps (t += u) and v realizations;
 // 3 set t = u
 __global__ void k64_edit(Dev64 d, int what, double x, uint32_t u, uint32_t v)

@@ -3,7 +3,22 @@
 
 namespace {
 
-struct Layout64 { size_t state, done, partials, values, phi, bits, list, list_counts, vec, acc, acc2, total; };
+struct Layout64 { size_t state, done, partials, values, phi, bits, list, list_counts, vec, acc, acc2, tstate, tile_meta, entries, total; };
+
+// tiles of the double-precision tile pass: 64 x 64 cores with a halo of 8 (4 sweeps per pass), lower cores of the same
+// pitch when 64 rows would not give every SM its two CTAs; lists by the fp32 path's kernels (frame offsets, pitch FC)
+void choose_tiles64(int rows, int cols, Geometry* g)
+{
+    int TR = 64;
+    const long ntx = (cols + 63) / 64;
+    if (ntx * ((rows + 63) / 64) < 148L * 2L)
+        for (int tr = 16; tr < 64; tr += 8)
+            if (ntx * ((rows + tr - 1) / tr) <= 148L * 2L) { TR = tr; break; }
+    g->TR = TR; g->TC = 64; g->H = 8; g->FR = TR + 16;
+    g->FC = ((64 + 16 + 1) & ~3) + 2;
+    g->ntx = (int)ntx; g->nty = (rows + TR - 1) / TR; g->ntiles = g->ntx * g->nty;
+    g->entry_stride = (size_t)g->ntiles * (((size_t)g->FR * g->FC + 31) & ~(size_t)15);
+}
 
 bool geometry64(int rows, int cols, uint32_t* N, uint32_t* words)
 {
@@ -17,6 +32,8 @@ bool geometry64(int rows, int cols, uint32_t* N, uint32_t* words)
 Layout64 make_layout64(int rows, int cols, uint32_t N, uint32_t words)
 {
     Layout64 L;
+    Geometry g;
+    choose_tiles64(rows, cols, &g);
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     L.state    = take(sizeof(mpr64::State64));
@@ -27,9 +44,12 @@ Layout64 make_layout64(int rows, int cols, uint32_t N, uint32_t words)
     L.bits     = take(sizeof(uint32_t) * words);
     L.list     = take(sizeof(uint32_t) * N);
     L.list_counts = take(sizeof(uint32_t) * 2 * cdiv(words, mpr64::LIST_THREADS));
-    L.vec      = take(sizeof(double2) * 2 * (size_t)rows * (size_t)((cols + 1) / 2));
+    L.vec      = take(sizeof(double2) * 2 * 2 * (size_t)rows * (size_t)((cols + 1) / 2));       // two buffers of two planes
     L.acc      = take(sizeof(double) * N);
     L.acc2     = take(sizeof(double) * N);
+    L.tstate   = take(sizeof(GridState));
+    L.tile_meta = take(sizeof(TileMeta) * (size_t)g.ntiles);
+    L.entries  = take(sizeof(uint16_t) * (g.entry_stride + 16));
     L.total = o;
     return L;
 }
@@ -48,6 +68,13 @@ struct mpr64_ctx {
     mpr64::State64 h_state;
     bool           qhalf, dirty;
     uint64_t       n_realizations;   // realizations accumulated since mpr64_set_params
+    // the tile pass (k64_tilepass): tiling and lists in the fp32 path's format, TMA descriptors [buffer][plane]
+    mpr::Dev       dt;
+    alignas(64) CUtensorMap map[2][2];
+    double2*       vec_buf[2];
+    uint32_t       cur;              // d.vec = vec_buf[cur]
+    size_t         tile_smem;
+    uint32_t       k_max;
 };
 
 namespace {
@@ -62,6 +89,59 @@ mpr_status fetch_state64(mpr64_ctx* ctx)
 }
 
 typedef void (*half_kernel)(mpr64::Dev64, const uint32_t*, uint32_t, uint32_t, int, int);
+typedef void (*tile_kernel64)(const CUtensorMap, const CUtensorMap, const mpr64::Dev64, const mpr::Dev, double2*, uint32_t, uint32_t);
+tile_kernel64 pick_tile_kernel64(bool qhalf, int or_mode)
+{
+    using namespace mpr64;
+    if (qhalf) return or_mode == 0 ? k64_tilepass<true, 0> : or_mode == 1 ? k64_tilepass<true, 1> : k64_tilepass<true, 2>;
+    return or_mode == 0 ? k64_tilepass<false, 0> : k64_tilepass<false, 2>;
+}
+
+void set_cur64(mpr64_ctx* ctx, uint32_t cur)
+{
+    ctx->cur = cur;
+    ctx->d.vec = ctx->vec_buf[cur]; ctx->d.vec_other = ctx->vec_buf[cur ^ 1u];
+}
+
+// n sweeps without the accepted count, as tile passes of up to k_max sweeps (sweep indices state.t + *t_off ...)
+mpr_status launch_passes64(mpr64_ctx* ctx, uint32_t n, uint32_t* t_off)
+{
+    const tile_kernel64 kern = pick_tile_kernel64(ctx->qhalf, (int)ctx->prm.or_mode);
+    while (n) {
+        const uint32_t K = n < ctx->k_max ? n : ctx->k_max;
+        kern<<<ctx->dt.ntiles, mpr64::T64_THREADS, ctx->tile_smem, ctx->stream>>>(ctx->map[ctx->cur][0], ctx->map[ctx->cur][1], ctx->d,
+                                                                                   ctx->dt, ctx->d.vec_other, K, *t_off);
+        CU_LAUNCH();
+        set_cur64(ctx, ctx->cur ^ 1u);
+        *t_off += K; n -= K;
+    }
+    ctx->dirty = true;
+    return MPR_OK;
+}
+
+// TMA descriptor of one colour plane of one vector buffer: [rows][2 * half] eight-byte words (a double2 is two), box =
+// one tile frame's share of the plane; out-of-grid elements arrive as zeros (open boundary, L109)
+mpr_status make_plane_map64(mpr64_ctx* ctx, int buf, int plane)
+{
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (!cuda_ok(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres), "cudaGetDriverEntryPoint") ||
+        qres != cudaDriverEntryPointSuccess || !fn) return MPR_ERR_CUDA;
+    const mpr64::Dev64& d = ctx->d;
+    const cuuint64_t dims[2] = {(cuuint64_t)d.half * 2u, (cuuint64_t)d.rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)d.half * sizeof(double2)};
+    const cuuint32_t box[2] = {(cuuint32_t)ctx->dt.FC, (cuuint32_t)ctx->dt.FR};          // FC / 2 double2 = FC words
+    const cuuint32_t estr[2] = {1u, 1u};
+    const CUresult r = ((PFN_cuTensorMapEncodeTiled)fn)(&ctx->map[buf][plane], CU_TENSOR_MAP_DATA_TYPE_UINT64, 2,
+                                                         (void*)(ctx->vec_buf[buf] + (size_t)plane * d.plane), dims, strides, box, estr,
+                                                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "cuTensorMapEncodeTiled (double planes) failed with CUresult %d", (int)r);
+        return MPR_ERR_CUDA;
+    }
+    return MPR_OK;
+}
 half_kernel pick_half_kernel(bool qhalf, int or_mode)
 {
     using namespace mpr64;
@@ -135,7 +215,9 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
     d.list = (uint32_t*)(base + lay.list);
     d.list_counts = (uint32_t*)(base + lay.list_counts);
     d.list_blocks = cdiv(words, mpr64::LIST_THREADS);
-    d.vec = (double2*)(base + lay.vec);
+    ctx->vec_buf[0] = (double2*)(base + lay.vec);
+    ctx->vec_buf[1] = ctx->vec_buf[0] + 2 * (size_t)rows * (size_t)((cols + 1) / 2);
+    set_cur64(ctx, 0);
     d.acc = (double*)(base + lay.acc);
     d.acc2 = (double*)(base + lay.acc2);
     d.rows = rows; d.cols = cols; d.N = N; d.words = words;
@@ -162,6 +244,42 @@ mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_val
     if (e & mpr::ERRF_DEGENERATE) return fail(MPR_ERR_DEGENERATE_RANGE);
     if (e & mpr::ERRF_NO_FREE) return fail(MPR_ERR_NO_FREE);
     ctx->n_colour[0] = ctx->h_state.n_colour[0]; ctx->n_colour[1] = ctx->h_state.n_colour[1];
+    // the tile pass: tiles and per-tile entry lists in the fp32 path's format, built by its kernels on this grid's bitmask
+    {
+        Geometry g;
+        choose_tiles64(rows, cols, &g);
+        mpr::Dev& t = ctx->dt;
+        memset(&t, 0, sizeof t);
+        t.states = (GridState*)(base + lay.tstate);
+        t.bits = d.bits; t.tile_meta = (TileMeta*)(base + lay.tile_meta); t.entries = (uint16_t*)(base + lay.entries);
+        t.batch = 1; t.rows = rows; t.cols = cols; t.chains = 1; t.nv = 1;
+        t.N = N; t.words = words;
+        t.entry_stride = g.entry_stride; t.tile_entries = (uint32_t)(g.entry_stride / (size_t)g.ntiles);
+        t.TR = g.TR; t.TC = g.TC; t.H = g.H; t.FR = g.FR; t.FC = g.FC; t.ntx = g.ntx; t.nty = g.nty; t.ntiles = g.ntiles;
+        t.fc_inv = (uint32_t)(((1u << 24) + (uint32_t)g.FC - 1u) / (uint32_t)g.FC);
+        t.own_r0 = 0; t.own_r1 = rows;
+        // the pads of an odd-width grid's planes stay zero (the frame loads read them as neighbours)
+        if (!cuda_ok(cudaMemsetAsync(ctx->vec_buf[0], 0, sizeof(double2) * 4 * (size_t)rows * (size_t)d.half, ctx->stream), "memset vec")) return fail(MPR_ERR_CUDA);
+        k_tile_count<<<dim3(g.ntiles, 1), 256, 0, ctx->stream>>>(t);
+        k_tile_scan<<<1, 32, 0, ctx->stream>>>(t);
+        const size_t fill_smem = (size_t)g.FR * g.FC * sizeof(uint16_t);
+        k_tile_fill<<<dim3(g.ntiles, 1), 256, fill_smem, ctx->stream>>>(t);       // <= 80 x 82 x 2 bytes: below the default limit
+        ctx->launches += 3;
+        GridState hs;
+        if (!cuda_ok(cudaMemcpyAsync(&hs, t.states, sizeof hs, cudaMemcpyDeviceToHost, ctx->stream), "copy") ||
+            !cuda_ok(cudaStreamSynchronize(ctx->stream), "sync") || !cuda_ok(cudaGetLastError(), "tile lists")) return fail(MPR_ERR_CUDA);
+        t.max_entries = (hs.max_tile_entries + 15u) & ~15u;
+        ctx->tile_smem = (size_t)2 * g.FR * (g.FC / 2) * sizeof(double2) + (size_t)t.max_entries * sizeof(uint16_t);
+        ctx->k_max = (uint32_t)(g.H / 2);
+        for (int qh = 0; qh < 2; ++qh)
+            for (int om = 0; om < 3; ++om) {
+                if (!qh && om == 1) continue;
+                if (!cuda_ok(cudaFuncSetAttribute((const void*)pick_tile_kernel64(qh, om), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                  (int)ctx->tile_smem), "cudaFuncSetAttribute")) return fail(MPR_ERR_CUDA);
+            }
+        for (int b = 0; b < 2; ++b)
+            for (int p = 0; p < 2; ++p) { st = make_plane_map64(ctx, b, p); if (st != MPR_OK) return fail(st); }
+    }
     *out = ctx;
     return MPR_OK;
 }
@@ -238,11 +356,9 @@ mpr_status mpr64_simulate(mpr64_ctx* ctx)
     if (ctx->prm.a_eq_mode == 1) { mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(d, 1, 1.0, 0u, 0u); CU_LAUNCH(); }
     uint32_t t_off = 0;
     for (uint32_t j = 0; j < ctx->prm.M; ++j) {
-        for (uint32_t w = 0; w < ctx->prm.sweeps_per_real; ++w, ++t_off) {
-            mpr_status s = launch_sweep64(ctx, t_off, 0);
-            if (s != MPR_OK) return s;
-        }
-        mpr64::k64_accumulate<<<cdiv(d.N, 256), 256, 0, ctx->stream>>>(d);          // step 6.3
+        mpr_status s = launch_passes64(ctx, ctx->prm.sweeps_per_real, &t_off);        // tile passes of up to 4 sweeps
+        if (s != MPR_OK) return s;
+        mpr64::k64_accumulate<<<cdiv(ctx->d.N, 256), 256, 0, ctx->stream>>>(ctx->d);    // step 6.3
         CU_LAUNCH();
     }
     mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(d, 2, 0.0, t_off, ctx->prm.M);
@@ -316,8 +432,14 @@ mpr_status mpr64_sweep(mpr64_ctx* ctx, uint32_t n_sweeps, double a, uint64_t* h_
     if (ctx->state != READY) return MPR_ERR_STATE;
     mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(ctx->d, 1, a, 0u, 0u);        // also zeroes the accepted counter
     CU_LAUNCH();
-    for (uint32_t w = 0; w < n_sweeps; ++w) {
-        mpr_status s = launch_sweep64(ctx, w, h_accepted ? 1 : 0);
+    if (h_accepted) {
+        for (uint32_t w = 0; w < n_sweeps; ++w) {
+            mpr_status s = launch_sweep64(ctx, w, 1);
+            if (s != MPR_OK) return s;
+        }
+    } else {
+        uint32_t t_off = 0;
+        mpr_status s = launch_passes64(ctx, n_sweeps, &t_off);
         if (s != MPR_OK) return s;
     }
     mpr64::k64_edit<<<1, 1, 0, ctx->stream>>>(ctx->d, 2, 0.0, n_sweeps, 0u);

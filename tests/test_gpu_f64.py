@@ -163,6 +163,39 @@ def test_equilibration_controller_and_full_run_follow_the_oracle(torch_cuda, mpr
     ctx.close()
 
 
+@pytest.mark.parametrize("rows,cols", [(64, 64), (150, 201), (37, 53), (2, 9), (300, 130), (65, 2)])
+@pytest.mark.parametrize("q,or_mode", [(0.5, 0), (0.5, 1), (0.3, 0), (0.5, 2)])
+def test_t2_tile_pass_several_sweeps_per_launch(torch_cuda, mpr, orc64, rows, cols, q, or_mode):
+    """mpr64_sweep without the accepted count runs the shared-memory tile pass (k64_tilepass: up to 4 sweeps per launch on
+    a frame with a halo of 8, colour planes loaded by TMA, every sweep its own Philox block): n = 1 ... 9 sweeps per call
+    (passes of 4, 4 + 1, 4 + 3, 4 + 4 + 1 sweeps, from even and odd sweep indices) against n oracle sweeps, at EVERY
+    prediction site within 1e-11 rad -- one and several tiles, ragged edges, odd widths (the planes' pad column)."""
+    torch = torch_cuda
+    if or_mode == 1 and q != 0.5:
+        pytest.skip("Eq. 6 as printed is q = 1/2 only")
+    z, m = _field(rows, cols, 5.0, 0.55, 900 + rows + cols)
+    z = z.astype(np.float64)
+    q = float(np.float32(q))               # mpr_params.q is a float field; the double path computes with its double value (R27)
+    seed, T = 77, 0.03
+    phi, _, _ = orc64.transform(z, m, seed)
+    ctx = mpr.Mpr64(_dev(torch, z), _dev(torch, m))
+    ctx.set_params(T, seed=seed, q=q, or_mode=or_mode)
+    t = 0
+    tol = 1e-8 if or_mode == 1 else 1e-11          # Eq. 6 as printed: atan2 of nearly cancelling q-less sums (hot state)
+    for n, a in ((1, 1.0), (4, 1.5), (5, 3.0), (7, 6.0), (9, 12.0), (2, 20.0), (3, 20.0)):
+        ctx.set_angles(torch.from_numpy(phi).cuda())
+        ctx.set_sweep_index(t)
+        assert ctx.sweep(n, a) is None
+        for k in range(n):
+            orc64.sweep(phi, m, q, T, a, seed, 0, t + k, or_mode)
+        t += n
+        got = ctx.get_angles().cpu().numpy()
+        assert ctx.get_stats().t == t
+        assert np.array_equal(got[m == 1], phi[m == 1])
+        assert np.abs(got - phi).max() < tol, (n, a, float(np.abs(got - phi).max()))
+    ctx.close()
+
+
 @pytest.mark.parametrize("cap,n_fit,n_f", [(21, 20, 5), (40, 20, 7), (300, 256, 7), (300, 20, 7), (23, 20, 5)])
 def test_equilibration_windows_not_aligned_with_the_check_interval(torch_cuda, mpr, orc64, cap, n_fit, n_f):
     """Alg. 2 step 5 with n_fit not a multiple of n_f (L201: the slope is checked at i >= n_fit, i % n_f == 0): the run
