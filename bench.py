@@ -138,8 +138,9 @@ ISSUE_PEAK_PER_S = 148 * 4 * 32 * 1.965e9
 # Instructions one UPDATE needs at the least: Philox4x32-10 is 40 per call and serves two
 # updates (20), about 40 fp32 / compare / select for Alg. 1 lines 1-6, 8 shared-memory accesses and addresses.
 ALGORITHMIC_INSTR_PER_UPDATE = 68.0
-# DRAM bytes of one 4-sweep tile-pass launch on cfg4 from the committed ncu capture (profiles/r01g_tilepass_v7.md)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4": 244.9e6}
+# DRAM bytes of one 4-sweep tile-pass launch from the committed ncu captures (NOT measured in this run: `traffic_source`)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"cfg4": (244.9e6, "profiles/r01g_tilepass_v7.md: ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one launch"),
+                                "cfg5": (2392.4e6, "profiles/r02b_cfg5_batch.md: ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one launch")}
 
 
 # ---------------------------------------------------------------------------
@@ -463,7 +464,8 @@ def run_b200(args, w):
             "clocks": clk.summary(),
             "roofline": {"bound": "hbm", "kernel": "k_tilepass", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w.name) if sweeps_per_launch == 4.0 else None,
+                         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH[w.name][0] if w.name in NCU_TRAFFIC_BYTES_PER_LAUNCH and sweeps_per_launch == 4.0 and not args.L and not args.batch else None,
+                         "traffic_source": NCU_TRAFFIC_BYTES_PER_LAUNCH[w.name][1] if w.name in NCU_TRAFFIC_BYTES_PER_LAUNCH and sweeps_per_launch == 4.0 and not args.L and not args.batch else None,
                          "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": bytes_per_launch, "sweeps_per_launch": sweeps_per_launch,
                          "us_per_launch": launch_s * 1e6, "us_per_sweep": sweep_s * 1e6,

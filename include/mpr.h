@@ -291,7 +291,7 @@ mpr_status mpr_create_slab(mpr_ctx** out, const mpr_slab* h_slab, const float* d
  * order (in double), the random streams are those of the fp32 path (same Philox counters, the same 24-bit
  * uniforms, grid word 0).  Calls mirror the fp32 ones (same statuses, same ordering rules, mpr_params as is;
  * T is one temperature).  mpr64_predict / mpr64_predict_std: d_out device double [rows][cols].  Angles are
- * exchanged as device double [rows][cols].  Workspace: mpr64_query_workspace bytes (52.2 B per site), 256-byte aligned. */
+ * exchanged as device double [rows][cols].  Workspace: mpr64_query_workspace bytes (71.4 B per site), 256-byte aligned. */
 typedef struct mpr64_ctx mpr64_ctx; /* opaque */
 mpr_status mpr64_query_workspace(int rows, int cols, size_t* h_bytes);
 mpr_status mpr64_create(mpr64_ctx** out, int rows, int cols, const double* d_values, const uint8_t* d_sample_mask,
