@@ -47,6 +47,19 @@ def build_microbench(force: bool = False) -> str:
     return MICROBENCH_LIB
 
 
+CHECKED_LIB = os.path.join(_HERE, "libmpr_b200_checked.so")
+
+
+def build_checked(force: bool = False) -> str:
+    """The library with -DMPR_CHECKED: device-side assertions on every shared-memory and accumulator index of the tile
+    passes (a stand-in for compute-sanitizer memcheck where that is not available).  `tests/sanitizer_driver.py --lib`."""
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS]
+    if force or not os.path.exists(CHECKED_LIB) or any(os.path.getmtime(d) > os.path.getmtime(CHECKED_LIB) for d in deps):
+        subprocess.run([_nvcc(), *NVCC_FLAGS, "-DMPR_CHECKED", "-I", INCLUDE, "-o", CHECKED_LIB] +
+                       [os.path.join(CSRC, f) for f in SOURCES], check=True)
+    return CHECKED_LIB
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     build_microbench(force)
     if force or _stale():

@@ -14,6 +14,15 @@
 #include <cstdint>
 #include <cuda.h>
 #include <cuda_runtime.h>
+// -DMPR_CHECKED (build.build_checked(): libmpr_b200_checked.so): bounds checks of every shared-memory and accumulator
+// index of the tile pass as device-side assertions.  compute-sanitizer is closed on the GPU pool this was developed
+// on (profiles/r02d); tests/sanitizer_driver.py --lib <checked library> runs every kernel family through them.
+#ifdef MPR_CHECKED
+#include <cassert>
+#define MPR_CHECK(cond) assert(cond)
+#else
+#define MPR_CHECK(cond) ((void)0)
+#endif
 
 namespace mpr {
 
@@ -967,7 +976,11 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         // sweep sit in one basic block (independent instruction streams for the scheduler to interleave).
         auto update_two = [&](auto draw_tag, uint32_t eA, uint32_t eB) {
             constexpr int DRAW = decltype(draw_tag)::value;
+            MPR_CHECK(h.cbase + eA < d.max_entries && h.cbase + eB < d.max_entries);
             const uint32_t offA = Ec[eA], offB = Ec[eB];
+            // the site and its four neighbours lie in the rows that were loaded, and never in the frame's first or last column
+            MPR_CHECK(offA >= (uint32_t)((H - HR + 1) * FC + 1) && offA + (uint32_t)FC + 1u < (uint32_t)((H - HR + FRK) * FC));
+            MPR_CHECK(offB >= (uint32_t)((H - HR + 1) * FC + 1) && offB + (uint32_t)FC + 1u < (uint32_t)((H - HR + FRK) * FC));
             float2 vA = S[offA], vB = S[offB];
             const float2 upA = S[offA - FC], dnA = S[offA + FC], lfA = S[offA - 1], rtA = S[offA + 1];
             const float2 upB = S[offB - FC], dnB = S[offB + FC], lfB = S[offB - 1], rtB = S[offB + 1];
@@ -1075,6 +1088,8 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
                 if (!on[u]) continue;
                 const uint32_t i = i0 + (uint32_t)u * NT;
                 const uint32_t off = E[i < n0 ? i : e1 + (i - a1)];
+                MPR_CHECK(i < d.acc_stride && (i < n0 ? i : e1 + (i - a1)) < d.max_entries);
+                MPR_CHECK(off >= (uint32_t)(H * FC + H) && off < (uint32_t)((H + tg.TRc) * FC));      // a core site
                 const float phi = angle_of(S[off], d.inv_q), before = a_[u], after = before + phi;
                 acc[i] = after;
                 if (k > 1u) m2[i] = m_[u] + (phi - before * inv_km1) * (phi - after * inv_k);
@@ -1377,6 +1392,7 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, double x_p, float* __res
         const uint32_t off = E[i < n0 ? i : e1 + (i - a1)];
         const uint32_t lr = off / (uint32_t)d.FC, lc = off - lr * (uint32_t)d.FC;
         const uint32_t n = (uint32_t)(tg.r0 - d.H + (int)lr) * d.cols + (uint32_t)(tg.c0 - d.H + (int)lc);
+        MPR_CHECK(n < d.N && i < d.acc_stride && !is_fixed(bits, n));
         double sum = 0.0, count = 0.0;
         for (int c = 0; c < d.chains; ++c) {
             const int v = g + c * d.batch;

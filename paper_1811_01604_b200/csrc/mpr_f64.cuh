@@ -586,6 +586,7 @@ k64_tilepass(const __grid_constant__ CUtensorMap map_p0, const __grid_constant__
             const int off = Ec[e];
             const int lr = (int)(((uint32_t)off * dt.fc_inv) >> 24), lc = off - lr * FC;
             const int o = lr * FCH + (lc >> 1);
+            MPR_CHECK(lr >= 1 && lr + 1 < FR && lc >= 1 && lc + 1 < FC && (c ? base1 : 0u) + e < dt.max_entries);
             const double2 up = oth[o - FCH], dn = oth[o + FCH], lf = oth[o - 1 + (lc & 1)], rt = oth[o + (lc & 1)];
             const uint32_t site = (uint32_t)((tg.r0 - H + lr) * d.cols + (tg.c0 - H + lc));
             const uint4 x = philox4x32_10(site, t >> 1, 2u, 0u, d.rk0, d.rk1);

@@ -54,10 +54,13 @@ def run_fp32(rows, cols, batch=1, chains=1, q=0.5, or_mode=0, a=None, cap=25, M=
 
 
 def main():
+    if "--lib" in sys.argv:                  # e.g. the -DMPR_CHECKED build (paper_1811_01604_b200.build.build_checked())
+        mpr.LIB_PATH = os.path.abspath(sys.argv[sys.argv.index("--lib") + 1])
+        print("library:", mpr.LIB_PATH)
     print("one tile (in-pass equilibration):", run_fp32(64, 64, a=2.0))
     print("multi-tile, low tiles:", run_fp32(130, 150, a=3.0))
     print("multi-tile, short polynomials, width not a multiple of 4:", run_fp32(150, 131, a=30.0))
-    print("64-row tiles (batch fills the device):", run_fp32(256, 256, batch=8, a=12.0, cap=22, M=1, s=4))
+    print("64-row tiles (batch fills the device):", run_fp32(256, 256, batch=8, a=12.0, cap=22, M=2, s=4))
     print("chains:", run_fp32(96, 200, chains=3, a=2.0))
     print("general q:", run_fp32(140, 140, q=0.3, a=2.0))
     print("Eq. 6 as printed:", run_fp32(140, 140, or_mode=1, a=2.0))
@@ -74,6 +77,11 @@ def main():
     c64.set_angles(out[2])
     c64.sweep(2, 2.0, count=True)
     assert np.isfinite(c64.energy()) and all(bool(torch.isfinite(o).all()) for o in out)
+    c64.close()
+    c64 = mpr.Mpr64(dev(z.astype(np.float64)), dev(m))
+    c64.set_params(synth.choose_T(z, m), seed=7, M=2, sweeps_per_real=7).simulate()     # the double tile pass: 4 + 3 sweeps
+    c64.sweep(9, 3.0)
+    assert bool(torch.isfinite(c64.predict()).all())
     c64.close()
     print("double-precision path: ok")
     torch.cuda.synchronize()
