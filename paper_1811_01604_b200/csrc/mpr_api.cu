@@ -56,9 +56,18 @@ void choose_tiles(int batch, int rows, int cols, Geometry* g)
     // a batch that does not fill the device with 64-row tiles gets lower ones (same frame pitch), as low as still
     // fits one wave: more CTAs in flight, shorter half-sweeps (measured: 256^2 2.7 instead of 4.1 us per sweep)
     const long ntx64 = (cols + 63) / 64;
-    if ((long)batch * ntx64 * ((rows + 63) / 64) < RESIDENT_TILE_PASSES)
+    if ((long)batch * ntx64 * ((rows + 63) / 64) < RESIDENT_TILE_PASSES) {
         for (int tr = 16; tr < 64; tr += 8)
             if ((long)batch * ntx64 * ((rows + tr - 1) / tr) <= RESIDENT_TILE_PASSES) { TR = tr; break; }
+        // still room at 16 rows: narrower tiles too (a pass of such a grid lasts as long as ONE tile's 2K half-sweeps, so
+        // halving a tile's sites matters more than the halo it recomputes; measured on 256^2: 64 tiles of 16 x 64 34.2 ms
+        // per grid, 128 of 16 x 32 26.3 ms, 256 of 16 x 16 21.9 ms)
+        if (TR == 16)
+            for (int tc = 32; tc >= 16; tc /= 2) {
+                if ((long)batch * ((cols + tc - 1) / tc) * ((rows + 15) / 16) > RESIDENT_TILE_PASSES) break;
+                TC = tc;
+            }
+    }
 #ifdef MPR_EXPERIMENT_HOOKS
     if (const char* e = getenv("MPR_TILE")) {
         int a, b, c;
