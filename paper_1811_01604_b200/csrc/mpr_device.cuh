@@ -870,7 +870,9 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     // rows above S_load are never touched (an entry of ring <= 2K - 1 has its upper neighbour in ring <= 2K).
     const int HR = (int)row_halo, FRK = d.TR + 2 * HR;
     float2*   S_load = reinterpret_cast<float2*>(smem_raw);
-    float2*   S  = S_load - (H - HR) * FC;
+    uint32_t  s_shift = (uint32_t)((H - HR) * FC) * (uint32_t)sizeof(float2);
+    asm volatile("" : "+r"(s_shift));    // opaque, so that the shifted base is formed once (else the shift is redone per site)
+    float2*   S  = reinterpret_cast<float2*>(smem_raw - s_shift);
     uint2*    SP = reinterpret_cast<uint2*>(S_load + FRK * FC);
     uint16_t* E  = reinterpret_cast<uint16_t*>(SP + (d.use_spare ? d.max_entries : 0u));
 
