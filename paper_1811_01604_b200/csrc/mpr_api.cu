@@ -172,7 +172,7 @@ mpr_status fetch_states(mpr_ctx* ctx)
     return MPR_OK;
 }
 
-typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t);
+typedef void (*pass_kernel)(const CUtensorMap, const CUtensorMap, const Dev, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t, uint32_t);
 
 // fused = with the accepted count / energy reduction / done check compiled in (equilibration, counted sweeps);
 // std_fc = the frame pitch is the compile-time STD_FC (standard tile shape)
@@ -223,7 +223,9 @@ void note_a(mpr_ctx* ctx, double a_min)
 // flip = 0 / 1: read buffer ctx->cur ^ flip (known to the host); PER_GRID: each grid reads its own GridState::cur
 enum : uint32_t { PER_GRID = 2u };
 mpr_status halo_exchange(mpr_ctx* ctx, uint32_t buf);
-mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags, uint32_t real_no = 0, bool equil = false)
+// acc_every (with PASS_ACCUMULATE): the core is accumulated after every acc_every-th sweep of the pass (0: after the last)
+mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, uint32_t flags, uint32_t real_no = 0, bool equil = false,
+                       uint32_t acc_every = 0)
 {
     ctx->dirty = true;
     const bool fused = flags & (PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
@@ -259,7 +261,7 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
     ++ctx->launches;
     const CUtensorMap* maps0 = &ctx->map[0][row_halo / 2], *maps1 = &ctx->map[1][row_halo / 2];
     if (!cuda_ok(cudaLaunchKernelEx(&cfg, kern, *maps0, *maps1, d, K, t_off, src_sel, flags, pf_dist, real_no, row_halo,
-                                    (uint32_t)ctx->first),
+                                    (uint32_t)ctx->first, acc_every ? acc_every : K),
                  "tile pass launch")) return MPR_ERR_CUDA;
     return MPR_OK;
 }
@@ -810,9 +812,21 @@ mpr_status mpr_simulate(mpr_ctx* ctx)
     for (int g0 = 0; g0 < n_states && s == MPR_OK; g0 += group) {
         ctx->first = g0; ctx->active = n_states - g0 < group ? n_states - g0 : group;
         t_off = 0; flip = 0;
-        for (uint32_t j = 0; j < n_real && s == MPR_OK; ++j)
-            // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
-            s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE, j + 1u);   // realization number: realizations so far + j + 1
+        if (s_per < ctx->k_max) {
+            // realizations of fewer sweeps than a pass holds (the paper's s = 1, L210): several of them per launch, the
+            // core accumulated inside the pass after every s_per-th sweep (step 6.3)
+            const uint32_t per_pass = ctx->k_max / s_per;
+            for (uint32_t j = 0; j < n_real && s == MPR_OK; j += per_pass) {
+                const uint32_t r = n_real - j < per_pass ? n_real - j : per_pass, K = r * s_per;
+                s = launch_pass(ctx, K, t_off, flip, PASS_ACCUMULATE, j + 1u, false, s_per);
+                t_off += K; flip ^= 1u;
+                if (s == MPR_OK && ctx->slab) s = halo_exchange(ctx, ctx->cur ^ flip);
+            }
+        } else {
+            for (uint32_t j = 0; j < n_real && s == MPR_OK; ++j)
+                // s sweeps, the last pass also accumulates phi at the prediction sites (step 6.3)
+                s = launch_sweeps(ctx, s_per, &t_off, &flip, 0, PASS_ACCUMULATE, j + 1u);   // realization number: realizations so far + j + 1
+        }
     }
     ctx->first = 0; ctx->active = d.batch;
     if (s != MPR_OK) return s;

@@ -824,7 +824,7 @@ __device__ __forceinline__ double core_energy_warp(const Dev& d, const float2* S
 
 // what one half-sweep of a tile pass needs to know (tabulated per CTA, see k_tilepass)
 struct __align__(16) HalfSweep { uint32_t n, cbase, c1, flags; };   // entries to walk, list offset, Philox counter word 1, HS_*
-enum : uint32_t { HS_ODD = 1u, HS_FRESH = 2u, HS_STASH = 4u, HS_RENORM = 8u };
+enum : uint32_t { HS_ODD = 1u, HS_FRESH = 2u, HS_STASH = 4u, HS_RENORM = 8u, HS_ACC = 16u };   // bits 8: colour, 16..: realization offset
 constexpr int HS_CHUNK = 16;
 
 // how a half-sweep gets its random words: the stored second pair, a Philox draw of an even sweep whose second pair is
@@ -835,14 +835,14 @@ template <int M> struct DrawTag { static constexpr int value = M; };
 // EQUIL (a grid that is ONE tile, with FUSED): Alg. 2 step 5 runs inside the pass -- after every sweep the energy and
 // the accepted count are reduced in the CTA, thread 0 takes steps 5.2-5.5 (controller_step) and the CTA goes on with the
 // new proposal width or stops; K is then the most sweeps this launch may do.  Bit for bit the sweeps of the K = 1
-// passes with k_controller between them (every sweep renormalises, as a K = 1 pass does), without 2 launches per sweep.
+// passes with k_controller between them, without 2 launches per sweep.
 // MINB: CTAs per SM the registers are budgeted for: 3 for the K-sweep passes (their shared memory allows no more), 4 for
 // single-sweep passes (row halo 2, no stored random words: 49 KB), whose length is mostly a CTA's own latency
 template <bool QHALF, int ORMODE, bool FUSED, int FCT, bool SMALLD, bool EQUIL = false, int MINB = 3>
 __global__ void __launch_bounds__(TILE_THREADS, MINB)
 k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1, const Dev d,
            uint32_t K, uint32_t t_off, uint32_t src_sel, uint32_t flags, uint32_t pf_dist, uint32_t real_no, uint32_t row_halo,
-           uint32_t g_first)
+           uint32_t g_first, uint32_t acc_every)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t s_bar[2];       // [0] frame, [1] entry list
@@ -943,6 +943,41 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     mbar_wait(&s_bar[1], 0);
     mbar_wait(&s_bar[0], 0);
 
+    auto accumulate_core = [&](uint32_t k) {
+        // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites; and for the spread of the
+        // realizations (L212) the sum of squared deviations, updated from the running mean so that nothing cancels:
+        // m2 += (phi - mean_{k-1}) (phi - mean_k), k = number of this realization.
+        // The accumulators are kept per tile in the order of the tile's core entries, so that a pass touches only
+        // prediction sites' words, consecutive lanes consecutive words (and the tile's range was sent for at the start).
+        float* acc = d.acc + ((size_t)g * d.ntiles + tile) * d.acc_stride;
+        float* m2 = d.m2 + ((size_t)g * d.ntiles + tile) * d.acc_stride;
+        const float inv_km1 = k > 1u ? 1.0f / (float)(k - 1u) : 0.0f, inv_k = 1.0f / (float)k;
+        const uint32_t n0 = s_cle[0][0], a1 = colour1_base(n0), n_acc = a1 + s_cle[1][0], e1 = colour1_base(s_cle[0][MAX_H - 1]);
+        // position i of the tile's accumulators: colour 0's core entry i (i < n0), colour 1's core entry i - a1 (i >= a1)
+#pragma unroll 1
+        for (uint32_t i0 = tid; i0 < n_acc; i0 += 4u * NT) {
+            float a_[4], m_[4];
+            bool on[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t i = i0 + (uint32_t)u * NT;
+                on[u] = i < n_acc && (i < n0 || i >= a1);
+                if (on[u]) { a_[u] = acc[i]; m_[u] = k > 1u ? m2[i] : 0.0f; }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (!on[u]) continue;
+                const uint32_t i = i0 + (uint32_t)u * NT;
+                const uint32_t off = E[i < n0 ? i : e1 + (i - a1)];
+                MPR_CHECK(i < d.acc_stride && (i < n0 ? i : e1 + (i - a1)) < d.max_entries);
+                MPR_CHECK(off >= (uint32_t)(H * FC + H) && off < (uint32_t)((H + tg.TRc) * FC));      // a core site
+                const float phi = angle_of(S[off], d.inv_q), before = a_[u], after = before + phi;
+                acc[i] = after;
+                if (k > 1u) m2[i] = m_[u] + (phi - before * inv_km1) * (phi - after * inv_k);
+            }
+        }
+    };
+
     // half-sweep j = 2 s + c: colour c of sweep s (Alg. 1: colour 0, then colour 1).  What a half-sweep needs to
     // know is tabulated by one warp for 16 half-sweeps at a time (HalfSweep), so that the other warps do not redo it.
 #pragma unroll 1
@@ -952,14 +987,20 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
             const bool odd = t & 1u;
             const bool fresh = !odd || s == 0 || !use_spare;            // draw a new Philox block for (site, t >> 1)
             const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
-            // |v| = 1 against rounding drift: in the sweep whose result leaves the tile, and every 8th sweep of a long pass
-            const bool renorm = EQUIL || s + 1 == K || (s & 7u) == 7u;
+            // |v| = 1 against rounding drift, every fourth sweep BY THE GLOBAL SWEEP INDEX: which sweeps renormalise does
+            // not depend on how they are grouped into passes, so neither does any bit of the state (a tile's halo
+            // sites and its neighbour's core sites must renormalise alike anyway)
+            const bool renorm = (t & 3u) == 3u;
+            // step 6.3 inside the pass: after every acc_every-th sweep the core is accumulated (several realizations of
+            // fewer than K sweeps per launch)
+            const bool acc = (flags & PASS_ACCUMULATE) && c == 1u && (s + 1u) % acc_every == 0u;
             const uint32_t R = 2u * K - 1u - j;                          // rings still needed: 0 .. R
             HalfSweep h;
             h.n = s_cle[c][R < (uint32_t)MAX_H ? R : (uint32_t)MAX_H - 1u];
             h.cbase = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
             h.c1 = t >> 1;
-            h.flags = (odd ? HS_ODD : 0u) | (fresh ? HS_FRESH : 0u) | (stash ? HS_STASH : 0u) | (renorm ? HS_RENORM : 0u) | (c << 8);
+            h.flags = (odd ? HS_ODD : 0u) | (fresh ? HS_FRESH : 0u) | (stash ? HS_STASH : 0u) | (renorm ? HS_RENORM : 0u) |
+                      (acc ? HS_ACC : 0u) | (c << 8) | (acc ? ((s + 1u) / acc_every - 1u) << 16 : 0u);
             s_hs[tid] = h;
         }
         __syncthreads();
@@ -969,7 +1010,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         const HalfSweep h = s_hs[jj];
         const bool odd = h.flags & HS_ODD, fresh = h.flags & HS_FRESH, stash = h.flags & HS_STASH, renorm = h.flags & HS_RENORM;
         const uint32_t n = h.n, tc1 = h.c1;
-        const uint32_t n_core = FUSED ? s_cle[h.flags >> 8][0] : 0u;
+        const uint32_t n_core = FUSED ? s_cle[(h.flags >> 8) & 1u][0] : 0u;
         const uint16_t* Ec = E + h.cbase;
         uint2* SPc = SP + h.cbase;
 
@@ -1029,8 +1070,12 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
         else if (!odd && stash) half_sweep(DrawTag<DRAW_EVEN_STORE>{});
         else half_sweep(DrawTag<DRAW_ANY>{});
         __syncthreads();
+        if (h.flags & HS_ACC) {                 // a realization is complete: its state into the sums (reads the core only)
+            accumulate_core(st.realizations + real_no + (h.flags >> 16));
+            __syncthreads();                    // before the next half-sweep writes core sites
+        }
         if constexpr (EQUIL) {
-            if (h.flags >> 8) {                 // a whole sweep is done (colour 1 was its second half): steps 5.2-5.5
+            if ((h.flags >> 8) & 1u) {          // a whole sweep is done (colour 1 was its second half): steps 5.2-5.5
                 n_accepted = __reduce_add_sync(0xFFFFFFFFu, n_accepted);
                 if (lane == 0 && n_accepted) atomicAdd(&s_accepted, n_accepted);
                 n_accepted = 0;
@@ -1063,41 +1108,6 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     for (int lr = warp + NW * lane; lr < tg.TRc; lr += NW * 32)
         bulk_store(dst + (size_t)(tg.r0 + lr) * d.pitch + tg.c0, S + (H + lr) * FC + H, row_bytes);
 
-    if (flags & PASS_ACCUMULATE) {
-        // a7 (Alg. 2 step 6, L207-211): acc += phi at the core's prediction sites; and for the spread of the
-        // realizations (L212) the sum of squared deviations, updated from the running mean so that nothing cancels:
-        // m2 += (phi - mean_{k-1}) (phi - mean_k), k = number of this realization.
-        // The accumulators are kept per tile in the order of the tile's core entries, so that a pass touches only
-        // prediction sites' words, consecutive lanes consecutive words (and the tile's range was sent for at the start).
-        float* acc = d.acc + ((size_t)g * d.ntiles + tile) * d.acc_stride;
-        float* m2 = d.m2 + ((size_t)g * d.ntiles + tile) * d.acc_stride;
-        const uint32_t k = st.realizations + real_no;
-        const float inv_km1 = k > 1u ? 1.0f / (float)(k - 1u) : 0.0f, inv_k = 1.0f / (float)k;
-        const uint32_t n0 = s_cle[0][0], a1 = colour1_base(n0), n_acc = a1 + s_cle[1][0], e1 = colour1_base(s_cle[0][MAX_H - 1]);
-        // position i of the tile's accumulators: colour 0's core entry i (i < n0), colour 1's core entry i - a1 (i >= a1)
-#pragma unroll 1
-        for (uint32_t i0 = tid; i0 < n_acc; i0 += 4u * NT) {
-            float a_[4], m_[4];
-            bool on[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const uint32_t i = i0 + (uint32_t)u * NT;
-                on[u] = i < n_acc && (i < n0 || i >= a1);
-                if (on[u]) { a_[u] = acc[i]; m_[u] = k > 1u ? m2[i] : 0.0f; }
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (!on[u]) continue;
-                const uint32_t i = i0 + (uint32_t)u * NT;
-                const uint32_t off = E[i < n0 ? i : e1 + (i - a1)];
-                MPR_CHECK(i < d.acc_stride && (i < n0 ? i : e1 + (i - a1)) < d.max_entries);
-                MPR_CHECK(off >= (uint32_t)(H * FC + H) && off < (uint32_t)((H + tg.TRc) * FC));      // a core site
-                const float phi = angle_of(S[off], d.inv_q), before = a_[u], after = before + phi;
-                acc[i] = after;
-                if (k > 1u) m2[i] = m_[u] + (phi - before * inv_km1) * (phi - after * inv_k);
-            }
-        }
-    }
     if (FUSED && !EQUIL) {
         if (count) {
             n_accepted = __reduce_add_sync(0xFFFFFFFFu, n_accepted);

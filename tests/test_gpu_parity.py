@@ -1147,3 +1147,32 @@ def test_cfg5_full_batch_t1_t2_t3(torch_cuda, mpr, orc):
     ctx.set_params(Ts, **kw).equilibrate().simulate()
     assert np.array_equal(ctx.predict().cpu().numpy().view(np.uint32), pred.view(np.uint32))
     ctx.close()
+
+
+@pytest.mark.parametrize("s", [1, 2, 3, 5])
+def test_pass_depth_changes_no_bit(torch_cuda, mpr, s):
+    """How the sweeps are grouped into tile passes is invisible in the result: halo sites are recomputed bit for bit (the
+    random numbers are keyed by site and sweep) and the renormalisation of |v| goes by the global sweep index.  Step 6 with
+    s sweeps per realization at pass depths 4 (several realizations per launch when s < 4, accumulated inside the pass),
+    3, 2 and 1: the same prediction, spread and final state, bit for bit."""
+    torch = torch_cuda
+    z, m = _field(200, 330, 7.0, 0.5, 4300)
+    T = synth.choose_T(z, m)
+    ctx = mpr.Mpr(_dev(torch, z), _dev(torch, m))
+    out = []
+    for depth in (0, 3, 2, 1):
+        ctx.set_pass_depth(depth)
+        ctx.set_params(T, seed=12, equil_cap=40, M=7, sweeps_per_real=s).equilibrate()
+        l0 = ctx.launch_count()
+        ctx.simulate()
+        launches = ctx.launch_count() - l0
+        st = ctx.get_stats()[0]
+        out.append((ctx.predict().cpu().numpy(), ctx.predict_std().cpu().numpy(), ctx.get_angles().cpu().numpy(), st.t, st.realizations,
+                    launches))
+    for o in out[1:]:
+        assert o[3:5] == out[0][3:5] == (out[0][3], 7)
+        for a, b in zip(o[:3], out[0][:3]):
+            assert np.array_equal(a.view(np.uint32), b.view(np.uint32))
+    if s < 4:
+        assert out[0][5] < out[3][5]          # fewer launches at depth 4 than at depth 1
+    ctx.close()
