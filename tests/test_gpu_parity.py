@@ -353,7 +353,7 @@ def _diamond(seed_mask, radius):
 def _compare_n_sweeps(orc, ctx, phi0, mask, q, T, a, seed, t, n, or_mode=0, g_list=(0,), tol=TOL_RAD, margin_thr=1e-3):
     """n sweeps in ONE mpr_sweep call without the accepted count (h_accepted = NULL): the NON-fused tile pass at the
     context's pass depth K -- halo rings 2K-1 .. 0, the ring-prefix walk of the entry lists, the stashed second
-    Philox pair, renormalisation in the last sweep of a pass only, and for a >= q pi / 0.2 the short sin / cos
+    Philox pair, the renormalising sweeps, and for a >= q pi / 0.2 the short sin / cos
     polynomials -- against n oracle sweeps (Alg. 1) from the same state.
 
     A decision that falls the other way on the two sides (Metropolis accept, interval-end test) changes the site and,
