@@ -750,8 +750,14 @@ mpr_status mpr_equilibrate(mpr_ctx* ctx)
                 // 5.2, 5.4, 5.5 and commits the sweep (t, buffer swap) for the grids still running
                 mpr_status s = launch_pass(ctx, 1, 0, PER_GRID, PASS_COUNT | PASS_ENERGY | PASS_CHECK_DONE);
                 if (s != MPR_OK) return s;
-                k_controller<<<d.batch, REDUCE_THREADS, 0, ctx->stream>>>(d);
-                CU_LAUNCH();
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3(d.batch); cfg.blockDim = dim3(REDUCE_THREADS); cfg.stream = ctx->stream;
+                cudaLaunchAttribute attr[1];
+                attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                attr[0].val.programmaticStreamSerializationAllowed = 1;
+                cfg.attrs = attr; cfg.numAttrs = ctx->no_pdl ? 0 : 1;
+                ++ctx->launches;
+                if (!cuda_ok(cudaLaunchKernelEx(&cfg, k_controller, d), "controller launch")) return MPR_ERR_CUDA;
             }
             issued += chunk;
             bool all = false;

@@ -1274,6 +1274,10 @@ __global__ void k_sample_energy_finish(Dev d, int n_partials)
 // ---------------------------------------------------------------------------
 __global__ void k_controller(Dev d)
 {
+    // launched with programmatic stream serialization behind a fused tile pass: it may be resident before that pass has
+    // drained (and lets the next pass load its tile lists meanwhile), but reads nothing before the pass is complete
+    griddep_launch_dependents();
+    griddep_wait();
     const int g = blockIdx.x;
     GridState& s = d.states[g];
     if (s.done) return;
