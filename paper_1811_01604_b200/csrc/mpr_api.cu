@@ -252,7 +252,7 @@ mpr_status launch_pass(mpr_ctx* ctx, uint32_t K, uint32_t t_off, uint32_t flip, 
     // programmatic stream serialization: this pass's CTAs may start (and load their tile lists) while the last
     // CTAs of the previous kernel still run; k_tilepass waits for that kernel before it reads any result of it
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(ctx->d.ntiles, ctx->active); cfg.blockDim = dim3(TILE_THREADS);      // states first .. first + active - 1
+    cfg.gridDim = dim3(ctx->d.ntx, ctx->d.nty, ctx->active); cfg.blockDim = dim3(TILE_THREADS);      // states first .. first + active - 1
     cfg.dynamicSmemBytes = smem; cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;

@@ -373,13 +373,17 @@ __global__ void __launch_bounds__(256) k_transform(Dev d, const float* __restric
 // ---------------------------------------------------------------------------
 struct TileGeom { int r0, c0, TRc, TCc; };
 
-__device__ __forceinline__ TileGeom tile_geom(const Dev& d, int tile)
+__device__ __forceinline__ TileGeom tile_geom_xy(const Dev& d, int tx, int ty)
 {
     TileGeom t;
-    const int ty = tile / d.ntx, tx = tile - ty * d.ntx;
     t.r0 = ty * d.TR; t.c0 = tx * d.TC;
     t.TRc = min(d.TR, d.rows - t.r0); t.TCc = min(d.TC, d.cols - t.c0);
     return t;
+}
+__device__ __forceinline__ TileGeom tile_geom(const Dev& d, int tile)
+{
+    const int ty = tile / d.ntx;
+    return tile_geom_xy(d, tile - ty * d.ntx, ty);
 }
 
 // class of frame site (lr, lc): returns false if outside the grid, fixed, or on the outermost ring
@@ -853,7 +857,8 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
 
     constexpr int NT = TILE_THREADS, NW = TILE_THREADS / 32;
     static_assert(TILE_THREADS >= 96 + 2 * MAX_H && TILE_THREADS >= HS_CHUNK, "the prologue gives warps 0-3 their own jobs");
-    const int tile = blockIdx.x, g = (int)(blockIdx.y + g_first);   // g: state (grid and chain), gd: the grid whose data it shares
+    // grid = (tiles across, tiles down, states): the tile's place without a division at the head of every CTA's life
+    const int tile = (int)(blockIdx.y * gridDim.x + blockIdx.x), g = (int)(blockIdx.z + g_first);   // g: state (grid and chain), gd: the grid whose data it shares
     const int gd = g < d.batch ? g : g % d.batch;
     const GridState& st = d.states[g];
     // Programmatic dependent launch: the next kernel of the stream may start its CTAs while the last of this
@@ -877,7 +882,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     uint16_t* E  = reinterpret_cast<uint16_t*>(SP + (d.use_spare ? d.max_entries : 0u));
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const TileGeom tg = tile_geom(d, tile);
+    const TileGeom tg = tile_geom_xy(d, (int)blockIdx.x, (int)blockIdx.y);
     const TileMeta& meta = d.tile_meta[(size_t)gd * d.ntiles + tile];
 
     // three warps start the tile: warp 1 the entry list (needs the tile's counts from global memory first), and,
@@ -940,6 +945,32 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     const bool use_spare = d.use_spare;
     uint32_t n_accepted = 0;
     __syncthreads();
+    // What a half-sweep needs to know is tabulated by one warp for 16 half-sweeps at a time (HalfSweep), so that the other
+    // warps do not redo it; the first 16 while the frame is still on its way.
+    auto fill_table = [&](uint32_t j0) {
+        if (tid < HS_CHUNK && j0 + tid < 2u * K) {
+            const uint32_t j = j0 + tid, s = j >> 1, c = j & 1u, t = t0 + s;
+            const bool odd = t & 1u;
+            const bool fresh = !odd || s == 0 || !use_spare;            // draw a new Philox block for (site, t >> 1)
+            const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
+            // |v| = 1 against rounding drift, every fourth sweep BY THE GLOBAL SWEEP INDEX: which sweeps renormalise does
+            // not depend on how they are grouped into passes, so neither does any bit of the state (a tile's halo
+            // sites and its neighbour's core sites must renormalise alike anyway)
+            const bool renorm = (t & 3u) == 3u;
+            // step 6.3 inside the pass: after every acc_every-th sweep the core is accumulated (several realizations of
+            // fewer than K sweeps per launch)
+            const bool acc = (flags & PASS_ACCUMULATE) && c == 1u && (s + 1u) % acc_every == 0u;
+            const uint32_t R = 2u * K - 1u - j;                          // rings still needed: 0 .. R
+            HalfSweep h;
+            h.n = s_cle[c][R < (uint32_t)MAX_H ? R : (uint32_t)MAX_H - 1u];
+            h.cbase = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
+            h.c1 = t >> 1;
+            h.flags = (odd ? HS_ODD : 0u) | (fresh ? HS_FRESH : 0u) | (stash ? HS_STASH : 0u) | (renorm ? HS_RENORM : 0u) |
+                      (acc ? HS_ACC : 0u) | (c << 8) | (acc ? ((s + 1u) / acc_every - 1u) << 16 : 0u);
+            s_hs[tid] = h;
+        }
+    };
+    fill_table(0u);
     mbar_wait(&s_bar[1], 0);
     mbar_wait(&s_bar[0], 0);
 
@@ -982,27 +1013,7 @@ k_tilepass(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUt
     // know is tabulated by one warp for 16 half-sweeps at a time (HalfSweep), so that the other warps do not redo it.
 #pragma unroll 1
     for (uint32_t j0 = 0; j0 < 2u * K && !(EQUIL && finished); j0 += HS_CHUNK) {
-        if (tid < HS_CHUNK && j0 + tid < 2u * K) {
-            const uint32_t j = j0 + tid, s = j >> 1, c = j & 1u, t = t0 + s;
-            const bool odd = t & 1u;
-            const bool fresh = !odd || s == 0 || !use_spare;            // draw a new Philox block for (site, t >> 1)
-            const bool stash = use_spare && !odd && s + 1 < K;          // keep words 2,3 for sweep t + 1
-            // |v| = 1 against rounding drift, every fourth sweep BY THE GLOBAL SWEEP INDEX: which sweeps renormalise does
-            // not depend on how they are grouped into passes, so neither does any bit of the state (a tile's halo
-            // sites and its neighbour's core sites must renormalise alike anyway)
-            const bool renorm = (t & 3u) == 3u;
-            // step 6.3 inside the pass: after every acc_every-th sweep the core is accumulated (several realizations of
-            // fewer than K sweeps per launch)
-            const bool acc = (flags & PASS_ACCUMULATE) && c == 1u && (s + 1u) % acc_every == 0u;
-            const uint32_t R = 2u * K - 1u - j;                          // rings still needed: 0 .. R
-            HalfSweep h;
-            h.n = s_cle[c][R < (uint32_t)MAX_H ? R : (uint32_t)MAX_H - 1u];
-            h.cbase = c ? colour1_base(s_cle[0][MAX_H - 1]) : 0u;
-            h.c1 = t >> 1;
-            h.flags = (odd ? HS_ODD : 0u) | (fresh ? HS_FRESH : 0u) | (stash ? HS_STASH : 0u) | (renorm ? HS_RENORM : 0u) |
-                      (acc ? HS_ACC : 0u) | (c << 8) | (acc ? ((s + 1u) / acc_every - 1u) << 16 : 0u);
-            s_hs[tid] = h;
-        }
+        if (j0) fill_table(j0);
         __syncthreads();
         const uint32_t j_end = min(2u * K - j0, (uint32_t)HS_CHUNK);
 #pragma unroll 1
