@@ -51,6 +51,9 @@ def parse_args():
     ap.add_argument("--sfu-peak", action="store_true",
                     help="run the pipe-rate micro-benchmarks (MUFU / FFMA / FFMA2 / IMAD.WIDE / LOP3 / IMAD) with the SM clock "
                          "held during each, print one JSON line and exit (BASELINE.md section 4)")
+    ap.add_argument("--probe", action="store_true",
+                    help="time the kinds of pass on the workload's equilibrated state (K-sweep pass, single-sweep pass, realization "
+                         "sweep with s = 1, equilibration sweep, both precisions), print one JSON line and exit (profiles/r02c, r02f)")
     ap.add_argument("--no-f64", action="store_true",
                     help="skip the double-precision run of the same workload (extra key 'double_precision', not in the step)")
     return ap.parse_args()
@@ -178,6 +181,58 @@ def run_sfu_peak():
                               "warp_instr_per_clk_per_subpartition": per_clk_sm / 128.0 if per_clk_sm else None}
     out["sfu_peak_per_s"] = min(out["rates"]["mufu_ex2"]["per_s"], out["rates"]["mufu_rcp"]["per_s"])
     out["sfu_peak_used_by_bench"] = SFU_PEAK_PER_S
+    print(json.dumps(out))
+
+
+# ---------------------------------------------------------------------------
+# the kinds of pass, timed one by one (profiles/r02c, r02f)
+# ---------------------------------------------------------------------------
+def run_probe(args, w):
+    """CUDA events around back-to-back calls through the C ABI on the workload's equilibrated state (best of three):
+    mpr_sweep at the default pass depth and at depth 1, mpr_simulate with one sweep per realization, mpr_equilibrate, and
+    the double-precision path's tile pass and half-sweep kernels."""
+    import torch
+    from paper_1811_01604_b200 import mpr
+    dev = torch.device("cuda", 0)
+    dv, dm = torch.from_numpy(w.truth).to(dev), torch.from_numpy(w.mask).to(dev)
+    T = [float(x) for x in w.T]
+    st = torch.cuda.current_stream(dev)
+
+    def timed(fn, per):
+        best = float("inf")
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st); fn(); e1.record(st); e1.synchronize()
+            best = min(best, e0.elapsed_time(e1) * 1e3 / per)
+        return best
+
+    ctx = mpr.Mpr(dv, dm)
+    prm = dict(seed=w.seed, q=w.q, equil_cap=w.equil_cap)
+    out = {"workload": w.name, "rows": w.rows, "cols": w.cols, "batch": w.batch, "tiling": ctx.get_tiling()}
+    out["us_per_equilibration_sweep"] = timed(lambda: ctx.set_params(T, **prm).equilibrate(), 1.0)     # divided below
+    stats = ctx.get_stats()
+    n_eq = max(s.equil_sweeps for s in stats)
+    out["equil_sweeps"] = [s.equil_sweeps for s in stats][:8]
+    out["us_per_equilibration_sweep"] /= n_eq            # includes mpr_set_params (one memset and one init kernel)
+    a = float(np.mean([s.a for s in stats]))
+    ctx.sweep(8, a)
+    out["us_per_sweep_k4_pass"] = timed(lambda: ctx.sweep(96, a), 96)
+    ctx.set_pass_depth(1)
+    out["us_per_sweep_single_sweep_pass"] = timed(lambda: ctx.sweep(32, a), 32)
+    ctx.set_pass_depth(0)
+    ctx.set_params(T, M=32, sweeps_per_real=1, equil_cap=0, **{k: v for k, v in prm.items() if k != "equil_cap"})
+    ctx.sweep(4, a)
+    ctx.simulate()
+    out["us_per_realization_s1"] = timed(lambda: ctx.simulate(), 32)
+    ctx.close()
+    if not args.no_f64:
+        c64 = mpr.Mpr64(torch.from_numpy(w.truth[0].astype(np.float64)).to(dev), dm[0])
+        c64.set_params(T[0], **prm).equilibrate()
+        a64 = c64.get_stats().a
+        c64.sweep(8, a64)
+        out["f64_us_per_sweep_tile_pass"] = timed(lambda: c64.sweep(32, a64), 32)
+        out["f64_us_per_sweep_halfsweep_kernels"] = timed(lambda: c64.sweep(8, a64, count=True), 8)
+        c64.close()
     print(json.dumps(out))
 
 
@@ -517,6 +572,10 @@ def main():
     if args.impl == "reference" and rank != 0:
         return
     w = synth.make_workload(args.workload, batch=args.batch, L=args.L)
+    if args.probe:
+        if rank == 0:
+            run_probe(args, w)
+        return
     if args.impl == "reference":
         run_reference(args, w)
     else:
