@@ -534,7 +534,10 @@ mpr_status create_impl(mpr_ctx** out, int batch, int chains, int rows, int cols,
             have = fill_smem;
         }
     }
-    k_tile_fill<<<dim3(g.ntiles, batch), 256, fill_smem, s>>>(d);
+    // the lists' order: fitted group by group by a serial walk (fewest bank conflicts) when the batch fills the device and
+    // the sweeps are bound by throughput; in closed form (k_tile_fill_rounds) when it does not
+    if ((long)(batch * chains) * g.ntiles >= RESIDENT_TILE_PASSES) k_tile_fill<<<dim3(g.ntiles, batch), 256, fill_smem, s>>>(d);
+    else k_tile_fill_rounds<<<dim3(g.ntiles, batch), 256, 0, s>>>(d);
     ctx->launches += 7;
     if (!cuda_ok(cudaGetLastError(), "create kernels")) return fail(MPR_ERR_CUDA);
     st = fetch_states(ctx);
