@@ -54,7 +54,8 @@ typedef enum {
     MPR_ERR_WORKSPACE = 7,        /* workspace too small or misaligned (256 B) */
     MPR_ERR_CUDA = 8,             /* a CUDA runtime call failed; see mpr_last_cuda_error */
     MPR_ERR_UNSUPPORTED = 9,      /* valid per the paper but not built (or_mode 1 with q != 1/2) */
-    MPR_ERR_COMM = 10             /* a communication callback of a slab context returned non-zero */
+    MPR_ERR_COMM = 10,            /* a communication callback of a slab context returned non-zero */
+    MPR_ERR_TOO_LARGE = 11        /* a size beyond the fixed scratch of the allocation-free entry point */
 } mpr_status;
 
 /* Alg. 2 step 1 parameters.  POD, host memory. */
@@ -310,6 +311,26 @@ mpr_status mpr64_energy(mpr64_ctx* ctx, double* h_e_per_bond);
 mpr_status mpr64_get_transform(mpr64_ctx* ctx, double* h_zmin, double* h_zmax);
 mpr_status mpr64_get_stats(mpr64_ctx* ctx, mpr_stats* h_out);          /* z_min / z_max rounded to float here */
 mpr_status mpr64_get_launch_count(mpr64_ctx* ctx, uint64_t* h_count);
+
+/* ---- allocation-free entry point ----
+ * For callers that can neither call cudaMalloc nor hand over a workspace (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid allocation): the energy per bond e = H / N_GP of Eq. 2 (the quantity
+ * Alg. 2 step 5.3 tracks, L199) of an angle field in device memory, without a context.  mpr_energy keeps its partial
+ * sums in the caller's workspace; this variant keeps one partial per grid row in a file-scope `static __device__` array
+ * of the library: MPR_NOALLOC_MAX_ROWS doubles + a counter = 128 KB + 256 B, held by every GPU that loads the library
+ * until the process exits.  The call makes no cudaMalloc, cudaFree or allocating library call.
+ *   d_phi         device float [rows][cols], angles in [0, 2 pi] (sample and prediction sites alike: every bond counts)
+ *   q             0 < q <= 1/2
+ *   d_e_per_bond  device double [1]: receives e; written when the work enqueued on cuda_stream is done
+ * Asynchronous (enqueues one 4-byte memset of the counter and one kernel on cuda_stream; no synchronisation).
+ * rows > MPR_NOALLOC_MAX_ROWS is MPR_ERR_TOO_LARGE (mpr_last_cuda_error names the limit); other bad arguments
+ * (null pointers, rows or cols < 2, cols > 65534, q out of range, d_phi not device memory) MPR_ERR_ARG.
+ * The scratch is SHARED by every call and keeps the last call's contents: what must start at zero is cleared by the call
+ * itself, but calls that overlap on the GPU (other streams, other host threads) race on it -- serialise them.  The first
+ * call on a device looks the array's address up (cudaGetSymbolAddress); make that call outside a graph capture. */
+#define MPR_NOALLOC_MAX_ROWS 16384
+mpr_status mpr_energy_of_angles_noalloc(const float* d_phi, int rows, int cols, double q, double* d_e_per_bond,
+                                        void* cuda_stream);
 
 /* ---- diagnostic / test / checkpoint surface ---- */
 

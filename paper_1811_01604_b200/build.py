@@ -14,7 +14,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libmpr_b200.so")
 SOURCES = ["mpr_api.cu"]
-HEADERS = ["mpr_device.cuh", "mpr_f64.cuh", "mpr_f64_api.inl"]
+HEADERS = ["mpr_device.cuh", "mpr_f64.cuh", "mpr_f64_api.inl", "mpr_noalloc.inl"]
 # pipe-rate micro-benchmarks behind `bench.py --sfu-peak` (the roofline's measured denominators); not part of the MPR library
 MICROBENCH_LIB = os.path.join(_HERE, "libmpr_microbench.so")
 MICROBENCH_SOURCES = ["mpr_microbench.cu"]

@@ -383,6 +383,7 @@ const char* mpr_status_string(mpr_status s)
     case MPR_ERR_CUDA: return "CUDA error";
     case MPR_ERR_UNSUPPORTED: return "parameter combination not supported";
     case MPR_ERR_COMM: return "a communication callback of a slab context failed";
+    case MPR_ERR_TOO_LARGE: return "size beyond the fixed scratch of the allocation-free entry point";
     }
     return "unknown status";
 }
@@ -1263,3 +1264,4 @@ mpr_status mpr_get_tiling(mpr_ctx* ctx, int* h_tile_rows, int* h_tile_cols, int*
 }  // extern "C"
 
 #include "mpr_f64_api.inl"
+#include "mpr_noalloc.inl"

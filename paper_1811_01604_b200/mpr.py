@@ -22,8 +22,9 @@ LIB_PATH = os.path.join(_HERE, "libmpr_b200.so")
 STATUS_NAMES = {
     0: "MPR_OK", 1: "MPR_ERR_ARG", 2: "MPR_ERR_NO_SAMPLES", 3: "MPR_ERR_NO_FREE",
     4: "MPR_ERR_DEGENERATE_RANGE", 5: "MPR_ERR_NONFINITE", 6: "MPR_ERR_STATE",
-    7: "MPR_ERR_WORKSPACE", 8: "MPR_ERR_CUDA", 9: "MPR_ERR_UNSUPPORTED", 10: "MPR_ERR_COMM",
+    7: "MPR_ERR_WORKSPACE", 8: "MPR_ERR_CUDA", 9: "MPR_ERR_UNSUPPORTED", 10: "MPR_ERR_COMM", 11: "MPR_ERR_TOO_LARGE",
 }
+NOALLOC_MAX_ROWS = 16384        # MPR_NOALLOC_MAX_ROWS of include/mpr.h
 
 # every symbol include/mpr.h declares
 EXPORTS = (
@@ -36,7 +37,7 @@ EXPORTS = (
     "mpr_predict_quantile", "mpr_set_pass_depth", "mpr_get_tiling",
     "mpr_default_ladder", "mpr_infer_temperature_auto", "mpr_set_grid_group",
     "mpr_slab_halo_bytes", "mpr_slab_local_rows", "mpr_query_workspace_slab", "mpr_create_slab",
-    "mpr_query_workspace_learn_q", "mpr_learn_q",
+    "mpr_query_workspace_learn_q", "mpr_learn_q", "mpr_energy_of_angles_noalloc",
     "mpr64_query_workspace", "mpr64_create", "mpr64_set_params", "mpr64_equilibrate", "mpr64_simulate", "mpr64_predict",
     "mpr64_predict_std", "mpr64_destroy", "mpr64_get_angles", "mpr64_set_angles", "mpr64_set_sweep_index", "mpr64_sweep",
     "mpr64_energy", "mpr64_get_transform", "mpr64_get_stats", "mpr64_get_launch_count",
@@ -131,6 +132,7 @@ def lib():
         L.mpr_slab_local_rows.argtypes = [C.POINTER(mpr_slab), C.POINTER(i), C.POINTER(i)]
         L.mpr_query_workspace_slab.argtypes = [C.POINTER(mpr_slab), C.POINTER(sz)]
         L.mpr_create_slab.argtypes = [C.POINTER(vp), C.POINTER(mpr_slab), vp, vp, vp, sz, vp]
+        L.mpr_energy_of_angles_noalloc.argtypes = [vp, i, i, C.c_double, vp, vp]
         L.mpr_query_workspace_learn_q.argtypes = [i, i, C.POINTER(sz)]
         L.mpr_learn_q.argtypes = [i, i, vp, vp, C.POINTER(mpr_params), C.POINTER(C.c_float), i, C.c_double, vp, sz, vp,
                                   C.POINTER(C.c_float), C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -159,7 +161,7 @@ def lib():
 
 def _check(status: int, where: str):
     if status != 0:
-        detail = lib().mpr_last_cuda_error().decode() if status == 8 else lib().mpr_status_string(status).decode()
+        detail = lib().mpr_last_cuda_error().decode() if status in (8, 11) else lib().mpr_status_string(status).decode()
         raise MprError(status, where, detail)
 
 
@@ -665,6 +667,22 @@ def infer_T(ctx: "Mpr", n_meas: int = 100, ladder=None, return_e_s: bool = False
     if return_e_s:
         return [float(x) for x in T_hat], [float(x) for x in e_s]
     return [float(x) for x in T_hat]
+
+
+def energy_of_angles_noalloc(phi, q: float = 0.5, out=None, rows: int | None = None, cols: int | None = None):
+    """mpr_energy_of_angles_noalloc: energy per bond of the angle field `phi` (float32 CUDA tensor [rows, cols]) into
+    `out` (float64 CUDA tensor of one element, made here when None: the CALLER's allocation; the library makes none).
+    Asynchronous on the current stream.  `rows` / `cols` override the tensor's shape (tests of the size check)."""
+    import torch
+    if not phi.is_cuda or phi.dtype != torch.float32 or phi.dim() != 2 or not phi.is_contiguous():
+        raise ValueError("phi: a contiguous float32 CUDA tensor [rows, cols]")
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=phi.device)
+    r, c = (int(x) for x in phi.shape)
+    stream = torch.cuda.current_stream(phi.device)
+    _check(lib().mpr_energy_of_angles_noalloc(phi.data_ptr(), r if rows is None else int(rows), c if cols is None else int(cols),
+                                              float(q), out.data_ptr(), stream.cuda_stream), "mpr_energy_of_angles_noalloc")
+    return out
 
 
 def learn_q(values, sample_mask, qs, holdout_fraction: float = 0.2, params: mpr_params | None = None, **overrides):

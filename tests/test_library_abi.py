@@ -79,11 +79,11 @@ def test_null_and_misuse_are_errors_not_crashes(lib):
 
 def test_status_strings(lib):
     seen = set()
-    for code in range(11):
+    for code in range(12):
         s = lib.mpr_status_string(code).decode()
         assert s and s != "unknown status"
         seen.add(s)
-    assert len(seen) == 11 and set(mpr.STATUS_NAMES) == set(range(11))
+    assert len(seen) == 12 and set(mpr.STATUS_NAMES) == set(range(12))
     assert lib.mpr_status_string(99).decode() == "unknown status"
 
 
