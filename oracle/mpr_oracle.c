@@ -54,6 +54,12 @@ typedef float real_t;
 #define ORC_TWO_PI_F 6.28318530717958647692f
 #endif
 static const double TWO_PI = (double)ORC_TWO_PI_F;
+
+/* The rows of one colour are swept by OpenMP threads only on grids of at least 4096 sites: a parallel region costs
+ * microseconds to milliseconds (on a busy or oversubscribed host), far more than a sweep of the tiny grids the pins use.
+ * Scheduling only: the sites of a colour are independent (L261-265), so the result does not depend on the thread
+ * count (pinned: test_sweep_independent_of_thread_count). */
+#define ORC_PARALLEL(rows, cols) ((long)(rows) * (long)(cols) >= 4096L)
 int orc_real_bytes(void) { return (int)sizeof(real_t); }
 
 /* ------------------------------------------------------------------------
@@ -228,7 +234,7 @@ uint64_t orc_sweep(real_t *phi, const uint8_t *mask, int rows, int cols,
     for (int colour = 0; colour < 2; ++colour) {
         uint64_t accepted = 0;
 #ifdef _OPENMP
-#pragma omp parallel for schedule(static) reduction(+:accepted)
+#pragma omp parallel for schedule(static) reduction(+:accepted) if(ORC_PARALLEL(rows, cols))
 #endif
         for (int r = 0; r < rows; ++r) {
             for (int c = (r + colour) & 1; c < cols; c += 2) {
@@ -288,7 +294,7 @@ double orc_energy(const real_t *phi, int rows, int cols, double q)
 {
     double *row_sum = (double *)malloc(sizeof(double) * (size_t)rows);
 #ifdef _OPENMP
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if(ORC_PARALLEL(rows, cols))
 #endif
     for (int r = 0; r < rows; ++r) {
         double h = 0.0;
