@@ -973,6 +973,55 @@ def test_t2_one_sweep_on_a_grid_whose_buffers_pass_4_GiB(torch_cuda, mpr, orc):
     assert e_g == pytest.approx(orc.energy_per_bond(phi), abs=2e-6)
 
 
+def test_t2_sampled_rows_of_a_context_of_a_billion_sites(torch_cuda, mpr, orc):
+    """A context of 4 grids of 16384 x 16384 = 1.07 G sites (38 GB of workspace: every per-grid base offset -- vectors,
+    lists, accumulators, bitmask -- far beyond 2^32 bytes), inputs made on the device.  The oracle cannot sweep that, but the
+    first rows of a grid are a problem of their own: the Philox site word of row r, column c is r * cols + c whatever the
+    number of rows, and one sweep carries information two rows far, so an oracle sweep of the window rows [0, W) (open at
+    its lower edge, which the real grid is not) is exact on rows [0, W - 3].  Compared there for the first and the LAST grid
+    (largest grid word and offsets): every prediction site within 1e-5 rad except decision flips (<= 1e-4 of the sites);
+    sample sites bit for bit over the whole context."""
+    torch = torch_cuda
+    if torch.cuda.get_device_properties(0).total_memory < 100 * 2 ** 30:
+        pytest.skip("needs 60 GB of device memory")
+    B, L, W = 4, 16384, 48
+    gen = torch.Generator(device="cuda"); gen.manual_seed(20261105)
+    r = torch.arange(L, device="cuda", dtype=torch.float32)[:, None]; c = torch.arange(L, device="cuda", dtype=torch.float32)[None, :]
+    z = torch.empty((B, L, L), dtype=torch.float32, device="cuda"); m = torch.empty((B, L, L), dtype=torch.uint8, device="cuda")
+    for g in range(B):
+        z[g] = torch.sin(r / (97.0 + 11.0 * g)) + torch.cos(c / 131.0) + 0.05 * torch.randn((L, L), device="cuda", generator=gen)
+        m[g] = (torch.rand((L, L), device="cuda", generator=gen) >= 0.33).to(torch.uint8)
+    del r, c
+    T, a, seed, t = 2e-3, 12.0, 4243, 7
+    ctx = mpr.Mpr(z, m)
+    ctx.set_params([T] * B, seed=seed)
+    lo, hi = ctx.get_transform()
+    phi0 = ctx.get_angles()                                   # Eq. 1 at the samples, the initial draw elsewhere
+    for g in range(B):                                        # a near-equilibrium state at the prediction sites
+        near = (z[g] - lo[g]) * (TWO_PI_F / (hi[g] - lo[g])) + math.sqrt(T) * torch.randn((L, L), device="cuda", generator=gen)
+        phi0[g] = torch.where(m[g] == 1, phi0[g], near.clamp_(0.0, TWO_PI_F))
+        del near
+    ctx.set_angles(phi0)
+    ctx.set_sweep_index(t)
+    acc = ctx.sweep(1, a, count=True)
+    got = ctx.get_angles()
+    e = ctx.energy()
+    st = ctx.get_stats()
+    assert bool(((got == phi0) | (m == 0)).all())             # sample sites bit for bit, everywhere
+    for g in range(B):
+        assert 0 < acc[g] < st[g].n_free and -1.0 < e[g] < -0.9 and st[g].t == t + 1
+    for g in (0, B - 1):
+        ref = phi0[g, :W].cpu().numpy().copy(); mw = m[g, :W].cpu().numpy()
+        orc.sweep(ref, mw, 0.5, T, a, seed, g, t)
+        keep = slice(0, W - 2)
+        d = np.abs(got[g, :W].cpu().numpy().astype(np.float64) - ref.astype(np.float64))[keep]
+        free = mw[keep] == 0
+        bad = int((d[free] > TOL_RAD).sum())
+        assert bad <= max(2, math.ceil(FLIP_FRACTION * free.sum())), (g, bad, int(free.sum()))
+        assert float(np.median(d[free])) < 1e-6
+    ctx.close()
+
+
 def test_t2_only_one_colour_has_prediction_sites(torch_cuda, mpr, orc):
     """Degenerate checkerboards: every prediction site on colour 0 (all of its neighbours are samples), then on colour 1;
     the other colour's list is empty.  Both precisions."""
