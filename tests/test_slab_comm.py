@@ -61,7 +61,9 @@ def test_dist_slab_comm_over_three_gloo_ranks(tmp_path):
 def test_slab_geometry_host_checks():
     sys.path.insert(0, ROOT)
     import pytest
+    from paper_1811_01604_b200 import build as mpr_build
     from paper_1811_01604_b200 import mpr
+    mpr_build.build()                        # a fresh checkout has no library yet (nvcc cross-compiles without a GPU)
     mpr.lib()
     assert mpr.slab_local_rows(4096, 4096, 0, 2048) == (0, 2056)
     assert mpr.slab_local_rows(4096, 4096, 2048, 4096) == (2040, 2056)
